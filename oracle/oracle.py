@@ -1,0 +1,406 @@
+"""CPU oracle for one SPH + shear-strength step -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Plain fp64: the pair passes call oracle/sph_oracle.c (straight loops over brute-force or
+cell-list neighbour sets); every per-particle step is written here in numpy, in the paper's
+order and notation, each function citing the passage of /root/reference/PAPER.md it follows
+(line numbers as PAPER.md:<line>; "reading Qn" = DESIGN.md section 3 / SURVEY.md section 8c).
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this module.  It shares no code with paper_2603_19764_b200/csrc or binding.py and
+imports neither; parameter records are duck-typed (attributes kappa, alpha, ..., materials).
+
+Parity-unpinned choices (no authority in PAPER.md; listed in DESIGN.md): the kernel's
+functional form and kappa (Q3), AV constants (Q6), the analytic EOS stand-in (Q13), the
+singular-C fallback rule (Q9), the fixed-particle rule (Q16).  Everything else is pinned by
+tests/test_oracle_*.py.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, Optional
+
+import numpy as np
+
+from . import build as _build
+
+FLAG_STRENGTH = 1
+FLAG_CORRECTION_TENSOR = 2
+FLAG_PCLIP_GLOBAL = 4
+FLAG_JAUMANN_COROTATIONAL = 8
+
+GATHER, SYMMETRIC = 0, 1
+CTOL = 1.0e-4          # reading Q9: C = I unless |det C^-1| > CTOL * ||C^-1||_F^3
+
+_lib = None
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int)
+_lp = C.POINTER(C.c_longlong)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(_build.build())
+        for name in ("orc_W", "orc_dWdr", "orc_dWdh"):
+            f = getattr(_lib, name)
+            f.restype = C.c_double
+            f.argtypes = [C.c_double, C.c_double, C.c_double]
+        _lib.orc_max_threads.restype = C.c_int
+    return _lib
+
+
+def _d(a):
+    assert a.dtype == np.float64 and a.flags.c_contiguous
+    return a.ctypes.data_as(_dp)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+# ---------------------------------------------------------------------------
+# kernel (reading Q3) -- scalar entry points for the pin tests
+# ---------------------------------------------------------------------------
+def W(r, h, kappa=2.0):
+    return lib().orc_W(float(r), float(h), float(kappa))
+
+
+def dWdr(r, h, kappa=2.0):
+    return lib().orc_dWdr(float(r), float(h), float(kappa))
+
+
+def dWdh(r, h, kappa=2.0):
+    return lib().orc_dWdh(float(r), float(h), float(kappa))
+
+
+# ---------------------------------------------------------------------------
+# Pass O1 -- neighbour sets
+# ---------------------------------------------------------------------------
+def neighbors(x, y, z, h, kappa, which, mode="brute"):
+    """CSR neighbour lists (counts, offsets[n+1], list), ascending j, fp32 predicate (reading Q4).
+
+    which = GATHER: {j : r2 < H_i^2} (contains i);
+    which = SYMMETRIC: {j != i : r2 < max(H_i^2, H_j^2)}.
+    """
+    x, y, z, h = map(_f64, (x, y, z, h))
+    n = x.shape[0]
+    fn = lib().orc_neighbors_brute if mode == "brute" else lib().orc_neighbors_grid
+    counts = np.zeros(n, dtype=np.int32)
+    fn(C.c_longlong(n), _d(x), _d(y), _d(z), _d(h), C.c_double(kappa), C.c_int(which),
+       counts.ctypes.data_as(_ip), None, None)
+    offsets = np.zeros(n + 1, dtype=np.int64)
+    np.cumsum(counts, out=offsets[1:])
+    lst = np.zeros(max(int(offsets[-1]), 1), dtype=np.int32)
+    fn(C.c_longlong(n), _d(x), _d(y), _d(z), _d(h), C.c_double(kappa), C.c_int(which),
+       counts.ctypes.data_as(_ip), offsets.ctypes.data_as(_lp), lst.ctypes.data_as(_ip))
+    return counts, offsets, lst
+
+
+# ---------------------------------------------------------------------------
+# Pass O2 -- density, Omega (PAPER.md:57 Eq. 1, :66 Eq. 3)
+# ---------------------------------------------------------------------------
+def density(x, y, z, m, h, kappa, offsets, lst):
+    x, y, z, m, h = map(_f64, (x, y, z, m, h))
+    n = x.shape[0]
+    rho = np.zeros(n); omega = np.zeros(n)
+    lib().orc_density(C.c_longlong(n), _d(x), _d(y), _d(z), _d(m), _d(h), C.c_double(kappa),
+                      offsets.ctypes.data_as(_lp), lst.ctypes.data_as(_ip), _d(rho), _d(omega))
+    return rho, omega
+
+
+# ---------------------------------------------------------------------------
+# Pass O3 -- EOS, shear modulus, yield strength, plastic projection (per particle)
+# ---------------------------------------------------------------------------
+def _matcol(params, mat, name):
+    return np.array([getattr(mm, name) for mm in params.materials], dtype=np.float64)[mat]
+
+
+def eos(params, rho, u, mat):
+    """Analytic stand-in for EOSlib (reading Q13, BASELINE.json configs[0]):
+    P = c0^2 (rho - rho0), c = c0, T = u / cv.  PCLIP_GLOBAL clips P >= 0 everywhere (Q8)."""
+    rho0 = _matcol(params, mat, "rho0"); c0 = _matcol(params, mat, "c0"); cv = _matcol(params, mat, "cv")
+    P = c0 * c0 * (rho - rho0)
+    if params.flags & FLAG_PCLIP_GLOBAL:
+        P = np.maximum(P, 0.0)
+    return P, c0.copy(), u / cv
+
+
+def shear_modulus(params, rho, cs, mat):
+    """Gamma = 3(1-2nu)/(2(1+nu)) K, K = rho c_s^2 (Eq. 30), or the runtime
+    constant per material when one is given."""
+    Gc = _matcol(params, mat, "Gamma"); nu = _matcol(params, mat, "nu")
+    G30 = 3.0 * (1.0 - 2.0 * nu) / (2.0 * (1.0 + nu)) * rho * cs * cs
+    return np.where(Gc > 0.0, Gc, G30)
+
+
+def yield_strength(params, P, T, mat):
+    """Y_i = Y0 + mu_i P/(1 + mu_i P/(Ym - Y0)) (Eq. 34) with P < 0 clipped to 0
+    (PAPER.md:202); Y_d = mu_d P (Eq. 35); Y = min(Y_i, Y_d) when mu_d is finite (Eq. 36,
+    reading Q10); Y -> Y tanh(xi (T_melt/T - 1)) (Eq. 37), clamped to >= 0 above
+    the melting point and equal to Y for T <= 0 (reading Q11)."""
+    Y0 = _matcol(params, mat, "Y0"); Ym = _matcol(params, mat, "Ym")
+    mu_i = _matcol(params, mat, "mu_i"); mu_d = _matcol(params, mat, "mu_d")
+    xi = _matcol(params, mat, "xi"); Tm = _matcol(params, mat, "Tmelt")
+    Pp = np.maximum(P, 0.0)
+    span = Ym - Y0
+    with np.errstate(divide="ignore", invalid="ignore"):
+        Yi = np.where(span > 0.0, Y0 + mu_i * Pp / (1.0 + mu_i * Pp / np.where(span > 0.0, span, 1.0)), Y0)
+        Y = np.where(np.isfinite(mu_d), np.minimum(Yi, np.where(np.isfinite(mu_d), mu_d, 0.0) * Pp), Yi)
+        soft = np.where(T > 0.0, np.maximum(0.0, np.tanh(xi * (Tm / np.where(T > 0.0, T, 1.0) - 1.0))), 1.0)
+    return Y * soft
+
+
+def J2(S):
+    """J2 = 1/2 S:S (Eq. 33) from the five stored components, S_zz = -S_xx - S_yy."""
+    sxx, syy, sxy, sxz, syz = S
+    szz = -sxx - syy
+    return 0.5 * (sxx * sxx + syy * syy + szz * szz) + sxy * sxy + sxz * sxz + syz * syz
+
+
+def project(S, Y):
+    """S -> f S, f = min(Y / sqrt(J2), 1) (Eq. 31-32); f = 1 if J2 = 0 (Q12)."""
+    sj = np.sqrt(J2(S))
+    with np.errstate(divide="ignore", invalid="ignore"):
+        f = np.where(sj > Y, Y / np.where(sj > 0.0, sj, 1.0), 1.0)
+    return S * f[None, :], f
+
+
+# ---------------------------------------------------------------------------
+# Pass O4 -- velocity gradient (Eq. 20-24)
+# ---------------------------------------------------------------------------
+def gradients(x, y, z, m, h, vx, vy, vz, rho, omega, kappa, offsets, lst):
+    """F (Eq. 20) and C^-1 (Eq. 21) as [9][n], component 3*alpha + beta."""
+    args = list(map(_f64, (x, y, z, m, h, vx, vy, vz, rho, omega)))
+    n = args[0].shape[0]
+    F = np.zeros((9, n)); Cinv = np.zeros((9, n))
+    lib().orc_gradients(C.c_longlong(n), *[_d(a) for a in args], C.c_double(kappa),
+                        offsets.ctypes.data_as(_lp), lst.ctypes.data_as(_ip), _d(F), _d(Cinv))
+    return F, Cinv
+
+
+def correct_gradient(F, Cinv, flags):
+    """G = F . C (Eq. 22).  C = (C^-1)^-1 by a 3x3 inverse; C = 1 when the correction
+    tensor is switched off or C^-1 is singular (reading Q9).  Returns G [9][n] and
+    the per-particle fallback flag."""
+    n = F.shape[1]
+    Fm = F.T.reshape(n, 3, 3)
+    Cm = Cinv.T.reshape(n, 3, 3)
+    det = np.linalg.det(Cm)
+    fro = np.sqrt((Cm * Cm).sum(axis=(1, 2)))
+    ok = np.abs(det) > CTOL * fro ** 3
+    if not (flags & FLAG_CORRECTION_TENSOR):
+        ok[:] = False
+    Cfull = np.tile(np.eye(3), (n, 1, 1))
+    if ok.any():
+        Cfull[ok] = np.linalg.inv(Cm[ok])
+    G = np.einsum("nag,ngb->nab", Fm, Cfull)
+    return np.ascontiguousarray(G.reshape(n, 9).T), (~ok).astype(np.int32)
+
+
+def strain_and_rotation(G):
+    """eps_dot = (G + G^T)/2 (Eq. 24), R = (G - G^T)/2 (Eq. 23)."""
+    n = G.shape[1]
+    Gm = G.T.reshape(n, 3, 3)
+    GT = np.transpose(Gm, (0, 2, 1))
+    return 0.5 * (Gm + GT), 0.5 * (Gm - GT)
+
+
+def _S3(S):
+    sxx, syy, sxy, sxz, syz = S
+    szz = -sxx - syy
+    return np.stack([np.stack([sxx, sxy, sxz], axis=1),
+                     np.stack([sxy, syy, syz], axis=1),
+                     np.stack([sxz, syz, szz], axis=1)], axis=1)
+
+
+def stress_rate(G, S, Gamma, flags):
+    """dS/dt = 2 Gamma (eps_dot - tr(eps_dot)/3 delta) + S.R + (S.R)^T  (Eq. 13, as
+    printed: S^{ag} R^{gb} + S^{bg} R^{ga}).  JAUMANN_COROTATIONAL flips the sign of the rotation
+    terms (reading Q1).  Evaluated as a full 3x3; returns the five stored components [5][n],
+    the full tensor and 1/2 eps_dot:eps_dot (Eq. 43)."""
+    eps, R = strain_and_rotation(G)
+    S3 = _S3(S)
+    tr = np.trace(eps, axis1=1, axis2=2)
+    elastic = 2.0 * Gamma[:, None, None] * (eps - tr[:, None, None] / 3.0 * np.eye(3)[None])
+    SR = np.einsum("nag,ngb->nab", S3, R)
+    sgn = -1.0 if (flags & FLAG_JAUMANN_COROTATIONAL) else 1.0
+    dS3 = elastic + sgn * (SR + np.transpose(SR, (0, 2, 1)))
+    dS = np.stack([dS3[:, 0, 0], dS3[:, 1, 1], dS3[:, 0, 1], dS3[:, 0, 2], dS3[:, 1, 2]], axis=0)
+    eps2 = 0.5 * (eps * eps).sum(axis=(1, 2))
+    return np.ascontiguousarray(dS), dS3, eps2
+
+
+def stress_rate_components(G, S, Gamma, flags):
+    """The component form Eq. 25-29 (garbled in the extraction, reconstructed from
+    Eq. 13 in SURVEY.md Appendix A / DESIGN.md reading Q2).  Used by the tests as a cross-check
+    of stress_rate(); G component index 3*alpha + beta."""
+    Gxx, Gxy, Gxz, Gyx, Gyy, Gyz, Gzx, Gzy, Gzz = G
+    Sxx, Syy, Sxy, Sxz, Syz = S
+    s = -1.0 if (flags & FLAG_JAUMANN_COROTATIONAL) else 1.0
+    dSxx = s * (Sxy * (Gyx - Gxy) + Sxz * (Gzx - Gxz)) - (2.0 / 3.0) * Gamma * (Gyy + Gzz - 2.0 * Gxx)
+    dSyy = s * (Sxy * (Gxy - Gyx) + Syz * (Gzy - Gyz)) - (2.0 / 3.0) * Gamma * (Gxx + Gzz - 2.0 * Gyy)
+    dSxy = Gamma * (Gxy + Gyx) + s * 0.5 * (Sxx * (Gxy - Gyx) + Syy * (Gyx - Gxy)
+                                            + Syz * (Gzx - Gxz) + Sxz * (Gzy - Gyz))
+    dSxz = Gamma * (Gxz + Gzx) + s * 0.5 * ((Sxx + Syy) * (Gxz - Gzx) + Sxx * (Gxz - Gzx)
+                                            + Sxy * (Gyz - Gzy) + Syz * (Gyx - Gxy))
+    dSyz = Gamma * (Gyz + Gzy) + s * 0.5 * ((Sxx + Syy) * (Gyz - Gzy) + Syy * (Gyz - Gzy)
+                                            + Sxz * (Gxy - Gyx) + Sxy * (Gxz - Gzx))
+    return np.stack([dSxx, dSyy, dSxy, dSxz, dSyz], axis=0)
+
+
+# ---------------------------------------------------------------------------
+# Pass O5 -- forces (PAPER.md:71 Eq. 4, :76-93 Eq. 5-8, :140-144 Eq. 18-19)
+# ---------------------------------------------------------------------------
+def forces(params, x, y, z, m, h, vx, vy, vz, rho, omega, P, cs, S, g, offsets, lst):
+    args = list(map(_f64, (x, y, z, m, h, vx, vy, vz, rho, omega, P, cs)))
+    n = args[0].shape[0]
+    S = _f64(S)
+    strength = 1 if (params.flags & FLAG_STRENGTH) else 0
+    a = np.zeros((3, n)); dudt = np.zeros(n); mumax = np.zeros(n)
+    if g is None:
+        gp = [None, None, None]
+    else:
+        g = _f64(g)
+        gp = [_d(g[0]), _d(g[1]), _d(g[2])]
+    lib().orc_forces(C.c_longlong(n), *[_d(q) for q in args], _d(S), C.c_int(strength),
+                     gp[0], gp[1], gp[2],
+                     C.c_double(params.kappa), C.c_double(params.alpha), C.c_double(params.beta),
+                     C.c_double(params.eps_av),
+                     offsets.ctypes.data_as(_lp), lst.ctypes.data_as(_ip), _d(a), _d(dudt), _d(mumax))
+    return a, dudt, mumax
+
+
+def timestep(params, h, cs, mumax, a=None):
+    """dt_i,CFL = eta_C h_i / ((1 + 0.6 alpha) c_i + 0.6 beta max_j |min(0, mu_ij)|)
+    (Eq. 39); optionally dt_i,a = eta_a sqrt(h_i/|a_i|) (Eq. 38 with
+    epsilon = h_i)."""
+    dt = params.eta_C * h / ((1.0 + 0.6 * params.alpha) * cs + 0.6 * params.beta * mumax)
+    if params.eta_a > 0.0 and a is not None:
+        an = np.sqrt((a * a).sum(axis=0))
+        with np.errstate(divide="ignore"):
+            dt = np.minimum(dt, params.eta_a * np.sqrt(h / np.where(an > 0, an, np.inf)))
+    return dt
+
+
+# ---------------------------------------------------------------------------
+# O1..O6 for one set of predicted values
+# ---------------------------------------------------------------------------
+def derivatives(params, x, y, z, m, h, vx, vy, vz, u, S, mat, g=None, mode="brute") -> Dict[str, np.ndarray]:
+    """Everything the step needs at one time level, from PREDICTED v, u, S (PAPER.md:240,
+    reading Q14): neighbour sets -> rho, Omega -> P, c, T, Gamma, Y -> S_pred rescaled (Eq. 31)
+    -> F, C^-1, G -> a, du/dt, mu_max -> dS/dt, 1/2 eps:eps, dt_i."""
+    kap = params.kappa
+    out: Dict[str, np.ndarray] = {}
+    cg, og, lg = neighbors(x, y, z, h, kap, GATHER, mode)
+    cs_, os_, ls_ = neighbors(x, y, z, h, kap, SYMMETRIC, mode)
+    out["n_gather"], out["n_symmetric"] = cg, cs_
+    rho, omega = density(x, y, z, m, h, kap, og, lg)
+    P, cs, T = eos(params, rho, _f64(u), mat)
+    Gamma = shear_modulus(params, rho, cs, mat)
+    Y = yield_strength(params, P, T, mat)
+    strength = bool(params.flags & FLAG_STRENGTH)
+    S = _f64(S)
+    if strength:
+        Sp, f = project(S, Y)
+    else:
+        Sp, f = np.zeros_like(S), np.ones_like(rho)
+    out.update(rho=rho, omega=omega, P=P, cs=cs, T=T, Gamma=Gamma, Y=Y, S_pred=Sp, f_pred=f)
+    a, dudt, mumax = forces(params, x, y, z, m, h, vx, vy, vz, rho, omega, P, cs, Sp, g, os_, ls_)
+    out.update(a=a, dudt=dudt, mumax=mumax)
+    if strength:
+        F, Cinv = gradients(x, y, z, m, h, vx, vy, vz, rho, omega, kap, os_, ls_)
+        G, cflag = correct_gradient(F, Cinv, params.flags)
+        dS, _, eps2 = stress_rate(G, Sp, Gamma, params.flags)
+    else:
+        n = rho.shape[0]
+        F = np.zeros((9, n)); Cinv = np.zeros((9, n)); G = np.zeros((9, n))
+        cflag = np.zeros(n, np.int32); dS = np.zeros((5, n)); eps2 = np.zeros(n)
+    out.update(F=F, Cinv=Cinv, G=G, cflag=cflag, dS=dS, eps2=eps2)
+    out["dt_i"] = timestep(params, _f64(h), cs, mumax, a)
+    return out
+
+
+def single_pass(wl, dt: Optional[float] = None, mode="brute") -> Dict[str, np.ndarray]:
+    """BASELINE.json configs[0]: one density + gradient + force + strength-update pass, i.e.
+    steps 4-7 of the step sequence with S_half = S_pred = S_in, v_pred = v_in, u_pred = u_in
+    (SURVEY.md Appendix B).  Adds the closed S, v, u (Eq. 41 + rescale)."""
+    A = {k: _f64(v) for k, v in wl.arrays.items()}
+    dt = wl.dt if dt is None else dt
+    S = np.stack([A["Sxx"], A["Syy"], A["Sxy"], A["Sxz"], A["Syz"]], axis=0)
+    g = np.stack([A["gx"], A["gy"], A["gz"]], axis=0)
+    d = derivatives(wl.params, A["x"], A["y"], A["z"], A["m"], A["h"], A["vx"], A["vy"], A["vz"],
+                    A["u"], S, wl.mat, g, mode)
+    free = (wl.fixed == 0)
+    v = np.stack([A["vx"], A["vy"], A["vz"]], axis=0)
+    d["v_close"] = v + 0.5 * dt * d["a"] * free[None, :]
+    d["u_close"] = A["u"] + 0.5 * dt * d["dudt"]
+    if wl.params.flags & FLAG_STRENGTH:
+        Sc = S + 0.5 * dt * d["dS"]
+        d["S_close"], d["f_close"] = project(Sc, d["Y"])
+    else:
+        d["S_close"], d["f_close"] = np.zeros_like(S), np.ones(S.shape[1])
+    return d
+
+
+# ---------------------------------------------------------------------------
+# the full step (Eq. 40-42)
+# ---------------------------------------------------------------------------
+class Stepper:
+    """Global-dt kick-drift-kick with predictor-corrector for u and S (reading Q17)."""
+
+    def __init__(self, wl, mode="grid"):
+        A = {k: _f64(v) for k, v in wl.arrays.items()}
+        self.params = wl.params
+        self.mode = mode
+        self.x = np.stack([A["x"], A["y"], A["z"]], axis=0)
+        self.v = np.stack([A["vx"], A["vy"], A["vz"]], axis=0)
+        self.u = A["u"].copy()
+        self.S = np.stack([A["Sxx"], A["Syy"], A["Sxy"], A["Sxz"], A["Syz"]], axis=0)
+        self.m, self.h = A["m"], A["h"]
+        self.g = np.stack([A["gx"], A["gy"], A["gz"]], axis=0)
+        self.mat = wl.mat
+        self.free = (wl.fixed == 0).astype(np.float64)
+        self.e_acc = np.zeros_like(self.u)
+        self.d = None              # derivatives at the current full step
+        self.dt_next = None
+        self.strength = bool(wl.params.flags & FLAG_STRENGTH)
+
+    def _derivs(self, v, u, S):
+        return derivatives(self.params, self.x[0], self.x[1], self.x[2], self.m, self.h,
+                           v[0], v[1], v[2], u, S, self.mat, self.g, self.mode)
+
+    def bootstrap(self):
+        """First step: a_0, du_0, dS_0 from the current state (pred = current, dt = 0)."""
+        self.d = self._derivs(self.v, self.u, self.S)
+        self.dt_next = float(self.d["dt_i"].min())
+
+    def step(self, dt: float = 0.0) -> float:
+        if self.d is None:
+            self.bootstrap()
+        if dt <= 0.0:
+            dt = self.dt_next
+        a, dudt, dS = self.d["a"], self.d["dudt"], self.d["dS"]
+        fr = self.free[None, :]
+        # 1. opening kick (Eq. 42); fixed particles keep x, v (reading Q16)
+        v_half = self.v + 0.5 * dt * a * fr
+        u_half = self.u + 0.5 * dt * dudt
+        S_half = self.S + 0.5 * dt * dS
+        # 2. drift
+        self.x = self.x + dt * v_half * fr
+        # 3. prediction from the derivatives of the previous step (Eq. 40)
+        v_pred = v_half + 0.5 * dt * a * fr
+        u_pred = u_half + 0.5 * dt * dudt
+        S_pred = S_half + 0.5 * dt * dS
+        # 4-6. new derivatives from the predicted (and rescaled, Eq. 31) values
+        d = self._derivs(v_pred, u_pred, S_pred)
+        # 7. closing kick (Eq. 41) and rescale again
+        self.v = v_half + 0.5 * dt * d["a"] * fr
+        self.u = u_half + 0.5 * dt * d["dudt"]
+        if self.strength:
+            self.S, _ = project(S_half + 0.5 * dt * d["dS"], d["Y"])
+        # 8. carried derivatives, accumulated strain-rate invariant (Eq. 43)
+        self.e_acc = self.e_acc + dt * d["eps2"]
+        self.d = d
+        self.dt_next = float(d["dt_i"].min())
+        return dt
