@@ -1,0 +1,195 @@
+/*
+ * sph.h -- C ABI of libsph.so: one SPH time step of a solid body with pressure-dependent
+ * shear strength (arxiv/paper_2603_19764, section 2), hand-written CUDA for sm_100a.
+ *
+ * Citations are PAPER.md:<line> (section / equation) of /root/reference/PAPER.md; "reading Qn"
+ * refers to DESIGN.md section 3.  No torch types cross this boundary: plain pointers and sizes.
+ *
+ * Conventions
+ *  - Every pointer marked DEVICE is a CUDA device pointer, HOST a host pointer.
+ *  - Every call returns SPH_OK (0) or a negative SPH_E* code; nothing throws.
+ *  - Every call except sph_get_timings, sph_get_counters and sph_step_host is asynchronous on
+ *    the CUDA stream given to sph_init and never synchronises the device.
+ *  - The caller owns every particle array and the workspace; the library owns only the small
+ *    host-side context.  The workspace must stay alive and untouched until sph_destroy.
+ *  - Internally particles are kept sorted by Morton key ("resident" state).  Outputs of
+ *    sph_get_field / sph_get_neighbors / sph_download_state are in CALLER order.
+ *  - Particle arrays are fp32 structure-of-arrays, length n (BASELINE.json north_star).
+ */
+#ifndef SPH_H_
+#define SPH_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SPH_MAX_MATERIALS 8
+
+/* sph_params.flags */
+#define SPH_STRENGTH              1u  /* evolve S, add the S terms of Eq. 18-19      */
+#define SPH_CORRECTION_TENSOR     2u  /* G = F.C (Eq. 22); off: C = 1      */
+#define SPH_PCLIP_GLOBAL          4u  /* clip P >= 0 in the EOS too, not only in Eq. 34 (reading Q8)    */
+#define SPH_JAUMANN_COROTATIONAL  8u  /* flip the sign of the rotation terms of Eq. 13 (reading Q1)     */
+
+/* error codes */
+#define SPH_OK         0
+#define SPH_EINVAL    (-1)  /* bad argument (NULL, n < 0, unknown id, bad material index count)        */
+#define SPH_ENOMEM    (-2)  /* workspace smaller than sph_workspace_bytes()                             */
+#define SPH_ECUDA     (-3)  /* a CUDA call failed; sph_last_cuda_error() has the cudaError_t            */
+#define SPH_EORDER    (-4)  /* pass called before its prerequisite (e.g. sph_forces before sph_density) */
+#define SPH_ECAPACITY (-5)  /* n > n_max given to sph_init                                              */
+
+/* sph_strength_update phases */
+#define SPH_PREDICT     0   /* EOS, Gamma, Y, rescale S_pred, pack pair-pass operands */
+#define SPH_CLOSE       1   /* G, eps_dot, R, dS/dt, closing kick + rescale       */
+#define SPH_DERIVATIVES 2   /* as SPH_CLOSE but leaves v, u, S untouched (bootstrap of the first step)       */
+
+/* sph_get_neighbors sets (reading Q4: fp32 predicate) */
+#define SPH_GATHER     0    /* { j : r2_ij < H_i^2 }, contains i            */
+#define SPH_SYMMETRIC  1    /* { j != i : r2_ij < max(H_i^2, H_j^2) } */
+
+/* sph_get_field ids; multi-component fields take id + component                                        */
+enum {
+    SPH_F_RHO = 0,      /* Eq. 1                                          */
+    SPH_F_OMEGA,        /* Eq. 3                                          */
+    SPH_F_P,            /* EOS pressure (after SPH_PCLIP_GLOBAL)          */
+    SPH_F_CS,           /* sound speed                                    */
+    SPH_F_T,            /* temperature u_pred / cv                        */
+    SPH_F_GAMMA,        /* shear modulus, Eq. 30 or constant              */
+    SPH_F_Y,            /* yield strength, Eq. 34-37                      */
+    SPH_F_MUMAX,        /* max_j |min(0, mu_ij)|, Eq. 39                  */
+    SPH_F_DUDT,         /* Eq. 8 + Eq. 19                                 */
+    SPH_F_DT,           /* per-particle time-step limit, Eq. 38-39        */
+    SPH_F_EACC,         /* accumulated 1/2 eps_dot:eps_dot dt, Eq. 43     */
+    SPH_F_EPS2,         /* 1/2 eps_dot:eps_dot of the last CLOSE          */
+    SPH_F_U,            /* u after the closing kick                       */
+    SPH_F_CFLAG,        /* 1.0 where C fell back to 1 (reading Q9)        */
+    SPH_F_NGATHER,      /* |gather set| as float                          */
+    SPH_F_NSYMMETRIC,   /* |symmetric set| as float                       */
+    SPH_F_A = 32,       /* +0..2   acceleration, Eq. 18 (+ a_ext)         */
+    SPH_F_V = 36,       /* +0..2   velocity after the closing kick        */
+    SPH_F_X = 40,       /* +0..2   position                               */
+    SPH_F_SPRED = 48,   /* +0..4   predicted + rescaled S (xx,yy,xy,xz,yz)*/
+    SPH_F_S = 56,       /* +0..4   S after the closing kick + rescale     */
+    SPH_F_DSDT = 64,    /* +0..4   dS/dt, Eq. 13 / 25-29                  */
+    SPH_F_F = 80,       /* +0..8   raw velocity gradient, Eq. 20, 3*a+b   */
+    SPH_F_CINV = 96,    /* +0..8   C^-1, Eq. 21                           */
+    SPH_F_G = 112       /* +0..8   corrected gradient, Eq. 22             */
+};
+
+/* sph_get_timings slots (milliseconds of the last call of each pass; CUDA events) */
+enum { SPH_T_BUILD = 0, SPH_T_DENSITY, SPH_T_PREDICT, SPH_T_GRADIENT, SPH_T_FORCE, SPH_T_CLOSE,
+       SPH_T_KICKDRIFT, SPH_T_STEP, SPH_T_COUNT };
+
+/* sph_get_counters slots (from the last pass of each kind) */
+enum { SPH_C_PAIRS_GATHER = 0,   /* sum_i |gather set(i)|   (true pairs of the density pass)    */
+       SPH_C_PAIRS_SYMMETRIC,    /* sum_i |symmetric set(i)| (true pairs of gradient/force)     */
+       SPH_C_TESTS_DENSITY,      /* candidate pairs the density pass tested                     */
+       SPH_C_TESTS_FORCE,        /* candidate pairs the gradient/force pass tested              */
+       SPH_C_CFALLBACK,          /* particles whose C fell back to 1                             */
+       SPH_C_COUNT };
+
+typedef struct sph_ctx sph_ctx;   /* opaque, library-owned (host memory) */
+
+/* Per-material constants.  EOS stand-in (reading Q13, BASELINE.json
+ * configs[0]): P = c0^2 (rho - rho0), c = c0, T = u / cv. */
+typedef struct sph_material {
+    float rho0, c0, cv;
+    float Gamma;   /* > 0: constant shear modulus; <= 0: Eq. 30 with nu            */
+    float nu;      /* Poisson ratio of Eq. 30                                  */
+    float Y0, Ym, mu_i;   /* Eq. 34                                               */
+    float mu_d;    /* Eq. 35-36; +INFINITY disables the min rule (reading Q10) */
+    float xi, Tmelt;      /* Eq. 37                                               */
+} sph_material;
+
+typedef struct sph_params {
+    float kappa;               /* support radius H = kappa h (reading Q3; default 2)              */
+    float alpha, beta, eps_av; /* Eq. 5-6                                        */
+    float eta_C, eta_a;        /* Eq. 38-39; eta_a <= 0 disables Eq. 38        */
+    int n_materials;           /* 1..SPH_MAX_MATERIALS                                            */
+    unsigned flags;            /* SPH_STRENGTH | ...                                              */
+    sph_material mat[SPH_MAX_MATERIALS];
+} sph_params;
+
+/* Caller-owned particle arrays, each of length n.  For the device entry points all pointers are
+ * DEVICE pointers; for sph_step_host all are HOST pointers.  S is symmetric and traceless, five
+ * stored components (Eq. 11).  gx,gy,gz (external acceleration, the "G" term of
+ * Eq. 18 supplied as input), mat and fixed may be NULL (= 0, material 0, nothing fixed). */
+typedef struct sph_state {
+    float *x, *y, *z, *m, *h, *vx, *vy, *vz, *u;
+    float *Sxx, *Syy, *Sxy, *Sxz, *Syz;
+    const float *gx, *gy, *gz;
+    const int *mat;              /* material index per particle, 0..n_materials-1                 */
+    const unsigned char *fixed;  /* 1: particle skips kick and drift (reading Q16)  */
+} sph_state;
+
+/* Bytes of DEVICE workspace sph_init needs for up to n_max particles (0 on bad arguments). */
+size_t sph_workspace_bytes(const sph_params *params, long long n_max);
+
+/* Create a context.  params: HOST.  workspace: DEVICE, >= sph_workspace_bytes(), 256-byte aligned.
+ * cuda_stream: a cudaStream_t (NULL = default stream).  Errors: EINVAL, ENOMEM, ECUDA. */
+int sph_init(sph_ctx **ctx, const sph_params *params, long long n_max,
+             void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* S1: Morton keys -> radix sort -> gather into the resident sorted arrays -> chunk bounding boxes
+ * and the chunk tree the pair passes walk (stands in for the paper's tree build).
+ * state != NULL: ingest the caller's arrays (DEVICE), n particles; derivatives carried between
+ * steps are reset.  state == NULL: re-sort the resident particles at their current positions.
+ * n = 0 is legal.  Errors: EINVAL, ECAPACITY, EORDER (state == NULL with nothing resident). */
+int sph_build_neighbors(sph_ctx *ctx, const sph_state *state, long long n);
+
+/* S2: rho_i (Eq. 1), Omega_i (Eq. 3), |gather set|.  Needs sph_build_neighbors. */
+int sph_density(sph_ctx *ctx);
+
+/* S3 / S6: per-particle strength update, phase = SPH_PREDICT | SPH_CLOSE | SPH_DERIVATIVES.
+ * PREDICT needs sph_density; CLOSE needs sph_gradients (if SPH_STRENGTH) and sph_forces.
+ * dt is the step of the closing half kick (ignored by PREDICT and DERIVATIVES). */
+int sph_strength_update(sph_ctx *ctx, int phase, float dt);
+
+/* S4: F_i (Eq. 20), C_i^-1 (Eq. 21) over the symmetric set.  Needs PREDICT. */
+int sph_gradients(sph_ctx *ctx);
+
+/* S5: a_i (Eq. 4, 7, 18 + a_ext), du_i/dt (Eq. 8, 19), mu_max (Eq. 39).  Needs PREDICT. */
+int sph_forces(sph_ctx *ctx);
+
+/* One full step (Eq. 40-42): opening kick, drift,
+ * prediction, S1..S6 (gradient and force passes fused), next dt.  state != NULL (DEVICE arrays):
+ * ingested first if nothing is resident, and written back (x, v, u, S) in caller order at the
+ * end; state == NULL: everything stays resident.  dt > 0: use it; dt <= 0: use the CFL step of
+ * the previous derivatives (Eq. 39).  dt_used: DEVICE pointer to one float, or NULL. */
+int sph_step(sph_ctx *ctx, sph_state *state, long long n, float dt, float *dt_used);
+
+/* The same step through HOST buffers: copies the state host->device into library-owned staging,
+ * steps, copies x, v, u, S back device->host, and synchronises the stream.  dt_used: HOST. */
+int sph_step_host(sph_ctx *ctx, sph_state *host_state, long long n, float dt, float *dt_used);
+
+/* Write x, v, u, S of the resident particles to the caller's DEVICE arrays in caller order. */
+int sph_download_state(sph_ctx *ctx, sph_state *state);
+
+/* Copy one scalar field (enum above, id + component) to dst (DEVICE, n floats, caller order). */
+int sph_get_field(sph_ctx *ctx, int field_id, float *dst);
+
+/* Test hook: neighbour sets as the pair passes see them, as ORIGINAL particle ids.
+ * counts: DEVICE int[n].  If list != NULL, offsets (DEVICE long long[n+1], exclusive prefix of
+ * counts, supplied by the caller) says where each particle's ids go; order within a row is
+ * unspecified.  list_capacity: entries available in list (ECAPACITY if offsets[n] exceeds it is
+ * NOT checked on the device; the caller sizes list from counts). */
+int sph_get_neighbors(sph_ctx *ctx, int which, int *counts, const long long *offsets, int *list);
+
+/* HOST outputs.  Both synchronise the stream. */
+int sph_get_timings(sph_ctx *ctx, float *ms, int n);            /* SPH_T_* slots              */
+int sph_get_counters(sph_ctx *ctx, long long *counters, int n); /* SPH_C_* slots              */
+
+/* Number of this library's kernel launches since sph_init (HOST; no synchronisation). */
+long long sph_launch_count(const sph_ctx *ctx);
+
+int sph_last_cuda_error(const sph_ctx *ctx);
+const char *sph_strerror(int code);
+void sph_destroy(sph_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPH_H_ */

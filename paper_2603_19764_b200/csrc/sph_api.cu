@@ -1,0 +1,463 @@
+// sph_api.cu -- the C ABI of include/sph.h: workspace layout, pass sequencing, timings.
+#include <math.h>
+#include <new>
+#include <stdlib.h>
+#include <string.h>
+
+#include "sph_internal.cuh"
+
+// ------------------------------------------------------------------------------------------
+// workspace layout: one bump allocation, 256-byte aligned pieces
+// ------------------------------------------------------------------------------------------
+struct Bump {
+    char *base;
+    size_t off;
+    template <class T> T *take(size_t count)
+    {
+        off = (off + 255) & ~(size_t)255;
+        T *p = base ? (T *)(base + off) : (T *)nullptr;
+        off += count * sizeof(T);
+        return p;
+    }
+};
+
+static void tree_counts(long long n_max, int *count, int *nlev)
+{
+    int cnt = sph_div_up(n_max > 0 ? n_max : 1, SPH_CHUNK), L = 0;
+    count[0] = cnt;
+    while (cnt > SPH_ARITY && L + 1 < SPH_MAX_LEVELS) {
+        cnt = sph_div_up(cnt, SPH_ARITY);
+        count[++L] = cnt;
+    }
+    *nlev = L + 1;
+}
+
+static size_t carve(Dev *d, float **stage, char *base, long long n_max)
+{
+    Bump b{base, 0};
+    size_t N = (size_t)(n_max > 0 ? n_max : 1);
+    Dev tmp;
+    Dev &o = d ? *d : tmp;
+    o.n_max = n_max;
+    for (int k = 0; k < 2; ++k) {
+        Resident &r = k ? o.alt : o.r;
+        r.pm = b.take<float4>(N);
+        r.vh = b.take<float4>(N);
+        for (int f = 0; f < SPH_NPP; ++f) r.s[f] = b.take<float>(N);
+    }
+    int count[SPH_MAX_LEVELS], nlev;
+    tree_counts(n_max, count, &nlev);
+    for (int L = 0; L < SPH_MAX_LEVELS; ++L) {
+        size_t c = L < nlev ? (size_t)count[L] : 1;
+        o.tree.lo[L] = b.take<float4>(c);
+        o.tree.hi[L] = b.take<float4>(c);
+    }
+    for (int k = 0; k < 3; ++k) o.vfull[k] = b.take<float>(N);
+    o.ufull = b.take<float>(N);
+    for (int k = 0; k < 5; ++k) o.Sfull[k] = b.take<float>(N);
+    for (int k = 0; k < 3; ++k) o.a[k] = b.take<float>(N);
+    o.dudt = b.take<float>(N);
+    for (int k = 0; k < 5; ++k) o.dS[k] = b.take<float>(N);
+    o.rho = b.take<float>(N); o.omega = b.take<float>(N); o.P = b.take<float>(N); o.cs = b.take<float>(N);
+    o.T = b.take<float>(N); o.Gamma = b.take<float>(N); o.Y = b.take<float>(N); o.mumax = b.take<float>(N);
+    o.dti = b.take<float>(N); o.eps2 = b.take<float>(N); o.cflag = b.take<float>(N);
+    o.ngather = b.take<int>(N); o.nsym = b.take<int>(N);
+    for (int k = 0; k < 9; ++k) o.F[k] = b.take<float>(N);
+    for (int k = 0; k < 9; ++k) o.Cinv[k] = b.take<float>(N);
+    for (int k = 0; k < 9; ++k) o.G[k] = b.take<float>(N);
+    o.A3 = b.take<float4>(N); o.A4 = b.take<float4>(N); o.A5 = b.take<float4>(N);
+    o.bbox = b.take<float>(8);
+    o.dt_cur = b.take<float>(1);
+    o.dt_next = b.take<float>(1);
+    o.counters = b.take<unsigned long long>(SPH_C_COUNT);
+    o.keys = b.take<unsigned long long>(N); o.keys_alt = b.take<unsigned long long>(N);
+    o.perm = b.take<unsigned>(N); o.perm_alt = b.take<unsigned>(N);
+    o.cub_tmp_bytes = sph_cub_temp_bytes(n_max);
+    o.cub_tmp = b.take<char>(o.cub_tmp_bytes);
+    float *st = b.take<float>(19 * N);      // sph_step_host staging: 17 float arrays + mat + fixed
+    if (stage) *stage = st;
+    return (b.off + 255) & ~(size_t)255;
+}
+
+static bool params_ok(const sph_params *p)
+{
+    if (!p) return false;
+    if (p->n_materials < 1 || p->n_materials > SPH_MAX_MATERIALS) return false;
+    if (!(p->kappa > 0.f)) return false;
+    for (int k = 0; k < p->n_materials; ++k)
+        if (!(p->mat[k].rho0 > 0.f) || !(p->mat[k].cv > 0.f) || !(p->mat[k].c0 > 0.f)) return false;
+    return true;
+}
+
+extern "C" size_t sph_workspace_bytes(const sph_params *params, long long n_max)
+{
+    if (!params_ok(params) || n_max < 0 || n_max > 2000000000ll) return 0;
+    return carve(nullptr, nullptr, nullptr, n_max);
+}
+
+extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max, void *workspace,
+                        size_t workspace_bytes, void *cuda_stream)
+{
+    if (!out) return SPH_EINVAL;
+    *out = nullptr;
+    if (!params_ok(params) || n_max < 0 || n_max > 2000000000ll || !workspace) return SPH_EINVAL;
+    if (((uintptr_t)workspace & 255u) != 0) return SPH_EINVAL;
+    size_t need = carve(nullptr, nullptr, nullptr, n_max);
+    if (workspace_bytes < need) return SPH_ENOMEM;
+    sph_ctx *c = new (std::nothrow) sph_ctx();
+    if (!c) return SPH_ENOMEM;
+    memset(c, 0, sizeof(*c));
+    c->p.kappa = params->kappa; c->p.alpha = params->alpha; c->p.beta = params->beta;
+    c->p.eps_av = params->eps_av; c->p.eta_C = params->eta_C; c->p.eta_a = params->eta_a;
+    c->p.flags = params->flags; c->p.n_materials = params->n_materials;
+    memcpy(c->p.mat, params->mat, sizeof(params->mat));
+    c->stream = (cudaStream_t)cuda_stream;
+    c->ws_bytes = carve(&c->d, &c->stage, (char *)workspace, n_max);
+    c->d.n = 0; c->d.nchunk = 0;
+    for (int k = 0; k < 2 * SPH_T_COUNT; ++k) {
+        cudaError_t e = cudaEventCreate(&c->ev[k]);
+        if (e != cudaSuccess) {
+            for (int j = 0; j < k; ++j) cudaEventDestroy(c->ev[j]);
+            delete c;
+            return SPH_ECUDA;
+        }
+    }
+    cudaError_t e = cudaMemsetAsync(c->d.counters, 0, SPH_C_COUNT * sizeof(unsigned long long), c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->d.dt_cur, 0, sizeof(float), c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->d.dt_next, 0, sizeof(float), c->stream);
+    if (e != cudaSuccess) { sph_destroy(c); return SPH_ECUDA; }
+    *out = c;
+    return SPH_OK;
+}
+
+extern "C" void sph_destroy(sph_ctx *c)
+{
+    if (!c) return;
+    for (int k = 0; k < 2 * SPH_T_COUNT; ++k) cudaEventDestroy(c->ev[k]);
+    delete c;
+}
+
+// ------------------------------------------------------------------------------------------
+// timing helpers
+// ------------------------------------------------------------------------------------------
+struct PassTimer {
+    sph_ctx *c;
+    int slot;
+    PassTimer(sph_ctx *c_, int s) : c(c_), slot(s) { cudaEventRecord(c->ev[2 * slot], c->stream); }
+    ~PassTimer()
+    {
+        cudaEventRecord(c->ev[2 * slot + 1], c->stream);
+        c->ev_used[slot] = true;
+    }
+};
+
+static bool state_ok(const sph_state *s)
+{
+    return s && s->x && s->y && s->z && s->m && s->h && s->vx && s->vy && s->vz && s->u && s->Sxx && s->Syy &&
+           s->Sxy && s->Sxz && s->Syz;
+}
+
+// ------------------------------------------------------------------------------------------
+// passes
+// ------------------------------------------------------------------------------------------
+extern "C" int sph_build_neighbors(sph_ctx *c, const sph_state *state, long long n)
+{
+    if (!c) return SPH_EINVAL;
+    int rc;
+    PassTimer t(c, SPH_T_BUILD);
+    if (state) {
+        if (n < 0 || (n > 0 && !state_ok(state))) return SPH_EINVAL;
+        if (n > c->d.n_max) return SPH_ECAPACITY;
+        rc = sph_launch_ingest(c, state, n);
+        if (rc) return rc;
+        c->resident = true;
+        c->have_derivs = false;
+    } else {
+        if (!c->resident) return SPH_EORDER;
+        rc = sph_launch_resort(c);
+        if (rc) return rc;
+    }
+    c->have_density = c->have_predict = c->have_grad = c->have_force = false;
+    return SPH_OK;
+}
+
+extern "C" int sph_density(sph_ctx *c)
+{
+    if (!c) return SPH_EINVAL;
+    if (!c->resident) return SPH_EORDER;
+    PassTimer t(c, SPH_T_DENSITY);
+    int rc = sph_launch_density(c);
+    if (rc) return rc;
+    c->have_density = true;
+    c->have_predict = c->have_grad = c->have_force = false;
+    return SPH_OK;
+}
+
+extern "C" int sph_gradients(sph_ctx *c)
+{
+    if (!c) return SPH_EINVAL;
+    if (!c->have_predict) return SPH_EORDER;
+    PassTimer t(c, SPH_T_GRADIENT);
+    int rc = sph_launch_pair(c, true, false);
+    if (rc) return rc;
+    c->have_grad = true;
+    return SPH_OK;
+}
+
+extern "C" int sph_forces(sph_ctx *c)
+{
+    if (!c) return SPH_EINVAL;
+    if (!c->have_predict) return SPH_EORDER;
+    PassTimer t(c, SPH_T_FORCE);
+    int rc = sph_launch_pair(c, false, true);
+    if (rc) return rc;
+    c->have_force = true;
+    return SPH_OK;
+}
+
+static int do_close(sph_ctx *c, int phase, float dt, bool dt_from_device)
+{
+    const bool strength = (c->p.flags & SPH_STRENGTH) != 0;
+    if (!c->have_force || (strength && !c->have_grad)) return SPH_EORDER;
+    PassTimer t(c, SPH_T_CLOSE);
+    int rc = sph_launch_close(c, phase, dt, dt_from_device);
+    if (rc) return rc;
+    c->have_derivs = true;
+    return SPH_OK;
+}
+
+extern "C" int sph_strength_update(sph_ctx *c, int phase, float dt)
+{
+    if (!c) return SPH_EINVAL;
+    if (phase == SPH_PREDICT) {
+        if (!c->have_density) return SPH_EORDER;
+        PassTimer t(c, SPH_T_PREDICT);
+        int rc = sph_launch_predict(c);
+        if (rc) return rc;
+        c->have_predict = true;
+        c->have_grad = c->have_force = false;
+        return SPH_OK;
+    }
+    if (phase == SPH_CLOSE || phase == SPH_DERIVATIVES) {
+        if (phase == SPH_CLOSE && !(dt >= 0.f)) return SPH_EINVAL;
+        return do_close(c, phase, dt, false);
+    }
+    return SPH_EINVAL;
+}
+
+// density -> predict -> fused gradient + force
+static int derivative_passes(sph_ctx *c)
+{
+    int rc = sph_density(c);
+    if (rc) return rc;
+    rc = sph_strength_update(c, SPH_PREDICT, 0.f);
+    if (rc) return rc;
+    const bool strength = (c->p.flags & SPH_STRENGTH) != 0;
+    {
+        PassTimer t(c, SPH_T_FORCE);
+        rc = sph_launch_pair(c, strength, true);
+        if (rc) return rc;
+        c->have_force = true;
+        c->have_grad = strength;
+    }
+    return SPH_OK;
+}
+
+extern "C" int sph_step(sph_ctx *c, sph_state *state, long long n, float dt, float *dt_used)
+{
+    if (!c) return SPH_EINVAL;
+    int rc;
+    PassTimer ts(c, SPH_T_STEP);
+    if (!c->resident) {
+        if (!state) return SPH_EORDER;
+        rc = sph_build_neighbors(c, state, n);
+        if (rc) return rc;
+    } else if (state && n != c->d.n) {
+        return SPH_EINVAL;
+    }
+    if (!c->have_derivs) {          // first step: a_0, du_0/dt, dS_0/dt from the current state
+        rc = derivative_passes(c);
+        if (rc) return rc;
+        rc = do_close(c, SPH_DERIVATIVES, 0.f, false);
+        if (rc) return rc;
+    }
+    {
+        PassTimer t(c, SPH_T_KICKDRIFT);
+        rc = sph_launch_kick_drift(c, dt);
+        if (rc) return rc;
+    }
+    rc = sph_build_neighbors(c, nullptr, 0);
+    if (rc) return rc;
+    rc = derivative_passes(c);
+    if (rc) return rc;
+    rc = do_close(c, SPH_CLOSE, 0.f, true);
+    if (rc) return rc;
+    if (dt_used) SPH_CUDA(c, cudaMemcpyAsync(dt_used, c->d.dt_cur, sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    if (state) {
+        rc = sph_launch_download(c, state);
+        if (rc) return rc;
+    }
+    return SPH_OK;
+}
+
+// refresh the resident state from caller-order device arrays, keeping order and derivatives
+__global__ void __launch_bounds__(256) k_refresh(Dev d, sph_state st)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    unsigned o = ((const unsigned *)d.r.s[PP_ORIG])[i];
+    d.r.pm[i] = make_float4(st.x[o], st.y[o], st.z[o], st.m[o]);
+    d.r.vh[i].w = st.h[o];
+    d.vfull[0][i] = st.vx[o]; d.vfull[1][i] = st.vy[o]; d.vfull[2][i] = st.vz[o];
+    d.ufull[i] = st.u[o];
+    d.Sfull[0][i] = st.Sxx[o]; d.Sfull[1][i] = st.Syy[o]; d.Sfull[2][i] = st.Sxy[o];
+    d.Sfull[3][i] = st.Sxz[o]; d.Sfull[4][i] = st.Syz[o];
+    d.r.s[PP_G + 0][i] = st.gx ? st.gx[o] : 0.f;
+    d.r.s[PP_G + 1][i] = st.gy ? st.gy[o] : 0.f;
+    d.r.s[PP_G + 2][i] = st.gz ? st.gz[o] : 0.f;
+}
+
+extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, float *dt_used)
+{
+    if (!c || n < 0 || (n > 0 && !state_ok(hs))) return SPH_EINVAL;
+    if (n > c->d.n_max) return SPH_ECAPACITY;
+    if (c->resident && n != c->d.n) return SPH_EINVAL;
+    size_t N = (size_t)(c->d.n_max > 0 ? c->d.n_max : 1);
+    float *base = c->stage;
+    float *dev[17];
+    for (int k = 0; k < 17; ++k) dev[k] = base + (size_t)k * N;
+    int *dmat = (int *)(base + 17 * N);
+    unsigned char *dfix = (unsigned char *)(base + 18 * N);
+    const float *src[17] = {hs->x, hs->y, hs->z, hs->m, hs->h, hs->vx, hs->vy, hs->vz, hs->u,
+                            hs->Sxx, hs->Syy, hs->Sxy, hs->Sxz, hs->Syz, hs->gx, hs->gy, hs->gz};
+    sph_state ds;
+    memset(&ds, 0, sizeof(ds));
+    for (int k = 0; k < 17; ++k) {
+        if (n > 0 && src[k])
+            SPH_CUDA(c, cudaMemcpyAsync(dev[k], src[k], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    }
+    ds.x = dev[0]; ds.y = dev[1]; ds.z = dev[2]; ds.m = dev[3]; ds.h = dev[4];
+    ds.vx = dev[5]; ds.vy = dev[6]; ds.vz = dev[7]; ds.u = dev[8];
+    ds.Sxx = dev[9]; ds.Syy = dev[10]; ds.Sxy = dev[11]; ds.Sxz = dev[12]; ds.Syz = dev[13];
+    ds.gx = hs->gx ? dev[14] : nullptr; ds.gy = hs->gy ? dev[15] : nullptr; ds.gz = hs->gz ? dev[16] : nullptr;
+    if (n > 0 && hs->mat) {
+        SPH_CUDA(c, cudaMemcpyAsync(dmat, hs->mat, (size_t)n * sizeof(int), cudaMemcpyHostToDevice, c->stream));
+        ds.mat = dmat;
+    }
+    if (n > 0 && hs->fixed) {
+        SPH_CUDA(c, cudaMemcpyAsync(dfix, hs->fixed, (size_t)n, cudaMemcpyHostToDevice, c->stream));
+        ds.fixed = dfix;
+    }
+    int rc;
+    if (c->resident && n > 0) {
+        k_refresh<<<sph_div_up(n, 256), 256, 0, c->stream>>>(c->d, ds);
+        c->launches++;
+        SPH_CUDA(c, cudaGetLastError());
+    }
+    rc = sph_step(c, &ds, n, dt, nullptr);
+    if (rc) return rc;
+    float *dst[14] = {hs->x, hs->y, hs->z, nullptr, nullptr, hs->vx, hs->vy, hs->vz, hs->u,
+                      hs->Sxx, hs->Syy, hs->Sxy, hs->Sxz, hs->Syz};
+    for (int k = 0; k < 14; ++k) {
+        if (n > 0 && dst[k])
+            SPH_CUDA(c, cudaMemcpyAsync(dst[k], dev[k], (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    }
+    if (dt_used) SPH_CUDA(c, cudaMemcpyAsync(dt_used, c->d.dt_cur, sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    return SPH_OK;
+}
+
+extern "C" int sph_download_state(sph_ctx *c, sph_state *state)
+{
+    if (!c || !state_ok(state)) return SPH_EINVAL;
+    if (!c->resident) return SPH_EORDER;
+    return sph_launch_download(c, state);
+}
+
+// ------------------------------------------------------------------------------------------
+// outputs
+// ------------------------------------------------------------------------------------------
+extern "C" int sph_get_field(sph_ctx *c, int id, float *dst)
+{
+    if (!c || !dst) return SPH_EINVAL;
+    if (!c->resident) return SPH_EORDER;
+    Dev &d = c->d;
+    const float *src = nullptr;
+    int as_int = 0;
+    switch (id) {
+    case SPH_F_RHO: src = d.rho; break;
+    case SPH_F_OMEGA: src = d.omega; break;
+    case SPH_F_P: src = d.P; break;
+    case SPH_F_CS: src = d.cs; break;
+    case SPH_F_T: src = d.T; break;
+    case SPH_F_GAMMA: src = d.Gamma; break;
+    case SPH_F_Y: src = d.Y; break;
+    case SPH_F_MUMAX: src = d.mumax; break;
+    case SPH_F_DUDT: src = d.dudt; break;
+    case SPH_F_DT: src = d.dti; break;
+    case SPH_F_EACC: src = d.r.s[PP_EACC]; break;
+    case SPH_F_EPS2: src = d.eps2; break;
+    case SPH_F_U: src = d.ufull; break;
+    case SPH_F_CFLAG: src = d.cflag; break;
+    case SPH_F_NGATHER: src = (const float *)d.ngather; as_int = 1; break;
+    case SPH_F_NSYMMETRIC: src = (const float *)d.nsym; as_int = 1; break;
+    default: break;
+    }
+    if (!src) {
+        if (id >= SPH_F_A && id < SPH_F_A + 3) src = d.a[id - SPH_F_A];
+        else if (id >= SPH_F_V && id < SPH_F_V + 3) src = d.vfull[id - SPH_F_V];
+        else if (id >= SPH_F_X && id < SPH_F_X + 3) return sph_launch_get_position(c, id - SPH_F_X, dst);
+        else if (id >= SPH_F_SPRED && id < SPH_F_SPRED + 5) src = d.r.s[PP_SPRED + id - SPH_F_SPRED];
+        else if (id >= SPH_F_S && id < SPH_F_S + 5) src = d.Sfull[id - SPH_F_S];
+        else if (id >= SPH_F_DSDT && id < SPH_F_DSDT + 5) src = d.dS[id - SPH_F_DSDT];
+        else if (id >= SPH_F_F && id < SPH_F_F + 9) src = d.F[id - SPH_F_F];
+        else if (id >= SPH_F_CINV && id < SPH_F_CINV + 9) src = d.Cinv[id - SPH_F_CINV];
+        else if (id >= SPH_F_G && id < SPH_F_G + 9) src = d.G[id - SPH_F_G];
+    }
+    if (!src) return SPH_EINVAL;
+    return sph_launch_get_field(c, src, dst, as_int);
+}
+
+extern "C" int sph_get_neighbors(sph_ctx *c, int which, int *counts, const long long *offsets, int *list)
+{
+    if (!c || !counts || (which != SPH_GATHER && which != SPH_SYMMETRIC) || (list && !offsets)) return SPH_EINVAL;
+    if (!c->resident) return SPH_EORDER;
+    return sph_launch_neighbors(c, which, counts, offsets, list);
+}
+
+extern "C" int sph_get_timings(sph_ctx *c, float *ms, int n)
+{
+    if (!c || !ms || n < 0) return SPH_EINVAL;
+    SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < n && k < SPH_T_COUNT; ++k) {
+        ms[k] = 0.f;
+        if (c->ev_used[k]) cudaEventElapsedTime(&ms[k], c->ev[2 * k], c->ev[2 * k + 1]);
+    }
+    return SPH_OK;
+}
+
+extern "C" int sph_get_counters(sph_ctx *c, long long *out, int n)
+{
+    if (!c || !out || n < 0) return SPH_EINVAL;
+    unsigned long long h[SPH_C_COUNT];
+    SPH_CUDA(c, cudaMemcpyAsync(h, c->d.counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    for (int k = 0; k < n && k < SPH_C_COUNT; ++k) out[k] = (long long)h[k];
+    return SPH_OK;
+}
+
+extern "C" long long sph_launch_count(const sph_ctx *c) { return c ? c->launches : 0; }
+extern "C" int sph_last_cuda_error(const sph_ctx *c) { return c ? c->last_cuda : 0; }
+
+extern "C" const char *sph_strerror(int code)
+{
+    switch (code) {
+    case SPH_OK: return "ok";
+    case SPH_EINVAL: return "invalid argument";
+    case SPH_ENOMEM: return "workspace too small";
+    case SPH_ECUDA: return "CUDA error (see sph_last_cuda_error)";
+    case SPH_EORDER: return "pass called before its prerequisite";
+    case SPH_ECAPACITY: return "n exceeds n_max";
+    default: return "unknown error";
+    }
+}

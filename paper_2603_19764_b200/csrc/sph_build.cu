@@ -1,0 +1,281 @@
+// sph_build.cu -- S1: Morton keys, radix sort, gather into the resident sorted arrays, chunk
+// bounding boxes and the implicit 32-ary chunk tree (stands in for the paper's tree build and
+// domain decomposition; BASELINE.json north_star "Morton-key sort and reorder").
+#include <cub/device/device_radix_sort.cuh>
+
+#include "sph_internal.cuh"
+
+// ------------------------------------------------------------------------------------------
+// bounding box of all particles (ordered-int atomics; 6 words: lo xyz, hi xyz)
+// ------------------------------------------------------------------------------------------
+__global__ void k_bbox_init(int *bbox)
+{
+    if (threadIdx.x < 3) bbox[threadIdx.x] = 0x7fffffff;          // +max ordered
+    else if (threadIdx.x < 6) bbox[threadIdx.x] = (int)0x80000000; // -max ordered
+}
+
+template <bool FROM_STATE>
+__global__ void __launch_bounds__(256) k_bbox(const float *__restrict__ x, const float *__restrict__ y,
+                                              const float *__restrict__ z, const float4 *__restrict__ pm,
+                                              long long n, int *bbox)
+{
+    float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        float p[3];
+        if (FROM_STATE) { p[0] = x[i]; p[1] = y[i]; p[2] = z[i]; }
+        else { float4 q = pm[i]; p[0] = q.x; p[1] = q.y; p[2] = q.z; }
+#pragma unroll
+        for (int a = 0; a < 3; ++a) { lo[a] = fminf(lo[a], p[a]); hi[a] = fmaxf(hi[a], p[a]); }
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+            hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+        }
+    }
+    if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            atomicMin(&bbox[a], sph_f2ord(lo[a]));
+            atomicMax(&bbox[3 + a], sph_f2ord(hi[a]));
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// 63-bit Morton key (3 x 21 bits) on a cubic grid spanning the bounding box
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long expand21(unsigned long long v)
+{
+    v &= 0x1fffffull;
+    v = (v | v << 32) & 0x1f00000000ffffull;
+    v = (v | v << 16) & 0x1f0000ff0000ffull;
+    v = (v | v << 8) & 0x100f00f00f00f00full;
+    v = (v | v << 4) & 0x10c30c30c30c30c3ull;
+    v = (v | v << 2) & 0x1249249249249249ull;
+    return v;
+}
+
+template <bool FROM_STATE>
+__global__ void __launch_bounds__(256) k_keys(const float *__restrict__ x, const float *__restrict__ y,
+                                              const float *__restrict__ z, const float4 *__restrict__ pm,
+                                              long long n, const int *__restrict__ bbox,
+                                              unsigned long long *__restrict__ keys, unsigned *__restrict__ perm)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float lo[3], ext = 0.f;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        lo[a] = sph_ord2f(bbox[a]);
+        ext = fmaxf(ext, sph_ord2f(bbox[3 + a]) - lo[a]);
+    }
+    float scale = ext > 0.f ? 2097151.0f / ext : 0.f;
+    float p[3];
+    if (FROM_STATE) { p[0] = x[i]; p[1] = y[i]; p[2] = z[i]; }
+    else { float4 q = pm[i]; p[0] = q.x; p[1] = q.y; p[2] = q.z; }
+    unsigned long long k = 0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        float f = (p[a] - lo[a]) * scale;
+        f = fminf(fmaxf(f, 0.f), 2097151.0f);
+        k |= expand21((unsigned long long)f) << a;
+    }
+    keys[i] = k;
+    perm[i] = (unsigned)i;
+}
+
+// ------------------------------------------------------------------------------------------
+// ingest: caller arrays (caller order) -> resident sorted arrays
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_ingest(sph_state st, Dev d, const unsigned *__restrict__ perm)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    unsigned p = perm[i];
+    float vx = st.vx[p], vy = st.vy[p], vz = st.vz[p], u = st.u[p];
+    float S[5] = {st.Sxx[p], st.Syy[p], st.Sxy[p], st.Sxz[p], st.Syz[p]};
+    d.r.pm[i] = make_float4(st.x[p], st.y[p], st.z[p], st.m[p]);
+    d.r.vh[i] = make_float4(vx, vy, vz, st.h[p]);
+    d.r.s[PP_UPRED][i] = u;
+    d.r.s[PP_UHALF][i] = u;
+    d.ufull[i] = u;
+    d.r.s[PP_VHALF + 0][i] = vx; d.r.s[PP_VHALF + 1][i] = vy; d.r.s[PP_VHALF + 2][i] = vz;
+    d.vfull[0][i] = vx; d.vfull[1][i] = vy; d.vfull[2][i] = vz;
+#pragma unroll
+    for (int c = 0; c < 5; ++c) {
+        d.r.s[PP_SPRED + c][i] = S[c];
+        d.r.s[PP_SHALF + c][i] = S[c];
+        d.Sfull[c][i] = S[c];
+        d.dS[c][i] = 0.f;
+    }
+    d.r.s[PP_EACC][i] = 0.f;
+    d.r.s[PP_G + 0][i] = st.gx ? st.gx[p] : 0.f;
+    d.r.s[PP_G + 1][i] = st.gy ? st.gy[p] : 0.f;
+    d.r.s[PP_G + 2][i] = st.gz ? st.gz[p] : 0.f;
+    ((unsigned *)d.r.s[PP_ORIG])[i] = p;
+    unsigned mf = (st.mat ? (unsigned)st.mat[p] & 0xffu : 0u) | (st.fixed ? ((unsigned)(st.fixed[p] != 0) << 8) : 0u);
+    ((unsigned *)d.r.s[PP_MATFIX])[i] = mf;
+    d.a[0][i] = 0.f; d.a[1][i] = 0.f; d.a[2][i] = 0.f;
+    d.dudt[i] = 0.f;
+}
+
+// re-sort: alt[i] = cur[perm[i]] for every array that moves with the particle
+__global__ void __launch_bounds__(256) k_permute(Dev d, const unsigned *__restrict__ perm)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    unsigned p = perm[i];
+    d.alt.pm[i] = d.r.pm[p];
+    d.alt.vh[i] = d.r.vh[p];
+#pragma unroll
+    for (int f = 0; f < SPH_NPP; ++f) d.alt.s[f][i] = d.r.s[f][p];
+}
+
+// ------------------------------------------------------------------------------------------
+// chunk boxes (level 0) and inner levels of the implicit tree
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_chunk_boxes(Dev d, float kappa)
+{
+    int chunk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (chunk >= d.nchunk) return;
+    int lane = threadIdx.x & 31;
+    long long i = (long long)chunk * SPH_CHUNK + lane;
+    float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, H = 0.f;
+    if (i < d.n) {
+        float4 q = d.r.pm[i];
+        lo[0] = hi[0] = q.x; lo[1] = hi[1] = q.y; lo[2] = hi[2] = q.z;
+        H = sph_H(kappa, d.r.vh[i].w);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+            hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+        }
+        H = fmaxf(H, __shfl_xor_sync(0xffffffffu, H, o));
+    }
+    if (lane == 0) {
+        d.tree.lo[0][chunk] = make_float4(lo[0], lo[1], lo[2], H);
+        d.tree.hi[0][chunk] = make_float4(hi[0], hi[1], hi[2], 0.f);
+    }
+}
+
+__global__ void __launch_bounds__(256) k_tree_level(Tree t, int L)
+{
+    int node = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (node >= t.count[L]) return;
+    int lane = threadIdx.x & 31;
+    int child = node * SPH_ARITY + lane;
+    float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, H = 0.f;
+    if (child < t.count[L - 1]) {
+        float4 a = t.lo[L - 1][child], b = t.hi[L - 1][child];
+        lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; H = a.w;
+        hi[0] = b.x; hi[1] = b.y; hi[2] = b.z;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
+            hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+        }
+        H = fmaxf(H, __shfl_xor_sync(0xffffffffu, H, o));
+    }
+    if (lane == 0) {
+        t.lo[L][node] = make_float4(lo[0], lo[1], lo[2], H);
+        t.hi[L][node] = make_float4(hi[0], hi[1], hi[2], 0.f);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------
+size_t sph_cub_temp_bytes(long long n_max)
+{
+    size_t bytes = 0;
+    cudaError_t e = cub::DeviceRadixSort::SortPairs(nullptr, bytes, (const unsigned long long *)nullptr,
+                                                    (unsigned long long *)nullptr, (const unsigned *)nullptr,
+                                                    (unsigned *)nullptr, (int)(n_max > 0 ? n_max : 1), 0, 63);
+    // no device to ask (sizing on a CPU-only box): a bound well above what onesweep needs
+    size_t bound = (size_t)(n_max > 0 ? n_max : 1) * 16 + ((size_t)1 << 20);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return bound; }
+    return bytes > bound ? bytes : bound;
+}
+
+static int sort_keys(sph_ctx *c)
+{
+    Dev &d = c->d;
+    size_t bytes = d.cub_tmp_bytes;
+    SPH_CUDA(c, cub::DeviceRadixSort::SortPairs(d.cub_tmp, bytes, d.keys, d.keys_alt, d.perm, d.perm_alt,
+                                                (int)d.n, 0, 63, c->stream));
+    c->launches += 8;   // onesweep: histogram + scan + 8-bit digit passes over 63 bits
+    return SPH_OK;
+}
+
+int sph_launch_tree(sph_ctx *c)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    k_chunk_boxes<<<sph_div_up(d.nchunk, 8), 256, 0, c->stream>>>(d, c->p.kappa);
+    c->launches++;
+    for (int L = 1; L < d.tree.nlev; ++L) {
+        k_tree_level<<<sph_div_up(d.tree.count[L], 8), 256, 0, c->stream>>>(d.tree, L);
+        c->launches++;
+    }
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+static void set_counts(sph_ctx *c, long long n)
+{
+    Dev &d = c->d;
+    d.n = n;
+    d.nchunk = sph_div_up(n, SPH_CHUNK);
+    int cnt = d.nchunk, L = 0;
+    d.tree.count[0] = cnt;
+    while (cnt > SPH_ARITY && L + 1 < SPH_MAX_LEVELS) {
+        cnt = sph_div_up(cnt, SPH_ARITY);
+        d.tree.count[++L] = cnt;
+    }
+    d.tree.nlev = L + 1;
+}
+
+int sph_launch_ingest(sph_ctx *c, const sph_state *st, long long n)
+{
+    set_counts(c, n);
+    Dev &d = c->d;
+    if (n == 0) return SPH_OK;
+    int nb = sph_div_up(n, 256);
+    k_bbox_init<<<1, 32, 0, c->stream>>>((int *)d.bbox);
+    k_bbox<true><<<nb < 1184 ? nb : 1184, 256, 0, c->stream>>>(st->x, st->y, st->z, nullptr, n, (int *)d.bbox);
+    k_keys<true><<<nb, 256, 0, c->stream>>>(st->x, st->y, st->z, nullptr, n, (const int *)d.bbox, d.keys, d.perm);
+    c->launches += 3;
+    int rc = sort_keys(c);
+    if (rc) return rc;
+    k_ingest<<<nb, 256, 0, c->stream>>>(*st, d, d.perm_alt);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return sph_launch_tree(c);
+}
+
+int sph_launch_resort(sph_ctx *c)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    int nb = sph_div_up(d.n, 256);
+    k_bbox_init<<<1, 32, 0, c->stream>>>((int *)d.bbox);
+    k_bbox<false><<<nb < 1184 ? nb : 1184, 256, 0, c->stream>>>(nullptr, nullptr, nullptr, d.r.pm, d.n, (int *)d.bbox);
+    k_keys<false><<<nb, 256, 0, c->stream>>>(nullptr, nullptr, nullptr, d.r.pm, d.n, (const int *)d.bbox, d.keys, d.perm);
+    c->launches += 3;
+    int rc = sort_keys(c);
+    if (rc) return rc;
+    k_permute<<<nb, 256, 0, c->stream>>>(d, d.perm_alt);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    Resident t = d.r; d.r = d.alt; d.alt = t;
+    return sph_launch_tree(c);
+}

@@ -1,0 +1,136 @@
+// sph_internal.cuh -- internal declarations of libsph.so (CUDA, sm_100a only).
+// Shares nothing with oracle/.  Equation numbers refer to /root/reference/PAPER.md.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/sph.h"
+
+#define SPH_CHUNK 32          // particles per target chunk = one warp of targets
+#define SPH_ARITY 32          // children per node of the implicit chunk tree (one lane each)
+#define SPH_MAX_LEVELS 7      // 32^6 chunks * 32 particles >> any n that fits in HBM
+#define SPH_NPP 21            // scalar (4-byte) resident arrays that are permuted at re-sort
+
+// indices into Resident::s (scalar ping-pong arrays)
+enum {
+    PP_UPRED = 0,
+    PP_SPRED = 1,   // +0..4
+    PP_VHALF = 6,   // +0..2
+    PP_UHALF = 9,
+    PP_SHALF = 10,  // +0..4
+    PP_EACC = 15,
+    PP_G = 16,      // +0..2
+    PP_ORIG = 19,   // uint32 original index
+    PP_MATFIX = 20  // uint32: material | fixed << 8
+};
+
+struct DevParams {
+    float kappa, alpha, beta, eps_av, eta_C, eta_a;
+    unsigned flags;
+    int n_materials;
+    sph_material mat[SPH_MAX_MATERIALS];
+};
+
+// Sorted ("resident") particle data that moves with the particle at re-sort.
+struct Resident {
+    float4 *pm;              // x, y, z, m
+    float4 *vh;              // predicted v (Eq. 40 analogue for v), h
+    float *s[SPH_NPP];       // see PP_*
+};
+
+// Implicit 32-ary tree over the Morton-sorted chunk array: node k of level L covers chunks
+// [k 32^L, (k+1) 32^L).  lo.w = max H of the node, hi.w unused.
+struct Tree {
+    int nlev;                        // levels stored; level nlev-1 has <= 32 nodes
+    int count[SPH_MAX_LEVELS];
+    float4 *lo[SPH_MAX_LEVELS];
+    float4 *hi[SPH_MAX_LEVELS];
+};
+
+// Everything the kernels need, passed by value.
+struct Dev {
+    long long n;       // particles resident
+    int nchunk;        // ceil(n / 32)
+    long long n_max;
+    Resident r;        // current
+    Resident alt;      // other half of the ping-pong
+    Tree tree;
+    // single-buffered, current sorted order
+    float *vfull[3], *ufull, *Sfull[5];     // state at the full step (after CLOSE)
+    float *a[3], *dudt, *dS[5];             // derivatives at the full step
+    float *rho, *omega, *P, *cs, *T, *Gamma, *Y, *mumax, *dti, *eps2, *cflag;
+    int *ngather, *nsym;
+    float *F[9], *Cinv[9], *G[9];
+    float4 *A3, *A4, *A5;                   // packed pair-pass operands (see k_predict)
+    // scalars on the device
+    float *bbox;                            // 6 floats as ordered ints: lo xyz, hi xyz
+    float *dt_cur, *dt_next;                // step in use / CFL step from the last CLOSE
+    unsigned long long *counters;           // SPH_C_COUNT
+    // sort scratch
+    unsigned long long *keys, *keys_alt;
+    unsigned *perm, *perm_alt;
+    void *cub_tmp;
+    size_t cub_tmp_bytes;
+};
+
+struct sph_ctx {
+    DevParams p;
+    Dev d;
+    cudaStream_t stream;
+    int last_cuda;
+    long long launches;
+    bool resident, have_density, have_predict, have_grad, have_force, have_derivs;
+    cudaEvent_t ev[2 * SPH_T_COUNT];
+    bool ev_used[SPH_T_COUNT];
+    // host staging for sph_step_host
+    float *stage;            // device: 17 floats + 2 words per particle
+    size_t ws_bytes;
+};
+
+#define SPH_CUDA(ctx, call)                                   \
+    do {                                                      \
+        cudaError_t e__ = (call);                             \
+        if (e__ != cudaSuccess) {                             \
+            (ctx)->last_cuda = (int)e__;                      \
+            return SPH_ECUDA;                                 \
+        }                                                     \
+    } while (0)
+
+static inline int sph_div_up(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+// ---- launchers implemented in the .cu files ---------------------------------------------
+size_t sph_cub_temp_bytes(long long n_max);
+int sph_launch_ingest(sph_ctx *c, const sph_state *st, long long n);
+int sph_launch_resort(sph_ctx *c);
+int sph_launch_tree(sph_ctx *c);
+int sph_launch_density(sph_ctx *c);
+int sph_launch_pair(sph_ctx *c, bool grad, bool force);
+int sph_launch_predict(sph_ctx *c);
+int sph_launch_close(sph_ctx *c, int phase, float dt, bool dt_from_device);
+int sph_launch_kick_drift(sph_ctx *c, float dt);
+int sph_launch_get_field(sph_ctx *c, const float *src, float *dst, int as_int);
+int sph_launch_get_position(sph_ctx *c, int comp, float *dst);
+int sph_launch_neighbors(sph_ctx *c, int which, int *counts, const long long *offsets, int *list);
+int sph_launch_download(sph_ctx *c, sph_state *st);
+
+// ---- small device helpers ----------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ float sph_r2(float dx, float dy, float dz)
+{
+    // reading Q4: every multiply and add rounded separately (no FMA contraction)
+    return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+}
+__device__ __forceinline__ float sph_H(float kappa, float h) { return __fmul_rn(kappa, h); }
+
+// order-preserving float <-> int map for atomicMin/atomicMax on floats
+__device__ __forceinline__ int sph_f2ord(float f)
+{
+    int i = __float_as_int(f);
+    return i >= 0 ? i : i ^ 0x7fffffff;
+}
+__device__ __forceinline__ float sph_ord2f(int i)
+{
+    return __int_as_float(i >= 0 ? i : i ^ 0x7fffffff);
+}
+#endif

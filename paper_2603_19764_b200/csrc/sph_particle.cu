@@ -1,0 +1,339 @@
+// sph_particle.cu -- the per-particle (HBM-bound) kernels: S3 predict / EOS / yield, S6 close,
+// S7 kick-drift-predict, S8 time-step reduction, and the caller-order scatter helpers.
+#include "sph_internal.cuh"
+
+#define WC2_SIGMA 3.3422538049298023f     // 21 / (2 pi), Wendland C2 in 3-D (reading Q3)
+#define SPH_CTOL 1.0e-4f                  // reading Q9: C = 1 unless |det C^-1| > CTOL ||C^-1||_F^3
+
+// ------------------------------------------------------------------------------------------
+// material laws
+// ------------------------------------------------------------------------------------------
+// Y_i = Y0 + mu_i P/(1 + mu_i P/(Ym - Y0)) with P < 0 clipped (Eq. 34);
+// Y = min(Y_i, mu_d P) for finite mu_d (Eq. 35-36); Y *= max(0, tanh(xi (Tm/T - 1))) (Eq. 37).
+__device__ __forceinline__ float yield_strength(const sph_material &m, float P, float T)
+{
+    float Pp = fmaxf(P, 0.f);
+    float span = m.Ym - m.Y0;
+    float Y = m.Y0;
+    if (span > 0.f) Y = m.Y0 + m.mu_i * Pp / (1.f + m.mu_i * Pp / span);
+    if (isfinite(m.mu_d)) Y = fminf(Y, m.mu_d * Pp);
+    float soft = 1.f;
+    if (T > 0.f) soft = fmaxf(0.f, tanhf(m.xi * (m.Tmelt / T - 1.f)));
+    return Y * soft;
+}
+
+// f = min(Y / sqrt(J2), 1) (Eq. 31-33); J2 from the five stored components
+__device__ __forceinline__ float plastic_factor(const float S[5], float Y)
+{
+    float szz = -S[0] - S[1];
+    float J2 = 0.5f * (S[0] * S[0] + S[1] * S[1] + szz * szz) + S[2] * S[2] + S[3] * S[3] + S[4] * S[4];
+    float sj = sqrtf(J2);
+    return sj > Y ? Y / sj : 1.f;
+}
+
+// ------------------------------------------------------------------------------------------
+// S3 PREDICT: EOS (reading Q13), Gamma (Eq. 30), Y (Eq. 34-37), S_pred <- f S_pred (Eq. 31,
+// PAPER.md:240), and the packed operands of the pair pass:
+//   A3 = {rho, c, K, 1/H}, A4 = {Sg_xx, Sg_yy, Sg_zz, Sg_xy}, A5 = {Sg_xz, Sg_yz, m w K, H^2}
+//   K = 20 SIGMA / H^5, w = 1/(Omega rho), Sg = m K (-P delta + S_pred)/(Omega rho^2)
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_predict(Dev d, DevParams p)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    unsigned mf = ((const unsigned *)d.r.s[PP_MATFIX])[i];
+    const sph_material &m = p.mat[mf & 0xffu];
+    float rho = d.rho[i], om = d.omega[i], u = d.r.s[PP_UPRED][i];
+    float P = m.c0 * m.c0 * (rho - m.rho0);
+    if (p.flags & SPH_PCLIP_GLOBAL) P = fmaxf(P, 0.f);
+    float cs = m.c0;
+    float T = u / m.cv;
+    float Gam = m.Gamma > 0.f ? m.Gamma : 3.f * (1.f - 2.f * m.nu) / (2.f * (1.f + m.nu)) * rho * cs * cs;
+    float Y = yield_strength(m, P, T);
+    float S[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
+    if (p.flags & SPH_STRENGTH) {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) S[c] = d.r.s[PP_SPRED + c][i];
+        float f = plastic_factor(S, Y);
+#pragma unroll
+        for (int c = 0; c < 5; ++c) { S[c] *= f; d.r.s[PP_SPRED + c][i] = S[c]; }
+    }
+    d.P[i] = P; d.cs[i] = cs; d.T[i] = T; d.Gamma[i] = Gam; d.Y[i] = Y;
+
+    float4 pm = d.r.pm[i];
+    float h = d.r.vh[i].w;
+    float H = sph_H(p.kappa, h);
+    float invH = 1.f / H;
+    float invH2 = invH * invH;
+    float K = 20.f * WC2_SIGMA * invH2 * invH2 * invH;
+    float w = 1.f / (om * rho);
+    float g = pm.w * K * w / rho;                     // m K / (Omega rho^2)
+    d.A3[i] = make_float4(rho, cs, K, invH);
+    d.A4[i] = make_float4(g * (S[0] - P), g * (S[1] - P), g * (-S[0] - S[1] - P), g * S[2]);
+    d.A5[i] = make_float4(g * S[3], g * S[4], pm.w * w * K, __fmul_rn(H, H));
+}
+
+// ------------------------------------------------------------------------------------------
+// S6 CLOSE: C = (C^-1)^-1, G = F.C (Eq. 22), eps_dot, R (Eq. 23-24), dS/dt (Eq. 25-29 as
+// reconstructed from Eq. 13, reading Q2), closing kick (Eq. 41) + rescale,
+// strain-rate invariant (Eq. 43), per-particle time-step limit (Eq. 38-39).
+// phase == SPH_DERIVATIVES leaves v, u, S, e_acc untouched (bootstrap of the first step).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_close(Dev d, DevParams p, int phase, float dt_arg, int dt_from_device)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    const float dt = dt_from_device ? *d.dt_cur : dt_arg;
+    const bool strength = (p.flags & SPH_STRENGTH) != 0;
+    unsigned mf = ((const unsigned *)d.r.s[PP_MATFIX])[i];
+    const bool fixed = (mf >> 8) & 1u;
+    float dS[5] = {0.f, 0.f, 0.f, 0.f, 0.f}, eps2 = 0.f, cflag = 0.f;
+    if (strength) {
+        float F[9], Ci[9], C[9], G[9];
+#pragma unroll
+        for (int k = 0; k < 9; ++k) { F[k] = d.F[k][i]; Ci[k] = d.Cinv[k][i]; }
+        // cofactors / determinant of C^-1
+        float c00 = Ci[4] * Ci[8] - Ci[5] * Ci[7], c01 = Ci[5] * Ci[6] - Ci[3] * Ci[8], c02 = Ci[3] * Ci[7] - Ci[4] * Ci[6];
+        float det = Ci[0] * c00 + Ci[1] * c01 + Ci[2] * c02;
+        float fro2 = 0.f;
+#pragma unroll
+        for (int k = 0; k < 9; ++k) fro2 = fmaf(Ci[k], Ci[k], fro2);
+        float fro = sqrtf(fro2);
+        bool ok = (p.flags & SPH_CORRECTION_TENSOR) && (fabsf(det) > SPH_CTOL * fro * fro * fro);
+        if (ok) {
+            float id = 1.f / det;
+            C[0] = c00 * id;
+            C[1] = (Ci[2] * Ci[7] - Ci[1] * Ci[8]) * id;
+            C[2] = (Ci[1] * Ci[5] - Ci[2] * Ci[4]) * id;
+            C[3] = c01 * id;
+            C[4] = (Ci[0] * Ci[8] - Ci[2] * Ci[6]) * id;
+            C[5] = (Ci[2] * Ci[3] - Ci[0] * Ci[5]) * id;
+            C[6] = c02 * id;
+            C[7] = (Ci[1] * Ci[6] - Ci[0] * Ci[7]) * id;
+            C[8] = (Ci[0] * Ci[4] - Ci[1] * Ci[3]) * id;
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int b = 0; b < 3; ++b)
+                    G[3 * a + b] = F[3 * a] * C[b] + F[3 * a + 1] * C[3 + b] + F[3 * a + 2] * C[6 + b];
+        } else {
+            cflag = 1.f;
+            atomicAdd(&d.counters[SPH_C_CFALLBACK], 1ull);
+#pragma unroll
+            for (int k = 0; k < 9; ++k) G[k] = F[k];
+        }
+#pragma unroll
+        for (int k = 0; k < 9; ++k) d.G[k][i] = G[k];
+        const float Gxx = G[0], Gxy = G[1], Gxz = G[2], Gyx = G[3], Gyy = G[4], Gyz = G[5], Gzx = G[6], Gzy = G[7], Gzz = G[8];
+        const float Sxx = d.r.s[PP_SPRED + 0][i], Syy = d.r.s[PP_SPRED + 1][i], Sxy = d.r.s[PP_SPRED + 2][i],
+                    Sxz = d.r.s[PP_SPRED + 3][i], Syz = d.r.s[PP_SPRED + 4][i];
+        const float Gam = d.Gamma[i];
+        const float s = (p.flags & SPH_JAUMANN_COROTATIONAL) ? -1.f : 1.f;
+        const float rxy = Gxy - Gyx, rxz = Gxz - Gzx, ryz = Gyz - Gzy;       // 2 R^{xy}, 2 R^{xz}, 2 R^{yz}
+        dS[0] = s * (-Sxy * rxy - Sxz * rxz) - (2.f / 3.f) * Gam * (Gyy + Gzz - 2.f * Gxx);
+        dS[1] = s * (Sxy * rxy - Syz * ryz) - (2.f / 3.f) * Gam * (Gxx + Gzz - 2.f * Gyy);
+        dS[2] = Gam * (Gxy + Gyx) + s * 0.5f * (Sxx * rxy - Syy * rxy - Syz * rxz - Sxz * ryz);
+        dS[3] = Gam * (Gxz + Gzx) + s * 0.5f * ((Sxx + Syy) * rxz + Sxx * rxz + Sxy * ryz - Syz * rxy);
+        dS[4] = Gam * (Gyz + Gzy) + s * 0.5f * ((Sxx + Syy) * ryz + Syy * ryz + Sxz * rxy + Sxy * rxz);
+        // 1/2 eps_dot : eps_dot with eps_dot = (G + G^T)/2
+        float exy = 0.5f * (Gxy + Gyx), exz = 0.5f * (Gxz + Gzx), eyz = 0.5f * (Gyz + Gzy);
+        eps2 = 0.5f * (Gxx * Gxx + Gyy * Gyy + Gzz * Gzz) + exy * exy + exz * exz + eyz * eyz;
+        d.cflag[i] = cflag;
+    }
+#pragma unroll
+    for (int c = 0; c < 5; ++c) d.dS[c][i] = dS[c];
+    d.eps2[i] = eps2;
+
+    // time-step limit, Eq. 39 (and Eq. 38 with epsilon = h when eta_a > 0)
+    float h = d.r.vh[i].w;
+    float ax = d.a[0][i], ay = d.a[1][i], az = d.a[2][i];
+    float dti = p.eta_C * h / ((1.f + 0.6f * p.alpha) * d.cs[i] + 0.6f * p.beta * d.mumax[i]);
+    if (p.eta_a > 0.f) {
+        float an = sqrtf(ax * ax + ay * ay + az * az);
+        if (an > 0.f) dti = fminf(dti, p.eta_a * sqrtf(h / an));
+    }
+    d.dti[i] = dti;
+
+    if (phase == SPH_CLOSE) {
+        float hdt = 0.5f * dt;
+        float vx = d.r.s[PP_VHALF + 0][i], vy = d.r.s[PP_VHALF + 1][i], vz = d.r.s[PP_VHALF + 2][i];
+        if (!fixed) { vx = fmaf(hdt, ax, vx); vy = fmaf(hdt, ay, vy); vz = fmaf(hdt, az, vz); }
+        d.vfull[0][i] = vx; d.vfull[1][i] = vy; d.vfull[2][i] = vz;
+        d.ufull[i] = fmaf(hdt, d.dudt[i], d.r.s[PP_UHALF][i]);
+        float S[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
+        if (strength) {
+#pragma unroll
+            for (int c = 0; c < 5; ++c) S[c] = fmaf(hdt, dS[c], d.r.s[PP_SHALF + c][i]);
+            float f = plastic_factor(S, d.Y[i]);
+#pragma unroll
+            for (int c = 0; c < 5; ++c) S[c] *= f;
+        }
+#pragma unroll
+        for (int c = 0; c < 5; ++c) d.Sfull[c][i] = S[c];
+        d.r.s[PP_EACC][i] = fmaf(dt, eps2, d.r.s[PP_EACC][i]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// S8: dt_next = min_i dt_i  (positive floats order like unsigned ints)
+// ------------------------------------------------------------------------------------------
+__global__ void k_dt_reset(float *dt_next) { *(unsigned *)dt_next = 0x7f800000u; }
+
+__global__ void __launch_bounds__(256) k_dt_min(const float *__restrict__ dti, long long n, float *dt_next)
+{
+    float m = __int_as_float(0x7f800000);
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        m = fminf(m, dti[i]);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fminf(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0 && m > 0.f) atomicMin((unsigned *)dt_next, __float_as_uint(m));
+}
+
+__global__ void k_dt_select(float dt_arg, float *dt_cur, const float *dt_next, float *dt_used)
+{
+    float dt = dt_arg > 0.f ? dt_arg : *dt_next;
+    *dt_cur = dt;
+    if (dt_used) *dt_used = dt;
+}
+
+// ------------------------------------------------------------------------------------------
+// S7 opening kick (Eq. 42), drift, prediction (Eq. 40); fixed particles keep x and v
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_kick_drift(Dev d, DevParams p)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    const float dt = *d.dt_cur, hdt = 0.5f * dt;
+    unsigned mf = ((const unsigned *)d.r.s[PP_MATFIX])[i];
+    const bool fixed = (mf >> 8) & 1u;
+    float4 pm = d.r.pm[i];
+    float h = d.r.vh[i].w;
+    float v[3] = {d.vfull[0][i], d.vfull[1][i], d.vfull[2][i]};
+    float a[3] = {d.a[0][i], d.a[1][i], d.a[2][i]};
+    float vh[3], vp[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        vh[k] = fixed ? v[k] : fmaf(hdt, a[k], v[k]);
+        vp[k] = fixed ? v[k] : fmaf(hdt, a[k], vh[k]);
+        d.r.s[PP_VHALF + k][i] = vh[k];
+    }
+    if (!fixed) { pm.x = fmaf(dt, vh[0], pm.x); pm.y = fmaf(dt, vh[1], pm.y); pm.z = fmaf(dt, vh[2], pm.z); }
+    d.r.pm[i] = pm;
+    d.r.vh[i] = make_float4(vp[0], vp[1], vp[2], h);
+    float du = d.dudt[i];
+    float uh = fmaf(hdt, du, d.ufull[i]);
+    d.r.s[PP_UHALF][i] = uh;
+    d.r.s[PP_UPRED][i] = fmaf(hdt, du, uh);
+#pragma unroll
+    for (int c = 0; c < 5; ++c) {
+        float ds = d.dS[c][i];
+        float sh = fmaf(hdt, ds, d.Sfull[c][i]);
+        d.r.s[PP_SHALF + c][i] = sh;
+        d.r.s[PP_SPRED + c][i] = fmaf(hdt, ds, sh);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// caller-order scatter helpers
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_scatter(const float *__restrict__ src, const unsigned *__restrict__ orig,
+                                                 long long n, float *__restrict__ dst, int as_int)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    dst[orig[i]] = as_int ? (float)((const int *)src)[i] : src[i];
+}
+
+__global__ void __launch_bounds__(256) k_scatter_pos(const float4 *__restrict__ pm, const unsigned *__restrict__ orig,
+                                                     long long n, float *__restrict__ dst, int comp)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float4 q = pm[i];
+    dst[orig[i]] = comp == 0 ? q.x : (comp == 1 ? q.y : q.z);
+}
+
+__global__ void __launch_bounds__(256) k_download(Dev d, sph_state st)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    unsigned o = ((const unsigned *)d.r.s[PP_ORIG])[i];
+    float4 pm = d.r.pm[i];
+    st.x[o] = pm.x; st.y[o] = pm.y; st.z[o] = pm.z;
+    st.vx[o] = d.vfull[0][i]; st.vy[o] = d.vfull[1][i]; st.vz[o] = d.vfull[2][i];
+    st.u[o] = d.ufull[i];
+    st.Sxx[o] = d.Sfull[0][i]; st.Syy[o] = d.Sfull[1][i]; st.Sxy[o] = d.Sfull[2][i];
+    st.Sxz[o] = d.Sfull[3][i]; st.Syz[o] = d.Sfull[4][i];
+}
+
+// ------------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------------
+int sph_launch_predict(sph_ctx *c)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    k_predict<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, c->p);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_close(sph_ctx *c, int phase, float dt, bool dt_from_device)
+{
+    Dev &d = c->d;
+    SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_CFALLBACK], 0, sizeof(unsigned long long), c->stream));
+    k_dt_reset<<<1, 1, 0, c->stream>>>(d.dt_next);
+    c->launches++;
+    if (d.n > 0) {
+        int nb = sph_div_up(d.n, 256);
+        k_close<<<nb, 256, 0, c->stream>>>(d, c->p, phase, dt, dt_from_device ? 1 : 0);
+        k_dt_min<<<nb < 592 ? nb : 592, 256, 0, c->stream>>>(d.dti, d.n, d.dt_next);
+        c->launches += 2;
+    }
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_kick_drift(sph_ctx *c, float dt)
+{
+    Dev &d = c->d;
+    k_dt_select<<<1, 1, 0, c->stream>>>(dt, d.dt_cur, d.dt_next, nullptr);
+    c->launches++;
+    if (d.n > 0) {
+        k_kick_drift<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, c->p);
+        c->launches++;
+    }
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_get_field(sph_ctx *c, const float *src, float *dst, int as_int)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    k_scatter<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(src, (const unsigned *)d.r.s[PP_ORIG], d.n, dst, as_int);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_get_position(sph_ctx *c, int comp, float *dst)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    k_scatter_pos<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d.r.pm, (const unsigned *)d.r.s[PP_ORIG], d.n, dst, comp);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_download(sph_ctx *c, sph_state *st)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    k_download<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, *st);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}

@@ -1,0 +1,90 @@
+"""GPU-vs-oracle comparison helpers (tests only).  Tolerances are BASELINE.json north_star's:
+neighbour sets identical; rho 1e-5 relative; a, du/dt, dS/dt max|gpu - oracle| <= 1e-4 max|oracle|
+per field; yielded state (S, v, u after the closing kick) 1e-4 relative in the same max norm."""
+import numpy as np
+
+TOL_RHO = 1e-5
+TOL_RATE = 1e-4
+TOL_STATE = 1e-4
+
+
+def maxnorm_err(gpu, ref):
+    ref = np.asarray(ref, dtype=np.float64)
+    gpu = np.asarray(gpu, dtype=np.float64)
+    scale = np.abs(ref).max()
+    if scale == 0.0:
+        return np.abs(gpu).max()
+    return np.abs(gpu - ref).max() / scale
+
+
+def rows(counts, offsets, lst):
+    counts = np.asarray(counts); offsets = np.asarray(offsets); lst = np.asarray(lst)
+    return [np.sort(lst[offsets[i]:offsets[i + 1]]) for i in range(counts.shape[0])]
+
+
+def gpu_single_pass(wl, dt=None, split=True):
+    """Run the BASELINE.json configs[0] pass sequence through the C ABI; returns numpy fields."""
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    s = B.Sph(wl.params, max(wl.n, 1))
+    t = s.upload(wl)
+    dt = wl.dt if dt is None else dt
+    s.build_neighbors(t, wl.n)
+    s.density()
+    s.strength_update(B.PREDICT)
+    strength = bool(wl.params.flags & B.STRENGTH)
+    if split:
+        if strength:
+            s.gradients()
+        s.forces()
+        s.strength_update(B.CLOSE, dt)
+    else:
+        raise NotImplementedError
+    out = {}
+    for name in ("RHO", "OMEGA", "P", "CS", "T", "GAMMA", "Y", "MUMAX", "DUDT", "DT", "EPS2", "U", "CFLAG",
+                 "NGATHER", "NSYMMETRIC"):
+        out[name.lower()] = s.get_field(name).cpu().numpy()
+    for name, nc in (("A", 3), ("V", 3), ("X", 3), ("SPRED", 5), ("S", 5), ("DSDT", 5), ("F", 9), ("CINV", 9), ("G", 9)):
+        out[name.lower()] = s.get_fields(name, nc).cpu().numpy()
+    out["counters"] = s.get_counters()
+    out["timings"] = s.get_timings()
+    out["_sph"] = s
+    torch.cuda.synchronize()
+    return out
+
+
+def compare_single_pass(g, d, wl, check_sets=None):
+    """g: gpu_single_pass output, d: oracle.single_pass output.  Returns dict of errors; asserts."""
+    from paper_2603_19764_b200 import binding as B
+    errs = {}
+    assert np.array_equal(g["ngather"].astype(np.int64), d["n_gather"].astype(np.int64)), "gather counts differ"
+    assert np.array_equal(g["nsymmetric"].astype(np.int64), d["n_symmetric"].astype(np.int64)), "symmetric counts differ"
+    errs["rho"] = np.abs(g["rho"] / d["rho"] - 1.0).max() if wl.n else 0.0
+    assert errs["rho"] <= TOL_RHO, errs
+    errs["omega"] = maxnorm_err(g["omega"], d["omega"])
+    assert errs["omega"] <= 1e-5, errs
+    for k, ref in (("p", d["P"]), ("y", d["Y"]), ("t", d["T"]), ("gamma", d["Gamma"])):
+        errs[k] = maxnorm_err(g[k], ref)
+        assert errs[k] <= TOL_RATE, errs
+    errs["a"] = maxnorm_err(g["a"], d["a"])
+    errs["dudt"] = maxnorm_err(g["dudt"], d["dudt"])
+    errs["mumax"] = maxnorm_err(g["mumax"], d["mumax"])
+    errs["dt"] = maxnorm_err(g["dt"], d["dt_i"])
+    for k in ("a", "dudt", "mumax", "dt"):
+        assert errs[k] <= TOL_RATE, errs
+    if wl.params.flags & B.STRENGTH:
+        errs["spred"] = maxnorm_err(g["spred"], d["S_pred"])
+        errs["F"] = maxnorm_err(g["f"], d["F"])
+        errs["Cinv"] = maxnorm_err(g["cinv"], d["Cinv"])
+        errs["G"] = maxnorm_err(g["g"], d["G"])
+        errs["dsdt"] = maxnorm_err(g["dsdt"], d["dS"])
+        errs["eps2"] = maxnorm_err(g["eps2"], d["eps2"])
+        assert np.array_equal(g["cflag"].astype(np.int64), d["cflag"].astype(np.int64)), "C fallback flags differ"
+        for k in ("spred", "F", "Cinv", "G", "dsdt", "eps2"):
+            assert errs[k] <= TOL_RATE, errs
+    errs["S_close"] = maxnorm_err(g["s"], d["S_close"])
+    errs["v_close"] = maxnorm_err(g["v"], d["v_close"])
+    errs["u_close"] = maxnorm_err(g["u"], d["u_close"])
+    for k in ("S_close", "v_close", "u_close"):
+        assert errs[k] <= TOL_STATE, errs
+    return errs
