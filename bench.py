@@ -1,0 +1,318 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line per run (contract: see DESIGN.md section 7).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c0|c1|c2|c3|c4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (sph_step: opening kick, drift, prediction, Morton
+re-sort + chunk tree, density, predict/EOS/yield, fused gradient+force, close, dt reduction) over
+one seeded synthetic particle set shaped like BASELINE.json's configs.  value = true neighbour pair
+evaluations per second (sum_i |gather set| + sum_i |symmetric set| per step) over all ranks, inputs
+resident in HBM; e2e = the same through sph_step_host (pinned host buffers, H2D + D2H inside the
+timed region).  N > 1 runs N independent replicas ("replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# Algorithmic flops per TRUE pair evaluation, hand-counted from the equations as the kernels
+# evaluate them (FMA = 2, rsqrt / div / min / max / compare = 1); DESIGN.md section 6.
+FLOPS_PAIR_FUSED = 148      # Eq. 18-21 + 5-8, gradient and force in one pass, with S
+FLOPS_PAIR_HYDRO = 82       # force pass with S == 0 (no gradient sums)
+FLOPS_PAIR_DENSITY = 44     # Eq. 1 + 3: 20 fp32 + 12 fp64 (counted as 2 each)
+FP32_LANES_PER_SM = 128
+
+
+def fp32_peak_tflops(n_sm: int, mhz: float) -> float:
+    """SMs x 128 FP32 lanes x 2 flop (FMA) x clock: the CUDA-core peak (guide's unit counts)."""
+    return n_sm * FP32_LANES_PER_SM * 2 * mhz * 1e6 / 1e12
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region."""
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            f = [c.strip() for c in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if f[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def make_workload(name: str):
+    from paper_2603_19764_b200 import workloads as W
+    k = int(name[1])
+    return W.config(k)
+
+
+def oracle_sample(wl, target_n: int = 60000):
+    """A bounded sample of the workload for the CPU oracle: the particles inside a cube around the
+    centre of mass that holds about target_n of them (complete neighbourhoods inside, cut faces)."""
+    import numpy as np
+    A = wl.arrays
+    if wl.n <= target_n:
+        return wl, "all %d particles" % wl.n
+    p = np.stack([A["x"], A["y"], A["z"]]).astype(np.float64)
+    c = np.median(p, axis=1, keepdims=True)
+    d = np.abs(p - c).max(axis=0)
+    half = np.partition(d, target_n)[target_n]
+    idx = np.nonzero(d <= half)[0]
+    return wl.subset(idx), "cube of %d particles around the median position (of %d)" % (idx.size, wl.n)
+
+
+def time_oracle(wl, steps: int = 1):
+    """One derivative evaluation (the pair work of one step) of the oracle, as it stands."""
+    from oracle import oracle as O
+    import numpy as np
+    A = {k: np.ascontiguousarray(v, dtype=np.float64) for k, v in wl.arrays.items()}
+    S = np.stack([A["Sxx"], A["Syy"], A["Sxy"], A["Sxz"], A["Syz"]])
+    g = np.stack([A["gx"], A["gy"], A["gz"]])
+    O.lib()
+    best = None
+    pairs = 0
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        d = O.derivatives(wl.params, A["x"], A["y"], A["z"], A["m"], A["h"], A["vx"], A["vy"], A["vz"],
+                          A["u"], S, wl.mat, g, "grid")
+        dt = time.perf_counter() - t0
+        pairs = int(d["n_gather"].sum()) + int(d["n_symmetric"].sum())
+        best = dt if best is None else min(best, dt)
+    return pairs, best, O.lib().orc_max_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    wl = make_workload(args.workload)
+    sample, what = oracle_sample(wl)
+    for _ in range(max(args.warmup, 0) and 1):
+        time_oracle(sample, 1)
+    times = []
+    pairs = 0
+    for _ in range(args.steps):
+        pairs, dt, cores = time_oracle(sample, 1)
+        times.append(dt)
+    total = sum(times)
+    val = pairs * len(times) / total
+    line = {
+        "impl": "reference", "metric": "pair_interactions_per_s", "value": val, "unit": "pairs/s",
+        "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * total / len(times), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": wl.name, "n_particles": wl.n, "sample": what},
+        "cpu_baseline": {"value": val, "unit": "pairs/s", "cores": cores, "kind": "oracle", "sample": what},
+        "e2e": {"value": val, "unit": "pairs/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "particle_steps_per_s": sample.n * len(times) / total,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2603_19764_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    torch.cuda.set_device(local)
+    dev = torch.device(f"cuda:{local}")
+    props = torch.cuda.get_device_properties(dev)
+
+    wl = make_workload(args.workload)
+    n = wl.n
+    strength = bool(wl.params.flags & B.STRENGTH)
+    s = B.Sph(wl.params, n, device=dev)
+    t = s.upload(wl)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB of L2
+    working_set = s.workspace_bytes
+    do_flush = True
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize(dev)
+
+    # ---- device-resident timing -----------------------------------------------------------
+    s.build_neighbors(t, n)
+    for _ in range(args.warmup):
+        s.step(None, 0, 0.0)
+    barrier()
+    launches0 = s.launch_count()
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    pass_ms = {k: 0.0 for k in B.T_SLOTS}
+    pairs_g = pairs_s = tests = 0
+    barrier()
+    for k in range(args.steps):
+        if do_flush:
+            flush.fill_(k & 0xff)
+        ev[k][0].record(s.stream)
+        s.step(None, 0, 0.0)
+        ev[k][1].record(s.stream)
+        tm = s.get_timings()                 # synchronises; outside the event pair of the next step
+        for q in B.T_SLOTS:
+            pass_ms[q] += tm[q]
+        c = s.get_counters()
+        pairs_g += c["pairs_gather"]; pairs_s += c["pairs_symmetric"]
+        tests += c["tests_density"] + c["tests_force"]
+    barrier()
+    clocks = sampler.stop()
+    launches = s.launch_count() - launches0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = sum(step_ms)
+    tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    total_ms_max = float(tmax.item())
+    pairs = pairs_g + pairs_s
+    value = world * pairs / (total_ms_max * 1e-3)
+
+    # ---- end to end through the host-buffer entry point -----------------------------------
+    host = {k: torch.from_numpy(v.copy()).pin_memory() for k, v in wl.arrays.items()}
+    host["mat"] = torch.from_numpy(wl.mat.copy()).pin_memory()
+    host["fixed"] = torch.from_numpy(wl.fixed.copy()).pin_memory()
+    s2 = B.Sph(wl.params, n, device=dev)
+    e2e_steps = max(1, min(args.steps, 5))
+    s2.step_host(host, n, 0.0)                                   # warm-up (also the bootstrap)
+    s2.step_host(host, n, 0.0)
+    barrier()
+    t0 = time.perf_counter()
+    e2e_pairs = 0
+    for _ in range(e2e_steps):
+        s2.step_host(host, n, 0.0)
+        c = s2.get_counters()
+        e2e_pairs += c["pairs_gather"] + c["pairs_symmetric"]
+    torch.cuda.synchronize(dev)
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = world * e2e_pairs / float(te.item())
+    h2d = n * (17 * 4 + 4 + 1)
+    d2h = n * 12 * 4 + 4
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the fused gradient + force pair pass) --------------
+    sm_max = clocks.get("sm_max_mhz") or 1965.0
+    peak = fp32_peak_tflops(props.multi_processor_count, sm_max)
+    kern_ms = pass_ms["force"] / args.steps
+    flops_pair = FLOPS_PAIR_FUSED if strength else FLOPS_PAIR_HYDRO
+    achieved = (pairs_s / args.steps) * flops_pair / (kern_ms * 1e-3) / 1e12 if kern_ms > 0 else 0.0
+    roofline = {"bound": "alu", "kernel": "k_pair (fused Eq. 18-21 + 5-8)", "achieved": achieved,
+                "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "peak_source": "%d SMs x 128 FP32 lanes x 2 x %.0f MHz (guide's unit counts; no FP32 entry in "
+                               "MEASURED_PEAKS.json)" % (props.multi_processor_count, sm_max),
+                "flops_per_pair": flops_pair, "pairs_per_launch": pairs_s / args.steps,
+                "kernel_ms": kern_ms, "share_of_step": kern_ms / (total_ms / args.steps),
+                "candidate_hit_rate": pairs / tests if tests else None, "traffic": None}
+
+    # ---- the oracle beside it ------------------------------------------------------------------
+    cpu = None
+    if not args.no_cpu_baseline:
+        sample, what = oracle_sample(wl)
+        op, ot, cores = time_oracle(sample, 1)
+        cpu = {"value": op / ot, "unit": "pairs/s", "cores": cores, "kind": "oracle", "sample": what,
+               "seconds": ot, "particle_steps_per_s": sample.n / ot}
+
+    line = {
+        "metric": "pair_interactions_per_s", "value": value, "unit": "pairs/s", "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": wl.name, "n_particles": n, "strength": strength,
+                   "mean_neighbours": pairs_s / args.steps / max(n, 1),
+                   "l2": "flushed between steps (256 MiB fill outside the timed events)",
+                   "working_set_bytes": working_set, "parallelism": "replicas x%d" % world},
+        "particle_steps_per_s": world * n * args.steps / (total_ms_max * 1e-3),
+        "pass_ms": {k: v / args.steps for k, v in pass_ms.items()},
+        "gpu_launches": launches,
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": "pairs/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                "steps": e2e_steps, "ms_per_step": 1e3 * float(te.item()) / e2e_steps},
+        "roofline": roofline,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", default="c2", choices=["c0", "c1", "c2", "c3", "c4"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -60,6 +60,7 @@ struct Dev {
     float *vfull[3], *ufull, *Sfull[5];     // state at the full step (after CLOSE)
     float *a[3], *dudt, *dS[5];             // derivatives at the full step
     float *rho, *omega, *P, *cs, *T, *Gamma, *Y, *mumax, *dti, *eps2, *cflag;
+    double *rho64;                          // fp64 density for the EOS (see k_density)
     int *ngather, *nsym;
     float *F[9], *Cinv[9], *G[9];
     float4 *A3, *A4, *A5;                   // packed pair-pass operands (see k_predict)

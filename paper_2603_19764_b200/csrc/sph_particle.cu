@@ -44,7 +44,8 @@ __global__ void __launch_bounds__(256) k_predict(Dev d, DevParams p)
     unsigned mf = ((const unsigned *)d.r.s[PP_MATFIX])[i];
     const sph_material &m = p.mat[mf & 0xffu];
     float rho = d.rho[i], om = d.omega[i], u = d.r.s[PP_UPRED][i];
-    float P = m.c0 * m.c0 * (rho - m.rho0);
+    // the subtraction rho - rho0 in fp64 (see k_density)
+    float P = (float)((double)m.c0 * (double)m.c0 * (d.rho64[i] - (double)m.rho0));
     if (p.flags & SPH_PCLIP_GLOBAL) P = fmaxf(P, 0.f);
     float cs = m.c0;
     float T = u / m.cv;
