@@ -32,6 +32,11 @@ extern "C" {
 #define SPH_CORRECTION_TENSOR     2u  /* G = F.C (Eq. 22); off: C = 1      */
 #define SPH_PCLIP_GLOBAL          4u  /* clip P >= 0 in the EOS too, not only in Eq. 34 (reading Q8)    */
 #define SPH_JAUMANN_COROTATIONAL  8u  /* flip the sign of the rotation terms of Eq. 13 (reading Q1)     */
+#define SPH_NO_LISTS             16u  /* pair passes walk the chunk tree themselves instead of reading
+                                         the per-particle neighbour lists (the round-1 "v0" kernels, kept
+                                         for A/B measurement and as the path with no capacity limits)       */
+#define SPH_MORTON_ORDER         32u  /* sort by Morton (Z-order) keys instead of Hilbert keys (A/B
+                                         measurement; results do not depend on the order)                  */
 
 /* error codes */
 #define SPH_OK         0
@@ -89,6 +94,10 @@ enum { SPH_C_PAIRS_GATHER = 0,   /* sum_i |gather set(i)|   (true pairs of the d
        SPH_C_TESTS_DENSITY,      /* candidate pairs the density pass tested                     */
        SPH_C_TESTS_FORCE,        /* candidate pairs the gradient/force pass tested              */
        SPH_C_CFALLBACK,          /* particles whose C fell back to 1                             */
+       SPH_C_TESTS_CULL,         /* candidate pairs the list build tested (sph_build_neighbors) */
+       SPH_C_CANDIDATES,         /* sum over tiles of the tile candidate-list lengths           */
+       SPH_C_LIST_OVERFLOW,      /* != 0: a list capacity was exceeded, results are incomplete:
+                                    raise sph_params.max_neighbors or set SPH_NO_LISTS           */
        SPH_C_COUNT };
 
 typedef struct sph_ctx sph_ctx;   /* opaque, library-owned (host memory) */
@@ -111,6 +120,8 @@ typedef struct sph_params {
     int n_materials;           /* 1..SPH_MAX_MATERIALS                                            */
     unsigned flags;            /* SPH_STRENGTH | ...                                              */
     sph_material mat[SPH_MAX_MATERIALS];
+    int max_neighbors;         /* capacity of each particle's neighbour list (symmetric set), rounded
+                                  up to a multiple of 8; <= 0 selects 256                             */
 } sph_params;
 
 /* Caller-owned particle arrays, each of length n.  For the device entry points all pointers are
@@ -134,7 +145,8 @@ int sph_init(sph_ctx **ctx, const sph_params *params, long long n_max,
              void *workspace, size_t workspace_bytes, void *cuda_stream);
 
 /* S1: Morton keys -> radix sort -> gather into the resident sorted arrays -> chunk bounding boxes
- * and the chunk tree the pair passes walk (stands in for the paper's tree build).
+ * and chunk tree -> per-tile candidate lists and per-particle neighbour lists (the symmetric set)
+ * that the pair passes read (stands in for the paper's tree build).
  * state != NULL: ingest the caller's arrays (DEVICE), n particles; derivatives carried between
  * steps are reset.  state == NULL: re-sort the resident particles at their current positions.
  * n = 0 is legal.  Errors: EINVAL, ECAPACITY, EORDER (state == NULL with nothing resident). */

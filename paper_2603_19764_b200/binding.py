@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libsph.so")
 
 MAX_MATERIALS = 8
-STRENGTH, CORRECTION_TENSOR, PCLIP_GLOBAL, JAUMANN_COROTATIONAL = 1, 2, 4, 8
+STRENGTH, CORRECTION_TENSOR, PCLIP_GLOBAL, JAUMANN_COROTATIONAL, NO_LISTS = 1, 2, 4, 8, 16
 OK, EINVAL, ENOMEM, ECUDA, EORDER, ECAPACITY = 0, -1, -2, -3, -4, -5
 PREDICT, CLOSE, DERIVATIVES = 0, 1, 2
 GATHER, SYMMETRIC = 0, 1
@@ -23,7 +23,8 @@ GATHER, SYMMETRIC = 0, 1
 F = dict(RHO=0, OMEGA=1, P=2, CS=3, T=4, GAMMA=5, Y=6, MUMAX=7, DUDT=8, DT=9, EACC=10, EPS2=11, U=12,
          CFLAG=13, NGATHER=14, NSYMMETRIC=15, A=32, V=36, X=40, SPRED=48, S=56, DSDT=64, F=80, CINV=96, G=112)
 T_SLOTS = ("build", "density", "predict", "gradient", "force", "close", "kickdrift", "step")
-C_SLOTS = ("pairs_gather", "pairs_symmetric", "tests_density", "tests_force", "cfallback")
+C_SLOTS = ("pairs_gather", "pairs_symmetric", "tests_density", "tests_force", "cfallback", "tests_cull",
+           "candidates", "list_overflow")
 
 FLOAT_FIELDS = ("x", "y", "z", "m", "h", "vx", "vy", "vz", "u", "Sxx", "Syy", "Sxy", "Sxz", "Syz")
 OPT_FIELDS = ("gx", "gy", "gz")
@@ -43,7 +44,7 @@ class sph_material(C.Structure):
 class sph_params(C.Structure):
     _fields_ = [("kappa", C.c_float), ("alpha", C.c_float), ("beta", C.c_float), ("eps_av", C.c_float),
                 ("eta_C", C.c_float), ("eta_a", C.c_float), ("n_materials", C.c_int), ("flags", C.c_uint),
-                ("mat", sph_material * MAX_MATERIALS)]
+                ("mat", sph_material * MAX_MATERIALS), ("max_neighbors", C.c_int)]
 
 
 class sph_state(C.Structure):
@@ -108,6 +109,7 @@ def make_params(p) -> sph_params:
     out.kappa, out.alpha, out.beta, out.eps_av = p.kappa, p.alpha, p.beta, p.eps_av
     out.eta_C, out.eta_a = p.eta_C, p.eta_a
     out.flags = int(p.flags)
+    out.max_neighbors = int(getattr(p, "max_neighbors", 0))
     out.n_materials = len(p.materials)
     for k, m in enumerate(p.materials):
         for name, _ in sph_material._fields_:

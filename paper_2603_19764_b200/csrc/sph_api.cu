@@ -32,7 +32,13 @@ static void tree_counts(long long n_max, int *count, int *nlev)
     *nlev = L + 1;
 }
 
-static size_t carve(Dev *d, float **stage, char *base, long long n_max)
+static int kcap_of(const sph_params *p)
+{
+    int k = p->max_neighbors > 0 ? p->max_neighbors : SPH_KCAP_DEFAULT;
+    return (k + 7) & ~7;
+}
+
+static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap, bool lists)
 {
     Bump b{base, 0};
     size_t N = (size_t)(n_max > 0 ? n_max : 1);
@@ -67,6 +73,14 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max)
     for (int k = 0; k < 9; ++k) o.Cinv[k] = b.take<float>(N);
     for (int k = 0; k < 9; ++k) o.G[k] = b.take<float>(N);
     o.A3 = b.take<float4>(N); o.A4 = b.take<float4>(N); o.A5 = b.take<float4>(N);
+    o.kcap = kcap;
+    size_t ntile = (N + SPH_TILE - 1) / SPH_TILE;
+    o.tile_ncand = b.take<int>(ntile);
+    o.tile_off = b.take<unsigned long long>(ntile);
+    o.cand_cursor = b.take<unsigned long long>(1);
+    o.cand_cap = lists ? (unsigned long long)ntile * SPH_TILE_SC : 1;
+    o.cand = b.take<unsigned>((size_t)o.cand_cap);
+    o.nbr = b.take<unsigned short>(lists ? N * (size_t)kcap : 8);
     o.bbox = b.take<float>(8);
     o.dt_cur = b.take<float>(1);
     o.dt_next = b.take<float>(1);
@@ -93,7 +107,7 @@ static bool params_ok(const sph_params *p)
 extern "C" size_t sph_workspace_bytes(const sph_params *params, long long n_max)
 {
     if (!params_ok(params) || n_max < 0 || n_max > 2000000000ll) return 0;
-    return carve(nullptr, nullptr, nullptr, n_max);
+    return carve(nullptr, nullptr, nullptr, n_max, kcap_of(params), !(params->flags & SPH_NO_LISTS));
 }
 
 extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max, void *workspace,
@@ -103,7 +117,7 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
     *out = nullptr;
     if (!params_ok(params) || n_max < 0 || n_max > 2000000000ll || !workspace) return SPH_EINVAL;
     if (((uintptr_t)workspace & 255u) != 0) return SPH_EINVAL;
-    size_t need = carve(nullptr, nullptr, nullptr, n_max);
+    size_t need = carve(nullptr, nullptr, nullptr, n_max, kcap_of(params), !(params->flags & SPH_NO_LISTS));
     if (workspace_bytes < need) return SPH_ENOMEM;
     sph_ctx *c = new (std::nothrow) sph_ctx();
     if (!c) return SPH_ENOMEM;
@@ -113,7 +127,8 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
     c->p.flags = params->flags; c->p.n_materials = params->n_materials;
     memcpy(c->p.mat, params->mat, sizeof(params->mat));
     c->stream = (cudaStream_t)cuda_stream;
-    c->ws_bytes = carve(&c->d, &c->stage, (char *)workspace, n_max);
+    c->use_lists = !(params->flags & SPH_NO_LISTS);
+    c->ws_bytes = carve(&c->d, &c->stage, (char *)workspace, n_max, kcap_of(params), c->use_lists);
     c->d.n = 0; c->d.nchunk = 0;
     for (int k = 0; k < 2 * SPH_T_COUNT; ++k) {
         cudaError_t e = cudaEventCreate(&c->ev[k]);
@@ -178,6 +193,10 @@ extern "C" int sph_build_neighbors(sph_ctx *c, const sph_state *state, long long
         rc = sph_launch_resort(c);
         if (rc) return rc;
     }
+    if (c->use_lists) {
+        rc = sph_launch_cull(c);
+        if (rc) return rc;
+    }
     c->have_density = c->have_predict = c->have_grad = c->have_force = false;
     return SPH_OK;
 }
@@ -187,7 +206,7 @@ extern "C" int sph_density(sph_ctx *c)
     if (!c) return SPH_EINVAL;
     if (!c->resident) return SPH_EORDER;
     PassTimer t(c, SPH_T_DENSITY);
-    int rc = sph_launch_density(c);
+    int rc = c->use_lists ? sph_launch_density_l(c) : sph_launch_density(c);
     if (rc) return rc;
     c->have_density = true;
     c->have_predict = c->have_grad = c->have_force = false;
@@ -199,7 +218,7 @@ extern "C" int sph_gradients(sph_ctx *c)
     if (!c) return SPH_EINVAL;
     if (!c->have_predict) return SPH_EORDER;
     PassTimer t(c, SPH_T_GRADIENT);
-    int rc = sph_launch_pair(c, true, false);
+    int rc = c->use_lists ? sph_launch_pair_l(c, true, false) : sph_launch_pair(c, true, false);
     if (rc) return rc;
     c->have_grad = true;
     return SPH_OK;
@@ -210,7 +229,7 @@ extern "C" int sph_forces(sph_ctx *c)
     if (!c) return SPH_EINVAL;
     if (!c->have_predict) return SPH_EORDER;
     PassTimer t(c, SPH_T_FORCE);
-    int rc = sph_launch_pair(c, false, true);
+    int rc = c->use_lists ? sph_launch_pair_l(c, false, true) : sph_launch_pair(c, false, true);
     if (rc) return rc;
     c->have_force = true;
     return SPH_OK;
@@ -256,7 +275,7 @@ static int derivative_passes(sph_ctx *c)
     const bool strength = (c->p.flags & SPH_STRENGTH) != 0;
     {
         PassTimer t(c, SPH_T_FORCE);
-        rc = sph_launch_pair(c, strength, true);
+        rc = c->use_lists ? sph_launch_pair_l(c, strength, true) : sph_launch_pair(c, strength, true);
         if (rc) return rc;
         c->have_force = true;
         c->have_grad = strength;
@@ -423,7 +442,8 @@ extern "C" int sph_get_neighbors(sph_ctx *c, int which, int *counts, const long 
 {
     if (!c || !counts || (which != SPH_GATHER && which != SPH_SYMMETRIC) || (list && !offsets)) return SPH_EINVAL;
     if (!c->resident) return SPH_EORDER;
-    return sph_launch_neighbors(c, which, counts, offsets, list);
+    return c->use_lists ? sph_launch_neighbors_l(c, which, counts, offsets, list)
+                        : sph_launch_neighbors(c, which, counts, offsets, list);
 }
 
 extern "C" int sph_get_timings(sph_ctx *c, float *ms, int n)

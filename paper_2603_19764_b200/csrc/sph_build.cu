@@ -45,7 +45,7 @@ __global__ void __launch_bounds__(256) k_bbox(const float *__restrict__ x, const
 }
 
 // ------------------------------------------------------------------------------------------
-// 63-bit Morton key (3 x 21 bits) on a cubic grid spanning the bounding box
+// 63-bit space-filling-curve key (3 x 21 bits) on a cubic grid spanning the bounding box
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned long long expand21(unsigned long long v)
 {
@@ -58,10 +58,34 @@ __device__ __forceinline__ unsigned long long expand21(unsigned long long v)
     return v;
 }
 
+// Hilbert index of a 3 x 21-bit lattice point (Skilling's transpose algorithm, AIP Conf. Proc. 707,
+// 2004): unlike the Morton curve it has no jumps, so ANY run of consecutive particles is a compact
+// connected blob -- which is what bounds the chunk / tile boxes of the pair passes.
+__device__ __forceinline__ unsigned long long hilbert63(unsigned X0, unsigned X1, unsigned X2)
+{
+    unsigned X[3] = {X0, X1, X2};
+    const unsigned M = 1u << 20;
+    for (unsigned Q = M; Q > 1; Q >>= 1) {
+        unsigned P = Q - 1;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            if (X[a] & Q) X[0] ^= P;
+            else { unsigned t = (X[0] ^ X[a]) & P; X[0] ^= t; X[a] ^= t; }
+        }
+    }
+    X[1] ^= X[0];
+    X[2] ^= X[1];
+    unsigned t = 0;
+    for (unsigned Q = M; Q > 1; Q >>= 1)
+        if (X[2] & Q) t ^= Q - 1;
+    X[0] ^= t; X[1] ^= t; X[2] ^= t;
+    return (expand21(X[0]) << 2) | (expand21(X[1]) << 1) | expand21(X[2]);
+}
+
 template <bool FROM_STATE>
 __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ x, const float *__restrict__ y,
                                               const float *__restrict__ z, const float4 *__restrict__ pm,
-                                              long long n, const int *__restrict__ bbox,
+                                              long long n, const int *__restrict__ bbox, int morton,
                                               unsigned long long *__restrict__ keys, unsigned *__restrict__ perm)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
@@ -76,14 +100,13 @@ __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ x, const
     float p[3];
     if (FROM_STATE) { p[0] = x[i]; p[1] = y[i]; p[2] = z[i]; }
     else { float4 q = pm[i]; p[0] = q.x; p[1] = q.y; p[2] = q.z; }
-    unsigned long long k = 0;
+    unsigned c[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
         float f = (p[a] - lo[a]) * scale;
-        f = fminf(fmaxf(f, 0.f), 2097151.0f);
-        k |= expand21((unsigned long long)f) << a;
+        c[a] = (unsigned)fminf(fmaxf(f, 0.f), 2097151.0f);
     }
-    keys[i] = k;
+    keys[i] = morton ? (expand21(c[0]) | (expand21(c[1]) << 1) | (expand21(c[2]) << 2)) : hilbert63(c[0], c[1], c[2]);
     perm[i] = (unsigned)i;
 }
 
@@ -252,7 +275,7 @@ int sph_launch_ingest(sph_ctx *c, const sph_state *st, long long n)
     int nb = sph_div_up(n, 256);
     k_bbox_init<<<1, 32, 0, c->stream>>>((int *)d.bbox);
     k_bbox<true><<<nb < 1184 ? nb : 1184, 256, 0, c->stream>>>(st->x, st->y, st->z, nullptr, n, (int *)d.bbox);
-    k_keys<true><<<nb, 256, 0, c->stream>>>(st->x, st->y, st->z, nullptr, n, (const int *)d.bbox, d.keys, d.perm);
+    k_keys<true><<<nb, 256, 0, c->stream>>>(st->x, st->y, st->z, nullptr, n, (const int *)d.bbox, (c->p.flags & SPH_MORTON_ORDER) ? 1 : 0, d.keys, d.perm);
     c->launches += 3;
     int rc = sort_keys(c);
     if (rc) return rc;
@@ -269,7 +292,7 @@ int sph_launch_resort(sph_ctx *c)
     int nb = sph_div_up(d.n, 256);
     k_bbox_init<<<1, 32, 0, c->stream>>>((int *)d.bbox);
     k_bbox<false><<<nb < 1184 ? nb : 1184, 256, 0, c->stream>>>(nullptr, nullptr, nullptr, d.r.pm, d.n, (int *)d.bbox);
-    k_keys<false><<<nb, 256, 0, c->stream>>>(nullptr, nullptr, nullptr, d.r.pm, d.n, (const int *)d.bbox, d.keys, d.perm);
+    k_keys<false><<<nb, 256, 0, c->stream>>>(nullptr, nullptr, nullptr, d.r.pm, d.n, (const int *)d.bbox, (c->p.flags & SPH_MORTON_ORDER) ? 1 : 0, d.keys, d.perm);
     c->launches += 3;
     int rc = sort_keys(c);
     if (rc) return rc;

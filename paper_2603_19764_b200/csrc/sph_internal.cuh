@@ -12,6 +12,14 @@
 #define SPH_MAX_LEVELS 7      // 32^6 chunks * 32 particles >> any n that fits in HBM
 #define SPH_NPP 21            // scalar (4-byte) resident arrays that are permuted at re-sort
 
+// neighbour-list machinery (sph_lists.cu)
+#define SPH_TILE_CHUNKS 16    // chunks per tile = warps per CTA of the list kernels
+#define SPH_TILE (SPH_TILE_CHUNKS * SPH_CHUNK)
+#define SPH_TILE_SC 4096      // capacity of a tile's candidate list (slots are u16)
+#define SPH_CULL_MAXSRC 1024  // source chunks a tile may accept in the tree walk
+#define SPH_PAIR_SE 2560      // candidates staged per round in the fused pair pass (5 float4 each)
+#define SPH_KCAP_DEFAULT 256  // neighbour-list capacity per particle
+
 // indices into Resident::s (scalar ping-pong arrays)
 enum {
     PP_UPRED = 0,
@@ -64,6 +72,14 @@ struct Dev {
     int *ngather, *nsym;
     float *F[9], *Cinv[9], *G[9];
     float4 *A3, *A4, *A5;                   // packed pair-pass operands (see k_predict)
+    // neighbour lists (sph_lists.cu)
+    int *tile_ncand;                        // candidates per tile
+    unsigned *cand;                         // candidate pool: global indices, tile after tile
+    unsigned long long *tile_off;           // where each tile's candidates start in the pool
+    unsigned long long *cand_cursor;        // bump allocator of the pool
+    unsigned long long cand_cap;            // pool capacity (entries)
+    unsigned short *nbr;                    // [particle][kcap] slots into the tile candidate list
+    int kcap;
     // scalars on the device
     float *bbox;                            // 6 floats as ordered ints: lo xyz, hi xyz
     float *dt_cur, *dt_next;                // step in use / CFL step from the last CLOSE
@@ -81,6 +97,7 @@ struct sph_ctx {
     cudaStream_t stream;
     int last_cuda;
     long long launches;
+    bool use_lists;
     bool resident, have_density, have_predict, have_grad, have_force, have_derivs;
     cudaEvent_t ev[2 * SPH_T_COUNT];
     bool ev_used[SPH_T_COUNT];
@@ -114,6 +131,10 @@ int sph_launch_get_field(sph_ctx *c, const float *src, float *dst, int as_int);
 int sph_launch_get_position(sph_ctx *c, int comp, float *dst);
 int sph_launch_neighbors(sph_ctx *c, int which, int *counts, const long long *offsets, int *list);
 int sph_launch_download(sph_ctx *c, sph_state *st);
+int sph_launch_cull(sph_ctx *c);
+int sph_launch_density_l(sph_ctx *c);
+int sph_launch_pair_l(sph_ctx *c, bool grad, bool force);
+int sph_launch_neighbors_l(sph_ctx *c, int which, int *counts, const long long *offsets, int *list);
 
 // ---- small device helpers ----------------------------------------------------------------
 #ifdef __CUDACC__

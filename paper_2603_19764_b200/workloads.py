@@ -29,6 +29,7 @@ FLAG_STRENGTH = 1
 FLAG_CORRECTION_TENSOR = 2
 FLAG_PCLIP_GLOBAL = 4
 FLAG_JAUMANN_COROTATIONAL = 8
+FLAG_NO_LISTS = 16
 
 G_NEWTON = 6.674e-11
 
@@ -61,6 +62,7 @@ class Params:
     eta_C: float = 0.3
     eta_a: float = 0.0
     flags: int = FLAG_STRENGTH | FLAG_CORRECTION_TENSOR
+    max_neighbors: int = 0     # neighbour-list capacity of the CUDA path (0 = library default)
     materials: List[Material] = field(default_factory=lambda: [Material()])
 
 

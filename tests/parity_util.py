@@ -47,6 +47,7 @@ def gpu_single_pass(wl, dt=None, split=True):
     for name, nc in (("A", 3), ("V", 3), ("X", 3), ("SPRED", 5), ("S", 5), ("DSDT", 5), ("F", 9), ("CINV", 9), ("G", 9)):
         out[name.lower()] = s.get_fields(name, nc).cpu().numpy()
     out["counters"] = s.get_counters()
+    assert out["counters"]["list_overflow"] == 0, "neighbour-list capacity exceeded"
     out["timings"] = s.get_timings()
     out["_sph"] = s
     torch.cuda.synchronize()

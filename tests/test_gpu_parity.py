@@ -157,3 +157,43 @@ def test_step_host_roundtrip_equals_device_step():
     s2.step_host(host, wl.n, 2e-7)
     for k in ("x", "vx", "u", "Sxy"):
         assert np.array_equal(host[k].numpy(), t[k].cpu().numpy()), k
+
+
+def test_tree_walk_kernels_still_match():
+    """SPH_NO_LISTS selects the round-1 v0 kernels (pair passes walk the chunk tree)."""
+    wl = W.elastic_block(12, h_spread=0.25, flags=F | W.FLAG_NO_LISTS)
+    g = U.gpu_single_pass(wl)
+    d = O.single_pass(wl)
+    U.compare_single_pass(g, d, wl)
+    _neighbor_sets_equal(g["_sph"], wl)
+
+
+def test_variable_h_impact_pair_scaled():
+    """configs[3] construction at parity size: two bodies, two materials, h varying ~5x."""
+    wl = W.impact_pair(30000, W.SEED_BASE + 3, 100.0, 1.214)
+    assert wl.arrays["h"].max() / wl.arrays["h"].min() > 3.0
+    g = U.gpu_single_pass(wl, dt=1e-3)
+    d = O.single_pass(wl, dt=1e-3, mode="grid")
+    errs = U.compare_single_pass(g, d, wl)
+    assert g["counters"]["list_overflow"] == 0
+    print("impact pair errors", {k: float(f"{v:.3g}") for k, v in errs.items()})
+
+
+def test_granular_column_scaled_with_fixed_floor():
+    """configs[1] construction at parity size: fixed floor layers, Y0 = 0, mu_d = 0.8, gravity."""
+    wl = W.granular_column(0.35)
+    g = U.gpu_single_pass(wl, dt=1e-4)
+    d = O.single_pass(wl, dt=1e-4, mode="grid")
+    U.compare_single_pass(g, d, wl)
+    fx = wl.fixed.astype(bool)
+    assert np.all(g["v"][:, fx] == 0.0)
+
+
+def test_list_overflow_is_reported():
+    from paper_2603_19764_b200 import binding as B
+    wl = W.elastic_block(10)
+    wl.params.max_neighbors = 16          # far below the ~70 neighbours of the lattice
+    s = B.Sph(wl.params, wl.n)
+    t = s.upload(wl)
+    s.build_neighbors(t, wl.n)
+    assert s.get_counters()["list_overflow"] > 0
