@@ -97,7 +97,7 @@ enum { SPH_C_PAIRS_GATHER = 0,   /* sum_i |gather set(i)|   (true pairs of the d
        SPH_C_TESTS_CULL,         /* candidate pairs the list build tested (sph_build_neighbors) */
        SPH_C_CANDIDATES,         /* sum over tiles of the tile candidate-list lengths           */
        SPH_C_LIST_OVERFLOW,      /* != 0: a list capacity was exceeded, results are incomplete:
-                                    raise sph_params.max_neighbors or set SPH_NO_LISTS           */
+                                    raise sph_params.list_budget or set SPH_NO_LISTS           */
        SPH_C_COUNT };
 
 typedef struct sph_ctx sph_ctx;   /* opaque, library-owned (host memory) */
@@ -120,8 +120,10 @@ typedef struct sph_params {
     int n_materials;           /* 1..SPH_MAX_MATERIALS                                            */
     unsigned flags;            /* SPH_STRENGTH | ...                                              */
     sph_material mat[SPH_MAX_MATERIALS];
-    int max_neighbors;         /* capacity of each particle's neighbour list (symmetric set), rounded
-                                  up to a multiple of 8; <= 0 selects 256                             */
+    int list_budget;           /* 32-bit words of neighbour-mask storage reserved per particle in the
+                                  workspace (pool average; a particle whose chunk sees c candidates uses
+                                  c/32 words); <= 0 selects 48.  Exhaustion is reported in
+                                  SPH_C_LIST_OVERFLOW, never silently truncated.                      */
 } sph_params;
 
 /* Caller-owned particle arrays, each of length n.  For the device entry points all pointers are

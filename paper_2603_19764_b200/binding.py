@@ -44,7 +44,7 @@ class sph_material(C.Structure):
 class sph_params(C.Structure):
     _fields_ = [("kappa", C.c_float), ("alpha", C.c_float), ("beta", C.c_float), ("eps_av", C.c_float),
                 ("eta_C", C.c_float), ("eta_a", C.c_float), ("n_materials", C.c_int), ("flags", C.c_uint),
-                ("mat", sph_material * MAX_MATERIALS), ("max_neighbors", C.c_int)]
+                ("mat", sph_material * MAX_MATERIALS), ("list_budget", C.c_int)]
 
 
 class sph_state(C.Structure):
@@ -109,7 +109,7 @@ def make_params(p) -> sph_params:
     out.kappa, out.alpha, out.beta, out.eps_av = p.kappa, p.alpha, p.beta, p.eps_av
     out.eta_C, out.eta_a = p.eta_C, p.eta_a
     out.flags = int(p.flags)
-    out.max_neighbors = int(getattr(p, "max_neighbors", 0))
+    out.list_budget = int(getattr(p, "list_budget", 0))
     out.n_materials = len(p.materials)
     for k, m in enumerate(p.materials):
         for name, _ in sph_material._fields_:

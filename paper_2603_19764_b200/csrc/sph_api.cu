@@ -34,12 +34,27 @@ static void tree_counts(long long n_max, int *count, int *nlev)
 
 static int kcap_of(const sph_params *p)
 {
-    int k = p->max_neighbors > 0 ? p->max_neighbors : SPH_KCAP_DEFAULT;
-    return (k + 7) & ~7;
+    return p->list_budget > 0 ? p->list_budget : SPH_LIST_BUDGET;
+}
+
+static int sm_count_cached = 0;
+static int device_sm_count()
+{
+    if (sm_count_cached > 0) return sm_count_cached;
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess &&
+        cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+        sm_count_cached = n;
+    else {
+        (void)cudaGetLastError();
+        return 148;                       // sizing on a box without a GPU: B200
+    }
+    return sm_count_cached;
 }
 
 static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap, bool lists)
 {
+    const int sm_count = device_sm_count();
     Bump b{base, 0};
     size_t N = (size_t)(n_max > 0 ? n_max : 1);
     Dev tmp;
@@ -73,14 +88,19 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
     for (int k = 0; k < 9; ++k) o.Cinv[k] = b.take<float>(N);
     for (int k = 0; k < 9; ++k) o.G[k] = b.take<float>(N);
     o.A3 = b.take<float4>(N); o.A4 = b.take<float4>(N); o.A5 = b.take<float4>(N);
-    o.kcap = kcap;
     size_t ntile = (N + SPH_TILE - 1) / SPH_TILE;
     o.tile_ncand = b.take<int>(ntile);
     o.tile_off = b.take<unsigned long long>(ntile);
-    o.cand_cursor = b.take<unsigned long long>(1);
+    o.cand_cursor = b.take<unsigned long long>(2);
+    o.mask_cursor = o.cand_cursor ? o.cand_cursor + 1 : nullptr;
     o.cand_cap = lists ? (unsigned long long)ntile * SPH_TILE_SC : 1;
     o.cand = b.take<unsigned>((size_t)o.cand_cap);
-    o.nbr = b.take<unsigned short>(lists ? N * (size_t)kcap : 8);
+    o.candflag = b.take<unsigned short>((size_t)o.cand_cap);
+    o.tile_nwm = b.take<int>(ntile);
+    o.tile_moff = b.take<unsigned long long>(ntile);
+    o.mask_cap = lists ? (unsigned long long)ntile * SPH_TILE * (unsigned long long)kcap : 4;
+    o.nmask = b.take<unsigned>((size_t)o.mask_cap);
+    o.cull_grid = (int)(ntile < (size_t)(2 * sm_count) ? ntile : (size_t)(2 * sm_count));
     o.bbox = b.take<float>(8);
     o.dt_cur = b.take<float>(1);
     o.dt_next = b.take<float>(1);

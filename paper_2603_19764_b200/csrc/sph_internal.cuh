@@ -15,10 +15,13 @@
 // neighbour-list machinery (sph_lists.cu)
 #define SPH_TILE_CHUNKS 16    // chunks per tile = warps per CTA of the list kernels
 #define SPH_TILE (SPH_TILE_CHUNKS * SPH_CHUNK)
-#define SPH_TILE_SC 4096      // capacity of a tile's candidate list (slots are u16)
+#define SPH_TILE_SC 3072      // candidates per round in k_cull / k_density_l (slots are u16)
 #define SPH_CULL_MAXSRC 1024  // source chunks a tile may accept in the tree walk
-#define SPH_PAIR_SE 2560      // candidates staged per round in the fused pair pass (5 float4 each)
-#define SPH_KCAP_DEFAULT 256  // neighbour-list capacity per particle
+#define SPH_PAIR_SE 2048      // candidates staged per round in the fused pair pass (5 float4 each)
+#define SPH_CULL_MAXPAR 128   // level-1 nodes a tile may expand in the last level of the walk
+#define SPH_WL_CAP 512        // entries of a warp's k -> slot table in the list-driven passes
+#define SPH_MASK_GROUP 16     // mask words a lane holds in shared memory at a time
+#define SPH_LIST_BUDGET 48    // default neighbour-mask words reserved per particle (pool average)
 
 // indices into Resident::s (scalar ping-pong arrays)
 enum {
@@ -78,8 +81,14 @@ struct Dev {
     unsigned long long *tile_off;           // where each tile's candidates start in the pool
     unsigned long long *cand_cursor;        // bump allocator of the pool
     unsigned long long cand_cap;            // pool capacity (entries)
-    unsigned short *nbr;                    // [particle][kcap] slots into the tile candidate list
-    int kcap;
+    unsigned short *candflag;               // parallel to cand: bit w = within reach of chunk w of the tile
+    unsigned *nmask;                        // neighbour masks: per tile [512 targets][nwm words]; bit k of a
+                                            // target's row = the k-th candidate flagged for its chunk
+    int *tile_nwm;                          // words per target in each tile (multiple of 4)
+    unsigned long long *tile_moff;          // where each tile's rows start in nmask
+    unsigned long long *mask_cursor;        // bump allocator of nmask (must follow cand_cursor)
+    unsigned long long mask_cap;            // capacity of nmask (words)
+    int cull_grid;                          // persistent CTAs of k_cull
     // scalars on the device
     float *bbox;                            // 6 floats as ordered ints: lo xyz, hi xyz
     float *dt_cur, *dt_next;                // step in use / CFL step from the last CLOSE

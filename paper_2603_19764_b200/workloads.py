@@ -62,7 +62,7 @@ class Params:
     eta_C: float = 0.3
     eta_a: float = 0.0
     flags: int = FLAG_STRENGTH | FLAG_CORRECTION_TENSOR
-    max_neighbors: int = 0     # neighbour-list capacity of the CUDA path (0 = library default)
+    list_budget: int = 0       # neighbour-mask words per particle of the CUDA path (0 = library default)
     materials: List[Material] = field(default_factory=lambda: [Material()])
 
 

@@ -192,7 +192,7 @@ def test_granular_column_scaled_with_fixed_floor():
 def test_list_overflow_is_reported():
     from paper_2603_19764_b200 import binding as B
     wl = W.elastic_block(10)
-    wl.params.max_neighbors = 16          # far below the ~70 neighbours of the lattice
+    wl.params.list_budget = 2             # far below the ~12 mask words per target this block needs
     s = B.Sph(wl.params, wl.n)
     t = s.upload(wl)
     s.build_neighbors(t, wl.n)
