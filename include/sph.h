@@ -33,8 +33,8 @@ extern "C" {
 #define SPH_PCLIP_GLOBAL          4u  /* clip P >= 0 in the EOS too, not only in Eq. 34 (reading Q8)    */
 #define SPH_JAUMANN_COROTATIONAL  8u  /* flip the sign of the rotation terms of Eq. 13 (reading Q1)     */
 #define SPH_NO_LISTS             16u  /* pair passes walk the chunk tree themselves instead of reading
-                                         the per-particle neighbour lists (the round-1 "v0" kernels, kept
-                                         for A/B measurement and as the path with no capacity limits)       */
+                                         the per-particle neighbour lists (the round-1 "v0" kernels: A/B
+                                         measurement; they also serve tiles over a list capacity)           */
 #define SPH_MORTON_ORDER         32u  /* sort by Morton (Z-order) keys instead of Hilbert keys (A/B
                                          measurement; results do not depend on the order)                  */
 
@@ -96,8 +96,9 @@ enum { SPH_C_PAIRS_GATHER = 0,   /* sum_i |gather set(i)|   (true pairs of the d
        SPH_C_CFALLBACK,          /* particles whose C fell back to 1                             */
        SPH_C_TESTS_CULL,         /* candidate pairs the list build tested (sph_build_neighbors) */
        SPH_C_CANDIDATES,         /* sum over tiles of the tile candidate-list lengths           */
-       SPH_C_LIST_OVERFLOW,      /* != 0: a list capacity was exceeded, results are incomplete:
-                                    raise sph_params.list_budget or set SPH_NO_LISTS           */
+       SPH_C_LIST_OVERFLOW,      /* tiles (256 particles) that exceeded a list capacity and were served
+                                    by the tree-walk kernels instead: results are complete, the step is
+                                    slower; raise sph_params.list_budget if this is large           */
        SPH_C_COUNT };
 
 typedef struct sph_ctx sph_ctx;   /* opaque, library-owned (host memory) */
@@ -120,10 +121,10 @@ typedef struct sph_params {
     int n_materials;           /* 1..SPH_MAX_MATERIALS                                            */
     unsigned flags;            /* SPH_STRENGTH | ...                                              */
     sph_material mat[SPH_MAX_MATERIALS];
-    int list_budget;           /* 32-bit words of neighbour-mask storage reserved per particle in the
-                                  workspace (pool average; a particle whose chunk sees c candidates uses
-                                  c/32 words); <= 0 selects 48.  Exhaustion is reported in
-                                  SPH_C_LIST_OVERFLOW, never silently truncated.                      */
+    int list_budget;           /* neighbour-list capacity: a quarter of the longest neighbour list a
+                                  particle may have (8 bytes of workspace per particle and unit);
+                                  <= 0 selects 64 (256 neighbours).  Tiles that need more are served by
+                                  the tree-walk kernels and counted in SPH_C_LIST_OVERFLOW.           */
 } sph_params;
 
 /* Caller-owned particle arrays, each of length n.  For the device entry points all pointers are

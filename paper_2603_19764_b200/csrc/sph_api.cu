@@ -32,9 +32,10 @@ static void tree_counts(long long n_max, int *count, int *nlev)
     *nlev = L + 1;
 }
 
-static int kcap_of(const sph_params *p)
+static int kcap_of(const sph_params *p)          // row-groups of the neighbour lists reserved per chunk
 {
-    return p->list_budget > 0 ? p->list_budget : SPH_LIST_BUDGET;
+    int r = p->list_budget > 0 ? p->list_budget : SPH_ROWS_DEFAULT;
+    return r > 16000 ? 16000 : r;                 // rowptr entries are 16-bit
 }
 
 static int sm_count_cached = 0;
@@ -87,20 +88,20 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
     for (int k = 0; k < 9; ++k) o.F[k] = b.take<float>(N);
     for (int k = 0; k < 9; ++k) o.Cinv[k] = b.take<float>(N);
     for (int k = 0; k < 9; ++k) o.G[k] = b.take<float>(N);
-    o.A3 = b.take<float4>(N); o.A4 = b.take<float4>(N); o.A5 = b.take<float4>(N);
+    o.B3 = b.take<float4>(N); o.B4 = b.take<float4>(N); o.B5 = b.take<float>(N);
     size_t ntile = (N + SPH_TILE - 1) / SPH_TILE;
+    size_t nchunk = (N + SPH_CHUNK - 1) / SPH_CHUNK;
     o.tile_ncand = b.take<int>(ntile);
     o.tile_off = b.take<unsigned long long>(ntile);
-    o.cand_cursor = b.take<unsigned long long>(2);
-    o.mask_cursor = o.cand_cursor ? o.cand_cursor + 1 : nullptr;
-    o.cand_cap = lists ? (unsigned long long)ntile * SPH_TILE_SC : 1;
+    o.tile_flag = b.take<unsigned char>(ntile);
+    o.cand_cursor = b.take<unsigned long long>(1);
+    o.cand_cap = lists ? (unsigned long long)ntile * (2 * SPH_SE) : 1;   // pool: twice the one-round average
     o.cand = b.take<unsigned>((size_t)o.cand_cap);
-    o.candflag = b.take<unsigned short>((size_t)o.cand_cap);
-    o.tile_nwm = b.take<int>(ntile);
-    o.tile_moff = b.take<unsigned long long>(ntile);
-    o.mask_cap = lists ? (unsigned long long)ntile * SPH_TILE * (unsigned long long)kcap : 4;
-    o.nmask = b.take<unsigned>((size_t)o.mask_cap);
-    o.cull_grid = (int)(ntile < (size_t)(2 * sm_count) ? ntile : (size_t)(2 * sm_count));
+    o.rows_cap = kcap;
+    o.rowptr = b.take<unsigned short>(lists ? nchunk * (SPH_MAXROUND + 1) : 1);
+    o.nlist = b.take<uint2>(lists ? nchunk * (size_t)kcap * 32 : 1);
+    o.cull_grid = (int)ntile;
+    o.walk_grid = 2 * sm_count;
     o.bbox = b.take<float>(8);
     o.dt_cur = b.take<float>(1);
     o.dt_next = b.take<float>(1);
@@ -226,7 +227,7 @@ extern "C" int sph_density(sph_ctx *c)
     if (!c) return SPH_EINVAL;
     if (!c->resident) return SPH_EORDER;
     PassTimer t(c, SPH_T_DENSITY);
-    int rc = c->use_lists ? sph_launch_density_l(c) : sph_launch_density(c);
+    int rc = c->use_lists ? sph_launch_density_l(c) : sph_launch_density(c, false);
     if (rc) return rc;
     c->have_density = true;
     c->have_predict = c->have_grad = c->have_force = false;
@@ -238,7 +239,7 @@ extern "C" int sph_gradients(sph_ctx *c)
     if (!c) return SPH_EINVAL;
     if (!c->have_predict) return SPH_EORDER;
     PassTimer t(c, SPH_T_GRADIENT);
-    int rc = c->use_lists ? sph_launch_pair_l(c, true, false) : sph_launch_pair(c, true, false);
+    int rc = c->use_lists ? sph_launch_pair_l(c, true, false) : sph_launch_pair(c, true, false, false);
     if (rc) return rc;
     c->have_grad = true;
     return SPH_OK;
@@ -249,7 +250,7 @@ extern "C" int sph_forces(sph_ctx *c)
     if (!c) return SPH_EINVAL;
     if (!c->have_predict) return SPH_EORDER;
     PassTimer t(c, SPH_T_FORCE);
-    int rc = c->use_lists ? sph_launch_pair_l(c, false, true) : sph_launch_pair(c, false, true);
+    int rc = c->use_lists ? sph_launch_pair_l(c, false, true) : sph_launch_pair(c, false, true, false);
     if (rc) return rc;
     c->have_force = true;
     return SPH_OK;
@@ -295,7 +296,7 @@ static int derivative_passes(sph_ctx *c)
     const bool strength = (c->p.flags & SPH_STRENGTH) != 0;
     {
         PassTimer t(c, SPH_T_FORCE);
-        rc = c->use_lists ? sph_launch_pair_l(c, strength, true) : sph_launch_pair(c, strength, true);
+        rc = c->use_lists ? sph_launch_pair_l(c, strength, true) : sph_launch_pair(c, strength, true, false);
         if (rc) return rc;
         c->have_force = true;
         c->have_grad = strength;
@@ -463,7 +464,7 @@ extern "C" int sph_get_neighbors(sph_ctx *c, int which, int *counts, const long 
     if (!c || !counts || (which != SPH_GATHER && which != SPH_SYMMETRIC) || (list && !offsets)) return SPH_EINVAL;
     if (!c->resident) return SPH_EORDER;
     return c->use_lists ? sph_launch_neighbors_l(c, which, counts, offsets, list)
-                        : sph_launch_neighbors(c, which, counts, offsets, list);
+                        : sph_launch_neighbors(c, which, counts, offsets, list, false);
 }
 
 extern "C" int sph_get_timings(sph_ctx *c, float *ms, int n)

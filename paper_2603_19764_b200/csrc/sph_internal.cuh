@@ -13,15 +13,14 @@
 #define SPH_NPP 21            // scalar (4-byte) resident arrays that are permuted at re-sort
 
 // neighbour-list machinery (sph_lists.cu)
-#define SPH_TILE_CHUNKS 16    // chunks per tile = warps per CTA of the list kernels
+#define SPH_TILE_CHUNKS 8     // chunks per tile = warps per CTA of the list kernels
 #define SPH_TILE (SPH_TILE_CHUNKS * SPH_CHUNK)
-#define SPH_TILE_SC 3072      // candidates per round in k_cull / k_density_l (slots are u16)
+#define SPH_SE 1632           // candidates staged per round; the cull, density and pair kernels agree on it
+#define SPH_MAXROUND 15       // rounds a tile may need (more: the tile falls back to the tree-walk kernels)
 #define SPH_CULL_MAXSRC 1024  // source chunks a tile may accept in the tree walk
-#define SPH_PAIR_SE 2048      // candidates staged per round in the fused pair pass (5 float4 each)
 #define SPH_CULL_MAXPAR 128   // level-1 nodes a tile may expand in the last level of the walk
-#define SPH_WL_CAP 512        // entries of a warp's k -> slot table in the list-driven passes
-#define SPH_MASK_GROUP 16     // mask words a lane holds in shared memory at a time
-#define SPH_LIST_BUDGET 48    // default neighbour-mask words reserved per particle (pool average)
+#define SPH_GCAP 256          // entries of a quarter-warp's candidate table in k_cull
+#define SPH_ROWS_DEFAULT 64   // default row-groups (4 neighbours per lane each) reserved per chunk
 
 // indices into Resident::s (scalar ping-pong arrays)
 enum {
@@ -74,21 +73,21 @@ struct Dev {
     double *rho64;                          // fp64 density for the EOS (see k_density)
     int *ngather, *nsym;
     float *F[9], *Cinv[9], *G[9];
-    float4 *A3, *A4, *A5;                   // packed pair-pass operands (see k_predict)
+    float4 *B3, *B4;                        // packed pair-pass operands (see k_predict):
+    float *B5;                              //   B3 = {rho, c, w, st_xx}, B4 = {st_yy, st_zz, st_xy, st_xz}, B5 = st_yz
     // neighbour lists (sph_lists.cu)
     int *tile_ncand;                        // candidates per tile
-    unsigned *cand;                         // candidate pool: global indices, tile after tile
+    unsigned *cand;                         // candidate pool: global indices, tile after tile, ascending per tile
     unsigned long long *tile_off;           // where each tile's candidates start in the pool
     unsigned long long *cand_cursor;        // bump allocator of the pool
     unsigned long long cand_cap;            // pool capacity (entries)
-    unsigned short *candflag;               // parallel to cand: bit w = within reach of chunk w of the tile
-    unsigned *nmask;                        // neighbour masks: per tile [512 targets][nwm words]; bit k of a
-                                            // target's row = the k-th candidate flagged for its chunk
-    int *tile_nwm;                          // words per target in each tile (multiple of 4)
-    unsigned long long *tile_moff;          // where each tile's rows start in nmask
-    unsigned long long *mask_cursor;        // bump allocator of nmask (must follow cand_cursor)
-    unsigned long long mask_cap;            // capacity of nmask (words)
+    uint2 *nlist;                           // [chunk][row-group][lane]: 4 x u16 per lane = byte offsets (slot * 16)
+                                            // into the round's staged arrays; 0xFFFF = no entry
+    int rows_cap;                           // row-groups reserved per chunk
+    unsigned short *rowptr;                 // [chunk][SPH_MAXROUND + 1]: first row-group of each round
+    unsigned char *tile_flag;               // != 0: the tile exceeded a capacity; the tree-walk kernels serve it
     int cull_grid;                          // persistent CTAs of k_cull
+    int walk_grid;                          // persistent CTAs of the tree-walk kernels when they serve flagged tiles
     // scalars on the device
     float *bbox;                            // 6 floats as ordered ints: lo xyz, hi xyz
     float *dt_cur, *dt_next;                // step in use / CFL step from the last CLOSE
@@ -131,14 +130,14 @@ size_t sph_cub_temp_bytes(long long n_max);
 int sph_launch_ingest(sph_ctx *c, const sph_state *st, long long n);
 int sph_launch_resort(sph_ctx *c);
 int sph_launch_tree(sph_ctx *c);
-int sph_launch_density(sph_ctx *c);
-int sph_launch_pair(sph_ctx *c, bool grad, bool force);
+int sph_launch_density(sph_ctx *c, bool flagged_only);
+int sph_launch_pair(sph_ctx *c, bool grad, bool force, bool flagged_only);
 int sph_launch_predict(sph_ctx *c);
 int sph_launch_close(sph_ctx *c, int phase, float dt, bool dt_from_device);
 int sph_launch_kick_drift(sph_ctx *c, float dt);
 int sph_launch_get_field(sph_ctx *c, const float *src, float *dst, int as_int);
 int sph_launch_get_position(sph_ctx *c, int comp, float *dst);
-int sph_launch_neighbors(sph_ctx *c, int which, int *counts, const long long *offsets, int *list);
+int sph_launch_neighbors(sph_ctx *c, int which, int *counts, const long long *offsets, int *list, bool flagged_only);
 int sph_launch_download(sph_ctx *c, sph_state *st);
 int sph_launch_cull(sph_ctx *c);
 int sph_launch_density_l(sph_ctx *c);

@@ -1,75 +1,98 @@
-// sph_lists.cu -- "v1" neighbour machinery: cull ONCE per step into compact lists, then let the
-// pair passes evaluate true pairs only.
+// sph_lists.cu -- neighbour lists: cull ONCE per step into explicit per-particle lists, then let the
+// pair passes evaluate true pairs only, one lane per target, with no search work in their inner loop.
 //
-//   tile        = 16 consecutive chunks = 512 Hilbert-consecutive targets = one CTA of 16 warps.
-//   k_cull      : persistent CTAs, one tile at a time:
+//   tile        = 8 consecutive chunks = 256 Hilbert-consecutive targets = one CTA of 8 warps.
+//   k_cull      : one CTA per tile:
 //                 (A) breadth-first walk of the chunk tree by all warps; every particle of the accepted
-//                     source chunks is tested against the tile's 16 chunk boxes; the survivors are
-//                     compacted into the tile CANDIDATE LIST (global indices, ascending) together with
-//                     a 16-bit FLAG word (bit w: within reach of chunk w of the tile);
-//                 (B) warp w runs the candidates flagged for its chunk, in slot order, past its 32
-//                     targets (exact fp32 predicate, reading Q4).  The k-th flagged candidate is bit k
-//                     of each target's NEIGHBOUR MASK: a dense bitmask (~18 % set, ~14 words per
-//                     target) emitted word by word straight from the test loop -- no append, no decode,
-//                     no per-particle capacity.  The symmetric set, self excluded.
-//   k_density_l : stages {x,y,z,m} of the tile's candidates in shared memory (coalesced gathers of
-//                 index runs); every warp rebuilds its k -> slot table from the flags, then every lane
-//                 walks the set bits of its own mask.  The gather set is the subset of the symmetric
-//                 set with r2 < H_i^2, plus the self term.
-//   k_pair_l    : same with the five float4 operand streams of the fused gradient + force pass.
+//                     source chunks is tested against the tile's chunk boxes; the survivors form the tile
+//                     CANDIDATE LIST (global indices, ascending), split into ROUNDS of SPH_SE slots, each
+//                     with a 32-bit flag word (bit 4w+g: within reach of the 8 targets of quarter g of
+//                     warp w);
+//                 (B) every quarter-warp runs the candidates flagged for it past its 8 targets (exact
+//                     fp32 predicate, reading Q4) and appends each hit to the target's NEIGHBOUR LIST:
+//                     the symmetric set, self excluded, as 16-bit byte offsets (slot * 16) into the
+//                     round's staged arrays, stored transposed ([chunk][row-group][lane], 4 entries per
+//                     lane per row-group) so that a warp reads one coalesced 256-byte row-group per four
+//                     pairs.  Rounds start at a common row-group (rowptr); 0xFFFF pads.
+//   k_density_l : stages {x,y,z,m} of the round's candidates in shared memory (coalesced gathers of index
+//                 runs) and walks the lists; the gather set is the subset with r2 < H_i^2, plus self.
+//   k_pair_l    : same with the 17 floats per source of the fused gradient + force pass.
+//   A tile that exceeds any capacity (tree-walk frontier, candidate pool, rounds, list rows) is FLAGGED
+//   and served by the tree-walk kernels of sph_pair.cu instead: slower, never wrong.
 //
-// Evidence for this design: profiles/r01_v0_launches_and_pair_kernel.md (candidate hit rate 3.5 %,
-// 18.65 of 32 threads active per instruction in the broadcast-tile kernels) and
-// profiles/r01_cull_iterations.md (append / decode variants of the list build).
+// Evidence for this design: profiles/r01_v0_launches_and_pair_kernel.md (broadcast tiles: candidate hit
+// rate 3.5 %, 18.65 of 32 threads active) and profiles/r01_v1_mask_lists.md (bitmask lists: 83 non-FP
+// instructions per pair, half of the shared-memory wavefronts were bank conflicts).
 #include "sph_internal.cuh"
+#include "sph_pairterm.cuh"
 
-#define WC2_SIGMA 3.3422538049298023f
 #define FULL 0xffffffffu
+#define ROWPTR_STRIDE (SPH_MAXROUND + 1)
 
-__device__ __forceinline__ bool box_reach_sym(float4 lo, float4 hi, float3 tlo, float3 thi, float tH)
+__device__ __forceinline__ bool box_reach_sym(float4 lo, float4 hi, float4 tlo, float4 thi)
 {
     float gx = fmaxf(0.f, fmaxf(lo.x - thi.x, tlo.x - hi.x));
     float gy = fmaxf(0.f, fmaxf(lo.y - thi.y, tlo.y - hi.y));
     float gz = fmaxf(0.f, fmaxf(lo.z - thi.z, tlo.z - hi.z));
     float d2 = gx * gx + gy * gy + gz * gz;
-    float R = fmaxf(lo.w, tH);
+    float R = fmaxf(lo.w, tlo.w);
     return d2 <= R * R * 1.00001f;        // conservative against the rounding of the exact predicate
+}
+
+__device__ __forceinline__ bool point_reach(float4 lo, float4 hi, float x, float y, float z, float Hj)
+{
+    float gx = fmaxf(0.f, fmaxf(lo.x - x, x - hi.x));
+    float gy = fmaxf(0.f, fmaxf(lo.y - y, y - hi.y));
+    float gz = fmaxf(0.f, fmaxf(lo.z - z, z - hi.z));
+    float d2 = gx * gx + gy * gy + gz * gz;
+    float R = fmaxf(lo.w, Hj);
+    return d2 <= R * R * 1.00001f;
 }
 
 // ------------------------------------------------------------------------------------------
 // k_cull
 // ------------------------------------------------------------------------------------------
 struct CullSmem {
-    float4 pos[SPH_TILE_SC];             // x, y, z, H^2 of the candidates of the current round
-    unsigned short flag[SPH_TILE_SC];    // bit w: within reach of chunk w of the tile
+    float4 pos[SPH_SE];                  // x, y, z, H^2 of the candidates of the current round
+    unsigned flag[SPH_SE];               // bit 4w+g: within reach of quarter g of warp w
     unsigned chunks[SPH_CULL_MAXSRC];    // frontier / accepted source chunks, ascending
     unsigned next[SPH_CULL_MAXSRC];      // next frontier
     unsigned mask[SPH_CULL_MAXSRC];      // surviving lanes (children / particles) of each entry
     unsigned off[SPH_CULL_MAXSRC];       // exclusive prefix of popc(mask)
-    unsigned short cmask[SPH_CULL_MAXSRC];       // chunk boxes of the tile a source chunk box reaches
-    unsigned short ctmp[SPH_CULL_MAXPAR][SPH_ARITY];   // per-child cmask of the leaf expansion
-    float4 blo[SPH_TILE_CHUNKS], bhi[SPH_TILE_CHUNKS];
+    unsigned char cmask[SPH_CULL_MAXSRC];                // chunk boxes of the tile a source chunk box reaches
+    unsigned char ctmp[SPH_CULL_MAXPAR][SPH_ARITY];      // per-child cmask of the leaf expansion
+    float4 blo[SPH_TILE_CHUNKS], bhi[SPH_TILE_CHUNKS];   // chunk boxes (lo.w = max H)
+    float4 glo[4 * SPH_TILE_CHUNKS], ghi[4 * SPH_TILE_CHUNKS];   // quarter-warp boxes
     float4 tlo, thi;                     // tile box (tlo.w = max H)
     unsigned selfslot[SPH_TILE];         // slot of each target of the tile in its own candidate list
-    unsigned wcount[SPH_TILE_CHUNKS];    // candidates flagged for each chunk of the tile
-    int nsrc, ntotal, nfront, overflow, nwm;
-    unsigned long long cand_off, mask_off;
+    unsigned short gl[SPH_TILE_CHUNKS][4][SPH_GCAP];     // per quarter-warp: slots still to test, ascending
+    int nsrc, ntotal, nfront, overflow;
+    unsigned long long cand_off;
 };
 
 // bits w of `among` whose chunk box is within reach of the point (x,y,z) with support Hj
-__device__ __forceinline__ unsigned reach_flags(const CullSmem &sm, unsigned among, float x, float y, float z, float Hj)
+__device__ __forceinline__ unsigned reach_chunks(const CullSmem &sm, unsigned among, float x, float y, float z, float Hj)
 {
     unsigned f = 0;
     while (among) {
         int w = __ffs(among) - 1;
         among &= among - 1;
-        float4 lo = sm.blo[w], hi = sm.bhi[w];
-        float gx = fmaxf(0.f, fmaxf(lo.x - x, x - hi.x));
-        float gy = fmaxf(0.f, fmaxf(lo.y - y, y - hi.y));
-        float gz = fmaxf(0.f, fmaxf(lo.z - z, z - hi.z));
-        float d2 = gx * gx + gy * gy + gz * gz;
-        float R = fmaxf(lo.w, Hj);
-        if (d2 <= R * R * 1.00001f) f |= 1u << w;
+        if (point_reach(sm.blo[w], sm.bhi[w], x, y, z, Hj)) f |= 1u << w;
+    }
+    return f;
+}
+
+// bits 4w+g: chunk box w passes AND the box of its quarter g passes
+__device__ __forceinline__ unsigned reach_groups(const CullSmem &sm, unsigned among, float x, float y, float z, float Hj)
+{
+    unsigned f = 0;
+    while (among) {
+        int w = __ffs(among) - 1;
+        among &= among - 1;
+        if (!point_reach(sm.blo[w], sm.bhi[w], x, y, z, Hj)) continue;
+#pragma unroll
+        for (int g = 0; g < 4; ++g)
+            if (point_reach(sm.glo[4 * w + g], sm.ghi[4 * w + g], x, y, z, Hj)) f |= 1u << (4 * w + g);
     }
     return f;
 }
@@ -95,15 +118,38 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     extern __shared__ __align__(16) unsigned char smem_raw[];
     CullSmem &sm = *reinterpret_cast<CullSmem *>(smem_raw);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
     for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
     const int chunk0 = tile * SPH_TILE_CHUNKS;
     const int nch = min(SPH_TILE_CHUNKS, d.nchunk - chunk0);
 
+    // ---- per-target state, chunk and quarter-warp boxes --------------------------------------------
+    const long long i = (long long)tile * SPH_TILE + threadIdx.x;
+    const bool valid = warp < nch && i < d.n;
+    const float4 pi = valid ? d.r.pm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+    const float Hi = sph_H(kappa, valid ? d.r.vh[i].w : 1.f);
+    const float H2i = valid ? __fmul_rn(Hi, Hi) : -1.f;
+    {
+        float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, Hm = 0.f;
+        if (valid) { lo[0] = hi[0] = pi.x; lo[1] = hi[1] = pi.y; lo[2] = hi[2] = pi.z; Hm = Hi; }
+#pragma unroll
+        for (int o = 4; o > 0; o >>= 1) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                lo[a] = fminf(lo[a], __shfl_xor_sync(FULL, lo[a], o));
+                hi[a] = fmaxf(hi[a], __shfl_xor_sync(FULL, hi[a], o));
+            }
+            Hm = fmaxf(Hm, __shfl_xor_sync(FULL, Hm, o));
+        }
+        if ((lane & 7) == 0) {
+            sm.glo[4 * warp + (lane >> 3)] = make_float4(lo[0], lo[1], lo[2], Hm);
+            sm.ghi[4 * warp + (lane >> 3)] = make_float4(hi[0], hi[1], hi[2], 0.f);
+        }
+    }
     if (threadIdx.x < nch) {
         sm.blo[threadIdx.x] = d.tree.lo[0][chunk0 + threadIdx.x];
         sm.bhi[threadIdx.x] = d.tree.hi[0][chunk0 + threadIdx.x];
     }
-    if (threadIdx.x < SPH_TILE_CHUNKS) sm.wcount[threadIdx.x] = 0u;
     if (threadIdx.x == 0) sm.overflow = 0;
     sm.selfslot[threadIdx.x] = 0xffffffffu;
     __syncthreads();
@@ -133,9 +179,9 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     __syncthreads();
 
     // ---- A1: breadth-first walk of the chunk tree by all warps (one parent per warp, one child per
-    //          lane).  A source chunk is accepted only if its box reaches one of the tile's chunk boxes.
-    const float3 tlo = make_float3(sm.tlo.x, sm.tlo.y, sm.tlo.z), thi = make_float3(sm.thi.x, sm.thi.y, sm.thi.z);
-    const float tH = sm.tlo.w;
+    //          lane).  A node is kept only if its box reaches one of the tile's CHUNK boxes: a tile that
+    //          straddles a gap of the space-filling curve has a huge union box but small chunk boxes.
+    const float4 tlo = sm.tlo, thi = sm.thi;
     for (int L = d.tree.nlev - 1; L >= 0; --L) {
         const int nf = sm.nfront;
         for (int k = warp; k < nf; k += SPH_TILE_CHUNKS) {
@@ -145,16 +191,12 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             bool pass = false;
             if (lane < cnt) {
                 float4 clo = d.tree.lo[L][first + lane], chi = d.tree.hi[L][first + lane];
-                pass = box_reach_sym(clo, chi, tlo, thi, tH);
-                if (pass && L == 0) {
-                    for (int w = 0; w < nch; ++w) {
-                        float4 tl = sm.blo[w], th = sm.bhi[w];
-                        if (box_reach_sym(clo, chi, make_float3(tl.x, tl.y, tl.z), make_float3(th.x, th.y, th.z), tl.w))
-                            cm |= 1u << w;
-                    }
+                if (box_reach_sym(clo, chi, tlo, thi)) {
+                    for (int w = 0; w < nch; ++w)
+                        if (box_reach_sym(clo, chi, sm.blo[w], sm.bhi[w])) cm |= 1u << w;
                     pass = cm != 0;
-                    sm.ctmp[k][lane] = (unsigned short)cm;
                 }
+                if (L == 0 && k < SPH_CULL_MAXPAR) sm.ctmp[k][lane] = (unsigned char)cm;
             }
             unsigned m = __ballot_sync(FULL, pass);
             if (lane == 0) sm.mask[k] = m;
@@ -171,7 +213,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
         for (int k = warp; k < nf; k += SPH_TILE_CHUNKS) {
             unsigned m = sm.mask[k];
             if ((m >> lane) & 1u) {
-                int o = (int)sm.off[k] + __popc(m & ((1u << lane) - 1u));
+                int o = (int)sm.off[k] + __popc(m & lt);
                 if (o < cap) {
                     sm.next[o] = sm.chunks[k] * SPH_ARITY + (unsigned)lane;
                     if (L == 0) sm.cmask[o] = sm.ctmp[k][lane];
@@ -184,172 +226,166 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     }
     const int nsrc = sm.nfront;
 
-    // ---- A2: which particles of the accepted source chunks reach a chunk box of the tile, and how
-    //          many candidates each chunk of the tile will see (-> length of its mask rows) ----------
+    // ---- A2: which particles of the accepted source chunks reach a chunk box of the tile ------------
     for (int k = warp; k < nsrc; k += SPH_TILE_CHUNKS) {
         long long j = (long long)sm.chunks[k] * SPH_CHUNK + lane;
         unsigned f = 0;
-        unsigned cm = sm.cmask[k];
         if (j < d.n) {
             float4 q = d.r.pm[j];
-            f = reach_flags(sm, cm, q.x, q.y, q.z, sph_H(kappa, d.r.vh[j].w));
+            f = reach_chunks(sm, sm.cmask[k], q.x, q.y, q.z, sph_H(kappa, d.r.vh[j].w));
         }
         unsigned m = __ballot_sync(FULL, f != 0);
         if (lane == 0) sm.mask[k] = m;
-        while (cm) {
-            int w = __ffs(cm) - 1;
-            cm &= cm - 1;
-            unsigned c = __popc(__ballot_sync(FULL, (f >> w) & 1u));
-            if (lane == 0 && c) atomicAdd(&sm.wcount[w], c);
-        }
     }
     __syncthreads();
     if (warp == 0) {
         int total = scan_popc(sm.mask, sm.off, nsrc, lane);
-        unsigned wc = lane < SPH_TILE_CHUNKS ? sm.wcount[lane] : 0u;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) wc = max(wc, __shfl_xor_sync(FULL, wc, o));
         if (lane == 0) {
-            unsigned long long nwm = (unsigned long long)((((wc + 31u) >> 5) + 3u) & ~3u);   // words per target
             unsigned long long co = atomicAdd(d.cand_cursor, (unsigned long long)total);
-            unsigned long long mo = atomicAdd(d.mask_cursor, nwm * SPH_TILE);
-            if (co + (unsigned long long)total > d.cand_cap) { sm.overflow |= 2; total = 0; co = 0; nwm = 0; }
-            if (mo + nwm * SPH_TILE > d.mask_cap) { sm.overflow |= 4; total = 0; nwm = 0; mo = 0; }
+            if (co + (unsigned long long)total > d.cand_cap) sm.overflow |= 2;
+            if (total > SPH_MAXROUND * SPH_SE) sm.overflow |= 4;
             sm.ntotal = total;
-            sm.nwm = (int)nwm;
             sm.cand_off = co;
-            sm.mask_off = mo;
-            d.tile_ncand[tile] = total;
-            d.tile_off[tile] = co;
-            d.tile_nwm[tile] = (int)nwm;
-            d.tile_moff[tile] = mo;
-            atomicAdd(&d.counters[SPH_C_CANDIDATES], (unsigned long long)total);
-            if (sm.overflow) atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], (unsigned long long)sm.overflow);
         }
     }
     __syncthreads();
+    if (sm.overflow) {                                 // flagged before any list was written
+        if (threadIdx.x == 0) {
+            d.tile_flag[tile] = 1;
+            d.tile_ncand[tile] = 0;
+            d.tile_off[tile] = 0;
+            atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], 1ull);
+        }
+        if (valid) d.nsym[i] = 0;
+        __syncthreads();
+        continue;
+    }
     const int ntotal = sm.ntotal;
-    const int nwm = sm.nwm;
     unsigned *cand = d.cand + sm.cand_off;
-    unsigned short *cflag = d.candflag + sm.cand_off;
+    if (threadIdx.x == 0) {
+        d.tile_ncand[tile] = ntotal;
+        d.tile_off[tile] = sm.cand_off;
+        atomicAdd(&d.counters[SPH_C_CANDIDATES], (unsigned long long)ntotal);
+    }
 
-    // ---- per-target state for phase B -------------------------------------------------------------
-    const long long i = (long long)tile * SPH_TILE + threadIdx.x;
-    const bool valid = warp < nch && i < d.n;
-    float4 pi = valid ? d.r.pm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
-    float Hi = sph_H(kappa, valid ? d.r.vh[i].w : 1.f);
-    const float H2i = valid ? __fmul_rn(Hi, Hi) : -1.f;
-    const unsigned wbit = 1u << warp;
-    uint4 *mrow = reinterpret_cast<uint4 *>(d.nmask + sm.mask_off + (size_t)threadIdx.x * nwm);
+    // ---- per-lane list state --------------------------------------------------------------------------
+    const int chunk = chunk0 + warp;
+    uint2 *lp = d.nlist + ((size_t)(warp < nch ? chunk : chunk0) * d.rows_cap) * 32 + lane;
+    unsigned short *rp = d.rowptr + (size_t)(warp < nch ? chunk : chunk0) * ROWPTR_STRIDE;
+    const int ncap = d.rows_cap * 4;
+    int n = 0, nhit = 0;                  // entries written (padding included) / true neighbours
+    unsigned w0 = 0, w1 = 0;              // the row-group being filled
     unsigned long long tests = 0;
-    int nsym = 0;
-    int kk = 0;                           // running index of this warp's flagged candidates (uniform)
-    unsigned hits = 0;
-    uint4 acc = make_uint4(0, 0, 0, 0);
-    const int nvalid = __popc(__ballot_sync(FULL, valid));
+    const int g = lane >> 3;
+    if (warp < nch && lane == 0) rp[0] = 0;
 
-    for (int r0 = 0; r0 < ntotal; r0 += SPH_TILE_SC) {
-        const int nr = min(SPH_TILE_SC, ntotal - r0);
+    int round = 0;
+    for (int r0 = 0; r0 < ntotal; r0 += SPH_SE, ++round) {
+        const int nr = min(SPH_SE, ntotal - r0);
         // ---- A3: compact this round's survivors into shared memory and the global candidate list
         for (int k = warp; k < nsrc; k += SPH_TILE_CHUNKS) {
             unsigned m = sm.mask[k];
             int o = (int)sm.off[k];
             if (o >= r0 + nr || o + 32 <= r0) continue;
             if (!((m >> lane) & 1u)) continue;
-            int slot = o + __popc(m & ((1u << lane) - 1u)) - r0;
+            int slot = o + __popc(m & lt) - r0;
             if (slot < 0 || slot >= nr) continue;
             long long j = (long long)sm.chunks[k] * SPH_CHUNK + lane;
             float4 q = d.r.pm[j];
             float Hj = sph_H(kappa, d.r.vh[j].w);
-            unsigned short f = (unsigned short)reach_flags(sm, sm.cmask[k], q.x, q.y, q.z, Hj);
             sm.pos[slot] = make_float4(q.x, q.y, q.z, __fmul_rn(Hj, Hj));
-            sm.flag[slot] = f;
+            sm.flag[slot] = reach_groups(sm, sm.cmask[k], q.x, q.y, q.z, Hj);
             cand[r0 + slot] = (unsigned)j;
-            cflag[r0 + slot] = f;
             long long rel = j - (long long)tile * SPH_TILE;
             if (rel >= 0 && rel < SPH_TILE) sm.selfslot[rel] = (unsigned)(r0 + slot);
         }
         __syncthreads();
-        // ---- B: the k-th candidate flagged for this warp's chunk is bit k of each target's mask -------
-        const int self = (int)sm.selfslot[threadIdx.x] - r0;       // self exclusion (j != i)
-        for (int base = 0; base < nr; base += 32) {
-            int s = base + lane;
-            unsigned m = __ballot_sync(FULL, s < nr && (sm.flag[s] & wbit));
-            tests += (unsigned long long)__popc(m);
-            while (m) {
-                int b = __ffs(m) - 1;
-                m &= m - 1;
-                float4 q = sm.pos[base + b];
-                float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
-                if (r2 < fmaxf(H2i, q.w) && base + b != self) hits |= 1u << (kk & 31);
-                ++kk;
-                if ((kk & 31) == 0) {                                // a word is complete (uniform branch)
-                    hits = valid ? hits : 0u;
-                    nsym += __popc(hits);
-                    int wi = ((kk - 1) >> 5) & 3;
-                    if (wi == 0) acc.x = hits; else if (wi == 1) acc.y = hits; else if (wi == 2) acc.z = hits; else acc.w = hits;
-                    if (wi == 3) { if (warp < nch && nwm) mrow[(kk - 1) >> 7] = acc; acc = make_uint4(0, 0, 0, 0); }
-                    hits = 0;
+        if (warp < nch) {
+            // ---- B: quarter g of this warp tests the candidates flagged for it, in slot order ---------
+            const int self = (int)sm.selfslot[threadIdx.x] - r0;       // self exclusion (j != i)
+            const int fshift = 4 * warp;
+            unsigned short(*gl)[SPH_GCAP] = sm.gl[warp];
+            int base = 0;
+            while (base < nr) {
+                int c0 = 0, c1 = 0, c2 = 0, c3 = 0;
+                while (base < nr && max(max(c0, c1), max(c2, c3)) + 32 <= SPH_GCAP) {
+                    const int s = base + lane;
+                    const unsigned f = s < nr ? (sm.flag[s] >> fshift) & 15u : 0u;
+                    const unsigned m0 = __ballot_sync(FULL, f & 1u), m1 = __ballot_sync(FULL, f & 2u),
+                                   m2 = __ballot_sync(FULL, f & 4u), m3 = __ballot_sync(FULL, f & 8u);
+                    if (f & 1u) gl[0][c0 + __popc(m0 & lt)] = (unsigned short)s;
+                    if (f & 2u) gl[1][c1 + __popc(m1 & lt)] = (unsigned short)s;
+                    if (f & 4u) gl[2][c2 + __popc(m2 & lt)] = (unsigned short)s;
+                    if (f & 8u) gl[3][c3 + __popc(m3 & lt)] = (unsigned short)s;
+                    c0 += __popc(m0); c1 += __popc(m1); c2 += __popc(m2); c3 += __popc(m3);
+                    base += 32;
                 }
+                __syncwarp();
+                const int gcnt = g == 0 ? c0 : (g == 1 ? c1 : (g == 2 ? c2 : c3));
+                const int mycnt = valid ? gcnt : 0;
+                const int cmax = max(max(c0, c1), max(c2, c3));
+                const unsigned short *mygl = gl[g];
+                for (int k = 0; k < cmax; ++k) {
+                    const bool act = k < mycnt;
+                    const int slot = act ? (int)mygl[k] : 0;
+                    const float4 q = sm.pos[slot];
+                    const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
+                    tests += act ? 1ull : 0ull;
+                    if (act && r2 < fmaxf(H2i, q.w) && slot != self) {
+                        ++nhit;
+                        if (n < ncap) {
+                            const unsigned v = ((unsigned)slot << 4) << ((n & 1) << 4);
+                            if (n & 2) w1 |= v; else w0 |= v;
+                            ++n;
+                            if ((n & 3) == 0) {
+                                lp[(size_t)((n >> 2) - 1) * 32] = make_uint2(w0, w1);
+                                w0 = w1 = 0u;
+                            }
+                        } else {
+                            sm.overflow = 8;          // list rows exhausted: the tile falls back
+                        }
+                    }
+                }
+                __syncwarp();
             }
+            // ---- end of the round: flush, pad every lane to the warp's longest list -------------------
+            const int G = (n + 3) >> 2;
+            if (n & 3) {
+                const int rem = n & 3;
+                if (rem == 1) { w0 |= 0xffff0000u; w1 = 0xffffffffu; }
+                else if (rem == 2) { w1 = 0xffffffffu; }
+                else { w1 |= 0xffff0000u; }
+                lp[(size_t)(G - 1) * 32] = make_uint2(w0, w1);
+                w0 = w1 = 0u;
+            }
+            int Gmax = G;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) Gmax = max(Gmax, __shfl_xor_sync(FULL, Gmax, o));
+            for (int gg = G; gg < Gmax; ++gg) lp[(size_t)gg * 32] = make_uint2(0xffffffffu, 0xffffffffu);
+            n = Gmax * 4;
+            if (lane == 0) rp[round + 1] = (unsigned short)Gmax;
         }
         __syncthreads();
     }
-    if (kk & 127) {                                                  // partial last word / last group of four
-        hits = valid ? hits : 0u;
-        nsym += __popc(hits);
-        int wi = (kk >> 5) & 3;
-        if (kk & 31) { if (wi == 0) acc.x = hits; else if (wi == 1) acc.y = hits; else if (wi == 2) acc.z = hits; else acc.w = hits; }
-        if (warp < nch && nwm) mrow[kk >> 7] = acc;
+    if (valid) d.nsym[i] = nhit;
+    if (warp < nch) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) tests += __shfl_xor_sync(FULL, tests, o);
+        if (lane == 0) atomicAdd(&d.counters[SPH_C_TESTS_CULL], tests);
     }
-    if (valid) d.nsym[i] = nwm ? nsym : 0;
-    if (lane == 0 && warp < nch) atomicAdd(&d.counters[SPH_C_TESTS_CULL], tests * (unsigned long long)nvalid);
+    if (threadIdx.x == 0) {
+        d.tile_flag[tile] = sm.overflow ? 1 : 0;
+        if (sm.overflow) atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], 1ull);
+    }
     __syncthreads();
     }   // tile loop
 }
 
-// ------------------------------------------------------------------------------------------
-// shared by the list-driven passes: k -> slot table of one warp, and the per-lane bit walk
-// ------------------------------------------------------------------------------------------
-// Appends to wl[] the slots (relative to r0) of this round's candidates in [base, nr) that are flagged
-// for this warp, until the table is full or the round ends; returns the new base.  Warp-uniform.
-__device__ __forceinline__ int build_wl(const unsigned short *s_flag, int nr, int base,
-                                        unsigned wbit, unsigned short *wl, int &nwl, int lane)
+// entry e (0..3) of a row-group word pair
+__device__ __forceinline__ unsigned list_entry(uint2 w, int e)
 {
-    nwl = 0;
-    while (base < nr && nwl + 32 <= SPH_WL_CAP) {
-        int s = base + lane;
-        bool f = s < nr && (s_flag[s] & wbit);
-        unsigned m = __ballot_sync(FULL, f);
-        if (f) wl[nwl + __popc(m & ((1u << lane) - 1u))] = (unsigned short)s;
-        nwl += __popc(m);
-        base += 32;
-    }
-    __syncwarp();
-    return base;
-}
-
-// Copies words [wg0, wg0 + SPH_MASK_GROUP) of this thread's mask row into its private column of the
-// shared scratch msk[word][thread] (bank-conflict free, read back only by the same thread), restricted
-// to bits k in [klo, khi).  Rows are multiples of four words, 16-byte aligned.
-__device__ __forceinline__ void load_mask_group(const unsigned *__restrict__ mrow, int nwm, int wg0, int klo, int khi,
-                                                unsigned *msk)
-{
-#pragma unroll
-    for (int q = 0; q < SPH_MASK_GROUP / 4; ++q) {
-        int w0 = wg0 + 4 * q;
-        uint4 v = make_uint4(0u, 0u, 0u, 0u);
-        if (w0 < nwm) v = *reinterpret_cast<const uint4 *>(mrow + w0);
-        unsigned w[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            int lo = klo - ((w0 + e) << 5), hi = khi - ((w0 + e) << 5);
-            unsigned x = w[e];
-            if (lo > 0) x = lo >= 32 ? 0u : (x & ~((1u << lo) - 1u));
-            if (hi < 32) x = hi <= 0 ? 0u : (x & ((1u << hi) - 1u));
-            msk[(4 * q + e) * SPH_TILE + threadIdx.x] = x;
-        }
-    }
+    const unsigned x = (e & 2) ? w.y : w.x;
+    return (e & 1) ? (x >> 16) : (x & 0xffffu);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -359,14 +395,13 @@ __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4 *s_pm = reinterpret_cast<float4 *>(smem_raw);
-    unsigned short *s_wl = reinterpret_cast<unsigned short *>(s_pm + SPH_TILE_SC);
-    unsigned *msk = reinterpret_cast<unsigned *>(s_wl + SPH_TILE_CHUNKS * SPH_WL_CAP);
-    unsigned short *s_flag = reinterpret_cast<unsigned short *>(msk + SPH_MASK_GROUP * SPH_TILE);
     const int tile = blockIdx.x;
+    if (d.tile_flag[tile]) return;
     const int ncand = d.tile_ncand[tile];
     const unsigned *cand = d.cand + d.tile_off[tile];
-    const unsigned short *cflag = d.candflag + d.tile_off[tile];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int chunk = tile * SPH_TILE_CHUNKS + warp;
+    const bool haschunk = chunk < d.nchunk;
     const long long i = (long long)tile * SPH_TILE + threadIdx.x;
     const bool valid = i < d.n;
     float4 pi = valid ? d.r.pm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -375,76 +410,56 @@ __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
     const float H2i = __fmul_rn(Hi, Hi);
     const float invH = 1.f / Hi;
     const double invHd = 1.0 / ((double)kappa * (double)hi);
-    const int nwm = d.tile_nwm[tile];
-    const unsigned *mrow = d.nmask + d.tile_moff[tile] + (size_t)threadIdx.x * nwm;
-    unsigned short *wl = s_wl + warp * SPH_WL_CAP;
-    const unsigned wbit = 1u << warp;
+    const double pxd = (double)pi.x, pyd = (double)pi.y, pzd = (double)pi.z;
+    const uint2 *lp = d.nlist + ((size_t)(haschunk ? chunk : 0) * d.rows_cap) * 32 + lane;
+    const unsigned short *rp = d.rowptr + (size_t)(haschunk ? chunk : 0) * ROWPTR_STRIDE;
     // self term: q = 0, t = 1
     double sum = (double)pi.w;
     float sh = 3.f * pi.w;
     int ng = 1, ntest = 1;
-    int kstart = 0;
-    for (int r0 = 0; r0 < ncand || r0 == 0; r0 += SPH_TILE_SC) {
-        const int nr = min(SPH_TILE_SC, ncand - r0);
-        for (int s = threadIdx.x; s < nr; s += SPH_TILE) {
-            s_pm[s] = d.r.pm[cand[r0 + s]];
-            s_flag[s] = cflag[r0 + s];
-        }
+    int round = 0;
+    for (int r0 = 0; r0 < ncand; r0 += SPH_SE, ++round) {
+        const int nr = min(SPH_SE, ncand - r0);
+        for (int s = threadIdx.x; s < nr; s += SPH_TILE) s_pm[s] = d.r.pm[cand[r0 + s]];
         __syncthreads();
-        int base = 0;
-        while (base < nr) {
-            int nwl;
-            base = build_wl(s_flag, nr, base, wbit, wl, nwl, lane);
-            const int klo = kstart, khi = kstart + nwl;      // warp-uniform: the walk below votes
-            // per-lane walk over the set bits of its mask words, one group of SPH_MASK_GROUP words at a
-            // time: `bits` is the word in hand, `nxt` the next one (read one refill ahead from the
-            // thread's shared-memory column); the refill is predicated, not a divergent branch
-            for (int wg0 = (klo >> 5) & ~3; (wg0 << 5) < khi; wg0 += SPH_MASK_GROUP) {
-            load_mask_group(mrow, nwm, wg0, klo, valid ? khi : klo, msk);   // padding lanes: all zero
-            int wcur = wg0;
-            const int wend = min(wg0 + SPH_MASK_GROUP, (khi + 31) >> 5);
-            unsigned bits = msk[threadIdx.x];
-            unsigned nxt = wcur + 1 < wend ? msk[SPH_TILE + threadIdx.x] : 0u;
-            while (true) {
-                if (bits == 0u && wcur < wend) {
-                    ++wcur;
-                    bits = nxt;
-                    nxt = wcur + 1 < wend ? msk[(wcur + 1 - wg0) * SPH_TILE + threadIdx.x] : 0u;
-                }
-                if (!__any_sync(FULL, wcur < wend)) break;
-                if (bits == 0u) continue;
-                int b = __ffs(bits) - 1;
-                bits &= bits - 1;
-                float4 q = s_pm[wl[(wcur << 5) + b - klo]];
-                ++ntest;
-                float dx = __fsub_rn(pi.x, q.x), dy = __fsub_rn(pi.y, q.y), dz = __fsub_rn(pi.z, q.z);
-                float r2 = sph_r2(dx, dy, dz);
-                if (r2 < H2i) {
-                    float rinv = rsqrtf(fmaxf(r2, 1.0e-37f));
-                    float r = r2 * rinv;
-                    float qq = r * invH;
-                    float t = fmaxf(0.f, 1.f - qq);
-                    float t3 = t * t * t;
-                    sh = fmaf(q.w * t3, fmaf(qq, fmaf(-32.f, qq, 9.f), 3.f), sh);
-                    double ex = (double)pi.x - (double)q.x, ey = (double)pi.y - (double)q.y, ez = (double)pi.z - (double)q.z;
-                    double r2d = fma(ex, ex, fma(ey, ey, ez * ez));
-                    double r0d = (double)r;
-                    double rd = fma(fma(-r0d, r0d, r2d), 0.5 * (double)rinv, r0d);
-                    double qd = rd * invHd;
-                    double td = fmax(0.0, 1.0 - qd);
-                    double t2 = td * td;
-                    sum = fma((double)q.w * t2 * t2, fma(4.0, qd, 1.0), sum);
-                    ++ng;
+        if (haschunk) {
+            const int g0 = rp[round], g1 = rp[round + 1];
+            uint2 nxt = g0 < g1 ? lp[(size_t)g0 * 32] : make_uint2(0xffffffffu, 0xffffffffu);
+            for (int gq = g0; gq < g1; ++gq) {
+                const uint2 w = nxt;
+                if (gq + 1 < g1) nxt = lp[(size_t)(gq + 1) * 32];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    const unsigned off = list_entry(w, e);
+                    if (off == 0xffffu) continue;
+                    const float4 q = *reinterpret_cast<const float4 *>(smem_raw + off);
+                    ++ntest;
+                    float dx = __fsub_rn(pi.x, q.x), dy = __fsub_rn(pi.y, q.y), dz = __fsub_rn(pi.z, q.z);
+                    float r2 = sph_r2(dx, dy, dz);
+                    if (r2 < H2i) {
+                        float rinv = rsqrtf(fmaxf(r2, 1.0e-37f));
+                        float r = r2 * rinv;
+                        float qq = r * invH;
+                        float t = fmaxf(0.f, 1.f - qq);
+                        float t3 = t * t * t;
+                        sh = fmaf(q.w * t3, fmaf(qq, fmaf(-32.f, qq, 9.f), 3.f), sh);
+                        double ex = pxd - (double)q.x, ey = pyd - (double)q.y, ez = pzd - (double)q.z;
+                        double r2d = fma(ex, ex, fma(ey, ey, ez * ez));
+                        double r0d = (double)r;
+                        double rd = fma(fma(-r0d, r0d, r2d), 0.5 * (double)rinv, r0d);
+                        double qd = rd * invHd;
+                        double td = fmax(0.0, 1.0 - qd);
+                        double t2 = td * td;
+                        sum = fma((double)q.w * t2 * t2, fma(4.0, qd, 1.0), sum);
+                        ++ng;
+                    }
                 }
             }
-            }   // mask groups
-            kstart += nwl;
-            __syncwarp();
         }
         __syncthreads();
     }
     if (valid) {
-        float kw = WC2_SIGMA * invH * invH * invH;
+        float kw = SPH_WC2_SIGMA * invH * invH * invH;
         double rhod = 3.3422538049298023 * invHd * invHd * invHd * sum;
         float rho = (float)rhod;
         d.rho64[i] = rhod;
@@ -465,144 +480,81 @@ __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
 }
 
 // ------------------------------------------------------------------------------------------
-// S4 + S5 from the lists.  Equations and operand packing: see k_pair in sph_pair.cu.
-// The tile's candidates are staged in rounds of SPH_PAIR_SE slots.
+// S4 + S5 from the lists.  Equations and operand packing: sph_pairterm.cuh.
+// Shared memory: four float4 arrays and one float array of SPH_SE slots (68 B per candidate; the
+// hydro-only variant stages the first three arrays only).
 // ------------------------------------------------------------------------------------------
-template <bool GRAD, bool FORCE>
-__global__ void __launch_bounds__(SPH_TILE) k_pair_l(Dev d, DevParams p)
+template <bool GRAD, bool FORCE, bool TENSOR>
+__global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float4 *s1 = reinterpret_cast<float4 *>(smem_raw);
-    float4 *s2 = s1 + SPH_PAIR_SE, *s3 = s2 + SPH_PAIR_SE, *s4 = s3 + SPH_PAIR_SE, *s5 = s4 + SPH_PAIR_SE;
-    unsigned short *s_wl = reinterpret_cast<unsigned short *>(s5 + SPH_PAIR_SE);
-    unsigned *msk = reinterpret_cast<unsigned *>(s_wl + SPH_TILE_CHUNKS * SPH_WL_CAP);
-    unsigned short *s_flag = reinterpret_cast<unsigned short *>(msk + SPH_MASK_GROUP * SPH_TILE);
+    unsigned char *s1 = smem_raw, *s2 = s1 + SPH_SE * 16, *s3 = s2 + SPH_SE * 16, *s4 = s3 + SPH_SE * 16,
+                  *s5 = s4 + SPH_SE * 16;
     const int tile = blockIdx.x;
+    if (d.tile_flag[tile]) return;
     const int ncand = d.tile_ncand[tile];
     const unsigned *cand = d.cand + d.tile_off[tile];
-    const unsigned short *cflag = d.candflag + d.tile_off[tile];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int chunk = tile * SPH_TILE_CHUNKS + warp;
+    const bool haschunk = chunk < d.nchunk;
     const long long i = (long long)tile * SPH_TILE + threadIdx.x;
     const bool valid = i < d.n;
-    const long long il = valid ? i : 0;
-    const float4 pi = d.r.pm[il], vi = d.r.vh[il], a3 = d.A3[il], a4 = d.A4[il], a5 = d.A5[il];
-    const float invHi = a3.w, Ki = a3.z, rhoi = a3.x, ci = a3.y, hi = vi.w;
-    const float invm = 1.f / pi.w;
-    const float wKi = a5.z * invm;
-    const float kxx = a4.x * invm, kyy = a4.y * invm, kzz = a4.z * invm, kxy = a4.w * invm, kxz = a5.x * invm,
-                kyz = a5.y * invm;
-    const int nwm = d.tile_nwm[tile];
-    const unsigned *mrow = d.nmask + d.tile_moff[tile] + (size_t)threadIdx.x * nwm;
-    unsigned short *wl = s_wl + warp * SPH_WL_CAP;
-    const unsigned wbit = 1u << warp;
+    const PairTarget t = pair_target_load(d, valid ? i : 0, p.kappa);
+    PairConst kc;
+    kc.beta = p.beta; kc.alpha2 = 0.5f * p.alpha; kc.eps = p.eps_av; kc.hk = 0.5f / p.kappa;
+    const uint2 *lp = d.nlist + ((size_t)(haschunk ? chunk : 0) * d.rows_cap) * 32 + lane;
+    const unsigned short *rp = d.rowptr + (size_t)(haschunk ? chunk : 0) * ROWPTR_STRIDE;
+    PairAcc A;
+    pair_acc_zero(A);
+    int cnt = 0;
 
-    float F[9], C[6];
-#pragma unroll
-    for (int k = 0; k < 9; ++k) F[k] = 0.f;
-#pragma unroll
-    for (int k = 0; k < 6; ++k) C[k] = 0.f;
-    float ax = 0.f, ay = 0.f, az = 0.f, du = 0.f, mumax = 0.f;
-    int kstart = 0, cnt = 0;
-
-    for (int r0 = 0; r0 < ncand || r0 == 0; r0 += SPH_PAIR_SE) {
-        const int nr = min(SPH_PAIR_SE, ncand - r0);
+    int round = 0;
+    for (int r0 = 0; r0 < ncand; r0 += SPH_SE, ++round) {
+        const int nr = min(SPH_SE, ncand - r0);
         for (int s = threadIdx.x; s < nr; s += SPH_TILE) {
-            unsigned j = cand[r0 + s];
-            s1[s] = d.r.pm[j];
-            s2[s] = d.r.vh[j];
-            s3[s] = d.A3[j];
-            s4[s] = d.A4[j];
-            s5[s] = d.A5[j];
-            s_flag[s] = cflag[r0 + s];
+            const unsigned j = cand[r0 + s];
+            float4 vh = d.r.vh[j];
+            vh.w = sph_H(p.kappa, vh.w);
+            reinterpret_cast<float4 *>(s1)[s] = d.r.pm[j];
+            reinterpret_cast<float4 *>(s2)[s] = vh;
+            reinterpret_cast<float4 *>(s3)[s] = d.B3[j];
+            if (TENSOR) {
+                reinterpret_cast<float4 *>(s4)[s] = d.B4[j];
+                reinterpret_cast<float *>(s5)[s] = d.B5[j];
+            }
         }
         __syncthreads();
-        int base = 0;
-        while (base < nr) {
-            int nwl;
-            base = build_wl(s_flag, nr, base, wbit, wl, nwl, lane);
-            const int klo = kstart, khi = kstart + nwl;      // warp-uniform: the walk below votes
-            for (int wg0 = (klo >> 5) & ~3; (wg0 << 5) < khi; wg0 += SPH_MASK_GROUP) {
-            load_mask_group(mrow, nwm, wg0, klo, valid ? khi : klo, msk);   // padding lanes: all zero
-            int wcur = wg0;
-            const int wend = min(wg0 + SPH_MASK_GROUP, (khi + 31) >> 5);
-            unsigned bits = msk[threadIdx.x];
-            unsigned nxt = wcur + 1 < wend ? msk[SPH_TILE + threadIdx.x] : 0u;
-            while (true) {
-                if (bits == 0u && wcur < wend) {
-                    ++wcur;
-                    bits = nxt;
-                    nxt = wcur + 1 < wend ? msk[(wcur + 1 - wg0) * SPH_TILE + threadIdx.x] : 0u;
-                }
-                if (!__any_sync(FULL, wcur < wend)) break;
-                if (bits == 0u) continue;
-                int b = __ffs(bits) - 1;
-                bits &= bits - 1;
-                const int slot = wl[(wcur << 5) + b - klo];
-                ++cnt;
-                const float4 q1 = s1[slot], q2 = s2[slot], q3 = s3[slot], q4 = s4[slot], q5 = s5[slot];
-                float dx = __fsub_rn(pi.x, q1.x), dy = __fsub_rn(pi.y, q1.y), dz = __fsub_rn(pi.z, q1.z);
-                float r2 = sph_r2(dx, dy, dz);
-                float r = r2 * rsqrtf(fmaxf(r2, 1.0e-37f));
-                float ti = fmaxf(0.f, 1.f - r * invHi);
-                float tj = fmaxf(0.f, 1.f - r * q3.w);
-                float ti3 = ti * ti * ti, tj3 = tj * tj * tj;
-                float mj = q1.w;
-                float dvx = vi.x - q2.x, dvy = vi.y - q2.y, dvz = vi.z - q2.z;
-                float wi_ = mj * ti3;
-                if (GRAD) {
-                    float s = 0.5f * fmaf(wi_, wKi, q5.z * tj3);
-                    float sx = s * dx, sy = s * dy, sz = s * dz;
-                    F[0] = fmaf(dvx, sx, F[0]); F[1] = fmaf(dvx, sy, F[1]); F[2] = fmaf(dvx, sz, F[2]);
-                    F[3] = fmaf(dvy, sx, F[3]); F[4] = fmaf(dvy, sy, F[4]); F[5] = fmaf(dvy, sz, F[5]);
-                    F[6] = fmaf(dvz, sx, F[6]); F[7] = fmaf(dvz, sy, F[7]); F[8] = fmaf(dvz, sz, F[8]);
-                    C[0] = fmaf(dx, sx, C[0]); C[1] = fmaf(dx, sy, C[1]); C[2] = fmaf(dx, sz, C[2]);
-                    C[3] = fmaf(dy, sy, C[3]); C[4] = fmaf(dy, sz, C[4]); C[5] = fmaf(dz, sz, C[5]);
-                }
-                if (FORCE) {
-                    float zx = fmaf(kxx, dx, fmaf(kxy, dy, kxz * dz));
-                    float zy = fmaf(kxy, dx, fmaf(kyy, dy, kyz * dz));
-                    float zz = fmaf(kxz, dx, fmaf(kyz, dy, kzz * dz));
-                    ax = fmaf(-wi_, zx, ax); ay = fmaf(-wi_, zy, ay); az = fmaf(-wi_, zz, az);
-                    du = fmaf(wi_, fmaf(zx, dvx, fmaf(zy, dvy, zz * dvz)), du);
-                    float yx = fmaf(q4.x, dx, fmaf(q4.w, dy, q5.x * dz));
-                    float yy = fmaf(q4.w, dx, fmaf(q4.y, dy, q5.y * dz));
-                    float yz = fmaf(q5.x, dx, fmaf(q5.y, dy, q4.z * dz));
-                    ax = fmaf(-tj3, yx, ax); ay = fmaf(-tj3, yy, ay); az = fmaf(-tj3, yz, az);
-                    float vr = fminf(fmaf(dvx, dx, fmaf(dvy, dy, dvz * dz)), 0.f);
-                    float hb = 0.5f * (hi + q2.w);
-                    float mu = __fdividef(hb * vr, fmaf(p.eps_av * hb, hb, r2));
-                    float Pi = __fdividef(mu * fmaf(p.beta, mu, -p.alpha * 0.5f * (ci + q3.y)), 0.5f * (rhoi + q3.x));
-                    float kk = 0.5f * mj * Pi * fmaf(Ki, ti3, q3.z * tj3);
-                    ax = fmaf(kk, dx, ax); ay = fmaf(kk, dy, ay); az = fmaf(kk, dz, az);
-                    du = fmaf(-0.5f * kk, vr, du);
-                    mumax = fmaxf(mumax, -mu);
+        if (haschunk) {
+            const int g0 = rp[round], g1 = rp[round + 1];
+            uint2 nxt = g0 < g1 ? lp[(size_t)g0 * 32] : make_uint2(0xffffffffu, 0xffffffffu);
+            for (int gq = g0; gq < g1; ++gq) {
+                const uint2 w = nxt;
+                if (gq + 1 < g1) nxt = lp[(size_t)(gq + 1) * 32];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    unsigned off = list_entry(w, e);
+                    const bool v = off != 0xffffu;
+                    off = v ? off : 0u;
+                    cnt += v ? 1 : 0;
+                    const float4 q1 = *reinterpret_cast<const float4 *>(s1 + off);
+                    const float4 q2 = *reinterpret_cast<const float4 *>(s2 + off);
+                    const float4 q3 = *reinterpret_cast<const float4 *>(s3 + off);
+                    float4 q4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                    float q5 = 0.f;
+                    if (TENSOR) {
+                        q4 = *reinterpret_cast<const float4 *>(s4 + off);
+                        q5 = *reinterpret_cast<const float *>(s5 + (off >> 2));
+                    }
+                    pair_term<GRAD, FORCE, TENSOR>(t, kc, A, q1, q2, q3, q4, q5, v);
                 }
             }
-            }   // mask groups
-            kstart += nwl;
-            __syncwarp();
         }
         __syncthreads();
     }
 
-    if (valid) {
-        if (GRAD) {
-#pragma unroll
-            for (int c = 0; c < 9; ++c) d.F[c][i] = F[c];
-            d.Cinv[0][i] = C[0]; d.Cinv[1][i] = C[1]; d.Cinv[2][i] = C[2];
-            d.Cinv[3][i] = C[1]; d.Cinv[4][i] = C[3]; d.Cinv[5][i] = C[4];
-            d.Cinv[6][i] = C[2]; d.Cinv[7][i] = C[4]; d.Cinv[8][i] = C[5];
-        }
-        if (FORCE) {
-            d.a[0][i] = ax + d.r.s[PP_G + 0][i];
-            d.a[1][i] = ay + d.r.s[PP_G + 1][i];
-            d.a[2][i] = az + d.r.s[PP_G + 2][i];
-            d.dudt[i] = du;
-            d.mumax[i] = mumax;
-        }
-    }
+    if (valid) pair_store<GRAD, FORCE>(d, i, A);
     if (FORCE) {
-        unsigned long long hits = (unsigned long long)cnt;
+        unsigned long long hits = valid ? (unsigned long long)cnt : 0ull;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) hits += __shfl_xor_sync(FULL, hits, o);
         if (lane == 0) {
@@ -620,14 +572,14 @@ __global__ void __launch_bounds__(256) k_neighbors_l(Dev d, float kappa, int *co
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= d.n) return;
-    const unsigned *orig = (const unsigned *)d.r.s[PP_ORIG];
     const int tile = (int)(i / SPH_TILE);
-    const int tid = (int)(i - (long long)tile * SPH_TILE);
-    const unsigned wbit = 1u << (tid >> 5);
+    if (d.tile_flag[tile]) return;
+    const unsigned *orig = (const unsigned *)d.r.s[PP_ORIG];
+    const int chunk = (int)(i / SPH_CHUNK), lane = (int)(i % SPH_CHUNK);
     const int ncand = d.tile_ncand[tile];
     const unsigned *cand = d.cand + d.tile_off[tile];
-    const unsigned short *cflag = d.candflag + d.tile_off[tile];
-    const unsigned *mrow = d.nmask + d.tile_moff[tile] + (size_t)tid * d.tile_nwm[tile];
+    const uint2 *lp = d.nlist + ((size_t)chunk * d.rows_cap) * 32 + lane;
+    const unsigned short *rp = d.rowptr + (size_t)chunk * ROWPTR_STRIDE;
     unsigned oi = orig[i];
     long long base = list ? offsets[oi] : 0;
     float4 pi = d.r.pm[i];
@@ -638,21 +590,24 @@ __global__ void __launch_bounds__(256) k_neighbors_l(Dev d, float kappa, int *co
         if (list) list[base] = (int)oi;
         out = 1;
     }
-    int k = 0;
-    for (int s = 0; s < ncand; ++s) {
-        if (!(cflag[s] & wbit)) continue;
-        bool set = (mrow[k >> 5] >> (k & 31)) & 1u;
-        ++k;
-        if (!set) continue;
-        unsigned j = cand[s];
-        bool hit = true;
-        if (!SYM) {
-            float4 q = d.r.pm[j];
-            hit = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z)) < H2i;
-        }
-        if (hit) {
-            if (list) list[base + out] = (int)orig[j];
-            ++out;
+    int round = 0;
+    for (int r0 = 0; r0 < ncand; r0 += SPH_SE, ++round) {
+        for (int gq = rp[round]; gq < rp[round + 1]; ++gq) {
+            const uint2 w = lp[(size_t)gq * 32];
+            for (int e = 0; e < 4; ++e) {
+                const unsigned off = list_entry(w, e);
+                if (off == 0xffffu) continue;
+                unsigned j = cand[r0 + (int)(off >> 4)];
+                bool hit = true;
+                if (!SYM) {
+                    float4 q = d.r.pm[j];
+                    hit = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z)) < H2i;
+                }
+                if (hit) {
+                    if (list) list[base + out] = (int)orig[j];
+                    ++out;
+                }
+            }
         }
     }
     counts[oi] = out;
@@ -671,12 +626,12 @@ int sph_launch_cull(sph_ctx *c)
 {
     Dev &d = c->d;
     SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_TESTS_CULL], 0, 3 * sizeof(unsigned long long), c->stream));
-    SPH_CUDA(c, cudaMemsetAsync(d.cand_cursor, 0, 2 * sizeof(unsigned long long), c->stream));
+    SPH_CUDA(c, cudaMemsetAsync(d.cand_cursor, 0, sizeof(unsigned long long), c->stream));
     if (d.n == 0) return SPH_OK;
     int rc = set_smem(c, (const void *)k_cull, sizeof(CullSmem));
     if (rc) return rc;
     int ntile = sph_div_up(d.nchunk, SPH_TILE_CHUNKS);
-    k_cull<<<ntile < d.cull_grid ? ntile : d.cull_grid, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, ntile);
+    k_cull<<<ntile, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, ntile);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
@@ -688,13 +643,23 @@ int sph_launch_density_l(sph_ctx *c)
     SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_PAIRS_GATHER], 0, sizeof(unsigned long long), c->stream));
     SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_TESTS_DENSITY], 0, sizeof(unsigned long long), c->stream));
     if (d.n == 0) return SPH_OK;
-    size_t bytes = (size_t)SPH_TILE_SC * sizeof(float4) + (size_t)SPH_TILE_CHUNKS * SPH_WL_CAP * sizeof(unsigned short) +
-                   (size_t)SPH_MASK_GROUP * SPH_TILE * sizeof(unsigned) + (size_t)SPH_TILE_SC * sizeof(unsigned short);
+    size_t bytes = (size_t)SPH_SE * sizeof(float4);
     int rc = set_smem(c, (const void *)k_density_l, bytes);
     if (rc) return rc;
     k_density_l<<<sph_div_up(d.nchunk, SPH_TILE_CHUNKS), SPH_TILE, bytes, c->stream>>>(d, c->p.kappa);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
+    return sph_launch_density(c, true);               // the flagged tiles, if any
+}
+
+template <bool GRAD, bool FORCE, bool TENSOR>
+static int launch_pair_l(sph_ctx *c)
+{
+    Dev &d = c->d;
+    size_t bytes = (size_t)SPH_SE * (TENSOR ? 68 : 48);
+    int rc = set_smem(c, (const void *)k_pair_l<GRAD, FORCE, TENSOR>, bytes);
+    if (rc) return rc;
+    k_pair_l<GRAD, FORCE, TENSOR><<<sph_div_up(d.nchunk, SPH_TILE_CHUNKS), SPH_TILE, bytes, c->stream>>>(d, c->p);
     return SPH_OK;
 }
 
@@ -706,23 +671,16 @@ int sph_launch_pair_l(sph_ctx *c, bool grad, bool force)
         SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_TESTS_FORCE], 0, sizeof(unsigned long long), c->stream));
     }
     if (d.n == 0) return SPH_OK;
-    size_t bytes = (size_t)5 * SPH_PAIR_SE * sizeof(float4) + (size_t)SPH_TILE_CHUNKS * SPH_WL_CAP * sizeof(unsigned short) +
-                   (size_t)SPH_MASK_GROUP * SPH_TILE * sizeof(unsigned) + (size_t)SPH_PAIR_SE * sizeof(unsigned short);
-    dim3 grid(sph_div_up(d.nchunk, SPH_TILE_CHUNKS)), block(SPH_TILE);
+    const bool tensor = (c->p.flags & SPH_STRENGTH) != 0;
     int rc;
-    if (grad && force) {
-        if ((rc = set_smem(c, (const void *)k_pair_l<true, true>, bytes))) return rc;
-        k_pair_l<true, true><<<grid, block, bytes, c->stream>>>(d, c->p);
-    } else if (grad) {
-        if ((rc = set_smem(c, (const void *)k_pair_l<true, false>, bytes))) return rc;
-        k_pair_l<true, false><<<grid, block, bytes, c->stream>>>(d, c->p);
-    } else {
-        if ((rc = set_smem(c, (const void *)k_pair_l<false, true>, bytes))) return rc;
-        k_pair_l<false, true><<<grid, block, bytes, c->stream>>>(d, c->p);
-    }
+    if (grad && force) rc = launch_pair_l<true, true, true>(c);
+    else if (grad) rc = launch_pair_l<true, false, true>(c);
+    else if (tensor) rc = launch_pair_l<false, true, true>(c);
+    else rc = launch_pair_l<false, true, false>(c);
+    if (rc) return rc;
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
-    return SPH_OK;
+    return sph_launch_pair(c, grad, force, true);     // the flagged tiles, if any
 }
 
 int sph_launch_neighbors_l(sph_ctx *c, int which, int *counts, const long long *offsets, int *list)
@@ -734,5 +692,5 @@ int sph_launch_neighbors_l(sph_ctx *c, int which, int *counts, const long long *
     else k_neighbors_l<false><<<nb, 256, 0, c->stream>>>(d, c->p.kappa, counts, offsets, list);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
-    return SPH_OK;
+    return sph_launch_neighbors(c, which, counts, offsets, list, true);
 }

@@ -1,0 +1,150 @@
+// sph_pairterm.cuh -- the arithmetic of one (i, j) pair of the gradient (S4) and force (S5) passes,
+// shared by the list-driven kernel (sph_lists.cu) and the tree-walk kernel (sph_pair.cu).
+//
+// With D(h) = -(dW/dr)/r = K t^3, t = max(0, 1 - r/H), K = 20 SIGMA / H^5 (Wendland C2, reading Q3),
+// grad_i W_ij(h) = -D x_ij, and st = sigma/(Omega rho^2) = (-P delta + S)/(Omega rho^2), w = 1/(Omega rho):
+//   F^{ab}    = +1/2 sum_j m_j (w_i D_i + w_j D_j) v_ij^a x_ij^b                         (Eq. 20)
+//   Cinv^{ab} = +1/2 sum_j m_j (w_i D_i + w_j D_j) x_ij^a x_ij^b                         (Eq. 21)
+//   a_i       = - sum_j m_j [ D_i st_i + D_j st_j ] x_ij + sum_j 1/2 m_j Pi_ij (D_i + D_j) x_ij   (Eq. 4, 7, 18)
+//   du_i/dt   = + sum_j m_j D_i (st_i x_ij).v_ij - sum_j 1/4 m_j Pi_ij (D_i + D_j) v_ij.x_ij      (Eq. 8, 19)
+//   mu_ij     = hbar v_ij.x_ij / (r^2 + eps hbar^2),  Pi_ij = (-alpha cbar mu + beta mu^2)/rhobar  if v_ij.x_ij < 0
+// (Eq. 5-6; means are arithmetic).  The accumulators F and C hold TWICE the sums of
+// Eq. 20-21; the caller halves them once at the end.
+#pragma once
+
+#define SPH_WC2_SIGMA 3.3422538049298023f     // 21 / (2 pi)
+#define SPH_WC2_K20 66.845076098596046f       // 20 * 21 / (2 pi)
+
+struct PairConst {
+    float beta;       // Eq. 5
+    float alpha2;     // alpha / 2: alpha cbar = alpha2 (c_i + c_j)
+    float eps;        // Eq. 6
+    float hk;         // 1 / (2 kappa): hbar = hk (H_i + H_j)
+};
+
+// per-target operands, constant over the neighbour loop
+struct PairTarget {
+    float x, y, z;
+    float vx, vy, vz;
+    float H, invH;    // support radius kappa h_i and its reciprocal
+    float K;          // 20 SIGMA / H_i^5
+    float wK;         // w_i K_i
+    float rho, c;
+    float kxx, kyy, kzz, kxy, kxz, kyz;   // K_i st_i
+};
+
+struct PairAcc {
+    float F[9], C[6];
+    float ax, ay, az, du, mumax;
+};
+
+__device__ __forceinline__ void pair_acc_zero(PairAcc &A)
+{
+#pragma unroll
+    for (int k = 0; k < 9; ++k) A.F[k] = 0.f;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) A.C[k] = 0.f;
+    A.ax = A.ay = A.az = A.du = A.mumax = 0.f;
+}
+
+// q1 = {x, y, z, m}_j   q2 = {vx, vy, vz, H}_j   q3 = {rho, c, w, st_xx}_j   q4 = {st_yy, st_zz, st_xy, st_xz}_j
+// q5 = st_yz_j.  valid == false: the entry contributes nothing (list padding).
+// TENSOR == false (hydro only, S == 0): st is the scalar -P/(Omega rho^2) held in t.kxx / q3.w.
+template <bool GRAD, bool FORCE, bool TENSOR = true>
+__device__ __forceinline__ void pair_term(const PairTarget &t, const PairConst &k, PairAcc &A, float4 q1, float4 q2,
+                                          float4 q3, float4 q4, float q5, bool valid)
+{
+    const float dx = t.x - q1.x, dy = t.y - q1.y, dz = t.z - q1.z;
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    const float r = r2 * rsqrtf(fmaxf(r2, 1.0e-37f));
+    const float invHj = __fdividef(1.f, q2.w);
+    const float ti = fmaxf(0.f, fmaf(-r, t.invH, 1.f));
+    const float tj = fmaxf(0.f, fmaf(-r, invHj, 1.f));
+    const float ti3 = ti * ti * ti, tj3 = tj * tj * tj;
+    const float g2 = invHj * invHj;
+    const float Kj = (SPH_WC2_K20 * invHj) * (g2 * g2);
+    const float mj = valid ? q1.w : 0.f;
+    const float di = mj * ti3;                       // m_j t_i^3       (D_i = K_i t_i^3)
+    const float dj = mj * Kj * tj3;                  // m_j D_j
+    const float dvx = t.vx - q2.x, dvy = t.vy - q2.y, dvz = t.vz - q2.z;
+    if (GRAD) {
+        const float s = fmaf(di, t.wK, dj * q3.z);   // m_j (w_i D_i + w_j D_j)
+        const float sx = s * dx, sy = s * dy, sz = s * dz;
+        A.F[0] = fmaf(dvx, sx, A.F[0]); A.F[1] = fmaf(dvx, sy, A.F[1]); A.F[2] = fmaf(dvx, sz, A.F[2]);
+        A.F[3] = fmaf(dvy, sx, A.F[3]); A.F[4] = fmaf(dvy, sy, A.F[4]); A.F[5] = fmaf(dvy, sz, A.F[5]);
+        A.F[6] = fmaf(dvz, sx, A.F[6]); A.F[7] = fmaf(dvz, sy, A.F[7]); A.F[8] = fmaf(dvz, sz, A.F[8]);
+        A.C[0] = fmaf(dx, sx, A.C[0]); A.C[1] = fmaf(dx, sy, A.C[1]); A.C[2] = fmaf(dx, sz, A.C[2]);
+        A.C[3] = fmaf(dy, sy, A.C[3]); A.C[4] = fmaf(dy, sz, A.C[4]); A.C[5] = fmaf(dz, sz, A.C[5]);
+    }
+    if (FORCE) {
+        const float vx_ = fmaf(dvx, dx, fmaf(dvy, dy, dvz * dz));          // v_ij . x_ij
+        if (TENSOR) {
+            // i side: z = K_i st_i x_ij
+            const float zx = fmaf(t.kxx, dx, fmaf(t.kxy, dy, t.kxz * dz));
+            const float zy = fmaf(t.kxy, dx, fmaf(t.kyy, dy, t.kyz * dz));
+            const float zz = fmaf(t.kxz, dx, fmaf(t.kyz, dy, t.kzz * dz));
+            A.ax = fmaf(-di, zx, A.ax); A.ay = fmaf(-di, zy, A.ay); A.az = fmaf(-di, zz, A.az);
+            A.du = fmaf(di, fmaf(zx, dvx, fmaf(zy, dvy, zz * dvz)), A.du);
+            // j side: y = st_j x_ij
+            const float yx = fmaf(q3.w, dx, fmaf(q4.z, dy, q4.w * dz));
+            const float yy = fmaf(q4.z, dx, fmaf(q4.x, dy, q5 * dz));
+            const float yz = fmaf(q4.w, dx, fmaf(q5, dy, q4.y * dz));
+            A.ax = fmaf(-dj, yx, A.ax); A.ay = fmaf(-dj, yy, A.ay); A.az = fmaf(-dj, yz, A.az);
+        } else {
+            const float si = di * t.kxx;                                     // m_j D_i st_i
+            const float sc = fmaf(dj, q3.w, si);                             // m_j (D_i st_i + D_j st_j)
+            A.ax = fmaf(-sc, dx, A.ax); A.ay = fmaf(-sc, dy, A.ay); A.az = fmaf(-sc, dz, A.az);
+            A.du = fmaf(si, vx_, A.du);
+        }
+        // artificial viscosity (only approaching pairs: min(v.x, 0))
+        float vr = fminf(vx_, 0.f);
+        vr = valid ? vr : 0.f;
+        const float hb = k.hk * (t.H + q2.w);
+        const float mu = __fdividef(hb * vr, fmaf(k.eps * hb, hb, r2));
+        const float P2 = __fdividef(mu * fmaf(k.beta, mu, -k.alpha2 * (t.c + q3.y)), t.rho + q3.x);   // Pi_ij / 2
+        const float kk = P2 * fmaf(t.K, di, dj);     // 1/2 m_j Pi_ij (D_i + D_j)
+        A.ax = fmaf(kk, dx, A.ax); A.ay = fmaf(kk, dy, A.ay); A.az = fmaf(kk, dz, A.az);
+        A.du = fmaf(-0.5f * kk, vr, A.du);
+        A.mumax = fmaxf(A.mumax, -mu);
+    }
+}
+
+// loads the per-target operands (resident arrays of sph_internal.cuh's Dev)
+__device__ __forceinline__ PairTarget pair_target_load(const Dev &d, long long i, float kappa)
+{
+    const float4 pi = d.r.pm[i], vi = d.r.vh[i], b3 = d.B3[i], b4 = d.B4[i];
+    const float b5 = d.B5[i];
+    PairTarget t;
+    t.x = pi.x; t.y = pi.y; t.z = pi.z;
+    t.vx = vi.x; t.vy = vi.y; t.vz = vi.z;
+    t.H = sph_H(kappa, vi.w);
+    t.invH = 1.f / t.H;
+    const float g2 = t.invH * t.invH;
+    t.K = (SPH_WC2_K20 * t.invH) * (g2 * g2);
+    t.wK = b3.z * t.K;
+    t.rho = b3.x; t.c = b3.y;
+    t.kxx = t.K * b3.w; t.kyy = t.K * b4.x; t.kzz = t.K * b4.y;
+    t.kxy = t.K * b4.z; t.kxz = t.K * b4.w; t.kyz = t.K * b5;
+    return t;
+}
+
+template <bool GRAD, bool FORCE>
+__device__ __forceinline__ void pair_store(const Dev &d, long long i, const PairAcc &A)
+{
+    if (GRAD) {
+#pragma unroll
+        for (int c = 0; c < 9; ++c) d.F[c][i] = 0.5f * A.F[c];
+        const float c0 = 0.5f * A.C[0], c1 = 0.5f * A.C[1], c2 = 0.5f * A.C[2], c3 = 0.5f * A.C[3], c4 = 0.5f * A.C[4],
+                    c5 = 0.5f * A.C[5];
+        d.Cinv[0][i] = c0; d.Cinv[1][i] = c1; d.Cinv[2][i] = c2;
+        d.Cinv[3][i] = c1; d.Cinv[4][i] = c3; d.Cinv[5][i] = c4;
+        d.Cinv[6][i] = c2; d.Cinv[7][i] = c4; d.Cinv[8][i] = c5;
+    }
+    if (FORCE) {
+        d.a[0][i] = A.ax + d.r.s[PP_G + 0][i];
+        d.a[1][i] = A.ay + d.r.s[PP_G + 1][i];
+        d.a[2][i] = A.az + d.r.s[PP_G + 2][i];
+        d.dudt[i] = A.du;
+        d.mumax[i] = A.mumax;
+    }
+}

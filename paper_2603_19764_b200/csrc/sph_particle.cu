@@ -33,9 +33,9 @@ __device__ __forceinline__ float plastic_factor(const float S[5], float Y)
 
 // ------------------------------------------------------------------------------------------
 // S3 PREDICT: EOS (reading Q13), Gamma (Eq. 30), Y (Eq. 34-37), S_pred <- f S_pred (Eq. 31,
-// PAPER.md:240), and the packed operands of the pair pass:
-//   A3 = {rho, c, K, 1/H}, A4 = {Sg_xx, Sg_yy, Sg_zz, Sg_xy}, A5 = {Sg_xz, Sg_yz, m w K, H^2}
-//   K = 20 SIGMA / H^5, w = 1/(Omega rho), Sg = m K (-P delta + S_pred)/(Omega rho^2)
+// PAPER.md:240), and the packed operands of the pair pass (sph_pairterm.cuh):
+//   B3 = {rho, c, w, st_xx}, B4 = {st_yy, st_zz, st_xy, st_xz}, B5 = st_yz
+//   w = 1/(Omega rho), st = (-P delta + S_pred)/(Omega rho^2)
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_predict(Dev d, DevParams p)
 {
@@ -61,17 +61,11 @@ __global__ void __launch_bounds__(256) k_predict(Dev d, DevParams p)
     }
     d.P[i] = P; d.cs[i] = cs; d.T[i] = T; d.Gamma[i] = Gam; d.Y[i] = Y;
 
-    float4 pm = d.r.pm[i];
-    float h = d.r.vh[i].w;
-    float H = sph_H(p.kappa, h);
-    float invH = 1.f / H;
-    float invH2 = invH * invH;
-    float K = 20.f * WC2_SIGMA * invH2 * invH2 * invH;
     float w = 1.f / (om * rho);
-    float g = pm.w * K * w / rho;                     // m K / (Omega rho^2)
-    d.A3[i] = make_float4(rho, cs, K, invH);
-    d.A4[i] = make_float4(g * (S[0] - P), g * (S[1] - P), g * (-S[0] - S[1] - P), g * S[2]);
-    d.A5[i] = make_float4(g * S[3], g * S[4], pm.w * w * K, __fmul_rn(H, H));
+    float g = w / rho;                                // 1 / (Omega rho^2)
+    d.B3[i] = make_float4(rho, cs, w, g * (S[0] - P));
+    d.B4[i] = make_float4(g * (S[1] - P), g * (-S[0] - S[1] - P), g * S[2], g * S[3]);
+    d.B5[i] = g * S[4];
 }
 
 // ------------------------------------------------------------------------------------------

@@ -22,7 +22,7 @@ def rows(counts, offsets, lst):
     return [np.sort(lst[offsets[i]:offsets[i + 1]]) for i in range(counts.shape[0])]
 
 
-def gpu_single_pass(wl, dt=None, split=True):
+def gpu_single_pass(wl, dt=None, split=True, allow_fallback=False):
     """Run the BASELINE.json configs[0] pass sequence through the C ABI; returns numpy fields."""
     import torch
     from paper_2603_19764_b200 import binding as B
@@ -47,7 +47,7 @@ def gpu_single_pass(wl, dt=None, split=True):
     for name, nc in (("A", 3), ("V", 3), ("X", 3), ("SPRED", 5), ("S", 5), ("DSDT", 5), ("F", 9), ("CINV", 9), ("G", 9)):
         out[name.lower()] = s.get_fields(name, nc).cpu().numpy()
     out["counters"] = s.get_counters()
-    assert out["counters"]["list_overflow"] == 0, "neighbour-list capacity exceeded"
+    assert allow_fallback or out["counters"]["list_overflow"] == 0, "tiles fell back to the tree-walk kernels"
     out["timings"] = s.get_timings()
     out["_sph"] = s
     torch.cuda.synchronize()

@@ -189,11 +189,13 @@ def test_granular_column_scaled_with_fixed_floor():
     assert np.all(g["v"][:, fx] == 0.0)
 
 
-def test_list_overflow_is_reported():
-    from paper_2603_19764_b200 import binding as B
-    wl = W.elastic_block(10)
-    wl.params.list_budget = 2             # far below the ~12 mask words per target this block needs
-    s = B.Sph(wl.params, wl.n)
-    t = s.upload(wl)
-    s.build_neighbors(t, wl.n)
-    assert s.get_counters()["list_overflow"] > 0
+def test_tiles_over_list_capacity_fall_back_to_the_tree_walk():
+    """A tile whose lists do not fit is flagged (counter) and served by the tree-walk kernels:
+    slower, never wrong."""
+    wl = W.elastic_block(12, h_spread=0.2)
+    wl.params.list_budget = 4             # 16 neighbours per lane; this block needs ~80
+    g = U.gpu_single_pass(wl, allow_fallback=True)
+    assert g["counters"]["list_overflow"] > 0
+    d = O.single_pass(wl)
+    U.compare_single_pass(g, d, wl)
+    _neighbor_sets_equal(g["_sph"], wl)
