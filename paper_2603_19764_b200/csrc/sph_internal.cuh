@@ -17,9 +17,10 @@
 #define SPH_TILE (SPH_TILE_CHUNKS * SPH_CHUNK)
 #define SPH_SE 1632           // candidates staged per round; the cull, density and pair kernels agree on it
 #define SPH_MAXROUND 15       // rounds a tile may need (more: the tile falls back to the tree-walk kernels)
-#define SPH_CULL_MAXSRC 1024  // source chunks a tile may accept in the tree walk
+#define SPH_CULL_MAXSRC 768   // source chunks a tile may accept in the tree walk
 #define SPH_CULL_MAXPAR 128   // level-1 nodes a tile may expand in the last level of the walk
-#define SPH_GCAP 256          // entries of a quarter-warp's candidate table in k_cull
+#define SPH_GCAP 192          // entries of a quarter-warp's candidate table in k_cull (multiple of 32)
+#define SPH_CULL_CFCACHE 128  // source chunks whose per-particle chunk flags are kept between the two passes
 #define SPH_ROWS_DEFAULT 64   // default row-groups (4 neighbours per lane each) reserved per chunk
 
 // indices into Resident::s (scalar ping-pong arrays)

@@ -53,7 +53,8 @@ __device__ __forceinline__ bool point_reach(float4 lo, float4 hi, float x, float
 // k_cull
 // ------------------------------------------------------------------------------------------
 struct CullSmem {
-    float4 pos[SPH_SE];                  // x, y, z, H^2 of the candidates of the current round
+    float4 pos[SPH_SE + 1];              // x, y, z, H^2 of the candidates of the current round; [SPH_SE] is a
+                                         // sentinel no target can reach (pads the quarter-warp tables)
     unsigned flag[SPH_SE];               // bit 4w+g: within reach of quarter g of warp w
     unsigned chunks[SPH_CULL_MAXSRC];    // frontier / accepted source chunks, ascending
     unsigned next[SPH_CULL_MAXSRC];      // next frontier
@@ -61,6 +62,7 @@ struct CullSmem {
     unsigned off[SPH_CULL_MAXSRC];       // exclusive prefix of popc(mask)
     unsigned char cmask[SPH_CULL_MAXSRC];                // chunk boxes of the tile a source chunk box reaches
     unsigned char ctmp[SPH_CULL_MAXPAR][SPH_ARITY];      // per-child cmask of the leaf expansion
+    unsigned char cf[SPH_CULL_CFCACHE][SPH_CHUNK];       // per-particle chunk flags of the first source chunks
     float4 blo[SPH_TILE_CHUNKS], bhi[SPH_TILE_CHUNKS];   // chunk boxes (lo.w = max H)
     float4 glo[4 * SPH_TILE_CHUNKS], ghi[4 * SPH_TILE_CHUNKS];   // quarter-warp boxes
     float4 tlo, thi;                     // tile box (tlo.w = max H)
@@ -82,14 +84,13 @@ __device__ __forceinline__ unsigned reach_chunks(const CullSmem &sm, unsigned am
     return f;
 }
 
-// bits 4w+g: chunk box w passes AND the box of its quarter g passes
-__device__ __forceinline__ unsigned reach_groups(const CullSmem &sm, unsigned among, float x, float y, float z, float Hj)
+// bits 4w+g for the chunks w of `fchunk` (which already passed reach_chunks) whose quarter-g box passes
+__device__ __forceinline__ unsigned reach_groups(const CullSmem &sm, unsigned fchunk, float x, float y, float z, float Hj)
 {
     unsigned f = 0;
-    while (among) {
-        int w = __ffs(among) - 1;
-        among &= among - 1;
-        if (!point_reach(sm.blo[w], sm.bhi[w], x, y, z, Hj)) continue;
+    while (fchunk) {
+        int w = __ffs(fchunk) - 1;
+        fchunk &= fchunk - 1;
 #pragma unroll
         for (int g = 0; g < 4; ++g)
             if (point_reach(sm.glo[4 * w + g], sm.ghi[4 * w + g], x, y, z, Hj)) f |= 1u << (4 * w + g);
@@ -126,7 +127,8 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     // ---- per-target state, chunk and quarter-warp boxes --------------------------------------------
     const long long i = (long long)tile * SPH_TILE + threadIdx.x;
     const bool valid = warp < nch && i < d.n;
-    const float4 pi = valid ? d.r.pm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+    // lanes without a particle sit where every r2 overflows to +inf (and differs from the table sentinel)
+    const float4 pi = valid ? d.r.pm[i] : make_float4(-1.0e30f, -1.0e30f, -1.0e30f, 0.f);
     const float Hi = sph_H(kappa, valid ? d.r.vh[i].w : 1.f);
     const float H2i = valid ? __fmul_rn(Hi, Hi) : -1.f;
     {
@@ -150,7 +152,10 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
         sm.blo[threadIdx.x] = d.tree.lo[0][chunk0 + threadIdx.x];
         sm.bhi[threadIdx.x] = d.tree.hi[0][chunk0 + threadIdx.x];
     }
-    if (threadIdx.x == 0) sm.overflow = 0;
+    if (threadIdx.x == 0) {
+        sm.overflow = 0;
+        sm.pos[SPH_SE] = make_float4(1.0e30f, 1.0e30f, 1.0e30f, -1.f);
+    }
     sm.selfslot[threadIdx.x] = 0xffffffffu;
     __syncthreads();
     if (warp == 0) {                                   // tile box = union of its chunk boxes
@@ -234,6 +239,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             float4 q = d.r.pm[j];
             f = reach_chunks(sm, sm.cmask[k], q.x, q.y, q.z, sph_H(kappa, d.r.vh[j].w));
         }
+        if (k < SPH_CULL_CFCACHE) sm.cf[k][lane] = (unsigned char)f;
         unsigned m = __ballot_sync(FULL, f != 0);
         if (lane == 0) sm.mask[k] = m;
     }
@@ -272,10 +278,23 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     const int chunk = chunk0 + warp;
     uint2 *lp = d.nlist + ((size_t)(warp < nch ? chunk : chunk0) * d.rows_cap) * 32 + lane;
     unsigned short *rp = d.rowptr + (size_t)(warp < nch ? chunk : chunk0) * ROWPTR_STRIDE;
+    uint2 *lpw = lp;                      // where the row-group being filled goes
     const int ncap = d.rows_cap * 4;
-    int n = 0, nhit = 0;                  // entries written (padding included) / true neighbours
-    unsigned w0 = 0, w1 = 0;              // the row-group being filled
-    unsigned long long tests = 0;
+    int n = 0, nhit = 0;                  // entries pushed (padding included) / true neighbours
+    unsigned w0 = 0, w1 = 0;              // the row-group being filled: a 4 x 16-bit shift register
+    unsigned tests = 0;
+    // push one 16-bit entry; a complete row-group goes to memory (rows beyond the capacity are dropped
+    // and the tile is flagged at the end)
+#define LIST_PUSH(v)                                              \
+    do {                                                          \
+        w0 = __byte_perm(w0, w1, 0x5432);                         \
+        w1 = __byte_perm(w1, (v), 0x5432);                        \
+        ++n;                                                      \
+        if ((n & 3) == 0) {                                       \
+            if (n <= ncap) *lpw = make_uint2(w0, w1);             \
+            lpw += 32;                                            \
+        }                                                         \
+    } while (0)
     const int g = lane >> 3;
     if (warp < nch && lane == 0) rp[0] = 0;
 
@@ -294,7 +313,9 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             float4 q = d.r.pm[j];
             float Hj = sph_H(kappa, d.r.vh[j].w);
             sm.pos[slot] = make_float4(q.x, q.y, q.z, __fmul_rn(Hj, Hj));
-            sm.flag[slot] = reach_groups(sm, sm.cmask[k], q.x, q.y, q.z, Hj);
+            const unsigned fc = k < SPH_CULL_CFCACHE ? (unsigned)sm.cf[k][lane]
+                                                     : reach_chunks(sm, sm.cmask[k], q.x, q.y, q.z, Hj);
+            sm.flag[slot] = reach_groups(sm, fc, q.x, q.y, q.z, Hj);
             cand[r0 + slot] = (unsigned)j;
             long long rel = j - (long long)tile * SPH_TILE;
             if (rel >= 0 && rel < SPH_TILE) sm.selfslot[rel] = (unsigned)(r0 + slot);
@@ -322,48 +343,49 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
                 }
                 __syncwarp();
                 const int gcnt = g == 0 ? c0 : (g == 1 ? c1 : (g == 2 ? c2 : c3));
-                const int mycnt = valid ? gcnt : 0;
                 const int cmax = max(max(c0, c1), max(c2, c3));
+                const int cpad = (cmax + 31) & ~31;
+                for (int k = c0 + lane; k < cpad; k += 32) gl[0][k] = (unsigned short)SPH_SE;
+                for (int k = c1 + lane; k < cpad; k += 32) gl[1][k] = (unsigned short)SPH_SE;
+                for (int k = c2 + lane; k < cpad; k += 32) gl[2][k] = (unsigned short)SPH_SE;
+                for (int k = c3 + lane; k < cpad; k += 32) gl[3][k] = (unsigned short)SPH_SE;
+                __syncwarp();
                 const unsigned short *mygl = gl[g];
-                for (int k = 0; k < cmax; ++k) {
-                    const bool act = k < mycnt;
-                    const int slot = act ? (int)mygl[k] : 0;
-                    const float4 q = sm.pos[slot];
-                    const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
-                    tests += act ? 1ull : 0ull;
-                    if (act && r2 < fmaxf(H2i, q.w) && slot != self) {
-                        ++nhit;
-                        if (n < ncap) {
-                            const unsigned v = ((unsigned)slot << 4) << ((n & 1) << 4);
-                            if (n & 2) w1 |= v; else w0 |= v;
-                            ++n;
-                            if ((n & 3) == 0) {
-                                lp[(size_t)((n >> 2) - 1) * 32] = make_uint2(w0, w1);
-                                w0 = w1 = 0u;
-                            }
-                        } else {
-                            sm.overflow = 8;          // list rows exhausted: the tile falls back
-                        }
+                tests += valid ? (unsigned)gcnt : 0u;
+                for (int kb = 0; kb < cmax; kb += 32) {
+                    // 32 candidates of the quarter's table -> one hit bit each
+                    unsigned bits = 0u;
+#pragma unroll
+                    for (int kk = 0; kk < 32; ++kk) {
+                        const int slot = (int)mygl[kb + kk];
+                        const float4 q = sm.pos[slot];
+                        const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
+                        if (r2 < fmaxf(H2i, q.w) && slot != self) bits |= 1u << kk;
+                    }
+                    nhit += __popc(bits);
+                    // every lane appends its own hits, in slot order
+                    while (bits) {
+                        const int b = __ffs(bits) - 1;
+                        bits &= bits - 1u;
+                        const unsigned v = (unsigned)mygl[kb + b] << 4;
+                        LIST_PUSH(v);
                     }
                 }
                 __syncwarp();
             }
             // ---- end of the round: flush, pad every lane to the warp's longest list -------------------
-            const int G = (n + 3) >> 2;
-            if (n & 3) {
-                const int rem = n & 3;
-                if (rem == 1) { w0 |= 0xffff0000u; w1 = 0xffffffffu; }
-                else if (rem == 2) { w1 = 0xffffffffu; }
-                else { w1 |= 0xffff0000u; }
-                lp[(size_t)(G - 1) * 32] = make_uint2(w0, w1);
-                w0 = w1 = 0u;
-            }
+            while (n & 3) LIST_PUSH(0xffffu);
+            const int G = n >> 2;
             int Gmax = G;
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) Gmax = max(Gmax, __shfl_xor_sync(FULL, Gmax, o));
-            for (int gg = G; gg < Gmax; ++gg) lp[(size_t)gg * 32] = make_uint2(0xffffffffu, 0xffffffffu);
+            for (int gg = G; gg < Gmax; ++gg) {
+                if (gg < d.rows_cap) *lpw = make_uint2(0xffffffffu, 0xffffffffu);
+                lpw += 32;
+            }
             n = Gmax * 4;
-            if (lane == 0) rp[round + 1] = (unsigned short)Gmax;
+            if (n > ncap) sm.overflow = 8;            // list rows exhausted: the tile falls back
+            if (lane == 0) rp[round + 1] = (unsigned short)min(Gmax, d.rows_cap);
         }
         __syncthreads();
     }
@@ -371,8 +393,9 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     if (warp < nch) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) tests += __shfl_xor_sync(FULL, tests, o);
-        if (lane == 0) atomicAdd(&d.counters[SPH_C_TESTS_CULL], tests);
+        if (lane == 0) atomicAdd(&d.counters[SPH_C_TESTS_CULL], (unsigned long long)tests);
     }
+#undef LIST_PUSH
     if (threadIdx.x == 0) {
         d.tile_flag[tile] = sm.overflow ? 1 : 0;
         if (sm.overflow) atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], 1ull);
