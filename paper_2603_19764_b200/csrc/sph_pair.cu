@@ -33,15 +33,37 @@ __device__ __forceinline__ bool box_reach(float4 lo, float4 hi, float3 tlo, floa
     return d2 <= R * R * 1.00001f;        // conservative against the rounding of the exact predicate
 }
 
-template <bool SYM, class Leaf>
-__device__ __forceinline__ void walk(const Tree &t, float3 tlo, float3 thi, float tH, unsigned *stack, Leaf &&leaf)
+// EXACT: a node must also be within reach of one of the warp's 32 TARGET PARTICLES (tgt[t] = {x, y, z, H},
+// H < 0: no particle), not only of their bounding box.  Thirty times the work per node, which pays for the
+// chunks this path exists for: a chunk that straddles a gap of the space-filling curve has a box that
+// covers the gap, and the box test alone would accept every source chunk in it.
+template <bool SYM, bool EXACT>
+__device__ __forceinline__ bool node_reach(float4 lo, float4 hi, float3 tlo, float3 thi, float tH, const float4 *tgt)
+{
+    bool pass = box_reach<SYM>(lo, hi, tlo, thi, tH);
+    if (!EXACT || !pass) return pass;
+    for (int t = 0; t < SPH_CHUNK; ++t) {
+        const float4 q = tgt[t];
+        if (q.w < 0.f) continue;
+        float gx = fmaxf(0.f, fmaxf(lo.x - q.x, q.x - hi.x));
+        float gy = fmaxf(0.f, fmaxf(lo.y - q.y, q.y - hi.y));
+        float gz = fmaxf(0.f, fmaxf(lo.z - q.z, q.z - hi.z));
+        float R = SYM ? fmaxf(lo.w, q.w) : q.w;
+        if (gx * gx + gy * gy + gz * gz <= R * R * 1.00001f) return true;
+    }
+    return false;
+}
+
+template <bool SYM, bool EXACT, class Leaf>
+__device__ __forceinline__ void walk(const Tree &t, float3 tlo, float3 thi, float tH, const float4 *tgt, unsigned *stack,
+                                     Leaf &&leaf)
 {
     const int lane = threadIdx.x & 31;
     int sp = 0;
     int L = t.nlev - 1, first = 0, cnt = t.count[L];
     while (true) {
         bool pass = false;
-        if (lane < cnt) pass = box_reach<SYM>(t.lo[L][first + lane], t.hi[L][first + lane], tlo, thi, tH);
+        if (lane < cnt) pass = node_reach<SYM, EXACT>(t.lo[L][first + lane], t.hi[L][first + lane], tlo, thi, tH, tgt);
         unsigned mask = __ballot_sync(0xffffffffu, pass);
         if (L == 0) {
             while (mask) {
@@ -76,9 +98,11 @@ __device__ __forceinline__ void walk(const Tree &t, float3 tlo, float3 thi, floa
 // fp32 rho misses the 1e-4 target on the yielded S.  B200 runs FP64 at half the FP32 rate, and the
 // extra work is ~12 DFMA per true pair.  r comes from the fp32 rsqrt plus one Newton step in fp64.
 // ------------------------------------------------------------------------------------------
+template <bool EXACT>
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_density(Dev d, float kappa, const unsigned char *__restrict__ tile_flag, int ntile)
 {
     __shared__ float4 s_src[PAIR_WARPS][SPH_CHUNK];
+    __shared__ float4 s_tgt[PAIR_WARPS][SPH_CHUNK];
     __shared__ unsigned s_stack[PAIR_WARPS][STACK_DEPTH];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
@@ -100,9 +124,13 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_density(Dev d, float kappa,
     int cnt_i = 0;
     unsigned long long tests = 0;
     const unsigned vmask = __ballot_sync(0xffffffffu, valid);
+    if (EXACT) {
+        s_tgt[warp][lane] = make_float4(pi.x, pi.y, pi.z, valid ? Hi : -1.f);
+        __syncwarp();
+    }
 
-    walk<false>(d.tree, make_float3(blo.x, blo.y, blo.z), make_float3(bhi.x, bhi.y, bhi.z), blo.w, s_stack[warp],
-                [&](int c) {
+    walk<false, EXACT>(d.tree, make_float3(blo.x, blo.y, blo.z), make_float3(bhi.x, bhi.y, bhi.z), blo.w, s_tgt[warp],
+                       s_stack[warp], [&](int c) {
         long long j0 = (long long)c * SPH_CHUNK;
         int cnt = (int)min((long long)SPH_CHUNK, d.n - j0);
         if (lane < cnt) s_src[warp][lane] = d.r.pm[j0 + lane];
@@ -159,11 +187,12 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_density(Dev d, float kappa,
 // S4 + S5 fused (or either alone): over the symmetric set r2 < max(H_i^2, H_j^2), j != i.
 // Equations and operand packing: sph_pairterm.cuh.
 // ------------------------------------------------------------------------------------------
-template <bool GRAD, bool FORCE>
+template <bool GRAD, bool FORCE, bool EXACT>
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(Dev d, DevParams p, const unsigned char *__restrict__ tile_flag, int ntile)
 {
     __shared__ float4 s_src[PAIR_WARPS][4][SPH_CHUNK];
     __shared__ float s_src5[PAIR_WARPS][SPH_CHUNK];
+    __shared__ float4 s_tgt[PAIR_WARPS][SPH_CHUNK];
     __shared__ unsigned s_stack[PAIR_WARPS][STACK_DEPTH];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     PairConst kc;
@@ -183,9 +212,13 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(Dev d, DevParams p, co
     int cnt_i = 0;
     unsigned long long tests = 0;
     const unsigned vmask = __ballot_sync(0xffffffffu, valid);
+    if (EXACT) {
+        s_tgt[warp][lane] = make_float4(t.x, t.y, t.z, valid ? t.H : -1.f);
+        __syncwarp();
+    }
 
-    walk<true>(d.tree, make_float3(blo.x, blo.y, blo.z), make_float3(bhi.x, bhi.y, bhi.z), blo.w, s_stack[warp],
-               [&](int c) {
+    walk<true, EXACT>(d.tree, make_float3(blo.x, blo.y, blo.z), make_float3(bhi.x, bhi.y, bhi.z), blo.w, s_tgt[warp],
+                      s_stack[warp], [&](int c) {
         long long j0 = (long long)c * SPH_CHUNK;
         int cnt = (int)min((long long)SPH_CHUNK, d.n - j0);
         if (lane < cnt) {
@@ -231,13 +264,14 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(Dev d, DevParams p, co
 // ------------------------------------------------------------------------------------------
 // test hook: neighbour sets as original ids
 // ------------------------------------------------------------------------------------------
-template <bool SYM>
+template <bool SYM, bool EXACT>
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_neighbors(Dev d, float kappa, int *counts, const long long *offsets,
                                                                int *list, const unsigned char *__restrict__ tile_flag, int ntile)
 {
     __shared__ float4 s_src[PAIR_WARPS][SPH_CHUNK];
     __shared__ float s_H2[PAIR_WARPS][SPH_CHUNK];
     __shared__ unsigned s_orig[PAIR_WARPS][SPH_CHUNK];
+    __shared__ float4 s_tgt[PAIR_WARPS][SPH_CHUNK];
     __shared__ unsigned s_stack[PAIR_WARPS][STACK_DEPTH];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
@@ -254,8 +288,12 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_neighbors(Dev d, float kapp
     long long base = (valid && list) ? offsets[oi] : 0;
     float4 blo = d.tree.lo[0][chunk], bhi = d.tree.hi[0][chunk];
     int cnt_i = 0;
-    walk<SYM>(d.tree, make_float3(blo.x, blo.y, blo.z), make_float3(bhi.x, bhi.y, bhi.z), blo.w, s_stack[warp],
-              [&](int c) {
+    if (EXACT) {
+        s_tgt[warp][lane] = make_float4(pi.x, pi.y, pi.z, valid ? Hi : -1.f);
+        __syncwarp();
+    }
+    walk<SYM, EXACT>(d.tree, make_float3(blo.x, blo.y, blo.z), make_float3(bhi.x, bhi.y, bhi.z), blo.w, s_tgt[warp],
+                     s_stack[warp], [&](int c) {
         long long j0 = (long long)c * SPH_CHUNK;
         int cnt = (int)min((long long)SPH_CHUNK, d.n - j0);
         if (lane < cnt) {
@@ -298,7 +336,10 @@ int sph_launch_density(sph_ctx *c, bool flagged_only)
     }
     if (d.n == 0) return SPH_OK;
     const int ntile = sph_div_up(d.nchunk, PAIR_WARPS);
-    k_density<<<walk_grid_of(d, flagged_only, ntile), PAIR_WARPS * 32, 0, c->stream>>>(d, c->p.kappa, flagged_only ? d.tile_flag : nullptr, ntile);
+    if (flagged_only)
+        k_density<true><<<walk_grid_of(d, true, ntile), PAIR_WARPS * 32, 0, c->stream>>>(d, c->p.kappa, d.tile_flag, ntile);
+    else
+        k_density<false><<<ntile, PAIR_WARPS * 32, 0, c->stream>>>(d, c->p.kappa, nullptr, ntile);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
@@ -315,9 +356,15 @@ int sph_launch_pair(sph_ctx *c, bool grad, bool force, bool flagged_only)
     const int ntile = sph_div_up(d.nchunk, PAIR_WARPS);
     dim3 grid(walk_grid_of(d, flagged_only, ntile)), block(PAIR_WARPS * 32);
     const unsigned char *tf = flagged_only ? d.tile_flag : nullptr;
-    if (grad && force) k_pair<true, true><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
-    else if (grad) k_pair<true, false><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
-    else k_pair<false, true><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
+    if (flagged_only) {
+        if (grad && force) k_pair<true, true, true><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
+        else if (grad) k_pair<true, false, true><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
+        else k_pair<false, true, true><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
+    } else {
+        if (grad && force) k_pair<true, true, false><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
+        else if (grad) k_pair<true, false, false><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
+        else k_pair<false, true, false><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
+    }
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
@@ -330,8 +377,13 @@ int sph_launch_neighbors(sph_ctx *c, int which, int *counts, const long long *of
     const int ntile = sph_div_up(d.nchunk, PAIR_WARPS);
     dim3 grid(walk_grid_of(d, flagged_only, ntile)), block(PAIR_WARPS * 32);
     const unsigned char *tf = flagged_only ? d.tile_flag : nullptr;
-    if (which == SPH_SYMMETRIC) k_neighbors<true><<<grid, block, 0, c->stream>>>(d, c->p.kappa, counts, offsets, list, tf, ntile);
-    else k_neighbors<false><<<grid, block, 0, c->stream>>>(d, c->p.kappa, counts, offsets, list, tf, ntile);
+    if (flagged_only) {
+        if (which == SPH_SYMMETRIC) k_neighbors<true, true><<<grid, block, 0, c->stream>>>(d, c->p.kappa, counts, offsets, list, tf, ntile);
+        else k_neighbors<false, true><<<grid, block, 0, c->stream>>>(d, c->p.kappa, counts, offsets, list, tf, ntile);
+    } else {
+        if (which == SPH_SYMMETRIC) k_neighbors<true, false><<<grid, block, 0, c->stream>>>(d, c->p.kappa, counts, offsets, list, tf, ntile);
+        else k_neighbors<false, false><<<grid, block, 0, c->stream>>>(d, c->p.kappa, counts, offsets, list, tf, ntile);
+    }
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
