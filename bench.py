@@ -225,6 +225,33 @@ def run_ours(args):
     pairs = pairs_g + pairs_s
     value = world * pairs / (total_ms_max * 1e-3)
 
+    # ---- the same step with strength off (S == 0, hydro only): BASELINE.json's "<= 30 % over hydro-only"
+    hydro = None
+    if strength and not args.no_hydro_only:
+        import dataclasses
+        wl_h = dataclasses.replace(wl, params=dataclasses.replace(wl.params, flags=wl.params.flags & ~B.STRENGTH))
+        sh = B.Sph(wl_h.params, n, device=dev)
+        th = sh.upload(wl_h)
+        sh.build_neighbors(th, n)
+        for _ in range(args.warmup):
+            sh.step(None, 0, 0.0)
+        barrier()
+        hev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        hpass = {k: 0.0 for k in B.T_SLOTS}
+        for k in range(args.steps):
+            flush.fill_(k & 0xff)
+            hev[k][0].record(sh.stream)
+            sh.step(None, 0, 0.0)
+            hev[k][1].record(sh.stream)
+            tmh = sh.get_timings()
+            for q in B.T_SLOTS:
+                hpass[q] += tmh[q]
+        barrier()
+        h_ms = sum(a.elapsed_time(b) for a, b in hev) / args.steps
+        hydro = {"ms_per_step": h_ms, "pass_ms": {k: v / args.steps for k, v in hpass.items()},
+                 "strength_overhead": (total_ms / args.steps) / h_ms - 1.0}
+        del sh, th
+
     # ---- end to end through the host-buffer entry point -----------------------------------
     host = {k: torch.from_numpy(v.copy()).pin_memory() for k, v in wl.arrays.items()}
     host["mat"] = torch.from_numpy(wl.mat.copy()).pin_memory()
@@ -293,6 +320,7 @@ def run_ours(args):
                 "steps": e2e_steps, "ms_per_step": 1e3 * float(te.item()) / e2e_steps},
         "roofline": roofline,
         "cpu_baseline": cpu,
+        "hydro_only": hydro,
     }
     print(json.dumps(line), flush=True)
     if world > 1:
@@ -307,6 +335,7 @@ def main():
     ap.add_argument("--workload", default="c2", choices=["c0", "c1", "c2", "c3", "c4"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-hydro-only", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

@@ -15,6 +15,15 @@
 #define SPH_WC2_SIGMA 3.3422538049298023f     // 21 / (2 pi)
 #define SPH_WC2_K20 66.845076098596046f       // 20 * 21 / (2 pi)
 
+// x / y and 1 / y by one MUFU.RCP and no range checks (__fdividef adds an FSETP and two scaling FMULs
+// per call); every operand here is far from the 2^126 limit of rcp.approx.
+__device__ __forceinline__ float sph_rcp(float y)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(y));
+    return r;
+}
+
 struct PairConst {
     float beta;       // Eq. 5
     float alpha2;     // alpha / 2: alpha cbar = alpha2 (c_i + c_j)
@@ -57,7 +66,7 @@ __device__ __forceinline__ void pair_term(const PairTarget &t, const PairConst &
     const float dx = t.x - q1.x, dy = t.y - q1.y, dz = t.z - q1.z;
     const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
     const float r = r2 * rsqrtf(fmaxf(r2, 1.0e-37f));
-    const float invHj = __fdividef(1.f, q2.w);
+    const float invHj = sph_rcp(q2.w);
     const float ti = fmaxf(0.f, fmaf(-r, t.invH, 1.f));
     const float tj = fmaxf(0.f, fmaf(-r, invHj, 1.f));
     const float ti3 = ti * ti * ti, tj3 = tj * tj * tj;
@@ -100,8 +109,8 @@ __device__ __forceinline__ void pair_term(const PairTarget &t, const PairConst &
         float vr = fminf(vx_, 0.f);
         vr = valid ? vr : 0.f;
         const float hb = k.hk * (t.H + q2.w);
-        const float mu = __fdividef(hb * vr, fmaf(k.eps * hb, hb, r2));
-        const float P2 = __fdividef(mu * fmaf(k.beta, mu, -k.alpha2 * (t.c + q3.y)), t.rho + q3.x);   // Pi_ij / 2
+        const float mu = (hb * vr) * sph_rcp(fmaf(k.eps * hb, hb, r2));
+        const float P2 = (mu * fmaf(k.beta, mu, -k.alpha2 * (t.c + q3.y))) * sph_rcp(t.rho + q3.x);   // Pi_ij / 2
         const float kk = P2 * fmaf(t.K, di, dj);     // 1/2 m_j Pi_ij (D_i + D_j)
         A.ax = fmaf(kk, dx, A.ax); A.ay = fmaf(kk, dy, A.ay); A.az = fmaf(kk, dz, A.az);
         A.du = fmaf(-0.5f * kk, vr, A.du);
