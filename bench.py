@@ -89,15 +89,38 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused pair kernel, from the committed
+# `ncu --set full` capture of this command (profiles/, latest round-1 summary); None where no capture exists.
+NCU_TRAFFIC_BYTES = {"c2": 338.8e6}
+
+
+def rank_reduce(ms: float, units: float, device):
+    """The N > 1 reduction of the contract: time = MAX over ranks, units = SUM over ranks (each rank
+    steps its own replica; there is no data-path collective).  Works on any initialised backend."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms), float(units)
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    u = torch.tensor([units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
 def make_workload(name: str):
     from paper_2603_19764_b200 import workloads as W
     k = int(name[1])
     return W.config(k)
 
 
-def oracle_sample(wl, target_n: int = 60000):
+ORACLE_SAMPLE_N = 1_000_000     # particles in the oracle's bounded sample (about 2 s per evaluation on 16 cores)
+ORACLE_BUDGET_S = 12.0          # the cpu_baseline leg repeats the evaluation until this much CPU time is spent
+
+
+def oracle_sample(wl, target_n: int = ORACLE_SAMPLE_N):
     """A bounded sample of the workload for the CPU oracle: the particles inside a cube around the
-    centre of mass that holds about target_n of them (complete neighbourhoods inside, cut faces)."""
+    median position that holds about target_n of them (complete neighbourhoods inside, cut faces)."""
     import numpy as np
     A = wl.arrays
     if wl.n <= target_n:
@@ -110,24 +133,26 @@ def oracle_sample(wl, target_n: int = 60000):
     return wl.subset(idx), "cube of %d particles around the median position (of %d)" % (idx.size, wl.n)
 
 
-def time_oracle(wl, steps: int = 1):
-    """One derivative evaluation (the pair work of one step) of the oracle, as it stands."""
+def time_oracle(wl, budget_s: float = 0.0, max_evals: int = 16):
+    """Derivative evaluations (the pair work of one step) of the oracle, as it stands: one, or as
+    many as fit in budget_s.  Returns (pairs per evaluation, mean seconds, threads, evaluations)."""
     from oracle import oracle as O
     import numpy as np
     A = {k: np.ascontiguousarray(v, dtype=np.float64) for k, v in wl.arrays.items()}
     S = np.stack([A["Sxx"], A["Syy"], A["Sxy"], A["Sxz"], A["Syz"]])
     g = np.stack([A["gx"], A["gy"], A["gz"]])
     O.lib()
-    best = None
+    times = []
     pairs = 0
-    for _ in range(steps):
+    while True:
         t0 = time.perf_counter()
         d = O.derivatives(wl.params, A["x"], A["y"], A["z"], A["m"], A["h"], A["vx"], A["vy"], A["vz"],
                           A["u"], S, wl.mat, g, "grid")
-        dt = time.perf_counter() - t0
+        times.append(time.perf_counter() - t0)
         pairs = int(d["n_gather"].sum()) + int(d["n_symmetric"].sum())
-        best = dt if best is None else min(best, dt)
-    return pairs, best, O.lib().orc_max_threads()
+        if sum(times) >= budget_s or len(times) >= max_evals:
+            break
+    return pairs, sum(times) / len(times), O.lib().orc_max_threads(), len(times)
 
 
 def run_reference(args):
@@ -137,11 +162,11 @@ def run_reference(args):
     wl = make_workload(args.workload)
     sample, what = oracle_sample(wl)
     for _ in range(max(args.warmup, 0) and 1):
-        time_oracle(sample, 1)
+        time_oracle(sample)
     times = []
     pairs = 0
     for _ in range(args.steps):
-        pairs, dt, cores = time_oracle(sample, 1)
+        pairs, dt, cores, _n = time_oracle(sample)
         times.append(dt)
     total = sum(times)
     val = pairs * len(times) / total
@@ -218,12 +243,9 @@ def run_ours(args):
     launches = s.launch_count() - launches0
     step_ms = [a.elapsed_time(b) for a, b in ev]
     total_ms = sum(step_ms)
-    tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    total_ms_max = float(tmax.item())
     pairs = pairs_g + pairs_s
-    value = world * pairs / (total_ms_max * 1e-3)
+    total_ms_max, pairs_all = rank_reduce(total_ms, pairs, dev)
+    value = pairs_all / (total_ms_max * 1e-3)
 
     # ---- the same step with strength off (S == 0, hydro only): BASELINE.json's "<= 30 % over hydro-only"
     hydro = None
@@ -269,10 +291,8 @@ def run_ours(args):
         e2e_pairs += c["pairs_gather"] + c["pairs_symmetric"]
     torch.cuda.synchronize(dev)
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = world * e2e_pairs / float(te.item())
+    e2e_s_max, e2e_pairs_all = rank_reduce(e2e_s, e2e_pairs, dev)
+    e2e_value = e2e_pairs_all / e2e_s_max
     h2d = n * (17 * 4 + 4 + 1)
     d2h = n * 12 * 4 + 4
 
@@ -293,15 +313,17 @@ def run_ours(args):
                                "MEASURED_PEAKS.json)" % (props.multi_processor_count, sm_max),
                 "flops_per_pair": flops_pair, "pairs_per_launch": pairs_s / args.steps,
                 "kernel_ms": kern_ms, "share_of_step": kern_ms / (total_ms / args.steps),
-                "candidate_hit_rate": pairs / tests if tests else None, "traffic": None}
+                "candidate_hit_rate": pairs / tests if tests else None,
+                "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if strength else None, "traffic_unit": "bytes per launch"}
 
     # ---- the oracle beside it ------------------------------------------------------------------
     cpu = None
     if not args.no_cpu_baseline:
         sample, what = oracle_sample(wl)
-        op, ot, cores = time_oracle(sample, 1)
-        cpu = {"value": op / ot, "unit": "pairs/s", "cores": cores, "kind": "oracle", "sample": what,
-               "seconds": ot, "particle_steps_per_s": sample.n / ot}
+        op, ot, cores, nev = time_oracle(sample, ORACLE_BUDGET_S)
+        cpu = {"value": op / ot, "unit": "pairs/s", "cores": cores, "kind": "oracle",
+               "sample": "%s, %d evaluations of the step's derivatives" % (what, nev),
+               "seconds": ot * nev, "particle_steps_per_s": sample.n / ot}
 
     line = {
         "metric": "pair_interactions_per_s", "value": value, "unit": "pairs/s", "n_gpus": world,
@@ -317,7 +339,7 @@ def run_ours(args):
         "gpu_launches": launches,
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "pairs/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": e2e_steps, "ms_per_step": 1e3 * float(te.item()) / e2e_steps},
+                "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s_max / e2e_steps},
         "roofline": roofline,
         "cpu_baseline": cpu,
         "hydro_only": hydro,

@@ -28,6 +28,8 @@
 
 #define FULL 0xffffffffu
 #define ROWPTR_STRIDE (SPH_MAXROUND + 1)
+#define LBUF_ENTRIES 64                    // u16 entries a lane can hold between two flushes
+#define LBUF_STRIDE (LBUF_ENTRIES * 2 + 8) // bytes per lane: 34 words, so lanes at the same fill level spread over banks
 
 __device__ __forceinline__ bool box_reach_sym(float4 lo, float4 hi, float4 tlo, float4 thi)
 {
@@ -67,7 +69,9 @@ struct CullSmem {
     float4 glo[4 * SPH_TILE_CHUNKS], ghi[4 * SPH_TILE_CHUNKS];   // quarter-warp boxes
     float4 tlo, thi;                     // tile box (tlo.w = max H)
     unsigned selfslot[SPH_TILE];         // slot of each target of the tile in its own candidate list
-    unsigned short gl[SPH_TILE_CHUNKS][4][SPH_GCAP];     // per quarter-warp: slots still to test, ascending
+    unsigned short gl[SPH_TILE_CHUNKS][4][SPH_GCAP];     // per quarter-warp: candidates still to test, ascending,
+                                                         // as byte offsets (slot * 16) into pos[]
+    unsigned char lbuf[SPH_TILE * LBUF_STRIDE];          // per lane: list entries found and not yet written out
     int nsrc, ntotal, nfront, overflow;
     unsigned long long cand_off;
 };
@@ -275,25 +279,29 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     }
 
     // ---- per-lane list state --------------------------------------------------------------------------
+    // A lane appends the byte offset of every hit to its own buffer in shared memory (one predicated
+    // store per test: no bit masks, no serial extraction loop).  Complete row-groups (4 entries) go to
+    // the transposed global list when some lane's buffer could overflow in the next block of tests and
+    // at the end of the round, all lanes in lockstep: by then the lanes hold similar numbers of rows.
     const int chunk = chunk0 + warp;
     uint2 *lp = d.nlist + ((size_t)(warp < nch ? chunk : chunk0) * d.rows_cap) * 32 + lane;
     unsigned short *rp = d.rowptr + (size_t)(warp < nch ? chunk : chunk0) * ROWPTR_STRIDE;
-    uint2 *lpw = lp;                      // where the row-group being filled goes
-    const int ncap = d.rows_cap * 4;
-    int n = 0, nhit = 0;                  // entries pushed (padding included) / true neighbours
-    unsigned w0 = 0, w1 = 0;              // the row-group being filled: a 4 x 16-bit shift register
+    unsigned char *const lb = sm.lbuf + threadIdx.x * LBUF_STRIDE;
+    unsigned char *wp = lb;               // where the next entry goes
+    int G = 0;                            // row-groups of this lane in the global list so far (padding included)
+    int nhit = 0;                         // true neighbours
     unsigned tests = 0;
-    // push one 16-bit entry; a complete row-group goes to memory (rows beyond the capacity are dropped
-    // and the tile is flagged at the end)
-#define LIST_PUSH(v)                                              \
-    do {                                                          \
-        w0 = __byte_perm(w0, w1, 0x5432);                         \
-        w1 = __byte_perm(w1, (v), 0x5432);                        \
-        ++n;                                                      \
-        if ((n & 3) == 0) {                                       \
-            if (n <= ncap) *lpw = make_uint2(w0, w1);             \
-            lpw += 32;                                            \
-        }                                                         \
+    // write the complete row-groups of the buffer out, keep the 0..3 entries left over
+#define LIST_FLUSH()                                                                        \
+    do {                                                                                    \
+        const int cnt_ = (int)(wp - lb) >> 1, rows_ = cnt_ >> 2;                            \
+        const int rmax_ = __reduce_max_sync(FULL, rows_);                                   \
+        for (int r_ = 0; r_ < rmax_; ++r_)                                                  \
+            if (r_ < rows_ && G + r_ < d.rows_cap)                                          \
+                lp[(size_t)(G + r_) * 32] = *reinterpret_cast<const uint2 *>(lb + 8 * r_);  \
+        if (cnt_ & 3) *reinterpret_cast<uint2 *>(lb) = *reinterpret_cast<const uint2 *>(lb + 8 * rows_); \
+        G += rows_;                                                                         \
+        wp = lb + 2 * (cnt_ & 3);                                                           \
     } while (0)
     const int g = lane >> 3;
     if (warp < nch && lane == 0) rp[0] = 0;
@@ -323,9 +331,12 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
         __syncthreads();
         if (warp < nch) {
             // ---- B: quarter g of this warp tests the candidates flagged for it, in slot order ---------
-            const int self = (int)sm.selfslot[threadIdx.x] - r0;       // self exclusion (j != i)
+            const int selfrel = (int)sm.selfslot[threadIdx.x] - r0;    // self exclusion (j != i)
+            const unsigned selfoff = (selfrel >= 0 && selfrel < nr) ? (unsigned)selfrel << 4 : 0xffffffffu;
             const int fshift = 4 * warp;
+            const int Gstart = G;
             unsigned short(*gl)[SPH_GCAP] = sm.gl[warp];
+            const unsigned char *const posb = reinterpret_cast<const unsigned char *>(sm.pos);
             int base = 0;
             while (base < nr) {
                 int c0 = 0, c1 = 0, c2 = 0, c3 = 0;
@@ -334,10 +345,11 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
                     const unsigned f = s < nr ? (sm.flag[s] >> fshift) & 15u : 0u;
                     const unsigned m0 = __ballot_sync(FULL, f & 1u), m1 = __ballot_sync(FULL, f & 2u),
                                    m2 = __ballot_sync(FULL, f & 4u), m3 = __ballot_sync(FULL, f & 8u);
-                    if (f & 1u) gl[0][c0 + __popc(m0 & lt)] = (unsigned short)s;
-                    if (f & 2u) gl[1][c1 + __popc(m1 & lt)] = (unsigned short)s;
-                    if (f & 4u) gl[2][c2 + __popc(m2 & lt)] = (unsigned short)s;
-                    if (f & 8u) gl[3][c3 + __popc(m3 & lt)] = (unsigned short)s;
+                    const unsigned short so = (unsigned short)(s << 4);
+                    if (f & 1u) gl[0][c0 + __popc(m0 & lt)] = so;
+                    if (f & 2u) gl[1][c1 + __popc(m1 & lt)] = so;
+                    if (f & 4u) gl[2][c2 + __popc(m2 & lt)] = so;
+                    if (f & 8u) gl[3][c3 + __popc(m3 & lt)] = so;
                     c0 += __popc(m0); c1 += __popc(m1); c2 += __popc(m2); c3 += __popc(m3);
                     base += 32;
                 }
@@ -345,46 +357,48 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
                 const int gcnt = g == 0 ? c0 : (g == 1 ? c1 : (g == 2 ? c2 : c3));
                 const int cmax = max(max(c0, c1), max(c2, c3));
                 const int cpad = (cmax + 31) & ~31;
-                for (int k = c0 + lane; k < cpad; k += 32) gl[0][k] = (unsigned short)SPH_SE;
-                for (int k = c1 + lane; k < cpad; k += 32) gl[1][k] = (unsigned short)SPH_SE;
-                for (int k = c2 + lane; k < cpad; k += 32) gl[2][k] = (unsigned short)SPH_SE;
-                for (int k = c3 + lane; k < cpad; k += 32) gl[3][k] = (unsigned short)SPH_SE;
+                const unsigned short sent = (unsigned short)(SPH_SE << 4);
+                for (int k = c0 + lane; k < cpad; k += 32) gl[0][k] = sent;
+                for (int k = c1 + lane; k < cpad; k += 32) gl[1][k] = sent;
+                for (int k = c2 + lane; k < cpad; k += 32) gl[2][k] = sent;
+                for (int k = c3 + lane; k < cpad; k += 32) gl[3][k] = sent;
                 __syncwarp();
-                const unsigned short *mygl = gl[g];
+                const uint4 *mygl = reinterpret_cast<const uint4 *>(gl[g]);
                 tests += valid ? (unsigned)gcnt : 0u;
                 for (int kb = 0; kb < cmax; kb += 32) {
-                    // 32 candidates of the quarter's table -> one hit bit each
-                    unsigned bits = 0u;
+                    // 32 candidates of the quarter's table (4 x 8 offsets per 16-byte read)
 #pragma unroll
-                    for (int kk = 0; kk < 32; ++kk) {
-                        const int slot = (int)mygl[kb + kk];
-                        const float4 q = sm.pos[slot];
-                        const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
-                        if (r2 < fmaxf(H2i, q.w) && slot != self) bits |= 1u << kk;
+                    for (int k8 = 0; k8 < 4; ++k8) {
+                        const uint4 tw = mygl[(kb >> 3) + k8];
+                        const unsigned wv[4] = {tw.x, tw.y, tw.z, tw.w};
+#pragma unroll
+                        for (int e = 0; e < 8; ++e) {
+                            const unsigned off = (e & 1) ? (wv[e >> 1] >> 16) : (wv[e >> 1] & 0xffffu);
+                            const float4 q = *reinterpret_cast<const float4 *>(posb + off);
+                            const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
+                            if (r2 < fmaxf(H2i, q.w) && off != selfoff) {
+                                *reinterpret_cast<unsigned short *>(wp) = (unsigned short)off;
+                                wp += 2;
+                            }
+                        }
                     }
-                    nhit += __popc(bits);
-                    // every lane appends its own hits, in slot order
-                    while (bits) {
-                        const int b = __ffs(bits) - 1;
-                        bits &= bits - 1u;
-                        const unsigned v = (unsigned)mygl[kb + b] << 4;
-                        LIST_PUSH(v);
-                    }
+                    // room for another 32 entries in every lane?  (3 may stay behind after a flush)
+                    if (__any_sync(FULL, (int)(wp - lb) > 2 * (LBUF_ENTRIES - 32))) LIST_FLUSH();
                 }
                 __syncwarp();
             }
-            // ---- end of the round: flush, pad every lane to the warp's longest list -------------------
-            while (n & 3) LIST_PUSH(0xffffu);
-            const int G = n >> 2;
-            int Gmax = G;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) Gmax = max(Gmax, __shfl_xor_sync(FULL, Gmax, o));
-            for (int gg = G; gg < Gmax; ++gg) {
-                if (gg < d.rows_cap) *lpw = make_uint2(0xffffffffu, 0xffffffffu);
-                lpw += 32;
+            // ---- end of the round: pad the last row-group, flush, pad every lane to the warp's longest list
+            nhit += 4 * (G - Gstart) + ((int)(wp - lb) >> 1);
+            while ((int)(wp - lb) & 7) {
+                *reinterpret_cast<unsigned short *>(wp) = 0xffffu;
+                wp += 2;
             }
-            n = Gmax * 4;
-            if (n > ncap) sm.overflow = 8;            // list rows exhausted: the tile falls back
+            LIST_FLUSH();
+            const int Gmax = __reduce_max_sync(FULL, G);
+            for (int gg = G; gg < Gmax; ++gg)
+                if (gg < d.rows_cap) lp[(size_t)gg * 32] = make_uint2(0xffffffffu, 0xffffffffu);
+            G = Gmax;
+            if (G > d.rows_cap) sm.overflow = 8;      // list rows exhausted: the tile falls back
             if (lane == 0) rp[round + 1] = (unsigned short)min(Gmax, d.rows_cap);
         }
         __syncthreads();
@@ -395,7 +409,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
         for (int o = 16; o > 0; o >>= 1) tests += __shfl_xor_sync(FULL, tests, o);
         if (lane == 0) atomicAdd(&d.counters[SPH_C_TESTS_CULL], (unsigned long long)tests);
     }
-#undef LIST_PUSH
+#undef LIST_FLUSH
     if (threadIdx.x == 0) {
         d.tile_flag[tile] = sm.overflow ? 1 : 0;
         if (sm.overflow) atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], 1ull);

@@ -22,8 +22,9 @@ def rows(counts, offsets, lst):
     return [np.sort(lst[offsets[i]:offsets[i + 1]]) for i in range(counts.shape[0])]
 
 
-def gpu_single_pass(wl, dt=None, split=True, allow_fallback=False):
-    """Run the BASELINE.json configs[0] pass sequence through the C ABI; returns numpy fields."""
+def gpu_single_pass(wl, dt=None, split=True, allow_fallback=False, select=None):
+    """Run the BASELINE.json configs[0] pass sequence through the C ABI; returns numpy fields
+    (of the particles ``select`` -- caller-order indices -- when given: full-size cases)."""
     import torch
     from paper_2603_19764_b200 import binding as B
     s = B.Sph(wl.params, max(wl.n, 1))
@@ -40,12 +41,14 @@ def gpu_single_pass(wl, dt=None, split=True, allow_fallback=False):
         s.strength_update(B.CLOSE, dt)
     else:
         raise NotImplementedError
+    sel = None if select is None else torch.as_tensor(np.asarray(select), dtype=torch.long, device="cuda")
+    pick = (lambda t: t) if sel is None else (lambda t: t[..., sel])
     out = {}
     for name in ("RHO", "OMEGA", "P", "CS", "T", "GAMMA", "Y", "MUMAX", "DUDT", "DT", "EPS2", "U", "CFLAG",
                  "NGATHER", "NSYMMETRIC"):
-        out[name.lower()] = s.get_field(name).cpu().numpy()
+        out[name.lower()] = pick(s.get_field(name)).cpu().numpy()
     for name, nc in (("A", 3), ("V", 3), ("X", 3), ("SPRED", 5), ("S", 5), ("DSDT", 5), ("F", 9), ("CINV", 9), ("G", 9)):
-        out[name.lower()] = s.get_fields(name, nc).cpu().numpy()
+        out[name.lower()] = pick(s.get_fields(name, nc)).cpu().numpy()
     out["counters"] = s.get_counters()
     assert allow_fallback or out["counters"]["list_overflow"] == 0, "tiles fell back to the tree-walk kernels"
     out["timings"] = s.get_timings()
@@ -89,3 +92,37 @@ def compare_single_pass(g, d, wl, check_sets=None):
     for k in ("S_close", "v_close", "u_close"):
         assert errs[k] <= TOL_STATE, errs
     return errs
+
+
+def dependency_closed_sample(wl, centre, n_valid):
+    """Indices for a SAMPLED full-size comparison.  V = the n_valid particles nearest to ``centre`` in
+    the max norm (a cube); N1 = every particle that can be a symmetric neighbour of a particle in V
+    (distance to V's box < max(H_j, max H in V)); N2 = every particle that can be a gather neighbour
+    of a particle in N1.  The oracle run on N2 alone reproduces rho, Omega, P, Y of all of N1 and hence
+    every field of V exactly as the run on the whole set would.  Pure geometry: no method arithmetic.
+    Returns (sample indices N2 ascending, positions of V inside the sample, V indices)."""
+    A = wl.arrays
+    p = np.stack([A["x"], A["y"], A["z"]]).astype(np.float64)
+    H = float(wl.params.kappa) * A["h"].astype(np.float64)
+    c = np.asarray(centre, dtype=np.float64)[:, None]
+    d = np.abs(p - c).max(axis=0)
+    V = np.sort(np.argpartition(d, n_valid)[:n_valid])
+
+    def box_dist(idx):
+        lo = p[:, idx].min(axis=1, keepdims=True); hi = p[:, idx].max(axis=1, keepdims=True)
+        g = np.maximum(0.0, np.maximum(lo - p, p - hi))
+        return np.sqrt((g * g).sum(axis=0))
+    slack = 1.0 + 1e-6
+    N1 = np.nonzero(box_dist(V) < slack * np.maximum(H, H[V].max()))[0]
+    N2 = np.nonzero(box_dist(N1) < slack * H[N1].max())[0]
+    pos = np.searchsorted(N2, V)
+    assert np.array_equal(N2[pos], V)
+    return N2, pos, V
+
+
+def restrict(fields, idx):
+    """Every array of a field dict whose last axis is the particle axis, restricted to idx."""
+    out = {}
+    for k, v in fields.items():
+        out[k] = v[..., idx] if isinstance(v, np.ndarray) and v.ndim >= 1 else v
+    return out

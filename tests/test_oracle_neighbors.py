@@ -81,3 +81,20 @@ def test_empty_and_single():
     assert c.tolist() == [1] and l[:1].tolist() == [0]
     c, o, l = O.neighbors(one, one, one, np.array([0.1]), 2.0, O.SYMMETRIC, "brute")
     assert c.tolist() == [0]
+
+
+def test_dependency_closed_sample_reproduces_the_full_run():
+    """The sampling used by the full-size GPU comparisons (tests/parity_util.py): the oracle on the
+    dependency-closed sample gives, for the sampled particles, what the oracle on the whole set gives."""
+    from tests import parity_util as U
+    wl = W.impact_pair(30000, W.SEED_BASE + 3, 100.0, 1.214)
+    full = O.single_pass(wl, dt=1e-3, mode="grid")
+    for centre in ((0.0, 0.0, 0.0), (5.0e4 / np.sqrt(2.0), 5.0e4 / np.sqrt(2.0), 0.0)):
+        idx, pos, V = U.dependency_closed_sample(wl, centre, 1500)
+        assert idx.size < wl.n
+        part = U.restrict(O.single_pass(wl.subset(idx), dt=1e-3, mode="grid"), pos)
+        ref = U.restrict(full, V)
+        assert np.array_equal(part["n_gather"], ref["n_gather"])
+        assert np.array_equal(part["n_symmetric"], ref["n_symmetric"])
+        for k in ("rho", "a", "dudt", "dS", "S_close", "G"):
+            assert np.allclose(part[k], ref[k], rtol=1e-12, atol=0.0), k
