@@ -197,6 +197,13 @@ int sph_get_neighbors(sph_ctx *ctx, int which, int *counts, const long long *off
 int sph_get_timings(sph_ctx *ctx, float *ms, int n);            /* SPH_T_* slots              */
 int sph_get_counters(sph_ctx *ctx, long long *counters, int n); /* SPH_C_* slots              */
 
+/* Diagnostic: per-tile statistics of the last neighbour build (tile = 256 curve-consecutive particles).
+ * ncand / cycles / flag: HOST arrays of `capacity` entries, each may be NULL: candidates staged for the
+ * tile, SM clock cycles the list builder spent on it, and whether it fell back to the tree-walk kernels.
+ * Returns the number of tiles (nothing is copied if capacity is smaller), or a negative SPH_E* code.
+ * Synchronises the stream. */
+int sph_get_tile_stats(sph_ctx *ctx, int *ncand, unsigned *cycles, unsigned char *flag, int capacity);
+
 /* Number of this library's kernel launches since sph_init (HOST; no synchronisation). */
 long long sph_launch_count(const sph_ctx *ctx);
 

@@ -32,7 +32,7 @@ OPT_FIELDS = ("gx", "gy", "gz")
 # every symbol include/sph.h declares (tests check the library exports all of them)
 SYMBOLS = ("sph_workspace_bytes", "sph_init", "sph_build_neighbors", "sph_density", "sph_strength_update",
            "sph_gradients", "sph_forces", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
-           "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_launch_count",
+           "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_launch_count",
            "sph_last_cuda_error", "sph_strerror", "sph_destroy")
 
 
@@ -88,6 +88,7 @@ def load():
     lib.sph_get_neighbors.argtypes = [vp, i, vp, vp, vp]
     lib.sph_get_timings.argtypes = [vp, C.POINTER(fl), i]
     lib.sph_get_counters.argtypes = [vp, C.POINTER(ll), i]
+    lib.sph_get_tile_stats.argtypes = [vp, vp, vp, vp, i]
     lib.sph_launch_count.restype = ll
     lib.sph_launch_count.argtypes = [vp]
     lib.sph_last_cuda_error.argtypes = [vp]
@@ -97,7 +98,8 @@ def load():
     lib.sph_destroy.argtypes = [vp]
     for s in ("sph_init", "sph_build_neighbors", "sph_density", "sph_strength_update", "sph_gradients",
               "sph_forces", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
-              "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_last_cuda_error"):
+              "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats",
+              "sph_last_cuda_error"):
         getattr(lib, s).restype = i
     _lib = lib
     return lib
@@ -258,6 +260,16 @@ class Sph:
         cs = (C.c_longlong * len(C_SLOTS))()
         self._check(self.lib.sph_get_counters(self.ctx, cs, len(C_SLOTS)), "sph_get_counters")
         return {k: int(cs[i]) for i, k in enumerate(C_SLOTS)}
+
+    def get_tile_stats(self):
+        """(candidates, cycles, fell_back) per tile of the last neighbour build, as numpy arrays (host)."""
+        import numpy as np
+        nt = self.lib.sph_get_tile_stats(self.ctx, None, None, None, 0)
+        self._check(min(nt, 0), "sph_get_tile_stats")
+        nc = np.zeros(nt, np.int32); cy = np.zeros(nt, np.uint32); fl = np.zeros(nt, np.uint8)
+        rc = self.lib.sph_get_tile_stats(self.ctx, nc.ctypes.data, cy.ctypes.data, fl.ctypes.data, nt)
+        self._check(min(rc, 0), "sph_get_tile_stats")
+        return nc, cy, fl
 
     def launch_count(self) -> int:
         return int(self.lib.sph_launch_count(self.ctx))

@@ -94,6 +94,12 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
     o.tile_ncand = b.take<int>(ntile);
     o.tile_off = b.take<unsigned long long>(ntile);
     o.tile_flag = b.take<unsigned char>(ntile);
+    o.tile_cycles = b.take<unsigned>(ntile);
+    o.cull_cycles = b.take<unsigned long long>(1);
+    o.heavy_cap = (int)(ntile / 16 < 16 ? 16 : (ntile / 16 > 2048 ? 2048 : ntile / 16));
+    o.heavy_list = b.take<unsigned>(o.heavy_cap);
+    o.nheavy = b.take<unsigned>(1);
+    o.heavy_mark = b.take<unsigned char>(ntile);
     o.cand_cursor = b.take<unsigned long long>(1);
     o.cand_cap = lists ? (unsigned long long)ntile * (2 * SPH_SE) : 1;   // pool: twice the one-round average
     o.cand = b.take<unsigned>((size_t)o.cand_cap);
@@ -161,6 +167,13 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
     }
     cudaError_t e = cudaMemsetAsync(c->d.counters, 0, SPH_C_COUNT * sizeof(unsigned long long), c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->d.dt_cur, 0, sizeof(float), c->stream);
+    {
+        const size_t ntile = ((size_t)c->d.n_max + SPH_TILE - 1) / SPH_TILE;
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d.tile_cycles, 0, ntile * sizeof(unsigned), c->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d.cull_cycles, 0, sizeof(unsigned long long), c->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d.nheavy, 0, sizeof(unsigned), c->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d.heavy_mark, 0, ntile, c->stream);
+    }
     if (e == cudaSuccess) e = cudaMemsetAsync(c->d.dt_next, 0, sizeof(float), c->stream);
     if (e != cudaSuccess) { sph_destroy(c); return SPH_ECUDA; }
     *out = c;
@@ -486,6 +499,19 @@ extern "C" int sph_get_counters(sph_ctx *c, long long *out, int n)
     SPH_CUDA(c, cudaStreamSynchronize(c->stream));
     for (int k = 0; k < n && k < SPH_C_COUNT; ++k) out[k] = (long long)h[k];
     return SPH_OK;
+}
+
+extern "C" int sph_get_tile_stats(sph_ctx *c, int *ncand, unsigned *cycles, unsigned char *flag, int capacity)
+{
+    if (!c || capacity < 0) return SPH_EINVAL;
+    if (!c->resident) return SPH_EORDER;
+    const int ntile = sph_div_up(c->d.nchunk, SPH_TILE_CHUNKS);
+    if (!c->use_lists || capacity < ntile) return ntile;
+    if (ncand) SPH_CUDA(c, cudaMemcpyAsync(ncand, c->d.tile_ncand, sizeof(int) * ntile, cudaMemcpyDeviceToHost, c->stream));
+    if (cycles) SPH_CUDA(c, cudaMemcpyAsync(cycles, c->d.tile_cycles, sizeof(unsigned) * ntile, cudaMemcpyDeviceToHost, c->stream));
+    if (flag) SPH_CUDA(c, cudaMemcpyAsync(flag, c->d.tile_flag, ntile, cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    return ntile;
 }
 
 extern "C" long long sph_launch_count(const sph_ctx *c) { return c ? c->launches : 0; }

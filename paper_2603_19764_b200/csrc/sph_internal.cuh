@@ -19,7 +19,7 @@
 #define SPH_MAXROUND 15       // rounds a tile may need (more: the tile falls back to the tree-walk kernels)
 #define SPH_CULL_MAXSRC 768   // source chunks a tile may accept in the tree walk
 #define SPH_CULL_MAXPAR 128   // level-1 nodes a tile may expand in the last level of the walk
-#define SPH_GCAP 192          // entries of a quarter-warp's candidate table in k_cull (multiple of 32)
+#define SPH_GCAP 128          // entries of a quarter-warp's candidate table in k_cull (multiple of 32)
 #define SPH_CULL_CFCACHE 128  // source chunks whose per-particle chunk flags are kept between the two passes
 #define SPH_ROWS_DEFAULT 64   // default row-groups (4 neighbours per lane each) reserved per chunk
 
@@ -86,6 +86,15 @@ struct Dev {
                                             // into the round's staged arrays; 0xFFFF = no entry
     int rows_cap;                           // row-groups reserved per chunk
     unsigned short *rowptr;                 // [chunk][SPH_MAXROUND + 1]: first row-group of each round
+    unsigned *tile_cycles;                  // SM clock cycles k_cull spent on each tile in the last build
+    unsigned long long *cull_cycles;        // their sum
+    // launch order of the tile kernels: the tiles that were expensive in the previous build go first
+    // (a tile that straddles gaps of the space-filling curve costs up to 5x the average and would
+    // otherwise finish long after everything else); see sph_tile_of_block
+    unsigned *heavy_list;                   // [heavy_cap] tiles that run first
+    unsigned *nheavy;                       // entries of heavy_list
+    unsigned char *heavy_mark;              // [tile] != 0: in heavy_list
+    int heavy_cap;                          // blocks reserved in front of the grid for heavy_list
     unsigned char *tile_flag;               // != 0: the tile exceeded a capacity; the tree-walk kernels serve it
     int cull_grid;                          // persistent CTAs of k_cull
     int walk_grid;                          // persistent CTAs of the tree-walk kernels when they serve flagged tiles
@@ -153,6 +162,15 @@ __device__ __forceinline__ float sph_r2(float dx, float dy, float dz)
     return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
 }
 __device__ __forceinline__ float sph_H(float kappa, float h) { return __fmul_rn(kappa, h); }
+
+// Block b of a tile kernel launched with grid = heavy_cap + ntile: blocks [0, heavy_cap) take the heavy
+// list, the rest take the remaining tiles in curve order; -1 = nothing to do for this block.
+__device__ __forceinline__ int sph_tile_of_block(const Dev &d, int b)
+{
+    if (b < d.heavy_cap) return b < (int)*d.nheavy ? (int)d.heavy_list[b] : -1;
+    const int t = b - d.heavy_cap;
+    return d.heavy_mark[t] ? -1 : t;
+}
 
 // order-preserving float <-> int map for atomicMin/atomicMax on floats
 __device__ __forceinline__ int sph_f2ord(float f)

@@ -28,8 +28,8 @@
 
 #define FULL 0xffffffffu
 #define ROWPTR_STRIDE (SPH_MAXROUND + 1)
-#define LBUF_ENTRIES 64                    // u16 entries a lane can hold between two flushes
-#define LBUF_STRIDE (LBUF_ENTRIES * 2 + 8) // bytes per lane: 34 words, so lanes at the same fill level spread over banks
+#define LBUF_ENTRIES 32                    // u16 entries a lane can hold between two flushes
+#define LBUF_STRIDE (LBUF_ENTRIES * 2 + 8) // bytes per lane: 18 words, so lanes at the same fill level spread over banks
 
 __device__ __forceinline__ bool box_reach_sym(float4 lo, float4 hi, float4 tlo, float4 thi)
 {
@@ -59,19 +59,24 @@ struct CullSmem {
                                          // sentinel no target can reach (pads the quarter-warp tables)
     unsigned flag[SPH_SE];               // bit 4w+g: within reach of quarter g of warp w
     unsigned chunks[SPH_CULL_MAXSRC];    // frontier / accepted source chunks, ascending
-    unsigned next[SPH_CULL_MAXSRC];      // next frontier
     unsigned mask[SPH_CULL_MAXSRC];      // surviving lanes (children / particles) of each entry
-    unsigned off[SPH_CULL_MAXSRC];       // exclusive prefix of popc(mask)
+    unsigned short off[SPH_CULL_MAXSRC]; // exclusive prefix of popc(mask) (< SPH_MAXROUND * SPH_SE + 32 < 65536)
     unsigned char cmask[SPH_CULL_MAXSRC];                // chunk boxes of the tile a source chunk box reaches
-    unsigned char ctmp[SPH_CULL_MAXPAR][SPH_ARITY];      // per-child cmask of the leaf expansion
+    union alignas(16) {
+        struct {                                         // the tree walk (A1) only
+            unsigned next[SPH_CULL_MAXSRC];              // next frontier
+            unsigned char ctmp[SPH_CULL_MAXPAR][SPH_ARITY];   // per-child cmask of the leaf expansion
+        } walk;
+        unsigned char lbuf[SPH_TILE * LBUF_STRIDE];      // the list phase (B) only: per lane, list entries found
+                                                         // and not yet written out
+    } u;
     unsigned char cf[SPH_CULL_CFCACHE][SPH_CHUNK];       // per-particle chunk flags of the first source chunks
     float4 blo[SPH_TILE_CHUNKS], bhi[SPH_TILE_CHUNKS];   // chunk boxes (lo.w = max H)
     float4 glo[4 * SPH_TILE_CHUNKS], ghi[4 * SPH_TILE_CHUNKS];   // quarter-warp boxes
     float4 tlo, thi;                     // tile box (tlo.w = max H)
     unsigned selfslot[SPH_TILE];         // slot of each target of the tile in its own candidate list
-    unsigned short gl[SPH_TILE_CHUNKS][4][SPH_GCAP];     // per quarter-warp: candidates still to test, ascending,
+    alignas(16) unsigned short gl[SPH_TILE_CHUNKS][4][SPH_GCAP];     // per quarter-warp: candidates still to test, ascending,
                                                          // as byte offsets (slot * 16) into pos[]
-    unsigned char lbuf[SPH_TILE * LBUF_STRIDE];          // per lane: list entries found and not yet written out
     int nsrc, ntotal, nfront, overflow;
     unsigned long long cand_off;
 };
@@ -103,7 +108,7 @@ __device__ __forceinline__ unsigned reach_groups(const CullSmem &sm, unsigned fc
 }
 
 // warp 0: off[k] = exclusive prefix of popc(mask[k]), k < n; returns the total (valid in every lane)
-__device__ __forceinline__ int scan_popc(const unsigned *mask, unsigned *off, int n, int lane)
+__device__ __forceinline__ int scan_popc(const unsigned *mask, unsigned short *off, int n, int lane)
 {
     int per = (n + 31) / 32, b0 = lane * per, local = 0;
     for (int k = b0; k < min(b0 + per, n); ++k) local += __popc(mask[k]);
@@ -114,7 +119,7 @@ __device__ __forceinline__ int scan_popc(const unsigned *mask, unsigned *off, in
         if (lane >= o) incl += v;
     }
     int run = incl - local;
-    for (int k = b0; k < min(b0 + per, n); ++k) { off[k] = (unsigned)run; run += __popc(mask[k]); }
+    for (int k = b0; k < min(b0 + per, n); ++k) { off[k] = (unsigned short)min(run, 65535); run += __popc(mask[k]); }
     return __shfl_sync(FULL, incl, 31);
 }
 
@@ -124,7 +129,10 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     CullSmem &sm = *reinterpret_cast<CullSmem *>(smem_raw);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
-    for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
+    {
+    const int tile = sph_tile_of_block(d, blockIdx.x);
+    if (tile < 0 || tile >= ntile) return;
+    const long long t_begin = clock64();
     const int chunk0 = tile * SPH_TILE_CHUNKS;
     const int nch = min(SPH_TILE_CHUNKS, d.nchunk - chunk0);
 
@@ -205,7 +213,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
                         if (box_reach_sym(clo, chi, sm.blo[w], sm.bhi[w])) cm |= 1u << w;
                     pass = cm != 0;
                 }
-                if (L == 0 && k < SPH_CULL_MAXPAR) sm.ctmp[k][lane] = (unsigned char)cm;
+                if (L == 0 && k < SPH_CULL_MAXPAR) sm.u.walk.ctmp[k][lane] = (unsigned char)cm;
             }
             unsigned m = __ballot_sync(FULL, pass);
             if (lane == 0) sm.mask[k] = m;
@@ -224,13 +232,13 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             if ((m >> lane) & 1u) {
                 int o = (int)sm.off[k] + __popc(m & lt);
                 if (o < cap) {
-                    sm.next[o] = sm.chunks[k] * SPH_ARITY + (unsigned)lane;
-                    if (L == 0) sm.cmask[o] = sm.ctmp[k][lane];
+                    sm.u.walk.next[o] = sm.chunks[k] * SPH_ARITY + (unsigned)lane;
+                    if (L == 0) sm.cmask[o] = sm.u.walk.ctmp[k][lane];
                 }
             }
         }
         __syncthreads();
-        for (int k = threadIdx.x; k < cap; k += SPH_TILE) sm.chunks[k] = sm.next[k];
+        for (int k = threadIdx.x; k < cap; k += SPH_TILE) sm.chunks[k] = sm.u.walk.next[k];
         __syncthreads();
     }
     const int nsrc = sm.nfront;
@@ -267,8 +275,12 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], 1ull);
         }
         if (valid) d.nsym[i] = 0;
-        __syncthreads();
-        continue;
+        if (threadIdx.x == 0) {
+            const unsigned cyc = (unsigned)(clock64() - t_begin);
+            d.tile_cycles[tile] = cyc;
+            atomicAdd(d.cull_cycles, (unsigned long long)cyc);
+        }
+        return;
     }
     const int ntotal = sm.ntotal;
     unsigned *cand = d.cand + sm.cand_off;
@@ -286,7 +298,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     const int chunk = chunk0 + warp;
     uint2 *lp = d.nlist + ((size_t)(warp < nch ? chunk : chunk0) * d.rows_cap) * 32 + lane;
     unsigned short *rp = d.rowptr + (size_t)(warp < nch ? chunk : chunk0) * ROWPTR_STRIDE;
-    unsigned char *const lb = sm.lbuf + threadIdx.x * LBUF_STRIDE;
+    unsigned char *const lb = sm.u.lbuf + threadIdx.x * LBUF_STRIDE;
     unsigned char *wp = lb;               // where the next entry goes
     int G = 0;                            // row-groups of this lane in the global list so far (padding included)
     int nhit = 0;                         // true neighbours
@@ -366,9 +378,11 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
                 const uint4 *mygl = reinterpret_cast<const uint4 *>(gl[g]);
                 tests += valid ? (unsigned)gcnt : 0u;
                 for (int kb = 0; kb < cmax; kb += 32) {
-                    // 32 candidates of the quarter's table (4 x 8 offsets per 16-byte read)
+                    // 32 candidates of the quarter's table (8 offsets per 16-byte read), 16 between two checks
+                    // of the buffer level
 #pragma unroll
                     for (int k8 = 0; k8 < 4; ++k8) {
+                        if (k8 == 2 && __any_sync(FULL, (int)(wp - lb) > 2 * (LBUF_ENTRIES - 16))) LIST_FLUSH();
                         const uint4 tw = mygl[(kb >> 3) + k8];
                         const unsigned wv[4] = {tw.x, tw.y, tw.z, tw.w};
 #pragma unroll
@@ -382,8 +396,8 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
                             }
                         }
                     }
-                    // room for another 32 entries in every lane?  (3 may stay behind after a flush)
-                    if (__any_sync(FULL, (int)(wp - lb) > 2 * (LBUF_ENTRIES - 32))) LIST_FLUSH();
+                    // room for another 16 entries in every lane?  (3 may stay behind after a flush)
+                    if (__any_sync(FULL, (int)(wp - lb) > 2 * (LBUF_ENTRIES - 16))) LIST_FLUSH();
                 }
                 __syncwarp();
             }
@@ -412,10 +426,33 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
 #undef LIST_FLUSH
     if (threadIdx.x == 0) {
         d.tile_flag[tile] = sm.overflow ? 1 : 0;
+        const unsigned cyc = (unsigned)(clock64() - t_begin);
+        d.tile_cycles[tile] = cyc;
+        atomicAdd(d.cull_cycles, (unsigned long long)cyc);
         if (sm.overflow) atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], 1ull);
     }
-    __syncthreads();
-    }   // tile loop
+    }
+}
+
+// Which tiles go first in this build: those that cost more than 1.5x the average in the previous one.
+__global__ void __launch_bounds__(256) k_tile_plan(Dev d, int ntile)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ntile) return;
+    const unsigned long long sum = *d.cull_cycles;
+    bool heavy = 2ull * (unsigned long long)d.tile_cycles[t] * (unsigned long long)ntile > 3ull * sum;
+    if (heavy) {
+        const unsigned k = atomicAdd(d.nheavy, 1u);
+        if (k < (unsigned)d.heavy_cap) d.heavy_list[k] = (unsigned)t;
+        else heavy = false;                // list full: the tile stays in curve order
+    }
+    d.heavy_mark[t] = heavy ? 1 : 0;
+}
+
+// nheavy may have counted past the capacity
+__global__ void k_tile_plan_clamp(Dev d)
+{
+    if (*d.nheavy > (unsigned)d.heavy_cap) *d.nheavy = (unsigned)d.heavy_cap;
 }
 
 // entry e (0..3) of a row-group word pair
@@ -432,8 +469,8 @@ __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4 *s_pm = reinterpret_cast<float4 *>(smem_raw);
-    const int tile = blockIdx.x;
-    if (d.tile_flag[tile]) return;
+    const int tile = sph_tile_of_block(d, blockIdx.x);
+    if (tile < 0 || d.tile_flag[tile]) return;
     const int ncand = d.tile_ncand[tile];
     const unsigned *cand = d.cand + d.tile_off[tile];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -527,8 +564,8 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     unsigned char *s1 = smem_raw, *s2 = s1 + SPH_SE * 16, *s3 = s2 + SPH_SE * 16, *s4 = s3 + SPH_SE * 16,
                   *s5 = s4 + SPH_SE * 16;
-    const int tile = blockIdx.x;
-    if (d.tile_flag[tile]) return;
+    const int tile = sph_tile_of_block(d, blockIdx.x);
+    if (tile < 0 || d.tile_flag[tile]) return;
     const int ncand = d.tile_ncand[tile];
     const unsigned *cand = d.cand + d.tile_off[tile];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -668,8 +705,12 @@ int sph_launch_cull(sph_ctx *c)
     int rc = set_smem(c, (const void *)k_cull, sizeof(CullSmem));
     if (rc) return rc;
     int ntile = sph_div_up(d.nchunk, SPH_TILE_CHUNKS);
-    k_cull<<<ntile, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, ntile);
-    c->launches++;
+    SPH_CUDA(c, cudaMemsetAsync(d.nheavy, 0, sizeof(unsigned), c->stream));
+    k_tile_plan<<<sph_div_up(ntile, 256), 256, 0, c->stream>>>(d, ntile);
+    k_tile_plan_clamp<<<1, 1, 0, c->stream>>>(d);
+    SPH_CUDA(c, cudaMemsetAsync(d.cull_cycles, 0, sizeof(unsigned long long), c->stream));
+    k_cull<<<d.heavy_cap + ntile, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, ntile);
+    c->launches += 3;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
 }
@@ -683,7 +724,7 @@ int sph_launch_density_l(sph_ctx *c)
     size_t bytes = (size_t)SPH_SE * sizeof(float4);
     int rc = set_smem(c, (const void *)k_density_l, bytes);
     if (rc) return rc;
-    k_density_l<<<sph_div_up(d.nchunk, SPH_TILE_CHUNKS), SPH_TILE, bytes, c->stream>>>(d, c->p.kappa);
+    k_density_l<<<d.heavy_cap + sph_div_up(d.nchunk, SPH_TILE_CHUNKS), SPH_TILE, bytes, c->stream>>>(d, c->p.kappa);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return sph_launch_density(c, true);               // the flagged tiles, if any
@@ -696,7 +737,7 @@ static int launch_pair_l(sph_ctx *c)
     size_t bytes = (size_t)SPH_SE * (TENSOR ? 68 : 48);
     int rc = set_smem(c, (const void *)k_pair_l<GRAD, FORCE, TENSOR>, bytes);
     if (rc) return rc;
-    k_pair_l<GRAD, FORCE, TENSOR><<<sph_div_up(d.nchunk, SPH_TILE_CHUNKS), SPH_TILE, bytes, c->stream>>>(d, c->p);
+    k_pair_l<GRAD, FORCE, TENSOR><<<d.heavy_cap + sph_div_up(d.nchunk, SPH_TILE_CHUNKS), SPH_TILE, bytes, c->stream>>>(d, c->p);
     return SPH_OK;
 }
 
