@@ -75,6 +75,7 @@ struct CullSmem {
     float4 glo[4 * SPH_TILE_CHUNKS], ghi[4 * SPH_TILE_CHUNKS];   // quarter-warp boxes
     float4 tlo, thi;                     // tile box (tlo.w = max H)
     unsigned selfslot[SPH_TILE];         // slot of each target of the tile in its own candidate list
+    alignas(16) unsigned short sentinels[32];            // a block of padding offsets (pos[SPH_SE])
     alignas(16) unsigned short gl[SPH_TILE_CHUNKS][4][SPH_GCAP];     // per quarter-warp: candidates still to test, ascending,
                                                          // as byte offsets (slot * 16) into pos[]
     int nsrc, ntotal, nfront, overflow;
@@ -168,6 +169,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
         sm.overflow = 0;
         sm.pos[SPH_SE] = make_float4(1.0e30f, 1.0e30f, 1.0e30f, -1.f);
     }
+    if (threadIdx.x < 32) sm.sentinels[threadIdx.x] = (unsigned short)(SPH_SE << 4);
     sm.selfslot[threadIdx.x] = 0xffffffffu;
     __syncthreads();
     if (warp == 0) {                                   // tile box = union of its chunk boxes
@@ -349,57 +351,75 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             const int Gstart = G;
             unsigned short(*gl)[SPH_GCAP] = sm.gl[warp];
             const unsigned char *const posb = reinterpret_cast<const unsigned char *>(sm.pos);
+            // Every quarter keeps a ring of SPH_GCAP offsets.  The rings are filled from the flag words
+            // until every quarter has a block of 32 (or one ring is full, or the round is exhausted);
+            // then each quarter that has a block tests it.  Quarters see different numbers of
+            // candidates: this way a lane tests padding only in the last block of a round.
             int base = 0;
-            while (base < nr) {
-                int c0 = 0, c1 = 0, c2 = 0, c3 = 0;
-                while (base < nr && max(max(c0, c1), max(c2, c3)) + 32 <= SPH_GCAP) {
+            int h0 = 0, h1 = 0, h2 = 0, h3 = 0;           // ring heads (entries consumed), multiples of 32
+            int t0 = 0, t1 = 0, t2 = 0, t3 = 0;           // ring tails (entries produced)
+            const unsigned short sent = (unsigned short)(SPH_SE << 4);
+            for (;;) {
+                while (base < nr) {
+                    const int a0 = t0 - h0, a1 = t1 - h1, a2 = t2 - h2, a3 = t3 - h3;
+                    if (max(max(a0, a1), max(a2, a3)) + 32 > SPH_GCAP) break;     // a ring could overflow
+                    if (min(min(a0, a1), min(a2, a3)) >= 32) break;               // every quarter has a block
                     const int s = base + lane;
                     const unsigned f = s < nr ? (sm.flag[s] >> fshift) & 15u : 0u;
                     const unsigned m0 = __ballot_sync(FULL, f & 1u), m1 = __ballot_sync(FULL, f & 2u),
                                    m2 = __ballot_sync(FULL, f & 4u), m3 = __ballot_sync(FULL, f & 8u);
                     const unsigned short so = (unsigned short)(s << 4);
-                    if (f & 1u) gl[0][c0 + __popc(m0 & lt)] = so;
-                    if (f & 2u) gl[1][c1 + __popc(m1 & lt)] = so;
-                    if (f & 4u) gl[2][c2 + __popc(m2 & lt)] = so;
-                    if (f & 8u) gl[3][c3 + __popc(m3 & lt)] = so;
-                    c0 += __popc(m0); c1 += __popc(m1); c2 += __popc(m2); c3 += __popc(m3);
+                    if (f & 1u) gl[0][(t0 + __popc(m0 & lt)) & (SPH_GCAP - 1)] = so;
+                    if (f & 2u) gl[1][(t1 + __popc(m1 & lt)) & (SPH_GCAP - 1)] = so;
+                    if (f & 4u) gl[2][(t2 + __popc(m2 & lt)) & (SPH_GCAP - 1)] = so;
+                    if (f & 8u) gl[3][(t3 + __popc(m3 & lt)) & (SPH_GCAP - 1)] = so;
+                    t0 += __popc(m0); t1 += __popc(m1); t2 += __popc(m2); t3 += __popc(m3);
                     base += 32;
                 }
+                const bool drain = base >= nr;
+                const int a0 = t0 - h0, a1 = t1 - h1, a2 = t2 - h2, a3 = t3 - h3;
+                // entries each quarter tests now: a full block, or what is left when the round is exhausted
+                const int n0 = a0 >= 32 ? 32 : (drain ? a0 : 0), n1 = a1 >= 32 ? 32 : (drain ? a1 : 0),
+                          n2 = a2 >= 32 ? 32 : (drain ? a2 : 0), n3 = a3 >= 32 ? 32 : (drain ? a3 : 0);
+                if ((n0 | n1 | n2 | n3) == 0) break;      // only when drained and empty
+                if (lane >= n0 && n0 > 0) gl[0][(h0 + lane) & (SPH_GCAP - 1)] = sent;
+                if (lane >= n1 && n1 > 0) gl[1][(h1 + lane) & (SPH_GCAP - 1)] = sent;
+                if (lane >= n2 && n2 > 0) gl[2][(h2 + lane) & (SPH_GCAP - 1)] = sent;
+                if (lane >= n3 && n3 > 0) gl[3][(h3 + lane) & (SPH_GCAP - 1)] = sent;
                 __syncwarp();
-                const int gcnt = g == 0 ? c0 : (g == 1 ? c1 : (g == 2 ? c2 : c3));
-                const int cmax = max(max(c0, c1), max(c2, c3));
-                const int cpad = (cmax + 31) & ~31;
-                const unsigned short sent = (unsigned short)(SPH_SE << 4);
-                for (int k = c0 + lane; k < cpad; k += 32) gl[0][k] = sent;
-                for (int k = c1 + lane; k < cpad; k += 32) gl[1][k] = sent;
-                for (int k = c2 + lane; k < cpad; k += 32) gl[2][k] = sent;
-                for (int k = c3 + lane; k < cpad; k += 32) gl[3][k] = sent;
-                __syncwarp();
-                const uint4 *mygl = reinterpret_cast<const uint4 *>(gl[g]);
-                tests += valid ? (unsigned)gcnt : 0u;
-                for (int kb = 0; kb < cmax; kb += 32) {
-                    // 32 candidates of the quarter's table (8 offsets per 16-byte read), 16 between two checks
-                    // of the buffer level
+                const int ng = g == 0 ? n0 : (g == 1 ? n1 : (g == 2 ? n2 : n3));
+                const int hg = g == 0 ? h0 : (g == 1 ? h1 : (g == 2 ? h2 : h3));
+                // a quarter without a block reads 32 sentinels
+                const uint4 *mygl = ng ? reinterpret_cast<const uint4 *>(&gl[g][hg & (SPH_GCAP - 1)])
+                                       : reinterpret_cast<const uint4 *>(sm.sentinels);
+                tests += valid ? (unsigned)ng : 0u;
+                // 32 candidates of the quarter's ring (8 offsets per 16-byte read), 16 between two checks of
+                // the list buffer level
 #pragma unroll
-                    for (int k8 = 0; k8 < 4; ++k8) {
-                        if (k8 == 2 && __any_sync(FULL, (int)(wp - lb) > 2 * (LBUF_ENTRIES - 16))) LIST_FLUSH();
-                        const uint4 tw = mygl[(kb >> 3) + k8];
-                        const unsigned wv[4] = {tw.x, tw.y, tw.z, tw.w};
+                for (int k8 = 0; k8 < 4; ++k8) {
+                    if (k8 == 2 && __any_sync(FULL, (int)(wp - lb) > 2 * (LBUF_ENTRIES - 16))) LIST_FLUSH();
+                    const uint4 tw = mygl[k8];
+                    const unsigned wv[4] = {tw.x, tw.y, tw.z, tw.w};
 #pragma unroll
-                        for (int e = 0; e < 8; ++e) {
-                            const unsigned off = (e & 1) ? (wv[e >> 1] >> 16) : (wv[e >> 1] & 0xffffu);
-                            const float4 q = *reinterpret_cast<const float4 *>(posb + off);
-                            const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
-                            if (r2 < fmaxf(H2i, q.w) && off != selfoff) {
-                                *reinterpret_cast<unsigned short *>(wp) = (unsigned short)off;
-                                wp += 2;
-                            }
+                    for (int e = 0; e < 8; ++e) {
+                        const unsigned off = (e & 1) ? (wv[e >> 1] >> 16) : (wv[e >> 1] & 0xffffu);
+                        const float4 q = *reinterpret_cast<const float4 *>(posb + off);
+                        const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
+                        if (r2 < fmaxf(H2i, q.w) && off != selfoff) {
+                            *reinterpret_cast<unsigned short *>(wp) = (unsigned short)off;
+                            wp += 2;
                         }
                     }
-                    // room for another 16 entries in every lane?  (3 may stay behind after a flush)
-                    if (__any_sync(FULL, (int)(wp - lb) > 2 * (LBUF_ENTRIES - 16))) LIST_FLUSH();
                 }
+                // room for another 16 entries in every lane?  (3 may stay behind after a flush)
+                if (__any_sync(FULL, (int)(wp - lb) > 2 * (LBUF_ENTRIES - 16))) LIST_FLUSH();
                 __syncwarp();
+                // consumed blocks leave the rings (a partial last block leaves it empty: head = tail, aligned)
+                h0 += n0 == 32 ? 32 : 0; h1 += n1 == 32 ? 32 : 0; h2 += n2 == 32 ? 32 : 0; h3 += n3 == 32 ? 32 : 0;
+                if (n0 < 32 && n0 > 0) { h0 = 0; t0 = 0; }
+                if (n1 < 32 && n1 > 0) { h1 = 0; t1 = 0; }
+                if (n2 < 32 && n2 > 0) { h2 = 0; t2 = 0; }
+                if (n3 < 32 && n3 > 0) { h3 = 0; t3 = 0; }
             }
             // ---- end of the round: pad the last row-group, flush, pad every lane to the warp's longest list
             nhit += 4 * (G - Gstart) + ((int)(wp - lb) >> 1);
