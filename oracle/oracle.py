@@ -11,7 +11,8 @@ imports neither; parameter records are duck-typed (attributes kappa, alpha, ...,
 
 Parity-unpinned choices (no authority in PAPER.md; listed in DESIGN.md): the kernel's
 functional form and kappa (Q3), AV constants (Q6), the analytic EOS stand-in (Q13), the
-singular-C fallback rule (Q9), the fixed-particle rule (Q16).  Everything else is pinned by
+singular-C fallback rule (Q9), the fixed-particle rule (Q16), the target mass and the
+safeguards of the smoothing-length iteration (Q20).  Everything else is pinned by
 tests/test_oracle_*.py.
 """
 from __future__ import annotations
@@ -107,6 +108,44 @@ def density(x, y, z, m, h, kappa, offsets, lst):
     lib().orc_density(C.c_longlong(n), _d(x), _d(y), _d(z), _d(m), _d(h), C.c_double(kappa),
                       offsets.ctypes.data_as(_lp), lst.ctypes.data_as(_ip), _d(rho), _d(omega))
     return rho, omega
+
+
+# ---------------------------------------------------------------------------
+# NEXT-1 -- adaptive smoothing length (Eq. 2)
+# ---------------------------------------------------------------------------
+H_OMEGA_FLOOR = 0.1        # reading Q20: the Newton slope uses max(Omega, 0.1)
+H_STEP_LIMITS = (0.8, 1.25)  # reading Q20: h changes by at most this factor per iteration
+
+
+def kernel_mass(rho, h, kappa):
+    """M_tot = (4/3) pi R_kernel(h)^3 rho with R_kernel = kappa h (Eq. 2)."""
+    return 4.0 / 3.0 * np.pi * (kappa * h) ** 3 * rho
+
+
+def adapt_h(x, y, z, m, h, kappa, n_target, iterations, mode="brute"):
+    """Newton-Raphson iterations on h_i towards a constant effective kernel mass:
+    solve f(h_i) = M_tot^i(h_i) - n_target m_i = 0, M_tot of Eq. 2 with rho_i(h_i) of Eq. 1.
+    "The density and its derivative with respect to h_i are computed and used": with Eq. 3,
+    d(h^3 rho)/dh = 3 h^2 rho + h^3 drho/dh = 3 h^2 rho Omega, hence
+        h <- h [1 - (1 - n_target m / M_tot) / (3 Omega)].
+    Readings (Q20, ours: the paper gives neither the target mass nor safeguards): the target is
+    n_target particle masses; the slope uses max(Omega, H_OMEGA_FLOOR); the factor is limited to
+    H_STEP_LIMITS; h is stored in fp32 between iterations (the neighbour predicate is defined on
+    fp32 h, reading Q4).  Returns (h [fp32 values as fp64], rho, Omega of the last density pass
+    -- taken at the h BEFORE the last update --, history of max |factor - 1|)."""
+    x, y, z, m = map(_f64, (x, y, z, m))
+    h = _f64(np.asarray(h, dtype=np.float32))
+    hist = []
+    rho = omega = None
+    for _ in range(iterations):
+        _, off, lst = neighbors(x, y, z, h, kappa, GATHER, mode)
+        rho, omega = density(x, y, z, m, h, kappa, off, lst)
+        ratio = n_target * m / kernel_mass(rho, h, kappa)
+        fac = 1.0 - (1.0 - ratio) / (3.0 * np.maximum(omega, H_OMEGA_FLOOR))
+        fac = np.clip(fac, H_STEP_LIMITS[0], H_STEP_LIMITS[1])
+        hist.append(float(np.abs(fac - 1.0).max()))
+        h = _f64((h * fac).astype(np.float32))
+    return h, rho, omega, hist
 
 
 # ---------------------------------------------------------------------------
