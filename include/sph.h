@@ -73,6 +73,7 @@ enum {
     SPH_F_CFLAG,        /* 1.0 where C fell back to 1 (reading Q9)        */
     SPH_F_NGATHER,      /* |gather set| as float                          */
     SPH_F_NSYMMETRIC,   /* |symmetric set| as float                       */
+    SPH_F_H,            /* smoothing length (after sph_adapt_h)           */
     SPH_F_A = 32,       /* +0..2   acceleration, Eq. 18 (+ a_ext)         */
     SPH_F_V = 36,       /* +0..2   velocity after the closing kick        */
     SPH_F_X = 40,       /* +0..2   position                               */
@@ -157,6 +158,18 @@ int sph_build_neighbors(sph_ctx *ctx, const sph_state *state, long long n);
 
 /* S2: rho_i (Eq. 1), Omega_i (Eq. 3), |gather set|.  Needs sph_build_neighbors. */
 int sph_density(sph_ctx *ctx);
+
+/* NEXT-1 (the step before the path): adaptive smoothing length.  `iterations`
+ * Newton-Raphson updates of the resident h_i towards a constant effective kernel mass (Eq. 2),
+ *   M_tot,i = (4/3) pi (kappa h_i)^3 rho_i(h_i) = n_target m_i,
+ * with the slope from Eq. 3: h <- h [1 - (1 - n_target m / M_tot) / (3 max(Omega, 0.1))], the factor
+ * limited to [0.8, 1.25] (reading Q20 in DESIGN.md).  Every iteration is one density pass (skipped when
+ * a current one exists), the per-particle update, and a rebuild of the chunk boxes, tree and neighbour
+ * lists for the new support radii; the particle order is kept.  Afterwards the lists are current and
+ * sph_density is the next call.  max_change: DEVICE pointer to one float (max_i |factor - 1| of the last
+ * iteration) or NULL.  The caller's h array is not written: read h with sph_get_field(SPH_F_H).
+ * Asynchronous.  Errors: EINVAL (n_target <= 0, iterations < 0), EORDER (nothing resident). */
+int sph_adapt_h(sph_ctx *ctx, float n_target, int iterations, float *max_change);
 
 /* S3 / S6: per-particle strength update, phase = SPH_PREDICT | SPH_CLOSE | SPH_DERIVATIVES.
  * PREDICT needs sph_density; CLOSE needs sph_gradients (if SPH_STRENGTH) and sph_forces.

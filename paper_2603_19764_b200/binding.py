@@ -21,7 +21,7 @@ PREDICT, CLOSE, DERIVATIVES = 0, 1, 2
 GATHER, SYMMETRIC = 0, 1
 
 F = dict(RHO=0, OMEGA=1, P=2, CS=3, T=4, GAMMA=5, Y=6, MUMAX=7, DUDT=8, DT=9, EACC=10, EPS2=11, U=12,
-         CFLAG=13, NGATHER=14, NSYMMETRIC=15, A=32, V=36, X=40, SPRED=48, S=56, DSDT=64, F=80, CINV=96, G=112)
+         CFLAG=13, NGATHER=14, NSYMMETRIC=15, H=16, A=32, V=36, X=40, SPRED=48, S=56, DSDT=64, F=80, CINV=96, G=112)
 T_SLOTS = ("build", "density", "predict", "gradient", "force", "close", "kickdrift", "step")
 C_SLOTS = ("pairs_gather", "pairs_symmetric", "tests_density", "tests_force", "cfallback", "tests_cull",
            "candidates", "list_overflow")
@@ -31,7 +31,7 @@ OPT_FIELDS = ("gx", "gy", "gz")
 
 # every symbol include/sph.h declares (tests check the library exports all of them)
 SYMBOLS = ("sph_workspace_bytes", "sph_init", "sph_build_neighbors", "sph_density", "sph_strength_update",
-           "sph_gradients", "sph_forces", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
+           "sph_gradients", "sph_forces", "sph_adapt_h", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
            "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_launch_count",
            "sph_last_cuda_error", "sph_strerror", "sph_destroy")
 
@@ -89,6 +89,8 @@ def load():
     lib.sph_get_timings.argtypes = [vp, C.POINTER(fl), i]
     lib.sph_get_counters.argtypes = [vp, C.POINTER(ll), i]
     lib.sph_get_tile_stats.argtypes = [vp, vp, vp, vp, i]
+    lib.sph_adapt_h.argtypes = [vp, fl, i, vp]
+    lib.sph_adapt_h.restype = i
     lib.sph_launch_count.restype = ll
     lib.sph_launch_count.argtypes = [vp]
     lib.sph_last_cuda_error.argtypes = [vp]
@@ -260,6 +262,11 @@ class Sph:
         cs = (C.c_longlong * len(C_SLOTS))()
         self._check(self.lib.sph_get_counters(self.ctx, cs, len(C_SLOTS)), "sph_get_counters")
         return {k: int(cs[i]) for i, k in enumerate(C_SLOTS)}
+
+    def adapt_h(self, n_target: float, iterations: int, max_change=None):
+        """sph_adapt_h; max_change: optional 1-element float32 device tensor."""
+        ptr = max_change.data_ptr() if max_change is not None else None
+        self._check(self.lib.sph_adapt_h(self.ctx, float(n_target), int(iterations), ptr), "sph_adapt_h")
 
     def get_tile_stats(self):
         """(candidates, cycles, fell_back) per tile of the last neighbour build, as numpy arrays (host)."""

@@ -111,6 +111,7 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
     o.bbox = b.take<float>(8);
     o.dt_cur = b.take<float>(1);
     o.dt_next = b.take<float>(1);
+    o.hchange = b.take<float>(1);
     o.counters = b.take<unsigned long long>(SPH_C_COUNT);
     o.keys = b.take<unsigned long long>(N); o.keys_alt = b.take<unsigned long long>(N);
     o.perm = b.take<unsigned>(N); o.perm_alt = b.take<unsigned>(N);
@@ -244,6 +245,32 @@ extern "C" int sph_density(sph_ctx *c)
     if (rc) return rc;
     c->have_density = true;
     c->have_predict = c->have_grad = c->have_force = false;
+    return SPH_OK;
+}
+
+extern "C" int sph_adapt_h(sph_ctx *c, float n_target, int iterations, float *max_change)
+{
+    if (!c || !(n_target > 0.f) || iterations < 0) return SPH_EINVAL;
+    if (!c->resident) return SPH_EORDER;
+    int rc;
+    for (int it = 0; it < iterations; ++it) {
+        if (!c->have_density) {
+            rc = sph_density(c);
+            if (rc) return rc;
+        }
+        rc = sph_launch_h_update(c, n_target);
+        if (rc) return rc;
+        // new support radii: chunk boxes, tree and lists again (the curve order stays)
+        rc = sph_launch_tree(c);
+        if (rc) return rc;
+        if (c->use_lists) {
+            rc = sph_launch_cull(c);
+            if (rc) return rc;
+        }
+        c->have_density = c->have_predict = c->have_grad = c->have_force = false;
+    }
+    if (iterations > 0 && max_change)
+        SPH_CUDA(c, cudaMemcpyAsync(max_change, c->d.hchange, sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
     return SPH_OK;
 }
 
@@ -455,6 +482,7 @@ extern "C" int sph_get_field(sph_ctx *c, int id, float *dst)
     case SPH_F_CFLAG: src = d.cflag; break;
     case SPH_F_NGATHER: src = (const float *)d.ngather; as_int = 1; break;
     case SPH_F_NSYMMETRIC: src = (const float *)d.nsym; as_int = 1; break;
+    case SPH_F_H: return sph_launch_get_h(c, dst);
     default: break;
     }
     if (!src) {

@@ -303,6 +303,62 @@ int sph_launch_kick_drift(sph_ctx *c, float dt)
     return SPH_OK;
 }
 
+// ------------------------------------------------------------------------------------------
+// NEXT-1: one Newton-Raphson update of h_i towards a constant kernel mass (Eq. 2):
+//   M_tot = (4/3) pi (kappa h)^3 rho(h),  d(h^3 rho)/dh = 3 h^2 rho Omega (Eq. 3)
+//   h <- h [1 - (1 - n_target m / M_tot) / (3 max(Omega, 0.1))], factor limited to [0.8, 1.25] (reading Q20)
+// Per particle, in fp64 from the fp64 density; h is stored back in fp32.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_h_update(Dev d, float kappa, float n_target, float *hchange)
+{
+    const long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    float change = 0.f;
+    if (i < d.n) {
+        float4 vh = d.r.vh[i];
+        const double h = (double)vh.w, H = (double)kappa * h;
+        const double mtot = 4.0 / 3.0 * 3.14159265358979323846 * H * H * H * d.rho64[i];
+        const double ratio = (double)n_target * (double)d.r.pm[i].w / mtot;
+        double fac = 1.0 - (1.0 - ratio) / (3.0 * fmax((double)d.omega[i], 0.1));
+        fac = fmin(fmax(fac, 0.8), 1.25);
+        vh.w = (float)(h * fac);
+        d.r.vh[i] = vh;
+        change = (float)fabs(fac - 1.0);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) change = fmaxf(change, __shfl_xor_sync(0xffffffffu, change, o));
+    if ((threadIdx.x & 31) == 0 && change > 0.f) atomicMax((unsigned *)hchange, __float_as_uint(change));
+}
+
+int sph_launch_h_update(sph_ctx *c, float n_target)
+{
+    Dev &d = c->d;
+    SPH_CUDA(c, cudaMemsetAsync(d.hchange, 0, sizeof(float), c->stream));
+    if (d.n > 0) {
+        k_h_update<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, c->p.kappa, n_target, d.hchange);
+        c->launches++;
+    }
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+// h in caller order (sph_get_field(SPH_F_H))
+__global__ void __launch_bounds__(256) k_scatter_h(const float4 *__restrict__ vh, const unsigned *__restrict__ orig,
+                                                   long long n, float *__restrict__ dst)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i < n) dst[orig[i]] = vh[i].w;
+}
+
+int sph_launch_get_h(sph_ctx *c, float *dst)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    k_scatter_h<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d.r.vh, (const unsigned *)d.r.s[PP_ORIG], d.n, dst);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
 int sph_launch_get_field(sph_ctx *c, const float *src, float *dst, int as_int)
 {
     Dev &d = c->d;
