@@ -206,6 +206,12 @@ int sph_get_field(sph_ctx *ctx, int field_id, float *dst);
  * NOT checked on the device; the caller sizes list from counts). */
 int sph_get_neighbors(sph_ctx *ctx, int which, int *counts, const long long *offsets, int *list);
 
+/* S8 diagnostics (the conservation checks of PAPER.md:349-357): out = DEVICE double[8] =
+ * { sum m, sum m v (3), sum m x cross v (3), sum m (v.v/2 + u) } over the resident particles at the
+ * full step (after the last closing kick; the ingested state before any step), accumulated in fp64
+ * in a fixed order (bitwise repeatable).  Asynchronous.  Errors: EINVAL, EORDER. */
+int sph_get_diagnostics(sph_ctx *ctx, double *out);
+
 /* HOST outputs.  Both synchronise the stream. */
 int sph_get_timings(sph_ctx *ctx, float *ms, int n);            /* SPH_T_* slots              */
 int sph_get_counters(sph_ctx *ctx, long long *counters, int n); /* SPH_C_* slots              */

@@ -32,7 +32,7 @@ OPT_FIELDS = ("gx", "gy", "gz")
 # every symbol include/sph.h declares (tests check the library exports all of them)
 SYMBOLS = ("sph_workspace_bytes", "sph_init", "sph_build_neighbors", "sph_density", "sph_strength_update",
            "sph_gradients", "sph_forces", "sph_adapt_h", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
-           "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_launch_count",
+           "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_get_diagnostics", "sph_launch_count",
            "sph_last_cuda_error", "sph_strerror", "sph_destroy")
 
 
@@ -89,6 +89,8 @@ def load():
     lib.sph_get_timings.argtypes = [vp, C.POINTER(fl), i]
     lib.sph_get_counters.argtypes = [vp, C.POINTER(ll), i]
     lib.sph_get_tile_stats.argtypes = [vp, vp, vp, vp, i]
+    lib.sph_get_diagnostics.argtypes = [vp, vp]
+    lib.sph_get_diagnostics.restype = i
     lib.sph_adapt_h.argtypes = [vp, fl, i, vp]
     lib.sph_adapt_h.restype = i
     lib.sph_launch_count.restype = ll
@@ -267,6 +269,12 @@ class Sph:
         """sph_adapt_h; max_change: optional 1-element float32 device tensor."""
         ptr = max_change.data_ptr() if max_change is not None else None
         self._check(self.lib.sph_adapt_h(self.ctx, float(n_target), int(iterations), ptr), "sph_adapt_h")
+
+    def get_diagnostics(self):
+        """float64 device tensor [8]: M, P (3), L (3), E = sum m (v^2/2 + u)."""
+        out = self.torch.zeros(8, dtype=self.torch.float64, device=self.device)
+        self._check(self.lib.sph_get_diagnostics(self.ctx, out.data_ptr()), "sph_get_diagnostics")
+        return out
 
     def get_tile_stats(self):
         """(candidates, cycles, fell_back) per tile of the last neighbour build, as numpy arrays (host)."""

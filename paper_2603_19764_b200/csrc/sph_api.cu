@@ -112,6 +112,7 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
     o.dt_cur = b.take<float>(1);
     o.dt_next = b.take<float>(1);
     o.hchange = b.take<float>(1);
+    o.diag_part = b.take<double>(592 * 8);
     o.counters = b.take<unsigned long long>(SPH_C_COUNT);
     o.keys = b.take<unsigned long long>(N); o.keys_alt = b.take<unsigned long long>(N);
     o.perm = b.take<unsigned>(N); o.perm_alt = b.take<unsigned>(N);
@@ -527,6 +528,13 @@ extern "C" int sph_get_counters(sph_ctx *c, long long *out, int n)
     SPH_CUDA(c, cudaStreamSynchronize(c->stream));
     for (int k = 0; k < n && k < SPH_C_COUNT; ++k) out[k] = (long long)h[k];
     return SPH_OK;
+}
+
+extern "C" int sph_get_diagnostics(sph_ctx *c, double *out)
+{
+    if (!c || !out) return SPH_EINVAL;
+    if (!c->resident) return SPH_EORDER;
+    return sph_launch_diagnostics(c, out);
 }
 
 extern "C" int sph_get_tile_stats(sph_ctx *c, int *ncand, unsigned *cycles, unsigned char *flag, int capacity)

@@ -101,6 +101,7 @@ struct Dev {
     // scalars on the device
     float *bbox;                            // 6 floats as ordered ints: lo xyz, hi xyz
     float *dt_cur, *dt_next;                // step in use / CFL step from the last CLOSE
+    double *diag_part;                      // [592][8] per-block partial sums of sph_get_diagnostics
     float *hchange;                         // max |factor - 1| of the last smoothing-length update
     unsigned long long *counters;           // SPH_C_COUNT
     // sort scratch
@@ -149,6 +150,7 @@ int sph_launch_kick_drift(sph_ctx *c, float dt);
 int sph_launch_get_field(sph_ctx *c, const float *src, float *dst, int as_int);
 int sph_launch_get_position(sph_ctx *c, int comp, float *dst);
 int sph_launch_get_h(sph_ctx *c, float *dst);
+int sph_launch_diagnostics(sph_ctx *c, double *out);
 int sph_launch_h_update(sph_ctx *c, float n_target);
 int sph_launch_neighbors(sph_ctx *c, int which, int *counts, const long long *offsets, int *list, bool flagged_only);
 int sph_launch_download(sph_ctx *c, sph_state *st);

@@ -341,6 +341,62 @@ int sph_launch_h_update(sph_ctx *c, float n_target)
     return SPH_OK;
 }
 
+// ------------------------------------------------------------------------------------------
+// S8 diagnostics (the conservation checks): M, sum m v, sum m x cross v, sum m (v^2/2 + u)
+// of the state at the full step, in fp64, in a fixed order (per-block partials, then one block):
+// bitwise repeatable.
+// ------------------------------------------------------------------------------------------
+#define DIAG_BLOCKS 592
+__global__ void __launch_bounds__(256) k_diag_partial(Dev d, double *__restrict__ part)
+{
+    double s[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < d.n; i += (long long)gridDim.x * blockDim.x) {
+        const float4 pm = d.r.pm[i];
+        const double m = pm.w, x = pm.x, y = pm.y, z = pm.z;
+        const double vx = d.vfull[0][i], vy = d.vfull[1][i], vz = d.vfull[2][i], u = d.ufull[i];
+        s[0] += m;
+        s[1] += m * vx; s[2] += m * vy; s[3] += m * vz;
+        s[4] += m * (y * vz - z * vy); s[5] += m * (z * vx - x * vz); s[6] += m * (x * vy - y * vx);
+        s[7] += m * (0.5 * (vx * vx + vy * vy + vz * vz) + u);
+    }
+    __shared__ double sh[8][8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s[k] += __shfl_xor_sync(0xffffffffu, s[k], o);
+        if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5][k] = s[k];
+    }
+    __syncthreads();
+    if (threadIdx.x < 8) {
+        double t = 0.0;
+        for (int w = 0; w < 8; ++w) t += sh[w][threadIdx.x];
+        part[blockIdx.x * 8 + threadIdx.x] = t;
+    }
+}
+
+__global__ void k_diag_final(const double *__restrict__ part, int nblocks, double *__restrict__ out)
+{
+    // 8 warps, one per quantity; lanes stride over the partials, then a shuffle tree: a fixed order
+    const int k = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double t = 0.0;
+    for (int b = lane; b < nblocks; b += 32) t += part[b * 8 + k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    if (lane == 0) out[k] = t;
+}
+
+int sph_launch_diagnostics(sph_ctx *c, double *out)
+{
+    Dev &d = c->d;
+    int nb = sph_div_up(d.n > 0 ? d.n : 1, 256);
+    if (nb > DIAG_BLOCKS) nb = DIAG_BLOCKS;
+    k_diag_partial<<<nb, 256, 0, c->stream>>>(d, d.diag_part);
+    k_diag_final<<<1, 256, 0, c->stream>>>(d.diag_part, nb, out);
+    c->launches += 2;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
 // h in caller order (sph_get_field(SPH_F_H))
 __global__ void __launch_bounds__(256) k_scatter_h(const float4 *__restrict__ vh, const unsigned *__restrict__ orig,
                                                    long long n, float *__restrict__ dst)
