@@ -88,6 +88,7 @@ struct CullSmem {
     float4 gc[4 * SPH_TILE_CHUNKS], ge[4 * SPH_TILE_CHUNKS];     // quarter-warp boxes, centre / half-extent
     float4 tlo, thi;                     // tile box (tlo.w = max H)
     unsigned selfslot[SPH_TILE];         // slot of each target of the tile in its own candidate list
+    unsigned short c1[SPH_TILE_CHUNKS][64];              // per warp: ring of the slots (as offsets) that reach its chunk
     alignas(16) unsigned short sentinels[32];            // a block of padding offsets (pos[SPH_SE])
     alignas(16) unsigned short gl[SPH_TILE_CHUNKS][4][SPH_GCAP];     // per quarter-warp: candidates still to test, ascending,
                                                          // as byte offsets (slot * 16) into pos[]
@@ -286,7 +287,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     __syncthreads();
     if (sm.overflow) {                                 // flagged before any list was written
         if (threadIdx.x == 0) {
-            d.tile_flag[tile] = 1;
+            d.tile_flag[tile] = (unsigned char)sm.overflow;     // which capacity: 1 walk, 2 pool, 4 rounds
             d.tile_ncand[tile] = 0;
             d.tile_off[tile] = 0;
             atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], 1ull);
@@ -374,25 +375,44 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             int base = 0;
             int h0 = 0, h1 = 0, h2 = 0, h3 = 0;           // ring heads (entries consumed), multiples of 32
             int t0 = 0, t1 = 0, t2 = 0, t3 = 0;           // ring tails (entries produced)
+            int ch = 0, ct = 0;                           // head / tail of the warp's ring of flagged slots
+            unsigned short *const c1 = sm.c1[warp];
             const unsigned short sent = (unsigned short)(SPH_SE << 4);
             for (;;) {
-                while (base < nr) {
+                // Two stages.  (1) one ballot per 32 slots keeps the slots that reach this warp's chunk at
+                // all (about a third); (2) 32 of those at a time are split over the four quarter rings
+                // (four ballots).  Every warp scans every slot of the round: stage 1 is the cheap part.
+                for (;;) {
                     const int a0 = t0 - h0, a1 = t1 - h1, a2 = t2 - h2, a3 = t3 - h3;
                     if (max(max(a0, a1), max(a2, a3)) + 32 > SPH_GCAP) break;     // a ring could overflow
                     if (min(min(a0, a1), min(a2, a3)) >= 32) break;               // every quarter has a block
-                    const int s = base + lane;
-                    const unsigned f = s < nr ? (sm.flag[s] >> fshift) & 15u : 0u;
+                    while (ct - ch < 32 && base < nr) {
+                        const int s = base + lane;
+                        const bool any = s < nr && ((sm.flag[s] >> fshift) & 15u) != 0u;
+                        const unsigned m = __ballot_sync(FULL, any);
+                        if (any) c1[(ct + __popc(m & lt)) & 63] = (unsigned short)(s << 4);
+                        ct += __popc(m);
+                        base += 32;
+                    }
+                    const int take = min(32, ct - ch);
+                    if (take == 0) break;                                         // round exhausted
+                    __syncwarp();
+                    unsigned f = 0u;
+                    unsigned short so = 0;
+                    if (lane < take) {
+                        so = c1[(ch + lane) & 63];
+                        f = (sm.flag[so >> 4] >> fshift) & 15u;
+                    }
+                    ch += take;
                     const unsigned m0 = __ballot_sync(FULL, f & 1u), m1 = __ballot_sync(FULL, f & 2u),
                                    m2 = __ballot_sync(FULL, f & 4u), m3 = __ballot_sync(FULL, f & 8u);
-                    const unsigned short so = (unsigned short)(s << 4);
                     if (f & 1u) gl[0][(t0 + __popc(m0 & lt)) & (SPH_GCAP - 1)] = so;
                     if (f & 2u) gl[1][(t1 + __popc(m1 & lt)) & (SPH_GCAP - 1)] = so;
                     if (f & 4u) gl[2][(t2 + __popc(m2 & lt)) & (SPH_GCAP - 1)] = so;
                     if (f & 8u) gl[3][(t3 + __popc(m3 & lt)) & (SPH_GCAP - 1)] = so;
                     t0 += __popc(m0); t1 += __popc(m1); t2 += __popc(m2); t3 += __popc(m3);
-                    base += 32;
                 }
-                const bool drain = base >= nr;
+                const bool drain = base >= nr && ct == ch;
                 const int a0 = t0 - h0, a1 = t1 - h1, a2 = t2 - h2, a3 = t3 - h3;
                 // entries each quarter tests now: a full block, or what is left when the round is exhausted
                 const int n0 = a0 >= 32 ? 32 : (drain ? a0 : 0), n1 = a1 >= 32 ? 32 : (drain ? a1 : 0),
@@ -461,7 +481,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     }
 #undef LIST_FLUSH
     if (threadIdx.x == 0) {
-        d.tile_flag[tile] = sm.overflow ? 1 : 0;
+        d.tile_flag[tile] = (unsigned char)sm.overflow;         // 8: list rows
         const unsigned cyc = (unsigned)(clock64() - t_begin);
         d.tile_cycles[tile] = cyc;
         atomicAdd(d.cull_cycles, (unsigned long long)cyc);
