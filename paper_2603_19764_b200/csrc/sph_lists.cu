@@ -546,7 +546,8 @@ __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
     // self term: q = 0, t = 1
     double sum = (double)pi.w;
     float sh = 3.f * pi.w;
-    int ng = 1, ntest = 1;
+    int ng = 1;
+    const int ntest = 1 + (valid ? d.nsym[i] : 0);      // every list entry is tested
     int round = 0;
     for (int r0 = 0; r0 < ncand; r0 += SPH_SE, ++round) {
         const int nr = min(SPH_SE, ncand - r0);
@@ -563,11 +564,10 @@ __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
                     const unsigned off = list_entry(w, e);
                     if (off == 0xffffu) continue;
                     const float4 q = *reinterpret_cast<const float4 *>(smem_raw + off);
-                    ++ntest;
                     float dx = __fsub_rn(pi.x, q.x), dy = __fsub_rn(pi.y, q.y), dz = __fsub_rn(pi.z, q.z);
                     float r2 = sph_r2(dx, dy, dz);
                     if (r2 < H2i) {
-                        float rinv = rsqrtf(fmaxf(r2, 1.0e-37f));
+                        float rinv = sph_rsqrt(fmaxf(r2, 1.0e-37f));
                         float r = r2 * rinv;
                         float qq = r * invH;
                         float t = fmaxf(0.f, 1.f - qq);
@@ -580,7 +580,9 @@ __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
                         const double yd = (double)rinv, td0 = r2d * yd;
                         double rd = fma(0.5 * td0, fma(-td0, yd, 1.0), td0);
                         double qd = rd * invHd;
-                        double td = fmax(0.0, 1.0 - qd);
+                        // no clamp at 0: membership (r2 < H_i^2 in fp32) already says q < 1 up to rounding, and
+                        // (1 - q)^4 of a q that exceeds 1 by 1e-7 is 1e-28 (fmax on doubles is nine instructions)
+                        double td = 1.0 - qd;
                         double t2 = td * td;
                         sum = fma((double)q.w * t2 * t2, fma(4.0, qd, 1.0), sum);
                         ++ng;

@@ -24,6 +24,15 @@ __device__ __forceinline__ float sph_rcp(float y)
     return r;
 }
 
+// 1 / sqrt(y) by one MUFU.RSQ (rsqrtf() adds a denormal-range rescue: three more instructions per call);
+// callers clamp y away from zero.
+__device__ __forceinline__ float sph_rsqrt(float y)
+{
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(y));
+    return r;
+}
+
 struct PairConst {
     float beta;       // Eq. 5
     float alpha2;     // alpha / 2: alpha cbar = alpha2 (c_i + c_j)
@@ -65,7 +74,7 @@ __device__ __forceinline__ void pair_term(const PairTarget &t, const PairConst &
 {
     const float dx = t.x - q1.x, dy = t.y - q1.y, dz = t.z - q1.z;
     const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    const float r = r2 * rsqrtf(fmaxf(r2, 1.0e-37f));
+    const float r = r2 * sph_rsqrt(fmaxf(r2, 1.0e-37f));
     const float invHj = sph_rcp(q2.w);
     const float ti = fmaxf(0.f, fmaf(-r, t.invH, 1.f));
     const float tj = fmaxf(0.f, fmaf(-r, invHj, 1.f));
