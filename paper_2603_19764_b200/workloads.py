@@ -309,6 +309,17 @@ def impact_pair(n_total: int = 4_400_000, seed: int = SEED_BASE + 3, contrast: f
                    f"number-density contrast {contrast:g}, eta_h {eta_h}; PCLIP_GLOBAL")
 
 
+def oblique_impact(n_total: int = 30_000, v_impact: float = 100.0, seed: int = SEED_BASE + 7) -> Workload:
+    """Stand-in for the paper's angular-momentum experiment (Fig. 7: oblique impact at
+    100 m/s and 45 degrees): two uniform lattice spheres (R = 50 km and 23 km, materials 0/1), just
+    touching, no external acceleration (self-gravity is not built here), h = 1.3 dx."""
+    wl = impact_pair(n_total, seed, 1.0, 1.3, v_impact=v_impact, name="oblique_impact")
+    for k in ("gx", "gy", "gz"):
+        wl.arrays[k][:] = 0.0
+    wl.notes = "uniform bodies, a_ext = 0, v = %g m/s at 45 degrees; PCLIP_GLOBAL" % v_impact
+    return wl
+
+
 def config(k: int, scale: float = 1.0) -> Workload:
     """BASELINE.json configs[k]; ``scale`` < 1 shrinks particle counts (parity-sized cases)."""
     if k == 0:
