@@ -215,32 +215,57 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     // ---- A1: breadth-first walk of the chunk tree by all warps (one parent per warp, one child per
     //          lane).  A node is kept only if its box reaches one of the tile's CHUNK boxes: a tile that
     //          straddles a gap of the space-filling curve has a huge union box but small chunk boxes.
+    //          If a level still overflows its capacity (a CHUNK that straddles such a gap has a huge box
+    //          too), the level is redone with the exact test: a node must be within reach of one of the
+    //          target PARTICLES of the chunks it was accepted for (32 point tests per chunk and node:
+    //          expensive, and needed by a few tiles in ten thousand).
     const float4 tlo = sm.tlo, thi = sm.thi;
+    sm.pos[threadIdx.x] = make_float4(pi.x, pi.y, pi.z, valid ? H2i * SPH_REACH_SLACK : -1.f);   // pos[] is free until A3
     for (int L = d.tree.nlev - 1; L >= 0; --L) {
         const int nf = sm.nfront;
-        for (int k = warp; k < nf; k += SPH_TILE_CHUNKS) {
-            int first = (int)sm.chunks[k] * SPH_ARITY;
-            int cnt = min(SPH_ARITY, d.tree.count[L] - first);
-            unsigned cm = 0;
-            bool pass = false;
-            if (lane < cnt) {
-                float4 clo = d.tree.lo[L][first + lane], chi = d.tree.hi[L][first + lane];
-                if (box_reach_sym(clo, chi, tlo, thi)) {
-                    for (int w = 0; w < nch; ++w)
-                        if (box_reach_sym(clo, chi, sm.blo[w], sm.bhi[w])) cm |= 1u << w;
-                    pass = cm != 0;
+        const int capL = (L == 1) ? SPH_CULL_MAXPAR : SPH_CULL_MAXSRC;         // level-1 parents index ctmp
+        for (int attempt = 0;; ++attempt) {
+            for (int k = warp; k < nf; k += SPH_TILE_CHUNKS) {
+                int first = (int)sm.chunks[k] * SPH_ARITY;
+                int cnt = min(SPH_ARITY, d.tree.count[L] - first);
+                unsigned cm = 0;
+                if (lane < cnt) {
+                    float4 clo = d.tree.lo[L][first + lane], chi = d.tree.hi[L][first + lane];
+                    if (box_reach_sym(clo, chi, tlo, thi)) {
+                        for (int w = 0; w < nch; ++w)
+                            if (box_reach_sym(clo, chi, sm.blo[w], sm.bhi[w])) cm |= 1u << w;
+                        if (attempt && cm) {
+                            float4 cc, ce;
+                            box_centre_form(clo, chi, cc, ce);
+                            unsigned left = cm;
+                            cm = 0;
+                            while (left) {
+                                const int w = __ffs(left) - 1;
+                                left &= left - 1;
+                                for (int t = 0; t < SPH_CHUNK; ++t) {
+                                    const float4 q = sm.pos[w * SPH_CHUNK + t];
+                                    if (q.w >= 0.f && point_reach(cc, ce, q.x, q.y, q.z, q.w)) { cm |= 1u << w; break; }
+                                }
+                            }
+                        }
+                    }
+                    if (L == 0 && k < SPH_CULL_MAXPAR) sm.u.walk.ctmp[k][lane] = (unsigned char)cm;
                 }
-                if (L == 0 && k < SPH_CULL_MAXPAR) sm.u.walk.ctmp[k][lane] = (unsigned char)cm;
+                unsigned m = __ballot_sync(FULL, cm != 0);
+                if (lane == 0) sm.mask[k] = m;
             }
-            unsigned m = __ballot_sync(FULL, pass);
-            if (lane == 0) sm.mask[k] = m;
+            __syncthreads();
+            if (warp == 0) {
+                const int total = scan_popc(sm.mask, sm.off, nf, lane);
+                if (lane == 0) sm.ntotal = total;
+            }
+            __syncthreads();
+            if (sm.ntotal <= capL || attempt == 1) break;
+            __syncthreads();                           // everyone has read ntotal before warp 0 writes it again
         }
-        __syncthreads();
-        if (warp == 0) {
-            int total = scan_popc(sm.mask, sm.off, nf, lane);
-            int cap = (L == 1) ? SPH_CULL_MAXPAR : SPH_CULL_MAXSRC;     // level-1 parents index ctmp
-            if (total > cap) { total = cap; if (lane == 0) sm.overflow |= 1; }
-            if (lane == 0) sm.nfront = total;
+        if (threadIdx.x == 0) {
+            if (sm.ntotal > capL) sm.overflow |= 1;
+            sm.nfront = min(sm.ntotal, capL);
         }
         __syncthreads();
         const int cap = sm.nfront;
