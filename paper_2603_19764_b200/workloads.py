@@ -332,6 +332,8 @@ def config(k: int, scale: float = 1.0) -> Workload:
         return impact_pair(int(4_400_000 * (scale ** 3 if scale < 1.0 else 1.0)), SEED_BASE + 3, 100.0, 1.214,
                            name="impact_pair_c3")
     if k == 4:
-        return impact_pair(int(32_000_000 * (scale ** 3 if scale < 1.0 else 1.0)), SEED_BASE + 4, 1000.0, 1.530,
-                           name="impact_pair_c4")
+        wl = impact_pair(int(32_000_000 * (scale ** 3 if scale < 1.0 else 1.0)), SEED_BASE + 4, 1000.0, 1.530,
+                         name="impact_pair_c4")
+        wl.params.list_budget = 96        # ~120 neighbours: room for 384 list entries per particle (default 256)
+        return wl
     raise ValueError(f"no config {k}")
