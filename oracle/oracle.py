@@ -155,14 +155,57 @@ def _matcol(params, mat, name):
     return np.array([getattr(mm, name) for mm in params.materials], dtype=np.float64)[mat]
 
 
+def table_lookup(f, x_min, x_max, x, y_min=None, y_max=None, y=None):
+    """Piecewise-linear (1-D) or bilinear (2-D) interpolation on a uniform grid, clamped to the grid's
+    edges (reading Q21: the paper says "tabulated", not how it interpolates).
+    f[i] sits at x_min + i (x_max - x_min)/(n_x - 1); f[i, j] likewise in y."""
+    f = np.asarray(f, dtype=np.float64)
+    nx = f.shape[0]
+    fx = np.clip((x - x_min) / (x_max - x_min) * (nx - 1), 0.0, nx - 1.0)
+    i = np.minimum(np.floor(fx).astype(np.int64), nx - 2)
+    tx = fx - i
+    if f.ndim == 1:
+        return (1.0 - tx) * f[i] + tx * f[i + 1]
+    ny = f.shape[1]
+    fy = np.clip((y - y_min) / (y_max - y_min) * (ny - 1), 0.0, ny - 1.0)
+    j = np.minimum(np.floor(fy).astype(np.int64), ny - 2)
+    ty = fy - j
+    return ((1.0 - tx) * (1.0 - ty) * f[i, j] + tx * (1.0 - ty) * f[i + 1, j]
+            + (1.0 - tx) * ty * f[i, j + 1] + tx * ty * f[i + 1, j + 1])
+
+
 def eos(params, rho, u, mat):
-    """Analytic stand-in for EOSlib (reading Q13, BASELINE.json configs[0]):
-    P = c0^2 (rho - rho0), c = c0, T = u / cv.  PCLIP_GLOBAL clips P >= 0 everywhere (Q8)."""
+    """P, c, T from (rho, u).  Materials without a table: the analytic stand-in for
+    EOSlib (reading Q13, BASELINE.json configs[0]): P = c0^2 (rho - rho0), c = c0, T = u / cv.
+    Materials with a table (NEXT-3): bilinear lookups (table_lookup).  PCLIP_GLOBAL clips P >= 0
+    everywhere (Q8)."""
     rho0 = _matcol(params, mat, "rho0"); c0 = _matcol(params, mat, "c0"); cv = _matcol(params, mat, "cv")
     P = c0 * c0 * (rho - rho0)
+    cs = c0.copy()
+    T = u / cv
+    for k, mm in enumerate(params.materials):
+        tab = getattr(mm, "table", None)
+        if tab is None:
+            continue
+        sel = mat == k
+        a = (tab.rho_min, tab.rho_max, rho[sel], tab.u_min, tab.u_max, u[sel])
+        P[sel] = table_lookup(tab.P, *a)
+        T[sel] = table_lookup(tab.T, *a)
+        cs[sel] = table_lookup(tab.cs, *a)
     if params.flags & FLAG_PCLIP_GLOBAL:
         P = np.maximum(P, 0.0)
-    return P, c0.copy(), u / cv
+    return P, cs, T
+
+
+def melt_temperature(params, rho, mat):
+    """T_melt: the material's constant, or "a tabulated function of density"."""
+    Tm = _matcol(params, mat, "Tmelt").copy()
+    for k, mm in enumerate(params.materials):
+        tab = getattr(mm, "table", None)
+        if tab is not None and tab.Tmelt is not None:
+            sel = mat == k
+            Tm[sel] = table_lookup(tab.Tmelt, tab.rho_min, tab.rho_max, rho[sel])
+    return Tm
 
 
 def shear_modulus(params, rho, cs, mat):
@@ -173,14 +216,15 @@ def shear_modulus(params, rho, cs, mat):
     return np.where(Gc > 0.0, Gc, G30)
 
 
-def yield_strength(params, P, T, mat):
+def yield_strength(params, P, T, mat, rho=None):
     """Y_i = Y0 + mu_i P/(1 + mu_i P/(Ym - Y0)) (Eq. 34) with P < 0 clipped to 0
     (PAPER.md:202); Y_d = mu_d P (Eq. 35); Y = min(Y_i, Y_d) when mu_d is finite (Eq. 36,
     reading Q10); Y -> Y tanh(xi (T_melt/T - 1)) (Eq. 37), clamped to >= 0 above
     the melting point and equal to Y for T <= 0 (reading Q11)."""
     Y0 = _matcol(params, mat, "Y0"); Ym = _matcol(params, mat, "Ym")
     mu_i = _matcol(params, mat, "mu_i"); mu_d = _matcol(params, mat, "mu_d")
-    xi = _matcol(params, mat, "xi"); Tm = _matcol(params, mat, "Tmelt")
+    xi = _matcol(params, mat, "xi")
+    Tm = _matcol(params, mat, "Tmelt") if rho is None else melt_temperature(params, rho, mat)
     Pp = np.maximum(P, 0.0)
     span = Ym - Y0
     with np.errstate(divide="ignore", invalid="ignore"):
@@ -337,7 +381,7 @@ def derivatives(params, x, y, z, m, h, vx, vy, vz, u, S, mat, g=None, mode="brut
     rho, omega = density(x, y, z, m, h, kap, og, lg)
     P, cs, T = eos(params, rho, _f64(u), mat)
     Gamma = shear_modulus(params, rho, cs, mat)
-    Y = yield_strength(params, P, T, mat)
+    Y = yield_strength(params, P, T, mat, rho)
     strength = bool(params.flags & FLAG_STRENGTH)
     S = _f64(S)
     if strength:

@@ -38,6 +38,23 @@ FIELDS = ("x", "y", "z", "m", "h", "vx", "vy", "vz", "u",
 
 
 @dataclass
+class EosTable:
+    """Tabulated EOS of one material on a uniform (rho, u) grid (P and T come from
+    EOSlib as functions of rho and u; T_melt is "a tabulated function of density").  Values are fp32;
+    P, T, cs have shape (n_rho, n_u); Tmelt has shape (n_melt,) over the same rho range, or is None
+    (constant T_melt of the material).  How the values are looked up is the method's business
+    (oracle / CUDA), not this module's."""
+    rho_min: float
+    rho_max: float
+    u_min: float
+    u_max: float
+    P: np.ndarray
+    T: np.ndarray
+    cs: np.ndarray
+    Tmelt: Optional[np.ndarray] = None
+
+
+@dataclass
 class Material:
     """Per-material constants (BASELINE.json configs[0])."""
     rho0: float = 2700.0
@@ -51,6 +68,7 @@ class Material:
     mu_d: float = math.inf     # +inf disables Eq. 35-36
     xi: float = 1.2
     Tmelt: float = 1500.0
+    table: Optional[EosTable] = None   # NEXT-3: tabulated EOS instead of the analytic stand-in
 
 
 @dataclass
@@ -149,17 +167,22 @@ def _lattice_block(nx, ny, nz, dx, seed, jitter=0.05, origin=(0.0, 0.0, 0.0), fi
 # ----------------------------------------------------------------------------
 def elastic_block(n_side: int = 16, seed: int = SEED_BASE, dx: float = 0.01,
                   flags: int = FLAG_STRENGTH | FLAG_CORRECTION_TENSOR,
-                  h_spread: float = 0.0, two_materials: bool = False) -> Workload:
+                  h_spread: float = 0.0, two_materials: bool = False,
+                  eos_table: Optional[str] = None) -> Workload:
     """BASELINE.json configs[0]: jittered n_side^3 lattice, shear flow, random S, T in [300,1600] K.
 
     ``h_spread`` > 0 multiplies h by U(1-h_spread, 1+h_spread) per particle (a parity
     case for the symmetric neighbour set with h_i != h_j); ``two_materials`` gives the
-    upper half (y > mid) material 1 (configs[3] second material).
+    upper half (y > mid) material 1 (configs[3] second material); ``eos_table`` ("linear" |
+    "curved") attaches a synthetic EOS table to every material (NEXT-3).
     """
     mat0 = Material()
     mats = [mat0]
     if two_materials:
         mats.append(Material(Y0=1.0e6, mu_i=1.0))
+    if eos_table:
+        for mm in mats:
+            mm.table = synthetic_eos_table(mm, eos_table)
     x, y, z, idx = _lattice_block(n_side, n_side, n_side, dx, seed)
     n = idx.size
     h = np.full(n, 1.3 * dx)
@@ -307,6 +330,31 @@ def impact_pair(n_total: int = 4_400_000, seed: int = SEED_BASE + 3, contrast: f
     params = Params(flags=FLAG_STRENGTH | FLAG_CORRECTION_TENSOR | FLAG_PCLIP_GLOBAL, materials=mats)
     return _finish(f"{name}_{n}", params, cols, mat, np.zeros(n, np.uint8), 0.0,
                    f"number-density contrast {contrast:g}, eta_h {eta_h}; PCLIP_GLOBAL")
+
+
+def synthetic_eos_table(mat: Material, kind: str = "curved", n_rho: int = 97, n_u: int = 33,
+                        n_melt: int = 49) -> EosTable:
+    """A synthetic table standing in for the paper's M-ANEOS quartz tables and SiO2 melt curve
+    (PAPER.md:221, 258), which are not available.  kind = "linear": the analytic stand-in of
+    BASELINE.json configs[0] sampled on the grid (P = c0^2 (rho - rho0), T = u / cv, c = c0, constant
+    T_melt) -- a bilinear lookup reproduces it; kind = "curved": a Tillotson-like smooth surface with
+    a density-dependent melt curve (coefficients arbitrary, fixed)."""
+    rho = np.linspace(0.1 * mat.rho0, 1.3 * mat.rho0, n_rho)      # free-surface particles sit near rho0 / 4
+    u = np.linspace(0.0, 2.5e6, n_u)
+    R, U = np.meshgrid(rho, u, indexing="ij")
+    mu = R / mat.rho0 - 1.0
+    if kind == "linear":
+        P = mat.c0 ** 2 * (R - mat.rho0)
+        T = U / mat.cv
+        cs = np.full_like(R, mat.c0)
+        tm = None
+    else:
+        P = mat.c0 ** 2 * mat.rho0 * (mu + 1.5 * mu * mu) + 0.5 * R * U * (1.0 + mu)
+        T = U / mat.cv * (1.0 + 0.3 * mu) + 40.0 * mu
+        cs = mat.c0 * np.sqrt(np.maximum(0.25, 1.0 + 1.5 * mu + 0.5 * U / mat.c0 ** 2))
+        rm = np.linspace(rho[0], rho[-1], n_melt)
+        tm = _f32(mat.Tmelt * np.maximum(0.2, 1.0 + 2.0 * (rm / mat.rho0 - 1.0)) ** 1.5)
+    return EosTable(float(rho[0]), float(rho[-1]), float(u[0]), float(u[-1]), _f32(P), _f32(T), _f32(cs), tm)
 
 
 def oblique_impact(n_total: int = 30_000, v_impact: float = 100.0, seed: int = SEED_BASE + 7) -> Workload:
