@@ -128,6 +128,18 @@ typedef struct sph_params {
                                   the tree-walk kernels and counted in SPH_C_LIST_OVERFLOW.           */
 } sph_params;
 
+/* NEXT-3: a tabulated EOS for one material (P and T are computed from rho and u by the EOS
+ * library; T_melt "is provided as a tabulated function of density").  Uniform grids; value k of an axis
+ * sits at min + k (max - min)/(n - 1).  P, T, cs: DEVICE, row-major [n_rho][n_u].  Tmelt: DEVICE [n_melt]
+ * over [rho_min, rho_max], or NULL (the material's constant Tmelt).  The arrays are caller-owned and
+ * must stay valid while the table is set. */
+typedef struct sph_eos_table {
+    int n_rho, n_u, n_melt;
+    float rho_min, rho_max, u_min, u_max;
+    const float *P, *T, *cs;
+    const float *Tmelt;
+} sph_eos_table;
+
 /* Caller-owned particle arrays, each of length n.  For the device entry points all pointers are
  * DEVICE pointers; for sph_step_host all are HOST pointers.  S is symmetric and traceless, five
  * stored components (Eq. 11).  gx,gy,gz (external acceleration, the "G" term of
@@ -205,6 +217,14 @@ int sph_get_field(sph_ctx *ctx, int field_id, float *dst);
  * unspecified.  list_capacity: entries available in list (ECAPACITY if offsets[n] exceeds it is
  * NOT checked on the device; the caller sizes list from counts). */
 int sph_get_neighbors(sph_ctx *ctx, int which, int *counts, const long long *offsets, int *list);
+
+/* NEXT-3: use `table` (HOST struct, DEVICE arrays) for P, T, c_s (and T_melt) of `material` in
+ * sph_strength_update(SPH_PREDICT) and every pass after it, instead of the analytic stand-in; NULL
+ * returns to the analytic EOS.  Lookup: bilinear (T_melt: piecewise linear), clamped to the grid's edges
+ * (reading Q21 in DESIGN.md); cell index and weights in fp64 from the fp64 density.  SPH_PCLIP_GLOBAL
+ * still clips P >= 0 afterwards.  Host-only call (no launch); passes from PREDICT on must be redone.
+ * Errors: EINVAL (material out of range, grid < 2 points, NULL arrays, empty ranges). */
+int sph_set_eos_table(sph_ctx *ctx, int material, const sph_eos_table *table);
 
 /* S8 diagnostics (the conservation checks of PAPER.md:349-357): out = DEVICE double[8] =
  * { sum m, sum m v (3), sum m x cross v (3), sum m (v.v/2 + u) } over the resident particles at the

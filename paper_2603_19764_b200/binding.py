@@ -31,9 +31,15 @@ OPT_FIELDS = ("gx", "gy", "gz")
 
 # every symbol include/sph.h declares (tests check the library exports all of them)
 SYMBOLS = ("sph_workspace_bytes", "sph_init", "sph_build_neighbors", "sph_density", "sph_strength_update",
-           "sph_gradients", "sph_forces", "sph_adapt_h", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
+           "sph_gradients", "sph_forces", "sph_adapt_h", "sph_set_eos_table", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
            "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_get_diagnostics", "sph_launch_count",
            "sph_last_cuda_error", "sph_strerror", "sph_destroy")
+
+
+class sph_eos_table(C.Structure):
+    _fields_ = [("n_rho", C.c_int), ("n_u", C.c_int), ("n_melt", C.c_int),
+                ("rho_min", C.c_float), ("rho_max", C.c_float), ("u_min", C.c_float), ("u_max", C.c_float),
+                ("P", C.c_void_p), ("T", C.c_void_p), ("cs", C.c_void_p), ("Tmelt", C.c_void_p)]
 
 
 class sph_material(C.Structure):
@@ -89,6 +95,8 @@ def load():
     lib.sph_get_timings.argtypes = [vp, C.POINTER(fl), i]
     lib.sph_get_counters.argtypes = [vp, C.POINTER(ll), i]
     lib.sph_get_tile_stats.argtypes = [vp, vp, vp, vp, i]
+    lib.sph_set_eos_table.argtypes = [vp, i, vp]
+    lib.sph_set_eos_table.restype = i
     lib.sph_get_diagnostics.argtypes = [vp, vp]
     lib.sph_get_diagnostics.restype = i
     lib.sph_adapt_h.argtypes = [vp, fl, i, vp]
@@ -148,6 +156,10 @@ class Sph:
                                       self.workspace.data_ptr(), need, self.stream.cuda_stream), "sph_init")
         self.n = 0
         self._dev_state: Dict[str, object] = {}
+        self._tables: Dict[int, object] = {}
+        for k, m in enumerate(params.materials):          # NEXT-3: materials that carry an EOS table
+            if getattr(m, "table", None) is not None:
+                self.set_eos_table(k, m.table)
 
     # ---- plumbing ---------------------------------------------------------------------------
     def _check(self, rc: int, what: str):
@@ -264,6 +276,25 @@ class Sph:
         cs = (C.c_longlong * len(C_SLOTS))()
         self._check(self.lib.sph_get_counters(self.ctx, cs, len(C_SLOTS)), "sph_get_counters")
         return {k: int(cs[i]) for i, k in enumerate(C_SLOTS)}
+
+    def set_eos_table(self, material: int, table):
+        """sph_set_eos_table; table: a workloads.EosTable-like record (numpy arrays) or None."""
+        if table is None:
+            self._check(self.lib.sph_set_eos_table(self.ctx, int(material), None), "sph_set_eos_table")
+            self._tables.pop(material, None)
+            return
+        torch = self.torch
+        dev = {k: torch.as_tensor(getattr(table, k), dtype=torch.float32, device=self.device).contiguous()
+               for k in ("P", "T", "cs")}
+        tm = None if table.Tmelt is None else torch.as_tensor(table.Tmelt, dtype=torch.float32, device=self.device).contiguous()
+        t = sph_eos_table()
+        t.n_rho, t.n_u = dev["P"].shape
+        t.n_melt = 0 if tm is None else tm.shape[0]
+        t.rho_min, t.rho_max, t.u_min, t.u_max = table.rho_min, table.rho_max, table.u_min, table.u_max
+        t.P, t.T, t.cs = dev["P"].data_ptr(), dev["T"].data_ptr(), dev["cs"].data_ptr()
+        t.Tmelt = None if tm is None else tm.data_ptr()
+        self._check(self.lib.sph_set_eos_table(self.ctx, int(material), C.byref(t)), "sph_set_eos_table")
+        self._tables[material] = (dev, tm)              # keep the device arrays alive
 
     def adapt_h(self, n_target: float, iterations: int, max_change=None):
         """sph_adapt_h; max_change: optional 1-element float32 device tensor."""

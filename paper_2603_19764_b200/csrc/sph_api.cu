@@ -530,6 +530,25 @@ extern "C" int sph_get_counters(sph_ctx *c, long long *out, int n)
     return SPH_OK;
 }
 
+extern "C" int sph_set_eos_table(sph_ctx *c, int material, const sph_eos_table *tab)
+{
+    if (!c || material < 0 || material >= c->p.n_materials) return SPH_EINVAL;
+    DevTab &t = c->tabs.t[material];
+    if (!tab) {
+        t = DevTab{};
+        c->have_predict = c->have_grad = c->have_force = false;
+        return SPH_OK;
+    }
+    if (tab->n_rho < 2 || tab->n_u < 2 || !tab->P || !tab->T || !tab->cs || !(tab->rho_max > tab->rho_min)
+        || !(tab->u_max > tab->u_min) || (tab->Tmelt && tab->n_melt < 2))
+        return SPH_EINVAL;
+    t.n_rho = tab->n_rho; t.n_u = tab->n_u; t.n_melt = tab->Tmelt ? tab->n_melt : 0;
+    t.rho_min = tab->rho_min; t.rho_max = tab->rho_max; t.u_min = tab->u_min; t.u_max = tab->u_max;
+    t.P = tab->P; t.T = tab->T; t.cs = tab->cs; t.Tmelt = tab->Tmelt;
+    c->have_predict = c->have_grad = c->have_force = false;
+    return SPH_OK;
+}
+
 extern "C" int sph_get_diagnostics(sph_ctx *c, double *out)
 {
     if (!c || !out) return SPH_EINVAL;

@@ -43,6 +43,16 @@ struct DevParams {
     sph_material mat[SPH_MAX_MATERIALS];
 };
 
+// NEXT-3: tabulated EOS per material (sph_set_eos_table); P == nullptr: the analytic stand-in
+struct DevTab {
+    int n_rho, n_u, n_melt;
+    float rho_min, rho_max, u_min, u_max;
+    const float *P, *T, *cs, *Tmelt;
+};
+struct DevTabs {
+    DevTab t[SPH_MAX_MATERIALS];
+};
+
 // Sorted ("resident") particle data that moves with the particle at re-sort.
 struct Resident {
     float4 *pm;              // x, y, z, m
@@ -113,6 +123,7 @@ struct Dev {
 
 struct sph_ctx {
     DevParams p;
+    DevTabs tabs;
     Dev d;
     cudaStream_t stream;
     int last_cuda;

@@ -10,7 +10,7 @@
 // ------------------------------------------------------------------------------------------
 // Y_i = Y0 + mu_i P/(1 + mu_i P/(Ym - Y0)) with P < 0 clipped (Eq. 34);
 // Y = min(Y_i, mu_d P) for finite mu_d (Eq. 35-36); Y *= max(0, tanh(xi (Tm/T - 1))) (Eq. 37).
-__device__ __forceinline__ float yield_strength(const sph_material &m, float P, float T)
+__device__ __forceinline__ float yield_strength(const sph_material &m, float P, float T, float Tmelt)
 {
     float Pp = fmaxf(P, 0.f);
     float span = m.Ym - m.Y0;
@@ -18,8 +18,25 @@ __device__ __forceinline__ float yield_strength(const sph_material &m, float P, 
     if (span > 0.f) Y = m.Y0 + m.mu_i * Pp / (1.f + m.mu_i * Pp / span);
     if (isfinite(m.mu_d)) Y = fminf(Y, m.mu_d * Pp);
     float soft = 1.f;
-    if (T > 0.f) soft = fmaxf(0.f, tanhf(m.xi * (m.Tmelt / T - 1.f)));
+    if (T > 0.f) soft = fmaxf(0.f, tanhf(m.xi * (Tmelt / T - 1.f)));
     return Y * soft;
+}
+
+// NEXT-3 (P and T from (rho, u) tables, T_melt "a tabulated function of density"): piecewise-
+// linear / bilinear lookup on a uniform grid, clamped to the grid's edges (reading Q21).  Index and weights
+// in fp64 from the fp64 density: (rho - rho_k) cancels like (rho - rho0) does in the analytic EOS.
+__device__ __forceinline__ void table_cell(double x, float x_min, float x_max, int n, int &i, double &t)
+{
+    double f = (x - (double)x_min) / ((double)x_max - (double)x_min) * (double)(n - 1);
+    f = fmin(fmax(f, 0.0), (double)(n - 1));
+    i = min((int)f, n - 2);
+    t = f - (double)i;
+}
+__device__ __forceinline__ float table_2d(const float *__restrict__ f, int n_u, int i, int j, double tx, double ty)
+{
+    const float *r0 = f + (size_t)i * n_u + j, *r1 = r0 + n_u;
+    return (float)((1.0 - tx) * (1.0 - ty) * (double)r0[0] + tx * (1.0 - ty) * (double)r1[0]
+                   + (1.0 - tx) * ty * (double)r0[1] + tx * ty * (double)r1[1]);
 }
 
 // f = min(Y / sqrt(J2), 1) (Eq. 31-33); J2 from the five stored components
@@ -37,20 +54,36 @@ __device__ __forceinline__ float plastic_factor(const float S[5], float Y)
 //   B3 = {rho, c, w, st_xx}, B4 = {st_yy, st_zz, st_xy, st_xz}, B5 = st_yz
 //   w = 1/(Omega rho), st = (-P delta + S_pred)/(Omega rho^2)
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_predict(Dev d, DevParams p)
+__global__ void __launch_bounds__(256) k_predict(Dev d, DevParams p, DevTabs tabs)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= d.n) return;
     unsigned mf = ((const unsigned *)d.r.s[PP_MATFIX])[i];
     const sph_material &m = p.mat[mf & 0xffu];
     float rho = d.rho[i], om = d.omega[i], u = d.r.s[PP_UPRED][i];
-    // the subtraction rho - rho0 in fp64 (see k_density)
-    float P = (float)((double)m.c0 * (double)m.c0 * (d.rho64[i] - (double)m.rho0));
+    const DevTab &tb = tabs.t[mf & 0xffu];
+    float P, cs, T, Tmelt = m.Tmelt;
+    if (tb.P) {
+        int ir, iu;
+        double tr, tu;
+        table_cell(d.rho64[i], tb.rho_min, tb.rho_max, tb.n_rho, ir, tr);
+        table_cell((double)u, tb.u_min, tb.u_max, tb.n_u, iu, tu);
+        P = table_2d(tb.P, tb.n_u, ir, iu, tr, tu);
+        T = table_2d(tb.T, tb.n_u, ir, iu, tr, tu);
+        cs = table_2d(tb.cs, tb.n_u, ir, iu, tr, tu);
+        if (tb.Tmelt) {
+            table_cell(d.rho64[i], tb.rho_min, tb.rho_max, tb.n_melt, ir, tr);
+            Tmelt = (float)((1.0 - tr) * (double)tb.Tmelt[ir] + tr * (double)tb.Tmelt[ir + 1]);
+        }
+    } else {
+        // the subtraction rho - rho0 in fp64 (see k_density)
+        P = (float)((double)m.c0 * (double)m.c0 * (d.rho64[i] - (double)m.rho0));
+        cs = m.c0;
+        T = u / m.cv;
+    }
     if (p.flags & SPH_PCLIP_GLOBAL) P = fmaxf(P, 0.f);
-    float cs = m.c0;
-    float T = u / m.cv;
     float Gam = m.Gamma > 0.f ? m.Gamma : 3.f * (1.f - 2.f * m.nu) / (2.f * (1.f + m.nu)) * rho * cs * cs;
-    float Y = yield_strength(m, P, T);
+    float Y = yield_strength(m, P, T, Tmelt);
     float S[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
     if (p.flags & SPH_STRENGTH) {
 #pragma unroll
@@ -268,7 +301,7 @@ int sph_launch_predict(sph_ctx *c)
 {
     Dev &d = c->d;
     if (d.n == 0) return SPH_OK;
-    k_predict<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, c->p);
+    k_predict<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, c->p, c->tabs);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;

@@ -223,3 +223,30 @@ def test_diagnostics_match_fp64_sums_and_momentum_is_conserved():
     pscale = (m * np.abs(v)).sum()
     assert np.abs(d1[1:4] - d0[1:4]).max() <= 1e-5 * pscale                # fp32 pair sums, antisymmetric terms
     assert d1[0] == d0[0]
+
+
+@pytest.mark.parametrize("kind", ["linear", "curved"])
+def test_tabulated_eos_matches_oracle(kind):
+    """NEXT-3: P, T, c_s from (rho, u) tables and T_melt(rho), two materials."""
+    wl = W.elastic_block(12, two_materials=True, eos_table=kind)
+    g = U.gpu_single_pass(wl)
+    d = O.single_pass(wl)
+    errs = U.compare_single_pass(g, d, wl)
+    assert U.maxnorm_err(g["cs"], d["cs"]) <= 1e-6
+    if kind == "curved":
+        assert np.ptp(d["cs"]) > 0.0 and (d["Y"] == 0.0).any()
+    print("table", kind, {k: float(f"{v:.3g}") for k, v in errs.items()})
+
+
+def test_eos_table_argument_checks_and_reset():
+    from paper_2603_19764_b200 import binding as B
+    wl = W.elastic_block(6, eos_table="curved")
+    ref = U.gpu_single_pass(W.elastic_block(6))
+    s = B.Sph(wl.params, wl.n)
+    with pytest.raises(B.SphError) as e:
+        s.set_eos_table(3, wl.params.materials[0].table)
+    assert e.value.code == B.EINVAL
+    s.set_eos_table(0, None)                       # back to the analytic EOS
+    t = s.upload(wl)
+    s.build_neighbors(t, wl.n); s.density(); s.strength_update(B.PREDICT)
+    assert np.array_equal(s.get_field("P").cpu().numpy(), ref["p"])
