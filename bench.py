@@ -198,8 +198,13 @@ def run_ours(args):
     torch.cuda.set_device(local)
     dev = torch.device(f"cuda:{local}")
     props = torch.cuda.get_device_properties(dev)
+    # everything (torch fills, copies, the library's kernels, the timing events) on one non-default stream:
+    # the library replays the resident step from a CUDA graph, and the default stream cannot be captured
+    torch.cuda.set_stream(torch.cuda.Stream(dev))
 
     wl = make_workload(args.workload)
+    if args.no_graph:
+        wl.params.flags |= 64          # SPH_NO_GRAPH
     n = wl.n
     strength = bool(wl.params.flags & B.STRENGTH)
     s = B.Sph(wl.params, n, device=dev)
@@ -333,7 +338,8 @@ def run_ours(args):
         "config": {"workload": wl.name, "n_particles": n, "strength": strength,
                    "mean_neighbours": pairs_s / args.steps / max(n, 1),
                    "l2": "flushed between steps (256 MiB fill outside the timed events)",
-                   "working_set_bytes": working_set, "parallelism": "replicas x%d" % world},
+                   "working_set_bytes": working_set, "parallelism": "replicas x%d" % world,
+                   "cuda_graph": not args.no_graph},
         "particle_steps_per_s": world * n * args.steps / (total_ms_max * 1e-3),
         "pass_ms": {k: v / args.steps for k, v in pass_ms.items()},
         "gpu_launches": launches,
@@ -358,6 +364,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-hydro-only", action="store_true")
+    ap.add_argument("--no-graph", action="store_true", help="launch the step kernel by kernel (A/B of the CUDA graph)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

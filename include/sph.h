@@ -35,6 +35,8 @@ extern "C" {
 #define SPH_NO_LISTS             16u  /* pair passes walk the chunk tree themselves instead of reading
                                          the per-particle neighbour lists (the round-1 "v0" kernels: A/B
                                          measurement; they also serve tiles over a list capacity)           */
+#define SPH_NO_GRAPH             64u  /* launch the resident step kernel by kernel instead of replaying its
+                                         CUDA graph (A/B measurement)                                      */
 #define SPH_MORTON_ORDER         32u  /* sort by Morton (Z-order) keys instead of Hilbert keys (A/B
                                          measurement; results do not depend on the order)                  */
 
@@ -156,7 +158,8 @@ typedef struct sph_state {
 size_t sph_workspace_bytes(const sph_params *params, long long n_max);
 
 /* Create a context.  params: HOST.  workspace: DEVICE, >= sph_workspace_bytes(), 256-byte aligned.
- * cuda_stream: a cudaStream_t (NULL = default stream).  Errors: EINVAL, ENOMEM, ECUDA. */
+ * cuda_stream: a cudaStream_t (NULL = default stream; the resident step is replayed from a CUDA graph
+ * only on a stream that can be captured, i.e. not on the default stream).  Errors: EINVAL, ENOMEM, ECUDA. */
 int sph_init(sph_ctx **ctx, const sph_params *params, long long n_max,
              void *workspace, size_t workspace_bytes, void *cuda_stream);
 

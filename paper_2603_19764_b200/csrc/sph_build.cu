@@ -329,5 +329,6 @@ int sph_launch_resort(sph_ctx *c)
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     Resident t = d.r; d.r = d.alt; d.alt = t;
+    c->parity ^= 1;
     return sph_launch_tree(c);
 }

@@ -129,6 +129,14 @@ struct sph_ctx {
     int last_cuda;
     long long launches;
     bool use_lists;
+    // CUDA graphs of the resident step (sph_step with state == NULL, dt <= 0): one per half of the
+    // ping-pong (the kernels take the array pointers by value); see sph_step
+    bool use_graph, capturing;
+    int parity;                      // which half of the ping-pong is current
+    cudaGraphExec_t gexec[2];
+    long long glaunches[2];          // launches one replay stands for
+    long long gkey_n[2];
+    const void *gkey_dtused[2];
     bool resident, have_density, have_predict, have_grad, have_force, have_derivs;
     cudaEvent_t ev[2 * SPH_T_COUNT];
     bool ev_used[SPH_T_COUNT];

@@ -250,3 +250,30 @@ def test_eos_table_argument_checks_and_reset():
     t = s.upload(wl)
     s.build_neighbors(t, wl.n); s.density(); s.strength_update(B.PREDICT)
     assert np.array_equal(s.get_field("P").cpu().numpy(), ref["p"])
+
+
+def test_graph_replay_equals_kernel_by_kernel_step():
+    """The resident step replayed from its CUDA graph (a capturable stream) against the same steps
+    launched kernel by kernel: bitwise equal state, timings and launch counts still reported."""
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    out = []
+    for no_graph in (False, True):
+        wl = W.elastic_block(12, h_spread=0.2, flags=F | (W.FLAG_NO_GRAPH if no_graph else 0))
+        with torch.cuda.stream(torch.cuda.Stream()):          # torch ops and the library on one capturable stream
+            s = B.Sph(wl.params, wl.n)
+            t = s.upload(wl)
+            s.build_neighbors(t, wl.n)
+            dtu = torch.zeros(1, dtype=torch.float32, device="cuda")
+            for _ in range(6):                    # bootstrap, two captures, three replays
+                s.step(None, 0, 0.0, dtu)
+            tm = s.get_timings()
+            assert tm["step"] > 0.0 and tm["force"] > 0.0 and tm["build"] > 0.0
+            s.download_state(t)
+            torch.cuda.synchronize()
+            out.append(({k: t[k].cpu().numpy().copy() for k in ("x", "vx", "u", "Sxy")}, float(dtu.item()),
+                        s.launch_count(), s.get_field("RHO").cpu().numpy()))
+    for k in out[0][0]:
+        assert np.array_equal(out[0][0][k], out[1][0][k]), k
+    assert out[0][1] == out[1][1] and out[0][2] == out[1][2]
+    assert np.array_equal(out[0][3], out[1][3])
