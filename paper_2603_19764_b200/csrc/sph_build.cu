@@ -248,13 +248,15 @@ size_t sph_cub_temp_bytes(long long n_max)
     return bytes > bound ? bytes : bound;
 }
 
-// bits per axis of the curve key: 2^6 cells per mean particle spacing and axis (room for a linear
-// density contrast of 64 before ties start to blur the order), within [10, 21]
+// bits per axis of the curve key: 2^3 cells per mean particle spacing and axis, within [10, 21].  Where the
+// particle spacing is below a cell (a linear density contrast above 8) the stable sort keeps ties in their
+// previous order, which is the previous step's curve order: measured on configs[3-4] (contrast 4.6 / 10) the
+// list build is as fast as with 2^6 cells, and the radix sort needs one pass less (30 key bits at 1e6).
 static int key_bits(long long n)
 {
     int b = 0;
     while (((long long)1 << (3 * b)) < n) ++b;      // ceil(log2(n) / 3)
-    b += 6;
+    b += 3;
     return b < 10 ? 10 : (b > 21 ? 21 : b);
 }
 
