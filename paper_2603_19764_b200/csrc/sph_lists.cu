@@ -69,7 +69,7 @@ __device__ __forceinline__ void box_centre_form(float4 lo, float4 hi, float4 &c,
 struct CullSmem {
     float4 pos[SPH_SE + 1];              // x, y, z, H^2 of the candidates of the current round; [SPH_SE] is a
                                          // sentinel no target can reach (pads the quarter-warp tables)
-    unsigned flag[SPH_SE];               // bit 4w+g: within reach of quarter g of warp w
+    unsigned char flag[SPH_SE];          // bit w: within reach of the box of chunk (warp) w of the tile
     unsigned chunks[SPH_CULL_MAXSRC];    // frontier / accepted source chunks, ascending
     unsigned mask[SPH_CULL_MAXSRC];      // surviving lanes (children / particles) of each entry
     unsigned short off[SPH_CULL_MAXSRC]; // exclusive prefix of popc(mask) (< SPH_MAXROUND * SPH_SE + 32 < 65536)
@@ -104,20 +104,6 @@ __device__ __forceinline__ unsigned reach_chunks(const CullSmem &sm, unsigned am
         int w = __ffs(among) - 1;
         among &= among - 1;
         if (point_reach(sm.bc[w], sm.be[w], x, y, z, H2s)) f |= 1u << w;
-    }
-    return f;
-}
-
-// bits 4w+g for the chunks w of `fchunk` (which already passed reach_chunks) whose quarter-g box passes
-__device__ __forceinline__ unsigned reach_groups(const CullSmem &sm, unsigned fchunk, float x, float y, float z, float H2s)
-{
-    unsigned f = 0;
-    while (fchunk) {
-        int w = __ffs(fchunk) - 1;
-        fchunk &= fchunk - 1;
-#pragma unroll
-        for (int g = 0; g < 4; ++g)
-            if (point_reach(sm.gc[4 * w + g], sm.ge[4 * w + g], x, y, z, H2s)) f |= 1u << (4 * w + g);
     }
     return f;
 }
@@ -379,7 +365,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             const float H2s = Hj * Hj * SPH_REACH_SLACK;
             const unsigned fc = k < SPH_CULL_CFCACHE ? (unsigned)sm.cf[k][lane]
                                                      : reach_chunks(sm, sm.cmask[k], q.x, q.y, q.z, H2s);
-            sm.flag[slot] = reach_groups(sm, fc, q.x, q.y, q.z, H2s);
+            sm.flag[slot] = (unsigned char)fc;
             cand[r0 + slot] = (unsigned)j;
             long long rel = j - (long long)tile * SPH_TILE;
             if (rel >= 0 && rel < SPH_TILE) sm.selfslot[rel] = (unsigned)(r0 + slot);
@@ -389,7 +375,6 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             // ---- B: quarter g of this warp tests the candidates flagged for it, in slot order ---------
             const int selfrel = (int)sm.selfslot[threadIdx.x] - r0;    // self exclusion (j != i)
             const unsigned selfoff = (selfrel >= 0 && selfrel < nr) ? (unsigned)selfrel << 4 : 0xffffffffu;
-            const int fshift = 4 * warp;
             const int Gstart = G;
             unsigned short(*gl)[SPH_GCAP] = sm.gl[warp];
             const unsigned char *const posb = reinterpret_cast<const unsigned char *>(sm.pos);
@@ -413,7 +398,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
                     if (min(min(a0, a1), min(a2, a3)) >= 32) break;               // every quarter has a block
                     while (ct - ch < 32 && base < nr) {
                         const int s = base + lane;
-                        const bool any = s < nr && ((sm.flag[s] >> fshift) & 15u) != 0u;
+                        const bool any = s < nr && ((sm.flag[s] >> warp) & 1u) != 0u;
                         const unsigned m = __ballot_sync(FULL, any);
                         if (any) c1[(ct + __popc(m & lt)) & 63] = (unsigned short)(s << 4);
                         ct += __popc(m);
@@ -425,8 +410,14 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
                     unsigned f = 0u;
                     unsigned short so = 0;
                     if (lane < take) {
+                        // which of the warp's four quarter boxes the candidate reaches (every lane has an
+                        // entry here: the quarter tests run at full width, unlike in A3)
                         so = c1[(ch + lane) & 63];
-                        f = (sm.flag[so >> 4] >> fshift) & 15u;
+                        const float4 q = *reinterpret_cast<const float4 *>(posb + so);
+                        const float H2s = q.w * SPH_REACH_SLACK;
+#pragma unroll
+                        for (int gq = 0; gq < 4; ++gq)
+                            if (point_reach(sm.gc[4 * warp + gq], sm.ge[4 * warp + gq], q.x, q.y, q.z, H2s)) f |= 1u << gq;
                     }
                     ch += take;
                     const unsigned m0 = __ballot_sync(FULL, f & 1u), m1 = __ballot_sync(FULL, f & 2u),
