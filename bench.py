@@ -91,7 +91,7 @@ class ClockSampler:
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused pair kernel, from the committed
 # `ncu --set full` capture of this command (profiles/, latest round-1 summary); None where no capture exists.
-NCU_TRAFFIC_BYTES = {"c2": 347.2e6}          # profiles/r01_v4_ring_tables_heavy_first.md: 273.9 MB read + 73.3 MB written
+NCU_TRAFFIC_BYTES = {"c2": 346.6e6}          # profiles/r01_v5_dense_flags_graph.md: 275.2 MB read + 71.4 MB written
 
 
 def rank_reduce(ms: float, units: float, device):
