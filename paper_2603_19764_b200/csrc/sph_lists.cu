@@ -2,18 +2,23 @@
 // pair passes evaluate true pairs only, one lane per target, with no search work in their inner loop.
 //
 //   tile        = 8 consecutive chunks = 256 Hilbert-consecutive targets = one CTA of 8 warps.
+//   k_tile_plan : the tiles that were expensive in the previous build are launched first (sph_tile_of_block).
 //   k_cull      : one CTA per tile:
-//                 (A) breadth-first walk of the chunk tree by all warps; every particle of the accepted
+//                 (A) breadth-first walk of the chunk tree by all warps (a level that overflows its
+//                     frontier is redone with per-target-particle tests); every particle of the accepted
 //                     source chunks is tested against the tile's chunk boxes; the survivors form the tile
 //                     CANDIDATE LIST (global indices, ascending), split into ROUNDS of SPH_SE slots, each
-//                     with a 32-bit flag word (bit 4w+g: within reach of the 8 targets of quarter g of
-//                     warp w);
-//                 (B) every quarter-warp runs the candidates flagged for it past its 8 targets (exact
-//                     fp32 predicate, reading Q4) and appends each hit to the target's NEIGHBOUR LIST:
-//                     the symmetric set, self excluded, as 16-bit byte offsets (slot * 16) into the
-//                     round's staged arrays, stored transposed ([chunk][row-group][lane], 4 entries per
-//                     lane per row-group) so that a warp reads one coalesced 256-byte row-group per four
-//                     pairs.  Rounds start at a common row-group (rowptr); 0xFFFF pads.
+//                     slot with one byte of flags (bit w: within reach of the box of chunk w);
+//                 (B) every warp keeps the slots that reach its chunk (one ballot per 32 slots), tests 32
+//                     of them at a time against its four quarter boxes and splits them over four rings of
+//                     offsets; every quarter-warp runs its ring, 32 candidates at a time, past its 8
+//                     targets (exact fp32 predicate, reading Q4) and appends each hit to the target's
+//                     NEIGHBOUR LIST: the symmetric set, self excluded, as 16-bit byte offsets (slot * 16)
+//                     into the round's staged arrays.  A hit is one predicated store into the lane's
+//                     buffer in shared memory; complete row-groups of 4 entries go to the global list,
+//                     which is stored transposed ([chunk][row-group][lane]) so that a warp reads one
+//                     coalesced 256-byte row-group per four pairs.  Rounds start at a common row-group
+//                     (rowptr); 0xFFFF pads.
 //   k_density_l : stages {x,y,z,m} of the round's candidates in shared memory (coalesced gathers of index
 //                 runs) and walks the lists; the gather set is the subset with r2 < H_i^2, plus self.
 //   k_pair_l    : same with the 17 floats per source of the fused gradient + force pass.
@@ -22,7 +27,8 @@
 //
 // Evidence for this design: profiles/r01_v0_launches_and_pair_kernel.md (broadcast tiles: candidate hit
 // rate 3.5 %, 18.65 of 32 threads active) and profiles/r01_v1_mask_lists.md (bitmask lists: 83 non-FP
-// instructions per pair, half of the shared-memory wavefronts were bank conflicts).
+// instructions per pair, half of the shared-memory wavefronts were bank conflicts); for the inside of
+// k_cull: profiles/r01_v4_ring_tables_heavy_first.md and profiles/r01_v5_dense_flags_graph.md.
 #include "sph_internal.cuh"
 #include "sph_pairterm.cuh"
 
