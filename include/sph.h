@@ -37,6 +37,9 @@ extern "C" {
                                          measurement; they also serve tiles over a list capacity)           */
 #define SPH_NO_GRAPH             64u  /* launch the resident step kernel by kernel instead of replaying its
                                          CUDA graph (A/B measurement)                                      */
+#define SPH_FUSED_DENSITY       128u  /* sph_step: run the density pass inside the list build instead of as its
+                                         own kernel (A/B measurement: same results bit for bit, 4 % slower
+                                         on configs[2]; off by default)                                    */
 #define SPH_MORTON_ORDER         32u  /* sort by Morton (Z-order) keys instead of Hilbert keys (A/B
                                          measurement; results do not depend on the order)                  */
 

@@ -246,11 +246,19 @@ extern "C" int sph_build_neighbors(sph_ctx *c, const sph_state *state, long long
         rc = sph_launch_resort(c);
         if (rc) return rc;
     }
-    if (c->use_lists) {
-        rc = sph_launch_cull(c);
-        if (rc) return rc;
-    }
     c->have_density = c->have_predict = c->have_grad = c->have_force = false;
+    if (c->use_lists) {
+        // inside sph_step the density pass of every tile runs in the list kernel itself (k_cull<true>)
+        const bool fuse = c->fuse_density_now;
+        rc = sph_launch_cull(c, fuse);
+        if (rc) return rc;
+        if (fuse) {
+            PassTimer td(c, SPH_T_DENSITY);           // what is left of S2: the tiles over a list capacity
+            rc = sph_launch_density(c, true);
+            if (rc) return rc;
+            c->have_density = true;
+        }
+    }
     return SPH_OK;
 }
 
@@ -282,7 +290,7 @@ extern "C" int sph_adapt_h(sph_ctx *c, float n_target, int iterations, float *ma
         rc = sph_launch_tree(c);
         if (rc) return rc;
         if (c->use_lists) {
-            rc = sph_launch_cull(c);
+            rc = sph_launch_cull(c, false);
             if (rc) return rc;
         }
         c->have_density = c->have_predict = c->have_grad = c->have_force = false;
@@ -347,7 +355,7 @@ extern "C" int sph_strength_update(sph_ctx *c, int phase, float dt)
 // density -> predict -> fused gradient + force
 static int derivative_passes(sph_ctx *c)
 {
-    int rc = sph_density(c);
+    int rc = c->have_density ? SPH_OK : sph_density(c);
     if (rc) return rc;
     rc = sph_strength_update(c, SPH_PREDICT, 0.f);
     if (rc) return rc;
@@ -384,7 +392,9 @@ static int step_body(sph_ctx *c, sph_state *state, long long n, float dt, float 
         rc = sph_launch_kick_drift(c, dt);
         if (rc) return rc;
     }
+    c->fuse_density_now = c->use_lists && (c->p.flags & SPH_FUSED_DENSITY) != 0;
     rc = sph_build_neighbors(c, nullptr, 0);
+    c->fuse_density_now = false;
     if (rc) return rc;
     rc = derivative_passes(c);
     if (rc) return rc;

@@ -130,6 +130,13 @@ __device__ __forceinline__ int scan_popc(const unsigned *mask, unsigned short *o
     return __shfl_sync(FULL, incl, 31);
 }
 
+// DENS (SPH_FUSED_DENSITY, off by default): the density pass (S2) of the tile runs inside this kernel, round
+// by round, right after the round's lists are written.  The idea was that its fp64 / conversion work fills
+// issue slots the integer-heavy list build leaves idle, with the candidates' positions already in shared
+// memory; measured, it is 4 % SLOWER per step on configs[2] (two more barriers per round, 80 registers, the
+// lists read back) -- kept as the A/B.  Same arithmetic in the same order as k_density_l: bitwise the same
+// rho, Omega and counts.
+template <bool DENS>
 __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -338,6 +345,11 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     int G = 0;                            // row-groups of this lane in the global list so far (padding included)
     int nhit = 0;                         // true neighbours
     unsigned tests = 0;
+    int Gstart = 0;                       // first row-group of the current round
+    // density state (DENS): self term q = 0, t = 1
+    double dsum = valid ? (double)pi.w : 0.0;
+    float dsh = 3.f * pi.w;
+    int dng = 1;
     // write the complete row-groups of the buffer out, keep the 0..3 entries left over
 #define LIST_FLUSH()                                                                        \
     do {                                                                                    \
@@ -381,7 +393,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             // ---- B: quarter g of this warp tests the candidates flagged for it, in slot order ---------
             const int selfrel = (int)sm.selfslot[threadIdx.x] - r0;    // self exclusion (j != i)
             const unsigned selfoff = (selfrel >= 0 && selfrel < nr) ? (unsigned)selfrel << 4 : 0xffffffffu;
-            const int Gstart = G;
+            Gstart = G;
             unsigned short(*gl)[SPH_GCAP] = sm.gl[warp];
             const unsigned char *const posb = reinterpret_cast<const unsigned char *>(sm.pos);
             // Every quarter keeps a ring of SPH_GCAP offsets.  The rings are filled from the flag words
@@ -493,7 +505,75 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             if (G > d.rows_cap) sm.overflow = 8;      // list rows exhausted: the tile falls back
             if (lane == 0) rp[round + 1] = (unsigned short)min(Gmax, d.rows_cap);
         }
+        if (DENS) {
+            // ---- C: density of this round's list entries.  The masses of the round's candidates go where
+            //         the rings were; positions are still in pos[].
+            __syncthreads();
+            float *const sm_m = reinterpret_cast<float *>(sm.gl);
+            for (int s = threadIdx.x; s < nr; s += SPH_TILE) sm_m[s] = d.r.pm[cand[r0 + s]].w;
+            __syncthreads();
+            if (warp < nch && valid) {
+                const float invH = 1.f / Hi;
+                const double invHd = 1.0 / ((double)kappa * (double)d.r.vh[i].w);
+                const double pxd = (double)pi.x, pyd = (double)pi.y, pzd = (double)pi.z;
+                const unsigned char *const posb = reinterpret_cast<const unsigned char *>(sm.pos);
+                const int gend = min(G, d.rows_cap);
+                for (int gq = Gstart; gq < gend; ++gq) {
+                    const uint2 w = lp[(size_t)gq * 32];
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        const unsigned x_ = (e & 2) ? w.y : w.x;
+                        const unsigned off = (e & 1) ? (x_ >> 16) : (x_ & 0xffffu);
+                        if (off == 0xffffu) continue;
+                        const float4 q = *reinterpret_cast<const float4 *>(posb + off);
+                        const float mj = sm_m[off >> 4];
+                        float dx = __fsub_rn(pi.x, q.x), dy = __fsub_rn(pi.y, q.y), dz = __fsub_rn(pi.z, q.z);
+                        float r2 = sph_r2(dx, dy, dz);
+                        if (r2 < H2i) {
+                            float rinv = sph_rsqrt(fmaxf(r2, 1.0e-37f));
+                            float r = r2 * rinv;
+                            float qq = r * invH;
+                            float t = fmaxf(0.f, 1.f - qq);
+                            float t3 = t * t * t;
+                            dsh = fmaf(mj * t3, fmaf(qq, fmaf(-32.f, qq, 9.f), 3.f), dsh);
+                            double ex = pxd - (double)q.x, ey = pyd - (double)q.y, ez = pzd - (double)q.z;
+                            double r2d = fma(ex, ex, fma(ey, ey, ez * ez));
+                            const double yd = (double)rinv, td0 = r2d * yd;
+                            double rd = fma(0.5 * td0, fma(-td0, yd, 1.0), td0);
+                            double qd = rd * invHd;
+                            double td = 1.0 - qd;
+                            double t2 = td * td;
+                            dsum = fma((double)mj * t2 * t2, fma(4.0, qd, 1.0), dsum);
+                            ++dng;
+                        }
+                    }
+                }
+            }
+        }
         __syncthreads();
+    }
+    if (DENS && valid && !sm.overflow) {
+        const float invH = 1.f / Hi;
+        const double invHd = 1.0 / ((double)kappa * (double)d.r.vh[i].w);
+        float kw = SPH_WC2_SIGMA * invH * invH * invH;
+        double rhod = 3.3422538049298023 * invHd * invHd * invHd * dsum;
+        float rho = (float)rhod;
+        d.rho64[i] = rhod;
+        d.rho[i] = rho;
+        d.omega[i] = 1.f - kw * dsh / (3.f * rho);
+        d.ngather[i] = dng;
+    }
+    if (DENS && !sm.overflow) {
+        unsigned long long hits = valid ? (unsigned long long)dng : 0ull, dt_ = valid ? (unsigned long long)(nhit + 1) : 0ull;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            hits += __shfl_xor_sync(FULL, hits, o);
+            dt_ += __shfl_xor_sync(FULL, dt_, o);
+        }
+        if (lane == 0) {
+            atomicAdd(&d.counters[SPH_C_PAIRS_GATHER], hits);
+            atomicAdd(&d.counters[SPH_C_TESTS_DENSITY], dt_);
+        }
     }
     if (valid) d.nsym[i] = nhit;
     if (warp < nch) {
@@ -778,20 +858,25 @@ static int set_smem(sph_ctx *c, const void *fn, size_t bytes)
     return SPH_OK;
 }
 
-int sph_launch_cull(sph_ctx *c)
+int sph_launch_cull(sph_ctx *c, bool with_density)
 {
     Dev &d = c->d;
     SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_TESTS_CULL], 0, 3 * sizeof(unsigned long long), c->stream));
     SPH_CUDA(c, cudaMemsetAsync(d.cand_cursor, 0, sizeof(unsigned long long), c->stream));
     if (d.n == 0) return SPH_OK;
-    int rc = set_smem(c, (const void *)k_cull, sizeof(CullSmem));
+    int rc = set_smem(c, with_density ? (const void *)k_cull<true> : (const void *)k_cull<false>, sizeof(CullSmem));
     if (rc) return rc;
+    if (with_density) {
+        SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_PAIRS_GATHER], 0, sizeof(unsigned long long), c->stream));
+        SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_TESTS_DENSITY], 0, sizeof(unsigned long long), c->stream));
+    }
     int ntile = sph_div_up(d.nchunk, SPH_TILE_CHUNKS);
     SPH_CUDA(c, cudaMemsetAsync(d.nheavy, 0, sizeof(unsigned), c->stream));
     k_tile_plan<<<sph_div_up(ntile, 256), 256, 0, c->stream>>>(d, ntile);
     k_tile_plan_clamp<<<1, 1, 0, c->stream>>>(d);
     SPH_CUDA(c, cudaMemsetAsync(d.cull_cycles, 0, sizeof(unsigned long long), c->stream));
-    k_cull<<<d.heavy_cap + ntile, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, ntile);
+    if (with_density) k_cull<true><<<d.heavy_cap + ntile, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, ntile);
+    else k_cull<false><<<d.heavy_cap + ntile, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, ntile);
     c->launches += 3;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;

@@ -31,6 +31,7 @@ FLAG_PCLIP_GLOBAL = 4
 FLAG_JAUMANN_COROTATIONAL = 8
 FLAG_NO_LISTS = 16
 FLAG_NO_GRAPH = 64
+FLAG_FUSED_DENSITY = 128
 
 G_NEWTON = 6.674e-11
 

@@ -277,3 +277,26 @@ def test_graph_replay_equals_kernel_by_kernel_step():
         assert np.array_equal(out[0][0][k], out[1][0][k]), k
     assert out[0][1] == out[1][1] and out[0][2] == out[1][2]
     assert np.array_equal(out[0][3], out[1][3])
+
+
+def test_fused_density_equals_density_kernel():
+    """SPH_FUSED_DENSITY makes sph_step run the density pass inside the list build (k_cull<true>) instead of
+    k_density_l.  Same arithmetic in the same order: rho, Omega, counts and the state agree bit for bit."""
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    out = []
+    for flag in (0, W.FLAG_FUSED_DENSITY):
+        wl = W.impact_pair(20000, W.SEED_BASE + 3, 100.0, 1.214)
+        wl.params.flags |= flag
+        s = B.Sph(wl.params, wl.n)
+        t = s.upload(wl)
+        for _ in range(3):
+            s.step(t, wl.n, 0.0)
+        torch.cuda.synchronize()
+        out.append({"rho": s.get_field("RHO").cpu().numpy(), "om": s.get_field("OMEGA").cpu().numpy(),
+                    "ng": s.get_field("NGATHER").cpu().numpy(), "x": t["x"].cpu().numpy().copy(),
+                    "S": t["Sxy"].cpu().numpy().copy(), "c": s.get_counters()})
+    for k in ("rho", "om", "ng", "x", "S"):
+        assert np.array_equal(out[0][k], out[1][k]), k
+    assert out[0]["c"]["pairs_gather"] == out[1]["c"]["pairs_gather"]
+    assert out[0]["c"]["tests_density"] == out[1]["c"]["tests_density"]
