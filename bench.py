@@ -205,6 +205,8 @@ def run_ours(args):
     wl = make_workload(args.workload)
     if args.no_graph:
         wl.params.flags |= 64          # SPH_NO_GRAPH
+    if args.sort_lists:
+        wl.params.flags |= 256         # SPH_SORT_LISTS
     if args.fused_density:
         wl.params.flags |= 128         # SPH_FUSED_DENSITY
     n = wl.n
@@ -367,6 +369,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-hydro-only", action="store_true")
+    ap.add_argument("--sort-lists", action="store_true", help="order the lists by bank class (A/B)")
     ap.add_argument("--fused-density", action="store_true", help="density pass inside the list build (A/B)")
     ap.add_argument("--no-graph", action="store_true", help="launch the step kernel by kernel (A/B of the CUDA graph)")
     args = ap.parse_args()

@@ -40,6 +40,9 @@ extern "C" {
 #define SPH_FUSED_DENSITY       128u  /* sph_step: run the density pass inside the list build instead of as its
                                          own kernel (A/B measurement: same results bit for bit, 4 % slower
                                          on configs[2]; off by default)                                    */
+#define SPH_SORT_LISTS          256u  /* after the list build, order every particle's list by the shared-memory
+                                         bank class of its entries (k_list_sort): the pair kernel's gathers
+                                         stop conflicting (A/B measurement)                                */
 #define SPH_MORTON_ORDER         32u  /* sort by Morton (Z-order) keys instead of Hilbert keys (A/B
                                          measurement; results do not depend on the order)                  */
 

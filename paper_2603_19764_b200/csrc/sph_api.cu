@@ -252,6 +252,10 @@ extern "C" int sph_build_neighbors(sph_ctx *c, const sph_state *state, long long
         const bool fuse = c->fuse_density_now;
         rc = sph_launch_cull(c, fuse);
         if (rc) return rc;
+        if (c->p.flags & SPH_SORT_LISTS) {
+            rc = sph_launch_list_sort(c);
+            if (rc) return rc;
+        }
         if (fuse) {
             PassTimer td(c, SPH_T_DENSITY);           // what is left of S2: the tiles over a list capacity
             rc = sph_launch_density(c, true);

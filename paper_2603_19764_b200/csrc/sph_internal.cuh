@@ -175,6 +175,7 @@ int sph_launch_h_update(sph_ctx *c, float n_target);
 int sph_launch_neighbors(sph_ctx *c, int which, int *counts, const long long *offsets, int *list, bool flagged_only);
 int sph_launch_download(sph_ctx *c, sph_state *st);
 int sph_launch_cull(sph_ctx *c, bool with_density);
+int sph_launch_list_sort(sph_ctx *c);
 int sph_launch_density_l(sph_ctx *c);
 int sph_launch_pair_l(sph_ctx *c, bool grad, bool force);
 int sph_launch_neighbors_l(sph_ctx *c, int which, int *counts, const long long *offsets, int *list);

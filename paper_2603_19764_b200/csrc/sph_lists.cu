@@ -613,6 +613,93 @@ __global__ void k_tile_plan_clamp(Dev d)
     if (*d.nheavy > (unsigned)d.heavy_cap) *d.nheavy = (unsigned)d.heavy_cap;
 }
 
+// ------------------------------------------------------------------------------------------
+// k_list_sort (SPH_SORT_LISTS): reorder every lane's list entries of a round so that lane l reads bank class
+// (l + n) mod 8 at step n (class = slot mod 8 = which 16-byte bank group the slot's float4 sits in).  The eight
+// lanes of a quarter-warp phase then hit eight different bank groups in the pair kernel's gathers instead of
+// random ones (2.47 wavefronts per phase).  Per lane: count the classes, bucket the entries by class in shared
+// memory (counting sort, cursors packed 8 x 8 bit), emit them round-robin over the classes starting at the
+// lane's own; when the wanted class has run out, the next one in cyclic order that has entries.  One warp per
+// chunk, all lanes in lockstep over the positions of the round; rounds with a lane over SORT_CAP entries stay as
+// they are.  The order of a lane's entries has no meaning (a set), so results change only by summation order.
+// ------------------------------------------------------------------------------------------
+#define SORT_CAP 160
+#define SORT_STRIDE (SORT_CAP * 2 + 4)       // bytes per lane: 81 words
+#define SORT_WARPS 4
+__global__ void __launch_bounds__(SORT_WARPS * 32) k_list_sort(Dev d)
+{
+    __shared__ __align__(4) unsigned char s_buf[SORT_WARPS * 32 * SORT_STRIDE];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int chunk = blockIdx.x * SORT_WARPS + warp;
+    if (chunk >= d.nchunk) return;
+    const int tile = chunk / SPH_TILE_CHUNKS;
+    if (d.tile_flag[tile]) return;
+    const int nround = (d.tile_ncand[tile] + SPH_SE - 1) / SPH_SE;
+    uint2 *lp = d.nlist + ((size_t)chunk * d.rows_cap) * 32 + lane;
+    const unsigned short *rp = d.rowptr + (size_t)chunk * ROWPTR_STRIDE;
+    unsigned short *buf = reinterpret_cast<unsigned short *>(s_buf + (size_t)threadIdx.x * SORT_STRIDE);
+    for (int r = 0; r < nround; ++r) {
+        const int g0 = rp[r], g1 = rp[r + 1];
+        if (g1 <= g0) continue;
+        // pass 1: class counts
+        unsigned long long cnt = 0ull;
+        int N = 0;
+        for (int gq = g0; gq < g1; ++gq) {
+            const uint2 w = lp[(size_t)gq * 32];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const unsigned x = (e & 2) ? w.y : w.x;
+                const unsigned off = (e & 1) ? (x >> 16) : (x & 0xffffu);
+                if (off != 0xffffu) { cnt += 1ull << (((off >> 4) & 7u) << 3); ++N; }
+            }
+        }
+        if (__any_sync(FULL, N > SORT_CAP)) continue;
+        const unsigned long long base = cnt * 0x0101010101010100ull;     // field c = entries of the classes below c
+        // pass 2: bucket by class
+        unsigned long long cur = base;
+        for (int gq = g0; gq < g1; ++gq) {
+            const uint2 w = lp[(size_t)gq * 32];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const unsigned x = (e & 2) ? w.y : w.x;
+                const unsigned off = (e & 1) ? (x >> 16) : (x & 0xffffu);
+                if (off != 0xffffu) {
+                    const unsigned c8 = ((off >> 4) & 7u) << 3;
+                    buf[(unsigned)(cur >> c8) & 0xffu] = (unsigned short)off;
+                    cur += 1ull << c8;
+                }
+            }
+        }
+        const unsigned long long end = cur;
+        unsigned long long tk = base;
+        // pass 3: emit round-robin over the classes, all lanes in lockstep over the positions
+        const int nmax = (g1 - g0) * 4;
+        unsigned w0 = 0u, w1 = 0u;
+        for (int n = 0; n < nmax; ++n) {
+            unsigned entry = 0xffffu;
+            if (n < N) {
+                unsigned c8 = ((unsigned)(lane + n) & 7u) << 3;
+                while (((unsigned)(tk >> c8) & 0xffu) >= ((unsigned)(end >> c8) & 0xffu)) c8 = (c8 + 8u) & 63u;
+                entry = buf[(unsigned)(tk >> c8) & 0xffu];
+                tk += 1ull << c8;
+            }
+            w0 = __byte_perm(w0, w1, 0x5432);
+            w1 = __byte_perm(w1, entry, 0x5432);
+            if ((n & 3) == 3) lp[(size_t)(g0 + (n >> 2)) * 32] = make_uint2(w0, w1);
+        }
+    }
+}
+
+int sph_launch_list_sort(sph_ctx *c)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    k_list_sort<<<sph_div_up(d.nchunk, SORT_WARPS), SORT_WARPS * 32, 0, c->stream>>>(d);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
 // entry e (0..3) of a row-group word pair
 __device__ __forceinline__ unsigned list_entry(uint2 w, int e)
 {

@@ -32,6 +32,7 @@ FLAG_JAUMANN_COROTATIONAL = 8
 FLAG_NO_LISTS = 16
 FLAG_NO_GRAPH = 64
 FLAG_FUSED_DENSITY = 128
+FLAG_SORT_LISTS = 256
 
 G_NEWTON = 6.674e-11
 

@@ -39,7 +39,7 @@ def test_config0_single_pass_all_fields():
 
 
 @pytest.mark.parametrize("case", ["ragged_11", "h_spread", "two_materials", "hydro_only", "no_correction",
-                                  "corotational", "pclip_global", "block_24"])
+                                  "corotational", "pclip_global", "block_24", "sort_lists"])
 def test_variants(case):
     kw = dict(n_side=12)
     if case == "ragged_11":
@@ -58,6 +58,8 @@ def test_variants(case):
         kw = dict(n_side=12, flags=F | W.FLAG_PCLIP_GLOBAL)
     elif case == "block_24":
         kw = dict(n_side=24)                                  # 432 chunks: two tree levels
+    elif case == "sort_lists":
+        kw = dict(n_side=12, h_spread=0.2, flags=F | W.FLAG_SORT_LISTS)   # lists reordered by bank class
     wl = W.elastic_block(**kw)
     g = U.gpu_single_pass(wl)
     d = O.single_pass(wl, mode="grid" if wl.n > 5000 else "brute")
