@@ -340,8 +340,9 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     const int chunk = chunk0 + warp;
     uint2 *lp = d.nlist + ((size_t)(warp < nch ? chunk : chunk0) * d.rows_cap) * 32 + lane;
     unsigned short *rp = d.rowptr + (size_t)(warp < nch ? chunk : chunk0) * ROWPTR_STRIDE;
-    unsigned char *const lb = sm.u.lbuf + threadIdx.x * LBUF_STRIDE;
-    unsigned char *wp = lb;               // where the next entry goes
+    // the lane's buffer and its write position as 32-bit byte offsets into the dynamic shared memory
+    const unsigned lb = (unsigned)(sm.u.lbuf - smem_raw) + threadIdx.x * LBUF_STRIDE;
+    unsigned wp = lb;                     // where the next entry goes
     int G = 0;                            // row-groups of this lane in the global list so far (padding included)
     int nhit = 0;                         // true neighbours
     unsigned tests = 0;
@@ -357,8 +358,8 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
         const int rmax_ = __reduce_max_sync(FULL, rows_);                                   \
         for (int r_ = 0; r_ < rmax_; ++r_)                                                  \
             if (r_ < rows_ && G + r_ < d.rows_cap)                                          \
-                lp[(size_t)(G + r_) * 32] = *reinterpret_cast<const uint2 *>(lb + 8 * r_);  \
-        if (cnt_ & 3) *reinterpret_cast<uint2 *>(lb) = *reinterpret_cast<const uint2 *>(lb + 8 * rows_); \
+                lp[(size_t)(G + r_) * 32] = *reinterpret_cast<const uint2 *>(smem_raw + lb + 8 * r_);  \
+        if (cnt_ & 3) *reinterpret_cast<uint2 *>(smem_raw + lb) = *reinterpret_cast<const uint2 *>(smem_raw + lb + 8 * rows_); \
         G += rows_;                                                                         \
         wp = lb + 2 * (cnt_ & 3);                                                           \
     } while (0)
@@ -476,7 +477,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
                         const float4 q = *reinterpret_cast<const float4 *>(posb + off);
                         const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
                         if (r2 < fmaxf(H2i, q.w) && off != selfoff) {
-                            *reinterpret_cast<unsigned short *>(wp) = (unsigned short)off;
+                            *reinterpret_cast<unsigned short *>(smem_raw + wp) = (unsigned short)off;
                             wp += 2;
                         }
                     }
@@ -494,7 +495,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             // ---- end of the round: pad the last row-group, flush, pad every lane to the warp's longest list
             nhit += 4 * (G - Gstart) + ((int)(wp - lb) >> 1);
             while ((int)(wp - lb) & 7) {
-                *reinterpret_cast<unsigned short *>(wp) = 0xffffu;
+                *reinterpret_cast<unsigned short *>(smem_raw + wp) = 0xffffu;
                 wp += 2;
             }
             LIST_FLUSH();
