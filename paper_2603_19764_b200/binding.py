@@ -9,6 +9,7 @@ from __future__ import annotations
 import ctypes as C
 import math
 import os
+import sys
 from typing import Dict, Optional
 
 HERE = os.path.dirname(os.path.abspath(__file__))
@@ -67,11 +68,28 @@ class SphError(RuntimeError):
 _lib = None
 
 
+def _ensure_built():
+    """Compile libsph.so when it is missing or older than its sources (nvcc is in the image; this is a
+    build step, not a fallback).  Under torchrun only local rank 0 compiles; the others wait for the file."""
+    import time
+    from . import build as _build
+    if os.environ.get("LOCAL_RANK", "0") == "0":
+        try:
+            _build.build()
+        except Exception as e:                      # reported by the missing-file check in load()
+            sys.stderr.write(f"building {LIB_PATH} failed: {e}\n")
+        return
+    t0 = time.time()
+    while not os.path.exists(LIB_PATH) and time.time() - t0 < 600.0:
+        time.sleep(1.0)
+
+
 def load():
     """dlopen libsph.so and declare the prototypes.  Fails loudly; never falls back."""
     global _lib
     if _lib is not None:
         return _lib
+    _ensure_built()
     if not os.path.exists(LIB_PATH):
         raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2603_19764_b200.build` "
                            "(there is no CPU fallback)")
