@@ -285,17 +285,34 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     const int nsrc = sm.nfront;
 
     // ---- A2: which particles of the accepted source chunks reach a chunk box of the tile ------------
-    for (int k = warp; k < nsrc; k += SPH_TILE_CHUNKS) {
-        long long j = (long long)sm.chunks[k] * SPH_CHUNK + lane;
-        unsigned f = 0;
+    // (two source chunks per trip: both pairs of loads are in flight before the first is used -- the loop is
+    //  bound by the latency of these L2 reads, not by its arithmetic)
+    for (int k = warp; k < nsrc; k += 2 * SPH_TILE_CHUNKS) {
+        const int k2 = k + SPH_TILE_CHUNKS;
+        const bool has2 = k2 < nsrc;
+        const long long j = (long long)sm.chunks[k] * SPH_CHUNK + lane;
+        const long long j2 = has2 ? (long long)sm.chunks[k2] * SPH_CHUNK + lane : d.n;
+        float4 q = make_float4(0.f, 0.f, 0.f, 0.f), q2 = q;
+        float h = 0.f, h2 = 0.f;
+        if (j < d.n) { q = d.r.pm[j]; h = d.r.vh[j].w; }
+        if (j2 < d.n) { q2 = d.r.pm[j2]; h2 = d.r.vh[j2].w; }
+        unsigned f = 0, f2 = 0;
         if (j < d.n) {
-            float4 q = d.r.pm[j];
-            const float Hj = sph_H(kappa, d.r.vh[j].w);
+            const float Hj = sph_H(kappa, h);
             f = reach_chunks(sm, sm.cmask[k], q.x, q.y, q.z, Hj * Hj * SPH_REACH_SLACK);
         }
+        if (j2 < d.n) {
+            const float Hj = sph_H(kappa, h2);
+            f2 = reach_chunks(sm, sm.cmask[k2], q2.x, q2.y, q2.z, Hj * Hj * SPH_REACH_SLACK);
+        }
         if (k < SPH_CULL_CFCACHE) sm.cf[k][lane] = (unsigned char)f;
-        unsigned m = __ballot_sync(FULL, f != 0);
+        const unsigned m = __ballot_sync(FULL, f != 0);
         if (lane == 0) sm.mask[k] = m;
+        if (has2) {
+            if (k2 < SPH_CULL_CFCACHE) sm.cf[k2][lane] = (unsigned char)f2;
+            const unsigned m2 = __ballot_sync(FULL, f2 != 0);
+            if (lane == 0) sm.mask[k2] = m2;
+        }
     }
     __syncthreads();
     if (warp == 0) {
@@ -370,24 +387,43 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     for (int r0 = 0; r0 < ntotal; r0 += SPH_SE, ++round) {
         const int nr = min(SPH_SE, ntotal - r0);
         // ---- A3: compact this round's survivors into shared memory and the global candidate list
-        for (int k = warp; k < nsrc; k += SPH_TILE_CHUNKS) {
-            unsigned m = sm.mask[k];
-            int o = (int)sm.off[k];
-            if (o >= r0 + nr || o + 32 <= r0) continue;
-            if (!((m >> lane) & 1u)) continue;
-            int slot = o + __popc(m & lt) - r0;
-            if (slot < 0 || slot >= nr) continue;
-            long long j = (long long)sm.chunks[k] * SPH_CHUNK + lane;
-            float4 q = d.r.pm[j];
-            float Hj = sph_H(kappa, d.r.vh[j].w);
-            sm.pos[slot] = make_float4(q.x, q.y, q.z, __fmul_rn(Hj, Hj));
-            const float H2s = Hj * Hj * SPH_REACH_SLACK;
-            const unsigned fc = k < SPH_CULL_CFCACHE ? (unsigned)sm.cf[k][lane]
-                                                     : reach_chunks(sm, sm.cmask[k], q.x, q.y, q.z, H2s);
-            sm.flag[slot] = (unsigned char)fc;
-            cand[r0 + slot] = (unsigned)j;
-            long long rel = j - (long long)tile * SPH_TILE;
-            if (rel >= 0 && rel < SPH_TILE) sm.selfslot[rel] = (unsigned)(r0 + slot);
+        // (two source chunks per trip, as in A2: the loads of both are issued before either is used)
+        for (int k = warp; k < nsrc; k += 2 * SPH_TILE_CHUNKS) {
+            int slot[2];
+            long long jj[2];
+            float4 q[2];
+            float hh[2];
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                const int kk = k + t * SPH_TILE_CHUNKS;
+                slot[t] = -1;
+                jj[t] = 0;
+                if (kk < nsrc) {
+                    const unsigned m = sm.mask[kk];
+                    const int o = (int)sm.off[kk];
+                    if (o < r0 + nr && o + 32 > r0 && ((m >> lane) & 1u)) {
+                        const int sl = o + __popc(m & lt) - r0;
+                        if (sl >= 0 && sl < nr) { slot[t] = sl; jj[t] = (long long)sm.chunks[kk] * SPH_CHUNK + lane; }
+                    }
+                }
+            }
+#pragma unroll
+            for (int t = 0; t < 2; ++t)
+                if (slot[t] >= 0) { q[t] = d.r.pm[jj[t]]; hh[t] = d.r.vh[jj[t]].w; }
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                if (slot[t] < 0) continue;
+                const int kk = k + t * SPH_TILE_CHUNKS;
+                const float Hj = sph_H(kappa, hh[t]);
+                sm.pos[slot[t]] = make_float4(q[t].x, q[t].y, q[t].z, __fmul_rn(Hj, Hj));
+                const float H2s = Hj * Hj * SPH_REACH_SLACK;
+                const unsigned fc = kk < SPH_CULL_CFCACHE ? (unsigned)sm.cf[kk][lane]
+                                                          : reach_chunks(sm, sm.cmask[kk], q[t].x, q[t].y, q[t].z, H2s);
+                sm.flag[slot[t]] = (unsigned char)fc;
+                cand[r0 + slot[t]] = (unsigned)jj[t];
+                const long long rel = jj[t] - (long long)tile * SPH_TILE;
+                if (rel >= 0 && rel < SPH_TILE) sm.selfslot[rel] = (unsigned)(r0 + slot[t]);
+            }
         }
         __syncthreads();
         if (warp < nch) {
