@@ -4,7 +4,10 @@ This module serves BOTH the CPU oracle (``oracle/``) and the CUDA path, so it
 holds none of the method's arithmetic: no kernel function, no EOS, no yield
 law.  It only lays particles out (lattices, spheres, a column on a floor), draws
 jitter / noise from a stateless counter-based generator and writes the material
-constants of BASELINE.json's configs into plain records.
+constants of BASELINE.json's configs into plain records.  The synthetic EOS tables
+(``synthetic_eos_table``) are input DATA in the same sense: smooth surfaces sampled on a grid,
+standing in for the paper's M-ANEOS tables; how a table is looked up is the method's business and
+lives in oracle/ and in the CUDA path, separately.
 
 Recipe: everything is generated in
 fp64 from splitmix64(seed + GOLDEN*(16*i + stream)) and cast ONCE to fp32; the
