@@ -266,3 +266,46 @@ def test_singular_correction_falls_back_to_identity():
     # an isolated particle: everything zero, flagged
     F0 = np.zeros((9, 1)); G0, f0 = O.correct_gradient(F0, F0.copy(), O.FLAG_CORRECTION_TENSOR)
     assert f0.tolist() == [1] and np.all(G0 == 0)
+
+
+# ------------------------------------------------------------------ two particles: Eq. 1, 3, 18, 19 by hand
+def test_two_particle_closed_forms():
+    """Two particles on the x axis, different m, h, rho, Omega, P and a full S: every sum has one term, so
+    Eq. 1, 3 and Eq. 18, 19 can be written out with the scalar kernel
+    functions (pinned in test_oracle_kernel.py).  A wrong sign, a swapped h_i / h_j, a missing Omega or a
+    transposed stress index fails here.  No artificial viscosity (receding pair)."""
+    r = 0.7
+    p = np.array([[0.0, r], [0.0, 0.0], [0.0, 0.0]])
+    m = np.array([2.0, 3.0]); h = np.array([0.5, 0.6]); kap = 2.0
+    # density and Omega
+    c, o, l = O.neighbors(p[0], p[1], p[2], h, kap, O.GATHER)
+    rho, om = O.density(p[0], p[1], p[2], m, h, kap, o, l)
+    for i, j in ((0, 1), (1, 0)):
+        rho_i = m[i] * O.W(0.0, h[i], kap) + m[j] * O.W(r, h[i], kap)
+        dh = m[i] * O.dWdh(0.0, h[i], kap) + m[j] * O.dWdh(r, h[i], kap)
+        assert rho[i] == pytest.approx(rho_i, rel=1e-13)
+        assert om[i] == pytest.approx(1.0 + h[i] / (3.0 * rho_i) * dh, rel=1e-12)
+    # forces with prescribed rho, Omega, P, S (five stored components xx, yy, xy, xz, yz; zz = -xx - yy)
+    rho_in = np.array([1.3, 0.9]); om_in = np.array([0.95, 1.1]); P = np.array([0.4, -0.2])
+    S = np.array([[0.3, -0.1], [0.2, 0.25], [0.15, -0.05], [-0.2, 0.1], [0.05, 0.3]])
+    v = np.array([[-0.5, 0.5], [0.2, -0.1], [0.0, 0.3]])              # v_ij . x_ij > 0: receding, Pi = 0
+    prm = params()
+    cs_, os_, ls_ = O.neighbors(p[0], p[1], p[2], h, kap, O.SYMMETRIC)
+    a, dudt, mumax = O.forces(prm, p[0], p[1], p[2], m, h, v[0], v[1], v[2], rho_in, om_in, P,
+                              np.array([1.0, 1.0]), S, None, os_, ls_)
+
+    def sigma(k):
+        sxx, syy, sxy, sxz, syz = S[:, k]
+        return np.array([[sxx, sxy, sxz], [sxy, syy, syz], [sxz, syz, -sxx - syy]]) - P[k] * np.eye(3)
+    for i, j in ((0, 1), (1, 0)):
+        xij = p[:, i] - p[:, j]
+        e = xij / r                                                      # grad_i W_ij(h) = W'(r, h) x_ij / r
+        gi = O.dWdr(r, h[i], kap) * e
+        gj = O.dWdr(r, h[j], kap) * e
+        a_i = m[j] * (sigma(i) @ gi / (om_in[i] * rho_in[i] ** 2) + sigma(j) @ gj / (om_in[j] * rho_in[j] ** 2))
+        vij = v[:, i] - v[:, j]
+        du_i = -m[j] * vij @ (sigma(i) @ gi) / (om_in[i] * rho_in[i] ** 2)
+        assert np.allclose(a[:, i], a_i, rtol=1e-12, atol=1e-14)
+        assert dudt[i] == pytest.approx(du_i, rel=1e-12)
+    assert np.all(mumax == 0.0)
+    assert np.allclose(m[0] * a[:, 0] + m[1] * a[:, 1], 0.0, atol=1e-13)
