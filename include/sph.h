@@ -31,7 +31,9 @@ extern "C" {
 #define SPH_STRENGTH              1u  /* evolve S, add the S terms of Eq. 18-19      */
 #define SPH_CORRECTION_TENSOR     2u  /* G = F.C (Eq. 22); off: C = 1      */
 #define SPH_PCLIP_GLOBAL          4u  /* clip P >= 0 in the EOS too, not only in Eq. 34 (reading Q8)    */
-#define SPH_JAUMANN_COROTATIONAL  8u  /* flip the sign of the rotation terms of Eq. 13 (reading Q1)     */
+#define SPH_JAUMANN_AS_PRINTED    8u  /* rotation terms of Eq. 13 with the index order AS PRINTED, S.R - R.S,
+                                         instead of the objective (co-rotational) Jaumann rate R.S - S.R that
+                                         is the default (reading Q1: the print contradicts "objective")     */
 #define SPH_NO_LISTS             16u  /* pair passes walk the chunk tree themselves instead of reading
                                          the per-particle neighbour lists (the round-1 "v0" kernels: A/B
                                          measurement; they also serve tiles over a list capacity)           */

@@ -28,7 +28,7 @@ from . import build as _build
 FLAG_STRENGTH = 1
 FLAG_CORRECTION_TENSOR = 2
 FLAG_PCLIP_GLOBAL = 4
-FLAG_JAUMANN_COROTATIONAL = 8
+FLAG_JAUMANN_AS_PRINTED = 8
 
 GATHER, SYMMETRIC = 0, 1
 CTOL = 1.0e-4          # reading Q9: C = I unless |det C^-1| > CTOL * ||C^-1||_F^3
@@ -298,16 +298,20 @@ def _S3(S):
 
 
 def stress_rate(G, S, Gamma, flags):
-    """dS/dt = 2 Gamma (eps_dot - tr(eps_dot)/3 delta) + S.R + (S.R)^T  (Eq. 13, as
-    printed: S^{ag} R^{gb} + S^{bg} R^{ga}).  JAUMANN_COROTATIONAL flips the sign of the rotation
-    terms (reading Q1).  Evaluated as a full 3x3; returns the five stored components [5][n],
-    the full tensor and 1/2 eps_dot:eps_dot (Eq. 43)."""
+    """dS/dt = 2 Gamma (eps_dot - tr(eps_dot)/3 delta) + rotation terms (Eq. 13).
+    Reading Q1: the paper "adopt[s] the Jaumann rate to obtain an objective stress rate"
+    (PAPER.md:122) after Benz & Asphaug, whose rotation terms are S^{ag} R^{bg} + S^{gb} R^{ag}
+    = R.S - S.R with R of Eq. 15: the rate that turns S with the body.  The index order AS PRINTED,
+    S^{ag} R^{gb} + S^{bg} R^{ga} = S.R + (S.R)^T = S.R - R.S, is the negative of that and is not
+    objective, so the text is at odds with itself; the default follows the words ("objective"),
+    JAUMANN_AS_PRINTED follows the indices.  Evaluated as a full 3x3; returns the five stored
+    components [5][n], the full tensor and 1/2 eps_dot:eps_dot (Eq. 43)."""
     eps, R = strain_and_rotation(G)
     S3 = _S3(S)
     tr = np.trace(eps, axis1=1, axis2=2)
     elastic = 2.0 * Gamma[:, None, None] * (eps - tr[:, None, None] / 3.0 * np.eye(3)[None])
     SR = np.einsum("nag,ngb->nab", S3, R)
-    sgn = -1.0 if (flags & FLAG_JAUMANN_COROTATIONAL) else 1.0
+    sgn = 1.0 if (flags & FLAG_JAUMANN_AS_PRINTED) else -1.0
     dS3 = elastic + sgn * (SR + np.transpose(SR, (0, 2, 1)))
     dS = np.stack([dS3[:, 0, 0], dS3[:, 1, 1], dS3[:, 0, 1], dS3[:, 0, 2], dS3[:, 1, 2]], axis=0)
     eps2 = 0.5 * (eps * eps).sum(axis=(1, 2))
@@ -320,7 +324,7 @@ def stress_rate_components(G, S, Gamma, flags):
     of stress_rate(); G component index 3*alpha + beta."""
     Gxx, Gxy, Gxz, Gyx, Gyy, Gyz, Gzx, Gzy, Gzz = G
     Sxx, Syy, Sxy, Sxz, Syz = S
-    s = -1.0 if (flags & FLAG_JAUMANN_COROTATIONAL) else 1.0
+    s = 1.0 if (flags & FLAG_JAUMANN_AS_PRINTED) else -1.0
     dSxx = s * (Sxy * (Gyx - Gxy) + Sxz * (Gzx - Gxz)) - (2.0 / 3.0) * Gamma * (Gyy + Gzz - 2.0 * Gxx)
     dSyy = s * (Sxy * (Gxy - Gyx) + Syz * (Gzy - Gyz)) - (2.0 / 3.0) * Gamma * (Gxx + Gzz - 2.0 * Gyy)
     dSxy = Gamma * (Gxy + Gyx) + s * 0.5 * (Sxx * (Gxy - Gyx) + Syy * (Gyx - Gxy)
@@ -356,13 +360,16 @@ def forces(params, x, y, z, m, h, vx, vy, vz, rho, omega, P, cs, S, g, offsets, 
 
 def timestep(params, h, cs, mumax, a=None):
     """dt_i,CFL = eta_C h_i / ((1 + 0.6 alpha) c_i + 0.6 beta max_j |min(0, mu_ij)|)
-    (Eq. 39); optionally dt_i,a = eta_a sqrt(h_i/|a_i|) (Eq. 38 with
-    epsilon = h_i)."""
+    (Eq. 39); when eta_a > 0 also dt_i,a = eta_a sqrt(epsilon/|a_i|) (PAPER.md:227,
+    Eq. 38) with epsilon = h_i (reading Q22: PAPER.md:234 offers "the gravitational softening length
+    or SPH kernel size"; gravity is not built here, so the SPH length it is) and a_i the full
+    acceleration of Eq. 18 including a_ext; "the minimum of these criteria".
+    |a_i| = 0 leaves Eq. 39 alone."""
     dt = params.eta_C * h / ((1.0 + 0.6 * params.alpha) * cs + 0.6 * params.beta * mumax)
     if params.eta_a > 0.0 and a is not None:
         an = np.sqrt((a * a).sum(axis=0))
-        with np.errstate(divide="ignore"):
-            dt = np.minimum(dt, params.eta_a * np.sqrt(h / np.where(an > 0, an, np.inf)))
+        dt_a = np.where(an > 0.0, params.eta_a * np.sqrt(h / np.where(an > 0.0, an, 1.0)), np.inf)
+        dt = np.minimum(dt, dt_a)
     return dt
 
 
@@ -430,9 +437,14 @@ def single_pass(wl, dt: Optional[float] = None, mode="brute") -> Dict[str, np.nd
 # the full step (Eq. 40-42)
 # ---------------------------------------------------------------------------
 class Stepper:
-    """Global-dt kick-drift-kick with predictor-corrector for u and S (reading Q17)."""
+    """Global-dt kick-drift-kick with predictor-corrector for u and S (reading Q17).
 
-    def __init__(self, wl, mode="grid"):
+    store_fp32: BASELINE.json's north_star fixes the STORAGE of the particle state as fp32.  With this
+    switch every quantity that is kept between two passes of a step (x after the drift; v, u, S at the
+    half step, predicted and at the full step; the carried derivatives a, du/dt, dS/dt; e_acc) is rounded
+    to fp32 once, where it would be stored; all arithmetic stays fp64.  The default carries fp64 state."""
+
+    def __init__(self, wl, mode="grid", store_fp32=False):
         A = {k: _f64(v) for k, v in wl.arrays.items()}
         self.params = wl.params
         self.mode = mode
@@ -443,15 +455,24 @@ class Stepper:
         self.m, self.h = A["m"], A["h"]
         self.g = np.stack([A["gx"], A["gy"], A["gz"]], axis=0)
         self.mat = wl.mat
+        self.store_fp32 = bool(store_fp32)
         self.free = (wl.fixed == 0).astype(np.float64)
         self.e_acc = np.zeros_like(self.u)
         self.d = None              # derivatives at the current full step
         self.dt_next = None
         self.strength = bool(wl.params.flags & FLAG_STRENGTH)
 
+    def _st(self, a):
+        """what the stored copy of ``a`` holds"""
+        return a.astype(np.float32).astype(np.float64) if self.store_fp32 else a
+
     def _derivs(self, v, u, S):
-        return derivatives(self.params, self.x[0], self.x[1], self.x[2], self.m, self.h,
-                           v[0], v[1], v[2], u, S, self.mat, self.g, self.mode)
+        d = derivatives(self.params, self.x[0], self.x[1], self.x[2], self.m, self.h,
+                        v[0], v[1], v[2], u, S, self.mat, self.g, self.mode)
+        if self.store_fp32:
+            for k in ("a", "dudt", "dS", "Y", "S_pred", "eps2"):
+                d[k] = self._st(d[k])
+        return d
 
     def bootstrap(self):
         """First step: a_0, du_0, dS_0 from the current state (pred = current, dt = 0)."""
@@ -466,24 +487,25 @@ class Stepper:
         a, dudt, dS = self.d["a"], self.d["dudt"], self.d["dS"]
         fr = self.free[None, :]
         # 1. opening kick (Eq. 42); fixed particles keep x, v (reading Q16)
-        v_half = self.v + 0.5 * dt * a * fr
-        u_half = self.u + 0.5 * dt * dudt
-        S_half = self.S + 0.5 * dt * dS
+        st = self._st
+        v_half = st(self.v + 0.5 * dt * a * fr)
+        u_half = st(self.u + 0.5 * dt * dudt)
+        S_half = st(self.S + 0.5 * dt * dS)
         # 2. drift
-        self.x = self.x + dt * v_half * fr
+        self.x = st(self.x + dt * v_half * fr)
         # 3. prediction from the derivatives of the previous step (Eq. 40)
-        v_pred = v_half + 0.5 * dt * a * fr
-        u_pred = u_half + 0.5 * dt * dudt
-        S_pred = S_half + 0.5 * dt * dS
+        v_pred = st(v_half + 0.5 * dt * a * fr)
+        u_pred = st(u_half + 0.5 * dt * dudt)
+        S_pred = st(S_half + 0.5 * dt * dS)
         # 4-6. new derivatives from the predicted (and rescaled, Eq. 31) values
         d = self._derivs(v_pred, u_pred, S_pred)
         # 7. closing kick (Eq. 41) and rescale again
-        self.v = v_half + 0.5 * dt * d["a"] * fr
-        self.u = u_half + 0.5 * dt * d["dudt"]
+        self.v = st(v_half + 0.5 * dt * d["a"] * fr)
+        self.u = st(u_half + 0.5 * dt * d["dudt"])
         if self.strength:
-            self.S, _ = project(S_half + 0.5 * dt * d["dS"], d["Y"])
+            self.S = st(project(S_half + 0.5 * dt * d["dS"], d["Y"])[0])
         # 8. carried derivatives, accumulated strain-rate invariant (Eq. 43)
-        self.e_acc = self.e_acc + dt * d["eps2"]
+        self.e_acc = st(self.e_acc + dt * d["eps2"])
         self.d = d
         self.dt_next = float(d["dt_i"].min())
         return dt

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libsph.so")
 
 MAX_MATERIALS = 8
-STRENGTH, CORRECTION_TENSOR, PCLIP_GLOBAL, JAUMANN_COROTATIONAL, NO_LISTS = 1, 2, 4, 8, 16
+STRENGTH, CORRECTION_TENSOR, PCLIP_GLOBAL, JAUMANN_AS_PRINTED, NO_LISTS = 1, 2, 4, 8, 16
 OK, EINVAL, ENOMEM, ECUDA, EORDER, ECAPACITY = 0, -1, -2, -3, -4, -5
 PREDICT, CLOSE, DERIVATIVES = 0, 1, 2
 GATHER, SYMMETRIC = 0, 1

@@ -156,7 +156,8 @@ __global__ void __launch_bounds__(256) k_close(Dev d, DevParams p, int phase, fl
         const float Sxx = d.r.s[PP_SPRED + 0][i], Syy = d.r.s[PP_SPRED + 1][i], Sxy = d.r.s[PP_SPRED + 2][i],
                     Sxz = d.r.s[PP_SPRED + 3][i], Syz = d.r.s[PP_SPRED + 4][i];
         const float Gam = d.Gamma[i];
-        const float s = (p.flags & SPH_JAUMANN_COROTATIONAL) ? -1.f : 1.f;
+        // reading Q1: the objective (co-rotational) Jaumann rate R.S - S.R by default; the index order as printed is its negative
+        const float s = (p.flags & SPH_JAUMANN_AS_PRINTED) ? 1.f : -1.f;
         const float rxy = Gxy - Gyx, rxz = Gxz - Gzx, ryz = Gyz - Gzy;       // 2 R^{xy}, 2 R^{xz}, 2 R^{yz}
         dS[0] = s * (-Sxy * rxy - Sxz * rxz) - (2.f / 3.f) * Gam * (Gyy + Gzz - 2.f * Gxx);
         dS[1] = s * (Sxy * rxy - Syz * ryz) - (2.f / 3.f) * Gam * (Gxx + Gzz - 2.f * Gyy);

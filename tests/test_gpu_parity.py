@@ -39,7 +39,7 @@ def test_config0_single_pass_all_fields():
 
 
 @pytest.mark.parametrize("case", ["ragged_11", "h_spread", "two_materials", "hydro_only", "no_correction",
-                                  "corotational", "pclip_global", "block_24", "sort_lists"])
+                                  "as_printed", "pclip_global", "block_24", "sort_lists"])
 def test_variants(case):
     kw = dict(n_side=12)
     if case == "ragged_11":
@@ -52,8 +52,8 @@ def test_variants(case):
         kw = dict(n_side=12, flags=W.FLAG_CORRECTION_TENSOR)
     elif case == "no_correction":
         kw = dict(n_side=12, flags=W.FLAG_STRENGTH)
-    elif case == "corotational":
-        kw = dict(n_side=12, flags=F | W.FLAG_JAUMANN_COROTATIONAL)
+    elif case == "as_printed":
+        kw = dict(n_side=12, flags=F | W.FLAG_JAUMANN_AS_PRINTED)
     elif case == "pclip_global":
         kw = dict(n_side=12, flags=F | W.FLAG_PCLIP_GLOBAL)
     elif case == "block_24":

@@ -1,4 +1,6 @@
 """Pins for the oracle's step sequence (Eq. 40-42)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -83,16 +85,104 @@ def test_fixed_particles_do_not_move_and_step_matches_single_pass():
     assert np.all(sj <= d["Y"] * (1 + 1e-12) + 1e-9)
 
 
-def test_cfl_timestep_eq39():
+def _golden_rows(golden_dir, name):
+    rows = []
+    for l in open(os.path.join(golden_dir, name)):
+        if l.strip() and not l.startswith("#"):
+            f = l.split()
+            rows.append((f[0], [float(q) for q in f[1:]]))
+    return rows
+
+
+def test_timestep_eq38_eq39_hand_evaluated(golden_dir):
+    """Eq. 38-39 against hand-evaluated numbers (tests/golden/timestep.txt): the CFL
+    branch, the acceleration branch with epsilon = h_i (reading Q22), both orders of the minimum, and
+    |a| = 0."""
+    p = W.Params(eta_C=0.3, eta_a=0.25, alpha=1.0, beta=2.0)
+    rows = _golden_rows(golden_dir, "timestep.txt")
+    assert [r[0] for r in rows] == ["A", "B", "C", "D", "E"]
+    v = np.array([r[1] for r in rows])
+    h, c, mu, a, want = v[:, 0], v[:, 1], v[:, 2], v[:, 3:6].T.copy(), v[:, 6]
+    got = O.timestep(p, h, c, mu, a)
+    assert np.allclose(got, want, rtol=1e-14, atol=0)
+    # eta_a <= 0 disables Eq. 38: rows B and E fall back to their CFL values 1.35/0.8 and 12/11
+    p0 = W.Params(eta_C=0.3, eta_a=0.0, alpha=1.0, beta=2.0)
+    got0 = O.timestep(p0, h, c, mu, a)
+    assert got0[1] == pytest.approx(1.6875, rel=1e-14) and got0[4] == pytest.approx(12.0 / 11.0, rel=1e-14)
+    assert np.array_equal(got0[[0, 2, 3]], got[[0, 2, 3]])
+
+
+def test_derivatives_apply_eq38_to_the_full_acceleration():
+    """derivatives() must hand the acceleration INCLUDING a_ext to Eq. 38: a block at rest in a strong
+    uniform external field has dt_i = eta_a sqrt(h/|g|) wherever the internal forces are negligible
+    (PAPER.md:227, 234), and the same call with eta_a = 0 gives the CFL value instead."""
+    wl = small_block(5)
+    A = wl.arrays
+    for k in ("vx", "vy", "vz", "Sxx", "Syy", "Sxy", "Sxz", "Syz"):
+        A[k][:] = 0
+    A["gy"][:] = -4.0e12                                       # |g| >> any internal acceleration here
+    wl.params.eta_a = 0.25
+    S = np.zeros((5, wl.n)); g = np.stack([A["gx"], A["gy"], A["gz"]]).astype(np.float64)
+    d = O.derivatives(wl.params, A["x"], A["y"], A["z"], A["m"], A["h"], A["vx"], A["vy"], A["vz"], A["u"], S,
+                      wl.mat, g)
+    h = A["h"].astype(np.float64)
+    an = np.sqrt((d["a"] ** 2).sum(axis=0))
+    assert np.allclose(an, 4.0e12, rtol=1e-2)
+    assert np.allclose(d["dt_i"], 0.25 * np.sqrt(h / an), rtol=1e-14)
+    assert np.allclose(d["dt_i"], 0.25 * np.sqrt(0.013 / 4.0e12), rtol=1e-2)      # h = 1.3 cm
+    wl.params.eta_a = 0.0
+    d0 = O.derivatives(wl.params, A["x"], A["y"], A["z"], A["m"], A["h"], A["vx"], A["vy"], A["vz"], A["u"], S,
+                       wl.mat, g)
+    assert np.all(d0["dt_i"] > 50.0 * d["dt_i"])
+    assert np.allclose(d0["dt_i"], 0.3 * h / (1.6 * 3000.0 + 1.2 * d0["mumax"]), rtol=1e-14)
+
+
+def test_forces_see_the_rescaled_predicted_stress():
+    """"The predicted deviatoric stress tensor is then rescaled according to Equation (31),
+    after which the updated time derivatives are computed from the predicted values."  Far above yield the
+    projected tensor Y S/sqrt(J2) does not depend on the magnitude of the input S (Y depends on P and T
+    only), so a, du/dt and dS/dt must be the same for S and 1000 S; had the force or the stress-rate pass
+    been fed the un-rescaled tensor they would differ by orders of magnitude."""
+    wl = small_block(5)
+    A = {k: v.astype(np.float64) for k, v in wl.arrays.items()}
+    A["u"][:] = 1000.0 * 400.0                                  # T = 400 K: Y > 0 everywhere
+    S1 = 3.0e4 * np.stack([A["Sxx"], A["Syy"], A["Sxy"], A["Sxz"], A["Syz"]])     # |S| ~ 1e11 >> Y <= Ym = 3.5e9
+    out = []
+    for lam in (1.0, 1000.0):
+        out.append(O.derivatives(wl.params, A["x"], A["y"], A["z"], A["m"], A["h"], A["vx"], A["vy"], A["vz"], A["u"],
+                                 lam * S1, wl.mat, None))
+    d1, d2 = out
+    assert np.all(d1["f_pred"] < 0.9) and np.all(d2["f_pred"] < 0.9e-3)         # every particle is far above yield
+    assert np.allclose(np.sqrt(O.J2(d1["S_pred"])), d1["Y"], rtol=1e-12)
+    for k in ("a", "dudt", "dS", "S_pred"):
+        assert np.allclose(d1[k], d2[k], rtol=1e-9, atol=1e-9 * np.abs(d1[k]).max()), k
+    # and S does enter the forces: with the stress switched off the acceleration is different
+    wl.params.flags &= ~O.FLAG_STRENGTH
+    d3 = O.derivatives(wl.params, A["x"], A["y"], A["z"], A["m"], A["h"], A["vx"], A["vy"], A["vz"], A["u"],
+                       S1, wl.mat, None)
+    wl.params.flags |= O.FLAG_STRENGTH
+    assert np.abs(d3["a"] - d1["a"]).max() > 1e-3 * np.abs(d1["a"]).max()
+
+
+def test_stepper_fp32_storage_mode_rounds_state_once_per_store():
+    """Stepper(store_fp32=True): every stored quantity is an fp32 value, the arithmetic is unchanged --
+    the trajectories of the two modes agree to fp32 rounding, and x of the fp32 mode is exactly what
+    rounding x + dt v_half of its own (stored) operands gives."""
     wl = small_block(6)
-    d = O.single_pass(wl)
-    p = wl.params
-    h = wl.arrays["h"].astype(np.float64)
-    # mu_max = 0 particle: dt = eta_C h / ((1 + 0.6 alpha) c)
-    i = int(np.argmin(d["mumax"]))
-    lo = p.eta_C * h[i] / ((1 + 0.6 * p.alpha) * 3000.0 + 0.6 * p.beta * d["mumax"][i])
-    assert d["dt_i"][i] == pytest.approx(lo, rel=1e-14)
-    assert np.all(d["dt_i"] <= p.eta_C * h / (1.6 * 3000.0) * (1 + 1e-14))
+    a = O.Stepper(wl, mode="brute"); b = O.Stepper(wl, mode="brute", store_fp32=True)
+    dt = 3e-7
+    for _ in range(2):
+        a.step(dt); b.step(dt)
+    for q in ("x", "v", "u", "S", "e_acc"):
+        vb = getattr(b, q)
+        assert np.array_equal(vb, vb.astype(np.float32).astype(np.float64)), q
+        va = getattr(a, q)
+        # S feels fp32 positions through rho -> P -> Y (an ulp of x moves rho by ~3e-7 here, P = c0^2 (rho - rho0)
+        # by ~5e3 Pa and the yield-limited S with it): the reason the multi-step GPU comparison uses this mode
+        assert np.abs(va - vb).max() <= (1e-4 if q == "S" else 1e-6) * np.abs(va).max(), q
+    assert not np.array_equal(a.x, b.x)
+    for q in ("a", "dudt", "dS"):
+        assert np.array_equal(b.d[q], b.d[q].astype(np.float32).astype(np.float64)), q
 
 
 def test_grid_mode_gives_the_same_step_as_brute():

@@ -115,7 +115,7 @@ def test_stress_rate_component_form_equals_eq13():
     rng = np.random.default_rng(1)
     n = 50
     G = rng.standard_normal((9, n)); S = rng.standard_normal((5, n)); Gam = 1.0 + rng.random(n)
-    for flags in (0, O.FLAG_JAUMANN_COROTATIONAL):
+    for flags in (0, O.FLAG_JAUMANN_AS_PRINTED):
         dS, dS3, eps2 = O.stress_rate(G, S, Gam, flags)
         comp = O.stress_rate_components(G, S, Gam, flags)
         assert np.allclose(dS, comp, rtol=1e-13, atol=1e-13)
@@ -154,8 +154,9 @@ def test_hooke_pure_shear_and_special_cases():
 def test_rotation_term_sign_documented():
     """Reading Q1.  Under a rigid rotation Q(t) about z with angular velocity w, a stress carried
     with the body is S(t) = Q S Q^T.  Its time derivative is W S - S W (W = spin = R of Eq. 15).
-    Eq. 13 AS PRINTED gives S.R + (S.R)^T = S R - R S, the opposite sign; the flag
-    JAUMANN_COROTATIONAL gives the co-rotating one.  Both are tested so a silent change fails."""
+    The default is that objective rate (the paper: "we adopt the Jaumann rate to obtain an objective
+    stress rate"); Eq. 13 with the index order AS PRINTED gives S.R + (S.R)^T = S R - R S,
+    the opposite sign, kept behind JAUMANN_AS_PRINTED.  Both are tested so a silent change fails."""
     w = 0.3
     S5 = np.array([1.0, -0.4, 0.25, 0.6, -0.8])
     S3 = O._S3(S5[:, None])[0]
@@ -166,8 +167,8 @@ def test_rotation_term_sign_documented():
         return np.array([[c, -s, 0.0], [s, c, 0.0], [0.0, 0.0, 1.0]])
     fd = (Q(dt) @ S3 @ Q(dt).T - Q(-dt) @ S3 @ Q(-dt).T) / (2 * dt)
     G = Wm.reshape(9, 1)
-    _, printed, _ = O.stress_rate(G, S5[:, None], np.zeros(1), 0)
-    _, corot, _ = O.stress_rate(G, S5[:, None], np.zeros(1), O.FLAG_JAUMANN_COROTATIONAL)
+    _, corot, _ = O.stress_rate(G, S5[:, None], np.zeros(1), 0)
+    _, printed, _ = O.stress_rate(G, S5[:, None], np.zeros(1), O.FLAG_JAUMANN_AS_PRINTED)
     assert np.allclose(corot[0], fd, atol=1e-8)
     assert np.allclose(printed[0], -fd, atol=1e-8)
     # the printed xx component, Eq. 25: S^{xy}(G^{yx}-G^{xy}) + S^{xz}(G^{zx}-G^{xz})
