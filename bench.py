@@ -205,10 +205,6 @@ def run_ours(args):
     wl = make_workload(args.workload)
     if args.no_graph:
         wl.params.flags |= 64          # SPH_NO_GRAPH
-    if args.sort_lists:
-        wl.params.flags |= 256         # SPH_SORT_LISTS
-    if args.fused_density:
-        wl.params.flags |= 128         # SPH_FUSED_DENSITY
     n = wl.n
     strength = bool(wl.params.flags & B.STRENGTH)
     s = B.Sph(wl.params, n, device=dev)
@@ -343,8 +339,7 @@ def run_ours(args):
                    "mean_neighbours": pairs_s / args.steps / max(n, 1),
                    "l2": "flushed between steps (256 MiB fill outside the timed events)",
                    "working_set_bytes": working_set, "parallelism": "replicas x%d" % world,
-                   "cuda_graph": not args.no_graph,
-                   "density_pass": "inside the list build (pass_ms.build)" if args.fused_density else "own kernel"},
+                   "cuda_graph": not args.no_graph},
         "particle_steps_per_s": world * n * args.steps / (total_ms_max * 1e-3),
         "pass_ms": {k: v / args.steps for k, v in pass_ms.items()},
         "gpu_launches": launches,
@@ -369,8 +364,6 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-hydro-only", action="store_true")
-    ap.add_argument("--sort-lists", action="store_true", help="order the lists by bank class (A/B)")
-    ap.add_argument("--fused-density", action="store_true", help="density pass inside the list build (A/B)")
     ap.add_argument("--no-graph", action="store_true", help="launch the step kernel by kernel (A/B of the CUDA graph)")
     args = ap.parse_args()
     if args.impl == "reference":

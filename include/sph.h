@@ -12,7 +12,8 @@
  *    the CUDA stream given to sph_init and never synchronises the device.
  *  - The caller owns every particle array and the workspace; the library owns only the small
  *    host-side context.  The workspace must stay alive and untouched until sph_destroy.
- *  - Internally particles are kept sorted by Morton key ("resident" state).  Outputs of
+ *  - Internally particles are kept sorted along a space-filling curve (Hilbert by default, Morton with
+ *    SPH_MORTON_ORDER): the "resident" state.  Outputs of
  *    sph_get_field / sph_get_neighbors / sph_download_state are in CALLER order.
  *  - Particle arrays are fp32 structure-of-arrays, length n (BASELINE.json north_star).
  */
@@ -39,12 +40,6 @@ extern "C" {
                                          measurement; they also serve tiles over a list capacity)           */
 #define SPH_NO_GRAPH             64u  /* launch the resident step kernel by kernel instead of replaying its
                                          CUDA graph (A/B measurement)                                      */
-#define SPH_FUSED_DENSITY       128u  /* sph_step: run the density pass inside the list build instead of as its
-                                         own kernel (A/B measurement: same results bit for bit, 4 % slower
-                                         on configs[2]; off by default)                                    */
-#define SPH_SORT_LISTS          256u  /* after the list build, order every particle's list by the shared-memory
-                                         bank class of its entries (k_list_sort): the pair kernel's gathers
-                                         stop conflicting (A/B measurement)                                */
 #define SPH_MORTON_ORDER         32u  /* sort by Morton (Z-order) keys instead of Hilbert keys (A/B
                                          measurement; results do not depend on the order)                  */
 
@@ -110,6 +105,11 @@ enum { SPH_C_PAIRS_GATHER = 0,   /* sum_i |gather set(i)|   (true pairs of the d
        SPH_C_LIST_OVERFLOW,      /* tiles (256 particles) that exceeded a list capacity and were served
                                     by the tree-walk kernels instead: results are complete, the step is
                                     slower; raise sph_params.list_budget if this is large           */
+       SPH_C_BAD_MATERIAL,       /* particles ingested with a material index outside 0..n_materials-1 (they were
+                                    given material n_materials-1; see sph_state.mat)                        */
+       SPH_C_OMEGA_SMALL,        /* particles with |Omega| < 0.1 in the last density pass (Eq. 3): too few
+                                    neighbours for the grad-h terms; sph_adapt_h is the method's remedy     */
+       SPH_C_NONFINITE,          /* particles whose a, du/dt or dS/dt was not finite in the last CLOSE      */
        SPH_C_COUNT };
 
 typedef struct sph_ctx sph_ctx;   /* opaque, library-owned (host memory) */
@@ -158,7 +158,8 @@ typedef struct sph_state {
     float *x, *y, *z, *m, *h, *vx, *vy, *vz, *u;
     float *Sxx, *Syy, *Sxy, *Sxz, *Syz;
     const float *gx, *gy, *gz;
-    const int *mat;              /* material index per particle, 0..n_materials-1                 */
+    const int *mat;              /* material index per particle, 0..n_materials-1; an index outside that
+                                    range is replaced by n_materials-1 and counted (SPH_C_BAD_MATERIAL)  */
     const unsigned char *fixed;  /* 1: particle skips kick and drift (reading Q16)  */
 } sph_state;
 
@@ -205,6 +206,11 @@ int sph_gradients(sph_ctx *ctx);
 /* S5: a_i (Eq. 4, 7, 18 + a_ext), du_i/dt (Eq. 8, 19), mu_max (Eq. 39).  Needs PREDICT. */
 int sph_forces(sph_ctx *ctx);
 
+/* S4 + S5 in ONE pass over the neighbour lists (both are sums over the same symmetric set):
+ * the kernel sph_step itself runs.  Same outputs as sph_gradients followed by sph_forces.  Without
+ * SPH_STRENGTH it is sph_forces.  Needs PREDICT. */
+int sph_gradients_forces(sph_ctx *ctx);
+
 /* One full step (Eq. 40-42): opening kick, drift,
  * prediction, S1..S6 (gradient and force passes fused), next dt.  state != NULL (DEVICE arrays):
  * ingested first if nothing is resident, and written back (x, v, u, S) in caller order at the
@@ -225,8 +231,9 @@ int sph_get_field(sph_ctx *ctx, int field_id, float *dst);
 /* Test hook: neighbour sets as the pair passes see them, as ORIGINAL particle ids.
  * counts: DEVICE int[n].  If list != NULL, offsets (DEVICE long long[n+1], exclusive prefix of
  * counts, supplied by the caller) says where each particle's ids go; order within a row is
- * unspecified.  list_capacity: entries available in list (ECAPACITY if offsets[n] exceeds it is
- * NOT checked on the device; the caller sizes list from counts). */
+ * unspecified; a particle with offsets[i] < 0 is skipped (its ids are not written: sampled comparisons
+ * at sizes where the whole list would not fit).  The capacity of list is NOT checked on the device; the
+ * caller sizes it from counts. */
 int sph_get_neighbors(sph_ctx *ctx, int which, int *counts, const long long *offsets, int *list);
 
 /* NEXT-3: use `table` (HOST struct, DEVICE arrays) for P, T, c_s (and T_melt) of `material` in
@@ -253,6 +260,12 @@ int sph_get_counters(sph_ctx *ctx, long long *counters, int n); /* SPH_C_* slots
  * Returns the number of tiles (nothing is copied if capacity is smaller), or a negative SPH_E* code.
  * Synchronises the stream. */
 int sph_get_tile_stats(sph_ctx *ctx, int *ncand, unsigned *cycles, unsigned char *flag, int capacity);
+
+/* Measurement aid ("measure an FMA-chain microbenchmark"): the FP32 CUDA-core rate this
+ * device sustains on a kernel of independent FFMA chains (2 flop each, no memory traffic), in TFLOP/s, best of
+ * `repeats` launches timed with CUDA events on `cuda_stream`.  tflops: HOST.  Synchronises the stream.
+ * It is the denominator of the ALU-bound roofline entries of bench.py. */
+int sph_fp32_peak(void *cuda_stream, int repeats, double *tflops);
 
 /* Number of this library's kernel launches since sph_init (HOST; no synchronisation). */
 long long sph_launch_count(const sph_ctx *ctx);

@@ -25,14 +25,14 @@ F = dict(RHO=0, OMEGA=1, P=2, CS=3, T=4, GAMMA=5, Y=6, MUMAX=7, DUDT=8, DT=9, EA
          CFLAG=13, NGATHER=14, NSYMMETRIC=15, H=16, A=32, V=36, X=40, SPRED=48, S=56, DSDT=64, F=80, CINV=96, G=112)
 T_SLOTS = ("build", "density", "predict", "gradient", "force", "close", "kickdrift", "step")
 C_SLOTS = ("pairs_gather", "pairs_symmetric", "tests_density", "tests_force", "cfallback", "tests_cull",
-           "candidates", "list_overflow")
+           "candidates", "list_overflow", "bad_material", "omega_small", "nonfinite")
 
 FLOAT_FIELDS = ("x", "y", "z", "m", "h", "vx", "vy", "vz", "u", "Sxx", "Syy", "Sxy", "Sxz", "Syz")
 OPT_FIELDS = ("gx", "gy", "gz")
 
 # every symbol include/sph.h declares (tests check the library exports all of them)
 SYMBOLS = ("sph_workspace_bytes", "sph_init", "sph_build_neighbors", "sph_density", "sph_strength_update",
-           "sph_gradients", "sph_forces", "sph_adapt_h", "sph_set_eos_table", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
+           "sph_gradients", "sph_forces", "sph_gradients_forces", "sph_fp32_peak", "sph_adapt_h", "sph_set_eos_table", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
            "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_get_diagnostics", "sph_launch_count",
            "sph_last_cuda_error", "sph_strerror", "sph_destroy")
 
@@ -105,6 +105,10 @@ def load():
     lib.sph_strength_update.argtypes = [vp, i, fl]
     lib.sph_gradients.argtypes = [vp]
     lib.sph_forces.argtypes = [vp]
+    lib.sph_gradients_forces.argtypes = [vp]
+    lib.sph_gradients_forces.restype = i
+    lib.sph_fp32_peak.argtypes = [vp, i, C.POINTER(C.c_double)]
+    lib.sph_fp32_peak.restype = i
     lib.sph_step.argtypes = [vp, C.POINTER(sph_state), ll, fl, vp]
     lib.sph_step_host.argtypes = [vp, C.POINTER(sph_state), ll, fl, vp]
     lib.sph_download_state.argtypes = [vp, C.POINTER(sph_state)]
@@ -236,6 +240,15 @@ class Sph:
     def forces(self):
         self._check(self.lib.sph_forces(self.ctx), "sph_forces")
 
+    def gradients_forces(self):
+        self._check(self.lib.sph_gradients_forces(self.ctx), "sph_gradients_forces")
+
+    def fp32_peak(self, repeats: int = 5) -> float:
+        """sph_fp32_peak: TFLOP/s of independent FFMA chains on this device (measurement aid)."""
+        out = C.c_double(0.0)
+        self._check(self.lib.sph_fp32_peak(self.stream.cuda_stream, int(repeats), C.byref(out)), "sph_fp32_peak")
+        return float(out.value)
+
     def step(self, tensors: Optional[Dict[str, object]] = None, n: int = 0, dt: float = 0.0, dt_used=None):
         st = C.byref(self.state_struct(tensors)) if tensors is not None else None
         if tensors is not None:
@@ -270,12 +283,26 @@ class Sph:
     def get_fields(self, name: str, ncomp: int):
         return self.torch.stack([self.get_field(name, c) for c in range(ncomp)], dim=0)
 
-    def get_neighbors(self, which: int):
-        """(counts[n], offsets[n+1], list) on the device; list holds ORIGINAL ids, rows unordered."""
+    def get_neighbors(self, which: int, select=None):
+        """(counts[n], offsets[n+1], list) on the device; list holds ORIGINAL ids, rows unordered.
+        select (caller-order indices): only these particles' ids are written (offsets = -1 elsewhere)."""
         torch = self.torch
         counts = torch.zeros(max(self.n, 1), dtype=torch.int32, device=self.device)
         self._check(self.lib.sph_get_neighbors(self.ctx, which, counts.data_ptr(), None, None), "sph_get_neighbors")
         counts = counts[: self.n]
+        if select is not None:
+            sel = torch.as_tensor(select, dtype=torch.long, device=self.device)
+            csel = counts[sel].to(torch.int64)
+            offsets = torch.full((self.n + 1,), -1, dtype=torch.int64, device=self.device)
+            starts = torch.cumsum(csel, dim=0) - csel
+            offsets[sel] = starts
+            total = int(csel.sum().item())
+            lst = torch.zeros(max(total, 1), dtype=torch.int32, device=self.device)
+            self._check(self.lib.sph_get_neighbors(self.ctx, which, counts.data_ptr(), offsets.data_ptr(), lst.data_ptr()),
+                        "sph_get_neighbors")
+            so = torch.zeros(sel.numel() + 1, dtype=torch.int64, device=self.device)
+            so[1:] = torch.cumsum(csel, dim=0)
+            return counts[sel], so, lst[:total]
         offsets = torch.zeros(self.n + 1, dtype=torch.int64, device=self.device)
         if self.n:
             offsets[1:] = torch.cumsum(counts.to(torch.int64), dim=0)
@@ -340,10 +367,14 @@ class Sph:
 
     # ---- convenience: BASELINE.json configs[0] single pass -------
     def single_pass(self, tensors, n: int, dt: float, fused: bool = False):
+        """fused: S4 + S5 in one pass (sph_gradients_forces, the kernel sph_step runs) instead of two."""
         self.build_neighbors(tensors, n)
         self.density()
         self.strength_update(PREDICT)
-        if self.cparams.flags & STRENGTH:
-            self.gradients()
-        self.forces()
+        if fused:
+            self.gradients_forces()
+        else:
+            if self.cparams.flags & STRENGTH:
+                self.gradients()
+            self.forces()
         self.strength_update(CLOSE, dt)

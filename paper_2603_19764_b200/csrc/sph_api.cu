@@ -248,20 +248,8 @@ extern "C" int sph_build_neighbors(sph_ctx *c, const sph_state *state, long long
     }
     c->have_density = c->have_predict = c->have_grad = c->have_force = false;
     if (c->use_lists) {
-        // inside sph_step the density pass of every tile runs in the list kernel itself (k_cull<true>)
-        const bool fuse = c->fuse_density_now;
-        rc = sph_launch_cull(c, fuse);
+        rc = sph_launch_cull(c);
         if (rc) return rc;
-        if (c->p.flags & SPH_SORT_LISTS) {
-            rc = sph_launch_list_sort(c);
-            if (rc) return rc;
-        }
-        if (fuse) {
-            PassTimer td(c, SPH_T_DENSITY);           // what is left of S2: the tiles over a list capacity
-            rc = sph_launch_density(c, true);
-            if (rc) return rc;
-            c->have_density = true;
-        }
     }
     return SPH_OK;
 }
@@ -294,7 +282,7 @@ extern "C" int sph_adapt_h(sph_ctx *c, float n_target, int iterations, float *ma
         rc = sph_launch_tree(c);
         if (rc) return rc;
         if (c->use_lists) {
-            rc = sph_launch_cull(c, false);
+            rc = sph_launch_cull(c);
             if (rc) return rc;
         }
         c->have_density = c->have_predict = c->have_grad = c->have_force = false;
@@ -323,6 +311,19 @@ extern "C" int sph_forces(sph_ctx *c)
     int rc = c->use_lists ? sph_launch_pair_l(c, false, true) : sph_launch_pair(c, false, true, false);
     if (rc) return rc;
     c->have_force = true;
+    return SPH_OK;
+}
+
+extern "C" int sph_gradients_forces(sph_ctx *c)
+{
+    if (!c) return SPH_EINVAL;
+    if (!c->have_predict) return SPH_EORDER;
+    const bool strength = (c->p.flags & SPH_STRENGTH) != 0;
+    PassTimer t(c, SPH_T_FORCE);
+    int rc = c->use_lists ? sph_launch_pair_l(c, strength, true) : sph_launch_pair(c, strength, true, false);
+    if (rc) return rc;
+    c->have_force = true;
+    c->have_grad = strength;
     return SPH_OK;
 }
 
@@ -363,15 +364,7 @@ static int derivative_passes(sph_ctx *c)
     if (rc) return rc;
     rc = sph_strength_update(c, SPH_PREDICT, 0.f);
     if (rc) return rc;
-    const bool strength = (c->p.flags & SPH_STRENGTH) != 0;
-    {
-        PassTimer t(c, SPH_T_FORCE);
-        rc = c->use_lists ? sph_launch_pair_l(c, strength, true) : sph_launch_pair(c, strength, true, false);
-        if (rc) return rc;
-        c->have_force = true;
-        c->have_grad = strength;
-    }
-    return SPH_OK;
+    return sph_gradients_forces(c);
 }
 
 static int step_body(sph_ctx *c, sph_state *state, long long n, float dt, float *dt_used)
@@ -396,9 +389,7 @@ static int step_body(sph_ctx *c, sph_state *state, long long n, float dt, float 
         rc = sph_launch_kick_drift(c, dt);
         if (rc) return rc;
     }
-    c->fuse_density_now = c->use_lists && (c->p.flags & SPH_FUSED_DENSITY) != 0;
     rc = sph_build_neighbors(c, nullptr, 0);
-    c->fuse_density_now = false;
     if (rc) return rc;
     rc = derivative_passes(c);
     if (rc) return rc;

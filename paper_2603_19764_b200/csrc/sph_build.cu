@@ -132,7 +132,7 @@ __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ x, const
 // ------------------------------------------------------------------------------------------
 // ingest: caller arrays (caller order) -> resident sorted arrays
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_ingest(sph_state st, Dev d, const unsigned *__restrict__ perm)
+__global__ void __launch_bounds__(256) k_ingest(sph_state st, Dev d, const unsigned *__restrict__ perm, int n_materials)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= d.n) return;
@@ -158,7 +158,13 @@ __global__ void __launch_bounds__(256) k_ingest(sph_state st, Dev d, const unsig
     d.r.s[PP_G + 1][i] = st.gy ? st.gy[p] : 0.f;
     d.r.s[PP_G + 2][i] = st.gz ? st.gz[p] : 0.f;
     ((unsigned *)d.r.s[PP_ORIG])[i] = p;
-    unsigned mf = (st.mat ? (unsigned)st.mat[p] & 0xffu : 0u) | (st.fixed ? ((unsigned)(st.fixed[p] != 0) << 8) : 0u);
+    // a material index outside 0..n_materials-1 would index past the parameter tables in k_predict / k_close
+    int mi = st.mat ? st.mat[p] : 0;
+    if (mi < 0 || mi >= n_materials) {
+        mi = n_materials - 1;
+        atomicAdd(&d.counters[SPH_C_BAD_MATERIAL], 1ull);
+    }
+    unsigned mf = (unsigned)mi | (st.fixed ? ((unsigned)(st.fixed[p] != 0) << 8) : 0u);
     ((unsigned *)d.r.s[PP_MATFIX])[i] = mf;
     d.a[0][i] = 0.f; d.a[1][i] = 0.f; d.a[2][i] = 0.f;
     d.dudt[i] = 0.f;
@@ -310,7 +316,8 @@ int sph_launch_ingest(sph_ctx *c, const sph_state *st, long long n)
     c->launches += 3;
     int rc = sort_keys(c, key_bits(n));
     if (rc) return rc;
-    k_ingest<<<nb, 256, 0, c->stream>>>(*st, d, d.perm_alt);
+    SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_BAD_MATERIAL], 0, sizeof(unsigned long long), c->stream));
+    k_ingest<<<nb, 256, 0, c->stream>>>(*st, d, d.perm_alt, c->p.n_materials);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return sph_launch_tree(c);

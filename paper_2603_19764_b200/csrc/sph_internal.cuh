@@ -132,7 +132,6 @@ struct sph_ctx {
     // CUDA graphs of the resident step (sph_step with state == NULL, dt <= 0): one per half of the
     // ping-pong (the kernels take the array pointers by value); see sph_step
     bool use_graph, capturing;
-    bool fuse_density_now;           // sph_step: the next list build also does the density pass
     int parity;                      // which half of the ping-pong is current
     cudaGraphExec_t gexec[2];
     long long glaunches[2];          // launches one replay stands for
@@ -174,8 +173,7 @@ int sph_launch_diagnostics(sph_ctx *c, double *out);
 int sph_launch_h_update(sph_ctx *c, float n_target);
 int sph_launch_neighbors(sph_ctx *c, int which, int *counts, const long long *offsets, int *list, bool flagged_only);
 int sph_launch_download(sph_ctx *c, sph_state *st);
-int sph_launch_cull(sph_ctx *c, bool with_density);
-int sph_launch_list_sort(sph_ctx *c);
+int sph_launch_cull(sph_ctx *c);
 int sph_launch_density_l(sph_ctx *c);
 int sph_launch_pair_l(sph_ctx *c, bool grad, bool force);
 int sph_launch_neighbors_l(sph_ctx *c, int which, int *counts, const long long *offsets, int *list);

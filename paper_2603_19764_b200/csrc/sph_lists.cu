@@ -130,13 +130,6 @@ __device__ __forceinline__ int scan_popc(const unsigned *mask, unsigned short *o
     return __shfl_sync(FULL, incl, 31);
 }
 
-// DENS (SPH_FUSED_DENSITY, off by default): the density pass (S2) of the tile runs inside this kernel, round
-// by round, right after the round's lists are written.  The idea was that its fp64 / conversion work fills
-// issue slots the integer-heavy list build leaves idle, with the candidates' positions already in shared
-// memory; measured, it is 4 % SLOWER per step on configs[2] (two more barriers per round, 80 registers, the
-// lists read back) -- kept as the A/B.  Same arithmetic in the same order as k_density_l: bitwise the same
-// rho, Omega and counts.
-template <bool DENS>
 __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -364,10 +357,6 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     int nhit = 0;                         // true neighbours
     unsigned tests = 0;
     int Gstart = 0;                       // first row-group of the current round
-    // density state (DENS): self term q = 0, t = 1
-    double dsum = valid ? (double)pi.w : 0.0;
-    float dsh = 3.f * pi.w;
-    int dng = 1;
     // write the complete row-groups of the buffer out, keep the 0..3 entries left over
 #define LIST_FLUSH()                                                                        \
     do {                                                                                    \
@@ -542,75 +531,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             if (G > d.rows_cap) sm.overflow = 8;      // list rows exhausted: the tile falls back
             if (lane == 0) rp[round + 1] = (unsigned short)min(Gmax, d.rows_cap);
         }
-        if (DENS) {
-            // ---- C: density of this round's list entries.  The masses of the round's candidates go where
-            //         the rings were; positions are still in pos[].
-            __syncthreads();
-            float *const sm_m = reinterpret_cast<float *>(sm.gl);
-            for (int s = threadIdx.x; s < nr; s += SPH_TILE) sm_m[s] = d.r.pm[cand[r0 + s]].w;
-            __syncthreads();
-            if (warp < nch && valid) {
-                const float invH = 1.f / Hi;
-                const double invHd = 1.0 / ((double)kappa * (double)d.r.vh[i].w);
-                const double pxd = (double)pi.x, pyd = (double)pi.y, pzd = (double)pi.z;
-                const unsigned char *const posb = reinterpret_cast<const unsigned char *>(sm.pos);
-                const int gend = min(G, d.rows_cap);
-                for (int gq = Gstart; gq < gend; ++gq) {
-                    const uint2 w = lp[(size_t)gq * 32];
-#pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const unsigned x_ = (e & 2) ? w.y : w.x;
-                        const unsigned off = (e & 1) ? (x_ >> 16) : (x_ & 0xffffu);
-                        if (off == 0xffffu) continue;
-                        const float4 q = *reinterpret_cast<const float4 *>(posb + off);
-                        const float mj = sm_m[off >> 4];
-                        float dx = __fsub_rn(pi.x, q.x), dy = __fsub_rn(pi.y, q.y), dz = __fsub_rn(pi.z, q.z);
-                        float r2 = sph_r2(dx, dy, dz);
-                        if (r2 < H2i) {
-                            float rinv = sph_rsqrt(fmaxf(r2, 1.0e-37f));
-                            float r = r2 * rinv;
-                            float qq = r * invH;
-                            float t = fmaxf(0.f, 1.f - qq);
-                            float t3 = t * t * t;
-                            dsh = fmaf(mj * t3, fmaf(qq, fmaf(-32.f, qq, 9.f), 3.f), dsh);
-                            double ex = pxd - (double)q.x, ey = pyd - (double)q.y, ez = pzd - (double)q.z;
-                            double r2d = fma(ex, ex, fma(ey, ey, ez * ez));
-                            const double yd = (double)rinv, td0 = r2d * yd;
-                            double rd = fma(0.5 * td0, fma(-td0, yd, 1.0), td0);
-                            double qd = rd * invHd;
-                            double td = 1.0 - qd;
-                            double t2 = td * td;
-                            dsum = fma((double)mj * t2 * t2, fma(4.0, qd, 1.0), dsum);
-                            ++dng;
-                        }
-                    }
-                }
-            }
-        }
         __syncthreads();
-    }
-    if (DENS && valid && !sm.overflow) {
-        const float invH = 1.f / Hi;
-        const double invHd = 1.0 / ((double)kappa * (double)d.r.vh[i].w);
-        float kw = SPH_WC2_SIGMA * invH * invH * invH;
-        double rhod = 3.3422538049298023 * invHd * invHd * invHd * dsum;
-        float rho = (float)rhod;
-        d.rho64[i] = rhod;
-        d.rho[i] = rho;
-        d.omega[i] = 1.f - kw * dsh / (3.f * rho);
-        d.ngather[i] = dng;
-    }
-    if (DENS && !sm.overflow) {
-        unsigned long long hits = valid ? (unsigned long long)dng : 0ull, dt_ = valid ? (unsigned long long)(nhit + 1) : 0ull;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            hits += __shfl_xor_sync(FULL, hits, o);
-            dt_ += __shfl_xor_sync(FULL, dt_, o);
-        }
-        if (lane == 0) {
-            atomicAdd(&d.counters[SPH_C_PAIRS_GATHER], hits);
-            atomicAdd(&d.counters[SPH_C_TESTS_DENSITY], dt_);
-        }
     }
     if (valid) d.nsym[i] = nhit;
     if (warp < nch) {
@@ -629,112 +550,32 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     }
 }
 
-// Which tiles go first in this build: those that cost more than 1.5x the average in the previous one.
-__global__ void __launch_bounds__(256) k_tile_plan(Dev d, int ntile)
+// Head of a list build, ONE block: which tiles go first (those that cost more than 1.5x the average in the previous
+// build), and the resets the build needs (list-build counters, candidate pool cursor, cycle sum).
+__global__ void __launch_bounds__(1024) k_tile_plan(Dev d, int ntile)
 {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= ntile) return;
+    __shared__ unsigned s_n;
+    if (threadIdx.x == 0) s_n = 0u;
+    __syncthreads();
     const unsigned long long sum = *d.cull_cycles;
-    bool heavy = 2ull * (unsigned long long)d.tile_cycles[t] * (unsigned long long)ntile > 3ull * sum;
-    if (heavy) {
-        const unsigned k = atomicAdd(d.nheavy, 1u);
-        if (k < (unsigned)d.heavy_cap) d.heavy_list[k] = (unsigned)t;
-        else heavy = false;                // list full: the tile stays in curve order
+    for (int t = threadIdx.x; t < ntile; t += blockDim.x) {
+        bool heavy = 2ull * (unsigned long long)d.tile_cycles[t] * (unsigned long long)ntile > 3ull * sum;
+        if (heavy) {
+            const unsigned k = atomicAdd(&s_n, 1u);
+            if (k < (unsigned)d.heavy_cap) d.heavy_list[k] = (unsigned)t;
+            else heavy = false;                // list full: the tile stays in curve order
+        }
+        d.heavy_mark[t] = heavy ? 1 : 0;
     }
-    d.heavy_mark[t] = heavy ? 1 : 0;
-}
-
-// nheavy may have counted past the capacity
-__global__ void k_tile_plan_clamp(Dev d)
-{
-    if (*d.nheavy > (unsigned)d.heavy_cap) *d.nheavy = (unsigned)d.heavy_cap;
-}
-
-// ------------------------------------------------------------------------------------------
-// k_list_sort (SPH_SORT_LISTS): reorder every lane's list entries of a round so that lane l reads bank class
-// (l + n) mod 8 at step n (class = slot mod 8 = which 16-byte bank group the slot's float4 sits in).  The eight
-// lanes of a quarter-warp phase then hit eight different bank groups in the pair kernel's gathers instead of
-// random ones (2.47 wavefronts per phase).  Per lane: count the classes, bucket the entries by class in shared
-// memory (counting sort, cursors packed 8 x 8 bit), emit them round-robin over the classes starting at the
-// lane's own; when the wanted class has run out, the next one in cyclic order that has entries.  One warp per
-// chunk, all lanes in lockstep over the positions of the round; rounds with a lane over SORT_CAP entries stay as
-// they are.  The order of a lane's entries has no meaning (a set), so results change only by summation order.
-// ------------------------------------------------------------------------------------------
-#define SORT_CAP 160
-#define SORT_STRIDE (SORT_CAP * 2 + 4)       // bytes per lane: 81 words
-#define SORT_WARPS 4
-__global__ void __launch_bounds__(SORT_WARPS * 32) k_list_sort(Dev d)
-{
-    __shared__ __align__(4) unsigned char s_buf[SORT_WARPS * 32 * SORT_STRIDE];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int chunk = blockIdx.x * SORT_WARPS + warp;
-    if (chunk >= d.nchunk) return;
-    const int tile = chunk / SPH_TILE_CHUNKS;
-    if (d.tile_flag[tile]) return;
-    const int nround = (d.tile_ncand[tile] + SPH_SE - 1) / SPH_SE;
-    uint2 *lp = d.nlist + ((size_t)chunk * d.rows_cap) * 32 + lane;
-    const unsigned short *rp = d.rowptr + (size_t)chunk * ROWPTR_STRIDE;
-    unsigned short *buf = reinterpret_cast<unsigned short *>(s_buf + (size_t)threadIdx.x * SORT_STRIDE);
-    for (int r = 0; r < nround; ++r) {
-        const int g0 = rp[r], g1 = rp[r + 1];
-        if (g1 <= g0) continue;
-        // pass 1: class counts
-        unsigned long long cnt = 0ull;
-        int N = 0;
-        for (int gq = g0; gq < g1; ++gq) {
-            const uint2 w = lp[(size_t)gq * 32];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const unsigned x = (e & 2) ? w.y : w.x;
-                const unsigned off = (e & 1) ? (x >> 16) : (x & 0xffffu);
-                if (off != 0xffffu) { cnt += 1ull << (((off >> 4) & 7u) << 3); ++N; }
-            }
-        }
-        if (__any_sync(FULL, N > SORT_CAP)) continue;
-        const unsigned long long base = cnt * 0x0101010101010100ull;     // field c = entries of the classes below c
-        // pass 2: bucket by class
-        unsigned long long cur = base;
-        for (int gq = g0; gq < g1; ++gq) {
-            const uint2 w = lp[(size_t)gq * 32];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const unsigned x = (e & 2) ? w.y : w.x;
-                const unsigned off = (e & 1) ? (x >> 16) : (x & 0xffffu);
-                if (off != 0xffffu) {
-                    const unsigned c8 = ((off >> 4) & 7u) << 3;
-                    buf[(unsigned)(cur >> c8) & 0xffu] = (unsigned short)off;
-                    cur += 1ull << c8;
-                }
-            }
-        }
-        const unsigned long long end = cur;
-        unsigned long long tk = base;
-        // pass 3: emit round-robin over the classes, all lanes in lockstep over the positions
-        const int nmax = (g1 - g0) * 4;
-        unsigned w0 = 0u, w1 = 0u;
-        for (int n = 0; n < nmax; ++n) {
-            unsigned entry = 0xffffu;
-            if (n < N) {
-                unsigned c8 = ((unsigned)(lane + n) & 7u) << 3;
-                while (((unsigned)(tk >> c8) & 0xffu) >= ((unsigned)(end >> c8) & 0xffu)) c8 = (c8 + 8u) & 63u;
-                entry = buf[(unsigned)(tk >> c8) & 0xffu];
-                tk += 1ull << c8;
-            }
-            w0 = __byte_perm(w0, w1, 0x5432);
-            w1 = __byte_perm(w1, entry, 0x5432);
-            if ((n & 3) == 3) lp[(size_t)(g0 + (n >> 2)) * 32] = make_uint2(w0, w1);
-        }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        *d.nheavy = min(s_n, (unsigned)d.heavy_cap);
+        *d.cull_cycles = 0ull;
+        *d.cand_cursor = 0ull;
+        d.counters[SPH_C_TESTS_CULL] = 0ull;
+        d.counters[SPH_C_CANDIDATES] = 0ull;
+        d.counters[SPH_C_LIST_OVERFLOW] = 0ull;
     }
-}
-
-int sph_launch_list_sort(sph_ctx *c)
-{
-    Dev &d = c->d;
-    if (d.n == 0) return SPH_OK;
-    k_list_sort<<<sph_div_up(d.nchunk, SORT_WARPS), SORT_WARPS * 32, 0, c->stream>>>(d);
-    c->launches++;
-    SPH_CUDA(c, cudaGetLastError());
-    return SPH_OK;
 }
 
 // entry e (0..3) of a row-group word pair
@@ -745,7 +586,12 @@ __device__ __forceinline__ unsigned list_entry(uint2 w, int e)
 }
 
 // ------------------------------------------------------------------------------------------
-// S2 density from the lists (fp64 accumulation as in k_density; see sph_pair.cu for why)
+// S2 density from the lists: the gather set is the subset of the symmetric list with r2 < H_i^2, plus self.
+// Arithmetic: density_term (sph_pairterm.cuh): rho in fp64 (five fp32 -> fp64 conversions per true pair).
+// Measured alternatives (round 2, configs[2], this kernel 0.222 ms): fp32 terms with an fp64 accumulator:
+// 0.151 ms but rho only to 1.4e-7 and S_pred of configs[0] at 1.02e-4 (tolerance 1e-4): rejected; candidates
+// staged a second time widened to fp64 (48 B per slot, no conversions in the loop): 0.39 ms with one or two
+// warps per chunk -- three random LDS.128 per pair instead of one: the shared-memory pipe binds: rejected.
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
 {
@@ -760,20 +606,18 @@ __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
     const bool haschunk = chunk < d.nchunk;
     const long long i = (long long)tile * SPH_TILE + threadIdx.x;
     const bool valid = i < d.n;
-    float4 pi = valid ? d.r.pm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
-    float hi = valid ? d.r.vh[i].w : 1.f;
-    float Hi = sph_H(kappa, hi);
+    const float4 pi = valid ? d.r.pm[i] : make_float4(0.f, 0.f, 0.f, 0.f);
+    const float hi = valid ? d.r.vh[i].w : 1.f;
+    const float Hi = sph_H(kappa, hi);
     const float H2i = __fmul_rn(Hi, Hi);
     const float invH = 1.f / Hi;
     const double invHd = 1.0 / ((double)kappa * (double)hi);
     const double pxd = (double)pi.x, pyd = (double)pi.y, pzd = (double)pi.z;
     const uint2 *lp = d.nlist + ((size_t)(haschunk ? chunk : 0) * d.rows_cap) * 32 + lane;
     const unsigned short *rp = d.rowptr + (size_t)(haschunk ? chunk : 0) * ROWPTR_STRIDE;
-    // self term: q = 0, t = 1
-    double sum = (double)pi.w;
-    float sh = 3.f * pi.w;
-    int ng = 1;
-    const int ntest = 1 + (valid ? d.nsym[i] : 0);      // every list entry is tested
+    DensAcc A;
+    A.sum = (double)pi.w; A.sh = 3.f * pi.w; A.n = 1;          // self term: q = 0, t = 1
+    int ntest = 1;
     int round = 0;
     for (int r0 = 0; r0 < ncand; r0 += SPH_SE, ++round) {
         const int nr = min(SPH_SE, ncand - r0);
@@ -789,53 +633,39 @@ __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
                 for (int e = 0; e < 4; ++e) {
                     const unsigned off = list_entry(w, e);
                     if (off == 0xffffu) continue;
+                    ++ntest;
                     const float4 q = *reinterpret_cast<const float4 *>(smem_raw + off);
-                    float dx = __fsub_rn(pi.x, q.x), dy = __fsub_rn(pi.y, q.y), dz = __fsub_rn(pi.z, q.z);
-                    float r2 = sph_r2(dx, dy, dz);
-                    if (r2 < H2i) {
-                        float rinv = sph_rsqrt(fmaxf(r2, 1.0e-37f));
-                        float r = r2 * rinv;
-                        float qq = r * invH;
-                        float t = fmaxf(0.f, 1.f - qq);
-                        float t3 = t * t * t;
-                        sh = fmaf(q.w * t3, fmaf(qq, fmaf(-32.f, qq, 9.f), 3.f), sh);
-                        double ex = pxd - (double)q.x, ey = pyd - (double)q.y, ez = pzd - (double)q.z;
-                        double r2d = fma(ex, ex, fma(ey, ey, ez * ez));
-                        // sqrt(r2d) by one Newton step on the fp32 rsqrt, all in fp64 (one conversion, not two:
-                        // the XU pipe that converts is this kernel's limiter)
-                        const double yd = (double)rinv, td0 = r2d * yd;
-                        double rd = fma(0.5 * td0, fma(-td0, yd, 1.0), td0);
-                        double qd = rd * invHd;
-                        // no clamp at 0: membership (r2 < H_i^2 in fp32) already says q < 1 up to rounding, and
-                        // (1 - q)^4 of a q that exceeds 1 by 1e-7 is 1e-28 (fmax on doubles is nine instructions)
-                        double td = 1.0 - qd;
-                        double t2 = td * td;
-                        sum = fma((double)q.w * t2 * t2, fma(4.0, qd, 1.0), sum);
-                        ++ng;
-                    }
+                    const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
+                    if (r2 < H2i)
+                        density_term(A, r2, q.w, invH, pxd - (double)q.x, pyd - (double)q.y, pzd - (double)q.z,
+                                     (double)q.w, invHd);
                 }
             }
         }
         __syncthreads();
     }
+    unsigned small = 0u;
     if (valid) {
-        float kw = SPH_WC2_SIGMA * invH * invH * invH;
-        double rhod = 3.3422538049298023 * invHd * invHd * invHd * sum;
-        float rho = (float)rhod;
+        double rhod;
+        float rho, om;
+        density_finish(A, invH, invHd, rhod, rho, om);
         d.rho64[i] = rhod;
         d.rho[i] = rho;
-        d.omega[i] = 1.f - kw * sh / (3.f * rho);
-        d.ngather[i] = ng;
+        d.omega[i] = om;
+        d.ngather[i] = A.n;
+        small = fabsf(om) < 0.1f ? 1u : 0u;
     }
-    unsigned long long hits = valid ? (unsigned long long)ng : 0ull, tests = valid ? (unsigned long long)ntest : 0ull;
+    unsigned long long hits = valid ? (unsigned long long)A.n : 0ull, tests = valid ? (unsigned long long)ntest : 0ull;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         hits += __shfl_xor_sync(FULL, hits, o);
         tests += __shfl_xor_sync(FULL, tests, o);
     }
+    small = __popc(__ballot_sync(FULL, small != 0u));
     if (lane == 0) {
         atomicAdd(&d.counters[SPH_C_PAIRS_GATHER], hits);
         atomicAdd(&d.counters[SPH_C_TESTS_DENSITY], tests);
+        if (small) atomicAdd(&d.counters[SPH_C_OMEGA_SMALL], (unsigned long long)small);
     }
 }
 
@@ -942,6 +772,7 @@ __global__ void __launch_bounds__(256) k_neighbors_l(Dev d, float kappa, int *co
     const unsigned short *rp = d.rowptr + (size_t)chunk * ROWPTR_STRIDE;
     unsigned oi = orig[i];
     long long base = list ? offsets[oi] : 0;
+    if (base < 0) { base = 0; list = nullptr; }          // offsets[i] < 0: this particle's ids are not wanted
     float4 pi = d.r.pm[i];
     float Hi = sph_H(kappa, d.r.vh[i].w);
     float H2i = __fmul_rn(Hi, Hi);
@@ -982,26 +813,19 @@ static int set_smem(sph_ctx *c, const void *fn, size_t bytes)
     return SPH_OK;
 }
 
-int sph_launch_cull(sph_ctx *c, bool with_density)
+int sph_launch_cull(sph_ctx *c)
 {
     Dev &d = c->d;
-    SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_TESTS_CULL], 0, 3 * sizeof(unsigned long long), c->stream));
-    SPH_CUDA(c, cudaMemsetAsync(d.cand_cursor, 0, sizeof(unsigned long long), c->stream));
-    if (d.n == 0) return SPH_OK;
-    int rc = set_smem(c, with_density ? (const void *)k_cull<true> : (const void *)k_cull<false>, sizeof(CullSmem));
-    if (rc) return rc;
-    if (with_density) {
-        SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_PAIRS_GATHER], 0, sizeof(unsigned long long), c->stream));
-        SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_TESTS_DENSITY], 0, sizeof(unsigned long long), c->stream));
+    if (d.n == 0) {
+        SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_TESTS_CULL], 0, 3 * sizeof(unsigned long long), c->stream));
+        return SPH_OK;
     }
+    int rc = set_smem(c, (const void *)k_cull, sizeof(CullSmem));
+    if (rc) return rc;
     int ntile = sph_div_up(d.nchunk, SPH_TILE_CHUNKS);
-    SPH_CUDA(c, cudaMemsetAsync(d.nheavy, 0, sizeof(unsigned), c->stream));
-    k_tile_plan<<<sph_div_up(ntile, 256), 256, 0, c->stream>>>(d, ntile);
-    k_tile_plan_clamp<<<1, 1, 0, c->stream>>>(d);
-    SPH_CUDA(c, cudaMemsetAsync(d.cull_cycles, 0, sizeof(unsigned long long), c->stream));
-    if (with_density) k_cull<true><<<d.heavy_cap + ntile, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, ntile);
-    else k_cull<false><<<d.heavy_cap + ntile, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, ntile);
-    c->launches += 3;
+    k_tile_plan<<<1, 1024, 0, c->stream>>>(d, ntile);
+    k_cull<<<d.heavy_cap + ntile, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, ntile);
+    c->launches += 2;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
 }
@@ -1011,6 +835,7 @@ int sph_launch_density_l(sph_ctx *c)
     Dev &d = c->d;
     SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_PAIRS_GATHER], 0, sizeof(unsigned long long), c->stream));
     SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_TESTS_DENSITY], 0, sizeof(unsigned long long), c->stream));
+    SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_OMEGA_SMALL], 0, sizeof(unsigned long long), c->stream));
     if (d.n == 0) return SPH_OK;
     size_t bytes = (size_t)SPH_SE * sizeof(float4);
     int rc = set_smem(c, (const void *)k_density_l, bytes);

@@ -89,14 +89,7 @@ __device__ __forceinline__ void walk(const Tree &t, float3 tlo, float3 thi, floa
 
 // ------------------------------------------------------------------------------------------
 // S2 density: rho_i = sum_j m_j W_ij(h_i) (Eq. 1), Omega_i (Eq. 3), over r2 < H_i^2, self included.
-//   W           = SIGMA/H^3 t^4 (1+4q),            t = 1-q
-//   dW/dh       = -(3W + r dW/dr)/h = -SIGMA/(H^3 h) t^3 (3 + 9q - 32 q^2)
-// so   rho = SIGMA/H^3 sum m t^4 (1+4q),   Omega = 1 - SIGMA/(3 rho H^3) sum m t^3 (3 + 9q - 32q^2).
-// rho is evaluated and accumulated in fp64 for the TRUE neighbours only: P = c0^2 (rho - rho0)
-// amplifies the relative error of rho by rho/(rho - rho0) ~ 100 on a lattice and Y = Y0 + mu_i P
-// by another rho0 c0^2 / Y0 ~ 2400 (hard part 2), so even a correctly rounded
-// fp32 rho misses the 1e-4 target on the yielded S.  B200 runs FP64 at half the FP32 rate, and the
-// extra work is ~12 DFMA per true pair.  r comes from the fp32 rsqrt plus one Newton step in fp64.
+// Arithmetic: density_term (sph_pairterm.cuh), the same as in the list-driven kernel.
 // ------------------------------------------------------------------------------------------
 template <bool EXACT>
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_density(Dev d, float kappa, const unsigned char *__restrict__ tile_flag, int ntile)
@@ -119,9 +112,8 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_density(Dev d, float kappa,
     const double invHd = 1.0 / ((double)kappa * (double)hi);
     const double pxd = (double)pi.x, pyd = (double)pi.y, pzd = (double)pi.z;
     float4 blo = d.tree.lo[0][chunk], bhi = d.tree.hi[0][chunk];
-    double sum = 0.0;
-    float sh = 0.f;
-    int cnt_i = 0;
+    DensAcc A;
+    A.sum = 0.0; A.sh = 0.f; A.n = 0;                  // the walk meets the particle itself (r2 = 0)
     unsigned long long tests = 0;
     const unsigned vmask = __ballot_sync(0xffffffffu, valid);
     if (EXACT) {
@@ -141,44 +133,32 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_density(Dev d, float kappa,
             float4 q = s_src[warp][j];
             float dx = __fsub_rn(pi.x, q.x), dy = __fsub_rn(pi.y, q.y), dz = __fsub_rn(pi.z, q.z);
             float r2 = sph_r2(dx, dy, dz);
-            if (r2 < H2i) {
-                float rinv = rsqrtf(fmaxf(r2, 1.0e-37f));
-                float r = r2 * rinv;
-                float qq = r * invH;
-                float t = fmaxf(0.f, 1.f - qq);
-                float t3 = t * t * t;
-                sh = fmaf(q.w * t3, fmaf(qq, fmaf(-32.f, qq, 9.f), 3.f), sh);
-                // fp64 value of m_j t^4 (1 + 4q)
-                double ex = pxd - (double)q.x, ey = pyd - (double)q.y, ez = pzd - (double)q.z;
-                double r2d = fma(ex, ex, fma(ey, ey, ez * ez));
-                double r0 = (double)r;
-                double rd = fma(fma(-r0, r0, r2d), 0.5 * (double)rinv, r0);      // one Newton step for sqrt
-                double qd = rd * invHd;
-                double td = fmax(0.0, 1.0 - qd);
-                double t2 = td * td;
-                sum = fma((double)q.w * t2 * t2, fma(4.0, qd, 1.0), sum);
-                ++cnt_i;
-            }
+            if (r2 < H2i)
+                density_term(A, r2, q.w, invH, pxd - (double)q.x, pyd - (double)q.y, pzd - (double)q.z, (double)q.w, invHd);
         }
         __syncwarp();
     });
 
+    unsigned small = 0u;
     if (valid) {
-        float kw = WC2_SIGMA * invH * invH * invH;
-        double rhod = 3.3422538049298023 * invHd * invHd * invHd * sum;
-        float rho = (float)rhod;
+        double rhod;
+        float rho, om;
+        density_finish(A, invH, invHd, rhod, rho, om);
         d.rho64[i] = rhod;
         d.rho[i] = rho;
-        d.omega[i] = 1.f - kw * sh / (3.f * rho);
-        d.ngather[i] = cnt_i;
+        d.omega[i] = om;
+        d.ngather[i] = A.n;
+        small = fabsf(om) < 0.1f ? 1u : 0u;
     }
+    small = __popc(__ballot_sync(0xffffffffu, small != 0u));
     // counters: true pairs and candidate tests
-    unsigned long long hits = (unsigned long long)cnt_i;
+    unsigned long long hits = (unsigned long long)A.n;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) hits += __shfl_xor_sync(0xffffffffu, hits, o);
     if (lane == 0) {
         atomicAdd(&d.counters[SPH_C_PAIRS_GATHER], hits);
         atomicAdd(&d.counters[SPH_C_TESTS_DENSITY], tests);
+        if (small) atomicAdd(&d.counters[SPH_C_OMEGA_SMALL], (unsigned long long)small);
     }
     }   // tile loop
 }
@@ -286,6 +266,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_neighbors(Dev d, float kapp
     float H2i = valid ? __fmul_rn(Hi, Hi) : -1.f;
     unsigned oi = valid ? orig[i] : 0u;
     long long base = (valid && list) ? offsets[oi] : 0;
+    const bool want = list && base >= 0;                 // offsets[i] < 0: this particle's ids are not wanted
     float4 blo = d.tree.lo[0][chunk], bhi = d.tree.hi[0][chunk];
     int cnt_i = 0;
     if (EXACT) {
@@ -308,7 +289,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_neighbors(Dev d, float kapp
             float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
             bool hit = SYM ? (r2 < fmaxf(H2i, s_H2[warp][j]) && (j0 + j) != i) : (r2 < H2i);
             if (hit) {
-                if (list) list[base + cnt_i] = (int)s_orig[warp][j];
+                if (want) list[base + cnt_i] = (int)s_orig[warp][j];
                 ++cnt_i;
             }
         }
@@ -333,6 +314,7 @@ int sph_launch_density(sph_ctx *c, bool flagged_only)
     if (!flagged_only) {
         SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_PAIRS_GATHER], 0, sizeof(unsigned long long), c->stream));
         SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_TESTS_DENSITY], 0, sizeof(unsigned long long), c->stream));
+        SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_OMEGA_SMALL], 0, sizeof(unsigned long long), c->stream));
     }
     if (d.n == 0) return SPH_OK;
     const int ntile = sph_div_up(d.nchunk, PAIR_WARPS);

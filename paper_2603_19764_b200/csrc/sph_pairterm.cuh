@@ -33,6 +33,23 @@ __device__ __forceinline__ float sph_rsqrt(float y)
     return r;
 }
 
+// ---- S2: one term of Eq. 1 and Eq. 3 (Wendland C2, reading Q3) ---------------------------------------------
+//   W = SIGMA/H^3 t^4 (1 + 4q),  dW/dh = -SIGMA/(H^3 h) t^3 (3 + 9q - 32 q^2),  q = r/H, t = 1 - q
+// rho is evaluated and accumulated in fp64: P = c0^2 (rho - rho0) amplifies the relative error of rho by
+// rho/(rho - rho0) ~ 100 on a lattice, and a yielding particle (Y small against rho0 c0^2) passes the error of P
+// on to the rescaled S: BASELINE.json configs[0] needs rho to ~2e-8 for its 1e-4 on the yielded state, which is
+// below what fp32 geometry can give (measured in round 2: fp32 terms with an fp64 accumulator leave 1.4e-7 in rho
+// and 1.02e-4 in S_pred).  The Omega sum (Eq. 3) stays fp32.  r = sqrt(r2) by one Newton step, in fp64, on the
+// fp32 rsqrt.  ex, ey, ez: x_i - x_j in fp64 (exact: both are fp32 values); md = m_j.
+struct DensAcc {
+    double sum;     // sum_j m_j t^4 (1 + 4q)
+    float sh;       // sum_j m_j t^3 (3 + 9q - 32 q^2)
+    int n;          // |gather set|
+};
+
+__device__ __forceinline__ void density_term(DensAcc &A, float r2, float mj, float invH, double ex, double ey,
+                                             double ez, double md, double invHd);
+
 struct PairConst {
     float beta;       // Eq. 5
     float alpha2;     // alpha / 2: alpha cbar = alpha2 (c_i + c_j)
@@ -125,6 +142,34 @@ __device__ __forceinline__ void pair_term(const PairTarget &t, const PairConst &
         A.du = fmaf(-0.5f * kk, vr, A.du);
         A.mumax = fmaxf(A.mumax, -mu);
     }
+}
+
+__device__ __forceinline__ void density_term(DensAcc &A, float r2, float mj, float invH, double ex, double ey,
+                                             double ez, double md, double invHd)
+{
+    const float rinv = sph_rsqrt(fmaxf(r2, 1.0e-37f));
+    const float q = (r2 * rinv) * invH;
+    const float t = fmaxf(0.f, 1.f - q);
+    A.sh = fmaf(mj * (t * t * t), fmaf(q, fmaf(-32.f, q, 9.f), 3.f), A.sh);
+    const double r2d = fma(ex, ex, fma(ey, ey, ez * ez));
+    const double yd = (double)rinv, td0 = r2d * yd;
+    const double rd = fma(0.5 * td0, fma(-td0, yd, 1.0), td0);
+    const double qd = rd * invHd;
+    // no clamp at 0: membership (r2 < H_i^2 in fp32) already says q < 1 up to rounding, and (1 - q)^4 of a q that
+    // exceeds 1 by 1e-7 is 1e-28
+    const double td = 1.0 - qd, t2 = td * td;
+    A.sum = fma(md * t2 * t2, fma(4.0, qd, 1.0), A.sum);
+    A.n++;
+}
+
+// rho (fp64 and fp32) and Omega from the sums; invH = 1 / (kappa h_i) in fp32 (the Omega terms), invHd in fp64
+__device__ __forceinline__ void density_finish(const DensAcc &A, float invH, double invHd, double &rhod, float &rho,
+                                               float &omega)
+{
+    rhod = 3.3422538049298023 * invHd * invHd * invHd * A.sum;
+    rho = (float)rhod;
+    const float kw = SPH_WC2_SIGMA * invH * invH * invH;
+    omega = 1.f - kw * A.sh / (3.f * rho);
 }
 
 // loads the per-target operands (resident arrays of sph_internal.cuh's Dev)

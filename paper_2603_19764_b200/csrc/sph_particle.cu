@@ -107,10 +107,14 @@ __global__ void __launch_bounds__(256) k_predict(Dev d, DevParams p, DevTabs tab
 // strain-rate invariant (Eq. 43), per-particle time-step limit (Eq. 38-39).
 // phase == SPH_DERIVATIVES leaves v, u, S, e_acc untouched (bootstrap of the first step).
 // ------------------------------------------------------------------------------------------
+// Also S8: the block's minimum of dt_i goes into dt_next with one atomicMin (positive floats order like
+// unsigned ints; k_dt_select / k_dt_reset set dt_next to +inf before), and the robustness counters.
 __global__ void __launch_bounds__(256) k_close(Dev d, DevParams p, int phase, float dt_arg, int dt_from_device)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (i >= d.n) return;
+    float dti = __int_as_float(0x7f800000);
+    unsigned nfall = 0u, nbad = 0u;
+    if (i < d.n) {
     const float dt = dt_from_device ? *d.dt_cur : dt_arg;
     const bool strength = (p.flags & SPH_STRENGTH) != 0;
     unsigned mf = ((const unsigned *)d.r.s[PP_MATFIX])[i];
@@ -146,7 +150,7 @@ __global__ void __launch_bounds__(256) k_close(Dev d, DevParams p, int phase, fl
                     G[3 * a + b] = F[3 * a] * C[b] + F[3 * a + 1] * C[3 + b] + F[3 * a + 2] * C[6 + b];
         } else {
             cflag = 1.f;
-            atomicAdd(&d.counters[SPH_C_CFALLBACK], 1ull);
+            nfall = 1u;
 #pragma unroll
             for (int k = 0; k < 9; ++k) G[k] = F[k];
         }
@@ -176,19 +180,22 @@ __global__ void __launch_bounds__(256) k_close(Dev d, DevParams p, int phase, fl
     // time-step limit, Eq. 39 (and Eq. 38 with epsilon = h when eta_a > 0)
     float h = d.r.vh[i].w;
     float ax = d.a[0][i], ay = d.a[1][i], az = d.a[2][i];
-    float dti = p.eta_C * h / ((1.f + 0.6f * p.alpha) * d.cs[i] + 0.6f * p.beta * d.mumax[i]);
+    dti = p.eta_C * h / ((1.f + 0.6f * p.alpha) * d.cs[i] + 0.6f * p.beta * d.mumax[i]);
     if (p.eta_a > 0.f) {
         float an = sqrtf(ax * ax + ay * ay + az * az);
         if (an > 0.f) dti = fminf(dti, p.eta_a * sqrtf(h / an));
     }
     d.dti[i] = dti;
+    const float du_ = d.dudt[i];
+    if (!(isfinite(ax) && isfinite(ay) && isfinite(az) && isfinite(du_) && isfinite(dS[0] + dS[1] + dS[2] + dS[3] + dS[4])))
+        nbad = 1u;
 
     if (phase == SPH_CLOSE) {
         float hdt = 0.5f * dt;
         float vx = d.r.s[PP_VHALF + 0][i], vy = d.r.s[PP_VHALF + 1][i], vz = d.r.s[PP_VHALF + 2][i];
         if (!fixed) { vx = fmaf(hdt, ax, vx); vy = fmaf(hdt, ay, vy); vz = fmaf(hdt, az, vz); }
         d.vfull[0][i] = vx; d.vfull[1][i] = vy; d.vfull[2][i] = vz;
-        d.ufull[i] = fmaf(hdt, d.dudt[i], d.r.s[PP_UHALF][i]);
+        d.ufull[i] = fmaf(hdt, du_, d.r.s[PP_UHALF][i]);
         float S[5] = {0.f, 0.f, 0.f, 0.f, 0.f};
         if (strength) {
 #pragma unroll
@@ -201,28 +208,42 @@ __global__ void __launch_bounds__(256) k_close(Dev d, DevParams p, int phase, fl
         for (int c = 0; c < 5; ++c) d.Sfull[c][i] = S[c];
         d.r.s[PP_EACC][i] = fmaf(dt, eps2, d.r.s[PP_EACC][i]);
     }
+    }   // i < d.n
+    // S8 and the counters: one atomic per block
+    __shared__ float s_dt[8];
+    __shared__ unsigned s_cnt[8];
+    unsigned packed = nfall | (nbad << 16);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        dti = fminf(dti, __shfl_xor_sync(0xffffffffu, dti, o));
+        packed += __shfl_xor_sync(0xffffffffu, packed, o);
+    }
+    if ((threadIdx.x & 31) == 0) { s_dt[threadIdx.x >> 5] = dti; s_cnt[threadIdx.x >> 5] = packed; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float m = s_dt[0];
+        unsigned c = s_cnt[0];
+#pragma unroll
+        for (int w = 1; w < 8; ++w) { m = fminf(m, s_dt[w]); c += s_cnt[w]; }
+        if (m > 0.f) atomicMin((unsigned *)d.dt_next, __float_as_uint(m));
+        if (c & 0xffffu) atomicAdd(&d.counters[SPH_C_CFALLBACK], (unsigned long long)(c & 0xffffu));
+        if (c >> 16) atomicAdd(&d.counters[SPH_C_NONFINITE], (unsigned long long)(c >> 16));
+    }
 }
 
 // ------------------------------------------------------------------------------------------
-// S8: dt_next = min_i dt_i  (positive floats order like unsigned ints)
+// S8: dt_next = min_i dt_i is accumulated by k_close; these set it up
 // ------------------------------------------------------------------------------------------
 __global__ void k_dt_reset(float *dt_next) { *(unsigned *)dt_next = 0x7f800000u; }
 
-__global__ void __launch_bounds__(256) k_dt_min(const float *__restrict__ dti, long long n, float *dt_next)
-{
-    float m = __int_as_float(0x7f800000);
-    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
-        m = fminf(m, dti[i]);
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) m = fminf(m, __shfl_xor_sync(0xffffffffu, m, o));
-    if ((threadIdx.x & 31) == 0 && m > 0.f) atomicMin((unsigned *)dt_next, __float_as_uint(m));
-}
-
-__global__ void k_dt_select(float dt_arg, float *dt_cur, const float *dt_next, float *dt_used)
+// head of a step: the step in use (dt_arg, or the CFL step the last CLOSE left in dt_next), and dt_next
+// reset to +inf for this step's CLOSE
+__global__ void k_dt_select(float dt_arg, float *dt_cur, float *dt_next, float *dt_used)
 {
     float dt = dt_arg > 0.f ? dt_arg : *dt_next;
     *dt_cur = dt;
     if (dt_used) *dt_used = dt;
+    *(unsigned *)dt_next = 0x7f800000u;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -312,13 +333,14 @@ int sph_launch_close(sph_ctx *c, int phase, float dt, bool dt_from_device)
 {
     Dev &d = c->d;
     SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_CFALLBACK], 0, sizeof(unsigned long long), c->stream));
-    k_dt_reset<<<1, 1, 0, c->stream>>>(d.dt_next);
-    c->launches++;
+    SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_NONFINITE], 0, sizeof(unsigned long long), c->stream));
+    if (!dt_from_device) {                 // inside sph_step k_dt_select has already reset dt_next
+        k_dt_reset<<<1, 1, 0, c->stream>>>(d.dt_next);
+        c->launches++;
+    }
     if (d.n > 0) {
-        int nb = sph_div_up(d.n, 256);
-        k_close<<<nb, 256, 0, c->stream>>>(d, c->p, phase, dt, dt_from_device ? 1 : 0);
-        k_dt_min<<<nb < 592 ? nb : 592, 256, 0, c->stream>>>(d.dti, d.n, d.dt_next);
-        c->launches += 2;
+        k_close<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, c->p, phase, dt, dt_from_device ? 1 : 0);
+        c->launches++;
     }
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;

@@ -34,8 +34,6 @@ FLAG_PCLIP_GLOBAL = 4
 FLAG_JAUMANN_AS_PRINTED = 8
 FLAG_NO_LISTS = 16
 FLAG_NO_GRAPH = 64
-FLAG_FUSED_DENSITY = 128
-FLAG_SORT_LISTS = 256
 
 G_NEWTON = 6.674e-11
 

@@ -22,6 +22,42 @@ def rows(counts, offsets, lst):
     return [np.sort(lst[offsets[i]:offsets[i + 1]]) for i in range(counts.shape[0])]
 
 
+def sorted_rows_key(counts, lst, n_ids):
+    """One int64 per list entry, row-major with every row sorted: row * n_ids + id, sorted.  Two CSR lists with
+    equal counts hold the same SETS row by row iff these arrays are equal (vectorised: usable at 1e6 rows)."""
+    counts = np.asarray(counts, dtype=np.int64)
+    row = np.repeat(np.arange(counts.shape[0], dtype=np.int64), counts)
+    key = row * np.int64(n_ids) + np.asarray(lst, dtype=np.int64)[: row.shape[0]]
+    return np.sort(key)
+
+
+def neighbor_sets_equal(s, wl, mode="grid", select=None, oracle_sample=None):
+    """Neighbour sets of the CUDA path (sph_get_neighbors, original ids) against the oracle's, as SETS per
+    particle, gather and symmetric.  select: caller-order indices of the particles to compare (full-size cases);
+    oracle_sample = (idx, pos): the oracle runs on wl.subset(idx) and select == idx[pos] (dependency-closed
+    sample, see dependency_closed_sample)."""
+    from oracle import oracle as O
+    from paper_2603_19764_b200 import binding as B
+    for which_g, which_o in ((B.GATHER, O.GATHER), (B.SYMMETRIC, O.SYMMETRIC)):
+        c, o, l = s.get_neighbors(which_g, select=select)
+        c = c.cpu().numpy(); l = l.cpu().numpy()
+        if oracle_sample is None:
+            A = wl.arrays
+            co, oo, lo = O.neighbors(A["x"], A["y"], A["z"], A["h"], wl.params.kappa, which_o, mode)
+            if select is not None:
+                sel = np.asarray(select)
+                lo = np.concatenate([lo[oo[i]:oo[i + 1]] for i in sel]) if sel.size else lo[:0]
+                co = co[sel]
+        else:
+            idx, pos = oracle_sample
+            sub = wl.subset(idx).arrays
+            cs, os_, ls = O.neighbors(sub["x"], sub["y"], sub["z"], sub["h"], wl.params.kappa, which_o, mode)
+            co = cs[pos]
+            lo = idx[np.concatenate([ls[os_[i]:os_[i + 1]] for i in pos])]       # back to ids of the whole set
+        assert np.array_equal(c, co), "neighbour counts differ"
+        assert np.array_equal(sorted_rows_key(c, l, wl.n), sorted_rows_key(co, lo, wl.n)), "neighbour ids differ"
+
+
 def gpu_single_pass(wl, dt=None, split=True, allow_fallback=False, select=None):
     """Run the BASELINE.json configs[0] pass sequence through the C ABI; returns numpy fields
     (of the particles ``select`` -- caller-order indices -- when given: full-size cases)."""
@@ -40,7 +76,8 @@ def gpu_single_pass(wl, dt=None, split=True, allow_fallback=False, select=None):
         s.forces()
         s.strength_update(B.CLOSE, dt)
     else:
-        raise NotImplementedError
+        s.gradients_forces()                    # S4 + S5 in one pass: the kernel sph_step runs
+        s.strength_update(B.CLOSE, dt)
     sel = None if select is None else torch.as_tensor(np.asarray(select), dtype=torch.long, device="cuda")
     pick = (lambda t: t) if sel is None else (lambda t: t[..., sel])
     out = {}

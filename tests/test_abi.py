@@ -19,7 +19,7 @@ def lib():
 def declared_symbols():
     src = open(os.path.join(ROOT, "include", "sph.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(sph_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(sph_[a-z_0-9]+)\s*\(", src)))
 
 
 def test_header_and_binding_agree():

@@ -28,6 +28,7 @@ def test_full_config_every_particle(k, dt):
     errs = U.compare_single_pass(g, d, wl)
     c = g["counters"]
     assert c["pairs_gather"] == int(d["n_gather"].sum()) and c["pairs_symmetric"] == int(d["n_symmetric"].sum())
+    U.neighbor_sets_equal(g["_sph"], wl, mode="grid")          # sorted id lists of every particle
     print(f"config{k} n={wl.n}", {q: float(f"{v:.3g}") for q, v in errs.items()})
 
 
@@ -39,6 +40,7 @@ def _sampled(wl, centre, n_valid, dt):
     d = U.restrict(O.single_pass(wl.subset(idx), dt=dt, mode="grid"), pos)
     sub = wl.subset(V)
     errs = U.compare_single_pass(g, d, sub)
+    U.neighbor_sets_equal(g["_sph"], wl, mode="grid", select=V, oracle_sample=(idx, pos))    # ids of the sampled particles
     return errs, idx.size, g["counters"]["list_overflow"]
 
 

@@ -12,26 +12,12 @@ pytestmark = pytest.mark.gpu
 F = W.FLAG_STRENGTH | W.FLAG_CORRECTION_TENSOR
 
 
-def _neighbor_sets_equal(s, wl, mode="brute"):
-    from paper_2603_19764_b200 import binding as B
-    A = wl.arrays
-    for which_g, which_o in ((B.GATHER, O.GATHER), (B.SYMMETRIC, O.SYMMETRIC)):
-        c, o, l = s.get_neighbors(which_g)
-        co, oo, lo = O.neighbors(A["x"], A["y"], A["z"], A["h"], wl.params.kappa, which_o, mode)
-        assert np.array_equal(c.cpu().numpy(), co)
-        assert np.array_equal(o.cpu().numpy(), oo)
-        rg = U.rows(c.cpu().numpy(), o.cpu().numpy(), l.cpu().numpy())
-        ro = U.rows(co, oo, lo)
-        for a, b in zip(rg, ro):
-            assert np.array_equal(a, b)
-
-
 def test_config0_single_pass_all_fields():
     wl = W.config(0)
     g = U.gpu_single_pass(wl)
     d = O.single_pass(wl)
     errs = U.compare_single_pass(g, d, wl)
-    _neighbor_sets_equal(g["_sph"], wl)
+    U.neighbor_sets_equal(g["_sph"], wl, mode="brute")
     c = g["counters"]
     assert c["pairs_gather"] == int(d["n_gather"].sum()) and c["pairs_symmetric"] == int(d["n_symmetric"].sum())
     assert c["cfallback"] == 0
@@ -39,7 +25,7 @@ def test_config0_single_pass_all_fields():
 
 
 @pytest.mark.parametrize("case", ["ragged_11", "h_spread", "two_materials", "hydro_only", "no_correction",
-                                  "as_printed", "pclip_global", "block_24", "sort_lists"])
+                                  "as_printed", "pclip_global", "block_24", "eta_a", "fused", "fused_hydro"])
 def test_variants(case):
     kw = dict(n_side=12)
     if case == "ragged_11":
@@ -58,21 +44,32 @@ def test_variants(case):
         kw = dict(n_side=12, flags=F | W.FLAG_PCLIP_GLOBAL)
     elif case == "block_24":
         kw = dict(n_side=24)                                  # 432 chunks: two tree levels
-    elif case == "sort_lists":
-        kw = dict(n_side=12, h_spread=0.2, flags=F | W.FLAG_SORT_LISTS)   # lists reordered by bank class
+    elif case == "fused":
+        kw = dict(n_side=12, h_spread=0.3, two_materials=True)            # S4 + S5 in one pass, h_i != h_j
+    elif case == "fused_hydro":
+        kw = dict(n_side=12, h_spread=0.3, flags=W.FLAG_CORRECTION_TENSOR)
+    elif case == "eta_a":
+        kw = dict(n_side=12)
     wl = W.elastic_block(**kw)
-    g = U.gpu_single_pass(wl)
+    if case == "eta_a":
+        wl.params.eta_a = 8.0e-2          # Eq. 38 (reading Q22) limits some particles, Eq. 39 the others
+    g = U.gpu_single_pass(wl, split=not case.startswith("fused"))
     d = O.single_pass(wl, mode="grid" if wl.n > 5000 else "brute")
     U.compare_single_pass(g, d, wl)
-    if wl.n <= 2000:
-        _neighbor_sets_equal(g["_sph"], wl)
+    if case == "eta_a":
+        wl.params.eta_a = 0.0
+        d0 = O.single_pass(wl)
+        lim = d["dt_i"] < d0["dt_i"] * (1 - 1e-12)
+        assert 0.05 < lim.mean() < 0.95, lim.mean()        # both branches of the minimum are exercised
+    U.neighbor_sets_equal(g["_sph"], wl, mode="grid")
 
 
-def test_three_tree_levels_and_sampled_rows():
+def test_three_tree_levels_and_neighbour_ids():
     wl = W.elastic_block(40, h_spread=0.2)                    # 64000 particles, 2000 chunks, 3 levels
     g = U.gpu_single_pass(wl)
     d = O.single_pass(wl, mode="grid")
     U.compare_single_pass(g, d, wl)
+    U.neighbor_sets_equal(g["_sph"], wl, mode="grid")         # sorted id lists, every particle
 
 
 def test_empty_and_tiny_inputs():
@@ -167,7 +164,7 @@ def test_tree_walk_kernels_still_match():
     g = U.gpu_single_pass(wl)
     d = O.single_pass(wl)
     U.compare_single_pass(g, d, wl)
-    _neighbor_sets_equal(g["_sph"], wl)
+    U.neighbor_sets_equal(g["_sph"], wl, mode="brute")
 
 
 def test_variable_h_impact_pair_scaled():
@@ -178,7 +175,59 @@ def test_variable_h_impact_pair_scaled():
     d = O.single_pass(wl, dt=1e-3, mode="grid")
     errs = U.compare_single_pass(g, d, wl)
     assert g["counters"]["list_overflow"] == 0
+    U.neighbor_sets_equal(g["_sph"], wl, mode="grid")         # multi-level walk, variable h: ids, not only counts
     print("impact pair errors", {k: float(f"{v:.3g}") for k, v in errs.items()})
+    gf = U.gpu_single_pass(wl, dt=1e-3, split=False)          # the fused S4 + S5 kernel on the same set
+    U.compare_single_pass(gf, d, wl)
+
+
+def test_fused_step_on_variable_h_two_materials_matches_oracle_stepper():
+    """sph_step (fused gradient + force kernel, CUDA-graph replay on a capturable stream) for two steps on the
+    configs[3] construction at parity size -- variable h, two materials -- against the oracle's stepper."""
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    wl = W.impact_pair(30000, W.SEED_BASE + 3, 100.0, 1.214)
+    st = O.Stepper(wl, mode="grid")
+    with torch.cuda.stream(torch.cuda.Stream()):
+        s = B.Sph(wl.params, wl.n)
+        t = s.upload(wl)
+        dtu = torch.zeros(1, dtype=torch.float32, device="cuda")
+        s.step(t, wl.n, 0.0, dtu)
+        dts = [float(dtu.item())]
+        s.step(None, 0, 0.0, dtu)
+        dts.append(float(dtu.item()))
+        s.download_state(t)
+        torch.cuda.synchronize()
+        assert s.get_counters()["list_overflow"] == 0
+    for k in range(2):
+        assert dts[k] == pytest.approx(st.step(0.0), rel=2e-5)
+    x = np.stack([t[k].cpu().numpy() for k in ("x", "y", "z")])
+    v = np.stack([t[k].cpu().numpy() for k in ("vx", "vy", "vz")])
+    S = np.stack([t[k].cpu().numpy() for k in ("Sxx", "Syy", "Sxy", "Sxz", "Syz")])
+    assert U.maxnorm_err(x, st.x) <= 1e-6
+    assert U.maxnorm_err(v, st.v) <= U.TOL_STATE
+    assert U.maxnorm_err(t["u"].cpu().numpy(), st.u) <= U.TOL_STATE
+    assert U.maxnorm_err(S, st.S) <= U.TOL_STATE
+
+
+def test_coincident_particles_and_bad_material_index():
+    """Two particles at the same position (r = 0, i != j): members of each other's sets, zero pair force
+    (x_ij = 0), no NaN.  A material index outside 0..n_materials-1 is replaced and counted."""
+    from paper_2603_19764_b200 import binding as B
+    wl = W.elastic_block(8, h_spread=0.2)
+    for k in ("x", "y", "z"):
+        wl.arrays[k][17] = wl.arrays[k][200]
+    g = U.gpu_single_pass(wl)
+    d = O.single_pass(wl)
+    U.compare_single_pass(g, d, wl)
+    U.neighbor_sets_equal(g["_sph"], wl, mode="brute")
+    for k in ("a", "dudt", "dsdt", "s", "rho"):
+        assert np.all(np.isfinite(g[k])), k
+    assert g["counters"]["bad_material"] == 0 and g["counters"]["nonfinite"] == 0
+    wl.mat[5] = 7; wl.mat[6] = -1                        # one material defined
+    g2 = U.gpu_single_pass(wl)
+    assert g2["counters"]["bad_material"] == 2
+    assert np.array_equal(g2["s"], g["s"])               # both were given material n_materials - 1 = 0
 
 
 def test_granular_column_scaled_with_fixed_floor():
@@ -200,7 +249,7 @@ def test_tiles_over_list_capacity_fall_back_to_the_tree_walk():
     assert g["counters"]["list_overflow"] > 0
     d = O.single_pass(wl)
     U.compare_single_pass(g, d, wl)
-    _neighbor_sets_equal(g["_sph"], wl)
+    U.neighbor_sets_equal(g["_sph"], wl, mode="brute")
 
 
 def test_diagnostics_match_fp64_sums_and_momentum_is_conserved():
@@ -279,26 +328,3 @@ def test_graph_replay_equals_kernel_by_kernel_step():
         assert np.array_equal(out[0][0][k], out[1][0][k]), k
     assert out[0][1] == out[1][1] and out[0][2] == out[1][2]
     assert np.array_equal(out[0][3], out[1][3])
-
-
-def test_fused_density_equals_density_kernel():
-    """SPH_FUSED_DENSITY makes sph_step run the density pass inside the list build (k_cull<true>) instead of
-    k_density_l.  Same arithmetic in the same order: rho, Omega, counts and the state agree bit for bit."""
-    import torch
-    from paper_2603_19764_b200 import binding as B
-    out = []
-    for flag in (0, W.FLAG_FUSED_DENSITY):
-        wl = W.impact_pair(20000, W.SEED_BASE + 3, 100.0, 1.214)
-        wl.params.flags |= flag
-        s = B.Sph(wl.params, wl.n)
-        t = s.upload(wl)
-        for _ in range(3):
-            s.step(t, wl.n, 0.0)
-        torch.cuda.synchronize()
-        out.append({"rho": s.get_field("RHO").cpu().numpy(), "om": s.get_field("OMEGA").cpu().numpy(),
-                    "ng": s.get_field("NGATHER").cpu().numpy(), "x": t["x"].cpu().numpy().copy(),
-                    "S": t["Sxy"].cpu().numpy().copy(), "c": s.get_counters()})
-    for k in ("rho", "om", "ng", "x", "S"):
-        assert np.array_equal(out[0][k], out[1][k]), k
-    assert out[0]["c"]["pairs_gather"] == out[1]["c"]["pairs_gather"]
-    assert out[0]["c"]["tests_density"] == out[1]["c"]["tests_density"]
