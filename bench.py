@@ -89,10 +89,6 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the fused pair kernel, from the committed
-# `ncu --set full` capture of this command (profiles/, latest round-1 summary); None where no capture exists.
-NCU_TRAFFIC_BYTES = {"c2": 346.6e6}          # profiles/r01_v5_dense_flags_graph.md: 275.2 MB read + 71.4 MB written
-
 
 def rank_reduce(ms: float, units: float, device):
     """The N > 1 reduction of the contract: time = MAX over ranks, units = SUM over ranks (each rank
@@ -183,6 +179,38 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# Algorithmic HBM bytes per particle of the HBM-bound passes
+BYTES_PER_PARTICLE = {"predict": 120, "close": 230, "kickdrift": 160,
+                      # S1 with a full build: keys 12 r + 12 w, radix sort 4-5 digit passes x 24, reorder 116 r + 116 w
+                      "build_full": 24 + 5 * 24 + 232}
+
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch, from the committed `ncu --set full` captures of this
+# command (profiles/r02_*.md); None where no capture exists for the workload.
+NCU_TRAFFIC_BYTES = {}
+try:
+    with open(os.path.join(ROOT, "profiles", "r02_traffic.json")) as _f:
+        NCU_TRAFFIC_BYTES = json.load(_f)
+except OSError:
+    pass
+
+
+def _respawn_under_torchrun(args) -> int:
+    """`python bench.py --gpus N` with N > 1 and no torchrun around it: start the N replica ranks ourselves
+    (one process per GPU, NCCL only for the barrier and the max / sum over ranks)."""
+    import socket
+    import torch
+    have = torch.cuda.device_count()
+    if have < args.gpus:
+        sys.stderr.write("bench.py: --gpus %d asked, %d visible: refusing to time fewer GPUs than asked\n" % (args.gpus, have))
+        return 2
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -205,19 +233,27 @@ def run_ours(args):
     wl = make_workload(args.workload)
     if args.no_graph:
         wl.params.flags |= 64          # SPH_NO_GRAPH
+    if args.skin is not None:
+        wl.params.skin = args.skin
+    if args.rebuild_every is not None:
+        wl.params.rebuild_every = args.rebuild_every
     n = wl.n
     strength = bool(wl.params.flags & B.STRENGTH)
+    reuse = wl.params.skin > 0.0
+    every = (wl.params.rebuild_every if wl.params.rebuild_every > 0 else 8) if reuse else 1
     s = B.Sph(wl.params, n, device=dev)
     t = s.upload(wl)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB of L2
     working_set = s.workspace_bytes
-    do_flush = True
 
     def barrier():
         torch.cuda.synchronize(dev)
         if world > 1:
             dist.barrier()
             torch.cuda.synchronize(dev)
+
+    # ---- the FP32 CUDA-core rate this device sustains (FFMA chains) ----------------------
+    peak_measured = s.fp32_peak(5)
 
     # ---- device-resident timing -----------------------------------------------------------
     s.build_neighbors(t, n)
@@ -229,20 +265,30 @@ def run_ours(args):
     sampler.start()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     pass_ms = {k: 0.0 for k in B.T_SLOTS}
-    pairs_g = pairs_s = tests = 0
+    pass_full = {k: 0.0 for k in B.T_SLOTS}
+    pass_reuse = {k: 0.0 for k in B.T_SLOTS}
+    n_full = n_reuse = 0
+    pairs_g = pairs_s = entries = tests_cull = tests_cull_steps = dirty_max = 0
     barrier()
     for k in range(args.steps):
-        if do_flush:
-            flush.fill_(k & 0xff)
+        flush.fill_(k & 0xff)
+        # the library's schedule (sph_internal: step_is_full): the step after a full build is number 1 of `every`
+        is_full = (not reuse) or ((args.warmup + k + 1) % every == 0)
         ev[k][0].record(s.stream)
         s.step(None, 0, 0.0)
         ev[k][1].record(s.stream)
         tm = s.get_timings()                 # synchronises; outside the event pair of the next step
         for q in B.T_SLOTS:
             pass_ms[q] += tm[q]
+            (pass_full if is_full else pass_reuse)[q] += tm[q]
+        n_full += 1 if is_full else 0
+        n_reuse += 0 if is_full else 1
         c = s.get_counters()
         pairs_g += c["pairs_gather"]; pairs_s += c["pairs_symmetric"]
-        tests += c["tests_density"] + c["tests_force"]
+        entries += c["tests_density"] + c["tests_force"]
+        if is_full:
+            tests_cull += c["tests_cull"]; tests_cull_steps += 1
+        dirty_max = max(dirty_max, c["tiles_dirty"])
     barrier()
     launches = s.launch_count() - launches0
     step_ms = [a.elapsed_time(b) for a, b in ev]
@@ -279,6 +325,8 @@ def run_ours(args):
         del sh, th
 
     # ---- end to end through the host-buffer entry point -----------------------------------
+    del s, t
+    torch.cuda.empty_cache()
     host = {k: torch.from_numpy(v.copy()).pin_memory() for k, v in wl.arrays.items()}
     host["mat"] = torch.from_numpy(wl.mat.copy()).pin_memory()
     host["fixed"] = torch.from_numpy(wl.fixed.copy()).pin_memory()
@@ -306,20 +354,55 @@ def run_ours(args):
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant kernel (the fused gradient + force pair pass) --------------
+    # ---- rooflines ------------------------------------------------------------------------------
     sm_max = clocks.get("sm_max_mhz") or 1965.0
-    peak = fp32_peak_tflops(props.multi_processor_count, sm_max)
-    kern_ms = pass_ms["force"] / args.steps
+    peak_nominal = fp32_peak_tflops(props.multi_processor_count, sm_max)
+    peak = peak_measured if peak_measured > 0 else peak_nominal
+    hbm_peak, hbm_src = measured_hbm_gbs()
+    K = args.steps
+    step_avg = total_ms / K
+    traffic = NCU_TRAFFIC_BYTES.get(args.workload, {})
+
+    def alu_entry(kernel, pass_key, units, flops_per_unit, what):
+        ms = pass_ms[pass_key] / K
+        ach = units / K * flops_per_unit / (ms * 1e-3) / 1e12 if ms > 0 else 0.0
+        return {"kernel": kernel, "bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                "frac_of_nominal": ach / peak_nominal, "kernel_ms": ms, "share_of_step": ms / step_avg,
+                "work": what, "traffic": traffic.get(kernel), "traffic_unit": "bytes per launch"}
+
     flops_pair = FLOPS_PAIR_FUSED if strength else FLOPS_PAIR_HYDRO
-    achieved = (pairs_s / args.steps) * flops_pair / (kern_ms * 1e-3) / 1e12 if kern_ms > 0 else 0.0
-    roofline = {"bound": "alu", "kernel": "k_pair (fused Eq. 18-21 + 5-8)", "achieved": achieved,
-                "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "peak_source": "%d SMs x 128 FP32 lanes x 2 x %.0f MHz (guide's unit counts; no FP32 entry in "
-                               "MEASURED_PEAKS.json)" % (props.multi_processor_count, sm_max),
-                "flops_per_pair": flops_pair, "pairs_per_launch": pairs_s / args.steps,
-                "kernel_ms": kern_ms, "share_of_step": kern_ms / (total_ms / args.steps),
-                "candidate_hit_rate": pairs / tests if tests else None,
-                "traffic": NCU_TRAFFIC_BYTES.get(args.workload) if strength else None, "traffic_unit": "bytes per launch"}
+    k_pair = alu_entry("k_pair_l", "force", pairs_s, flops_pair,
+                       "%d flop per TRUE pair (gather counts exclude self), %.0f true pairs per launch"
+                       % (flops_pair, pairs_s / K))
+    k_dens = alu_entry("k_density_l", "density", pairs_g, FLOPS_PAIR_DENSITY,
+                       "%d flop-equivalents per gather pair incl. self (20 fp32 + 12 fp64 x 2)" % FLOPS_PAIR_DENSITY)
+    kernels = [k_pair, k_dens]
+    if n_full:
+        ms = pass_full["build"] / n_full
+        by = BYTES_PER_PARTICLE["build_full"] * n
+        kernels.append({"kernel": "S1 full build (keys, radix sort, k_permute, tree, k_cull, k_list_sort)", "bound": "hbm",
+                        "achieved": by / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                        "frac": by / (ms * 1e-3) / 1e9 / hbm_peak, "kernel_ms": ms,
+                        "share_of_step": pass_ms["build"] / K / step_avg, "steps_per_full_build": every,
+                        "work": "%d B per particle (SURVEY.md section 8d, S1)" % BYTES_PER_PARTICLE["build_full"],
+                        "traffic": traffic.get("k_cull"), "traffic_unit": "bytes per launch of k_cull"})
+    for key in ("predict", "close", "kickdrift"):
+        ms = pass_ms[key] / K
+        by = BYTES_PER_PARTICLE[key] * n
+        kernels.append({"kernel": "k_" + ("kick_drift" if key == "kickdrift" else key), "bound": "hbm",
+                        "achieved": by / (ms * 1e-3) / 1e9 if ms > 0 else 0.0, "peak": hbm_peak, "unit": "GB/s",
+                        "frac": (by / (ms * 1e-3) / 1e9 / hbm_peak) if ms > 0 else 0.0, "kernel_ms": ms,
+                        "share_of_step": ms / step_avg, "work": "%d B per particle" % BYTES_PER_PARTICLE[key]})
+    roofline = dict(k_pair)
+    roofline.update({"kernel": "k_pair_l<1,1,1> (fused Eq. 18-21 + 5-8)" if strength else "k_pair_l<0,1,0>",
+                     "peak_source": "sph_fp32_peak: FFMA chains measured in this run (nominal %d SMs x 128 lanes x 2 x %.0f MHz = %.1f)"
+                                    % (props.multi_processor_count, sm_max, peak_nominal),
+                     "peak_nominal": peak_nominal, "peak_measured": peak_measured, "hbm_peak_source": hbm_src,
+                     "flops_per_pair": flops_pair, "pairs_per_launch": pairs_s / K,
+                     "list_entries_per_true_pair": entries / pairs if pairs else None,
+                     "cull_tests_per_true_pair": (tests_cull / tests_cull_steps) / (pairs_s / K) if tests_cull_steps and pairs_s else None,
+                     "candidate_hit_rate": (pairs_s / K) / (tests_cull / tests_cull_steps) if tests_cull else None,
+                     "kernels": kernels})
 
     # ---- the oracle beside it ------------------------------------------------------------------
     cpu = None
@@ -339,13 +422,20 @@ def run_ours(args):
                    "mean_neighbours": pairs_s / args.steps / max(n, 1),
                    "l2": "flushed between steps (256 MiB fill outside the timed events)",
                    "working_set_bytes": working_set, "parallelism": "replicas x%d" % world,
-                   "cuda_graph": not args.no_graph},
+                   "cuda_graph": not args.no_graph,
+                   "list_reuse": {"skin": wl.params.skin, "full_build_every": every, "full_steps_timed": n_full,
+                                  "reuse_steps_timed": n_reuse, "dirty_tiles_max": dirty_max,
+                                  "tiles": (n + 255) // 256} if reuse else None},
         "particle_steps_per_s": world * n * args.steps / (total_ms_max * 1e-3),
         "pass_ms": {k: v / args.steps for k, v in pass_ms.items()},
+        "pass_ms_full_step": {k: v / n_full for k, v in pass_full.items()} if n_full else None,
+        "pass_ms_reuse_step": {k: v / n_reuse for k, v in pass_reuse.items()} if n_reuse else None,
+        "ms_per_step_min_max": [min(step_ms), max(step_ms)],
         "gpu_launches": launches,
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": "pairs/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s_max / e2e_steps},
+                "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s_max / e2e_steps,
+                "note": "every host-buffer step ingests the caller's positions: a full neighbour build per step"},
         "roofline": roofline,
         "cpu_baseline": cpu,
         "hydro_only": hydro,
@@ -355,19 +445,33 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def measured_hbm_gbs():
+    """MEASURED_PEAKS.json (driver-written) if present, else the profiling guide's fallback."""
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+    except (OSError, KeyError, ValueError):
+        return 6650.0, "of fallback (B200_PROFILING.md; MEASURED_PEAKS.json absent)"
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=16)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="c2", choices=["c0", "c1", "c2", "c3", "c4"])
+    ap.add_argument("--workload", default="c4", choices=["c0", "c1", "c2", "c3", "c4"],
+                    help="BASELINE.json configs[k]; default: the largest single-GPU configuration")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-hydro-only", action="store_true")
     ap.add_argument("--no-graph", action="store_true", help="launch the step kernel by kernel (A/B of the CUDA graph)")
+    ap.add_argument("--skin", type=float, default=None, help="list reuse: skin as a fraction of H (0 = off; A/B)")
+    ap.add_argument("--rebuild-every", type=int, default=None, help="list reuse: steps between full builds (A/B)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(_respawn_under_torchrun(args))
     else:
         run_ours(args)
 

@@ -110,6 +110,8 @@ enum { SPH_C_PAIRS_GATHER = 0,   /* sum_i |gather set(i)|   (true pairs of the d
        SPH_C_OMEGA_SMALL,        /* particles with |Omega| < 0.1 in the last density pass (Eq. 3): too few
                                     neighbours for the grad-h terms; sph_adapt_h is the method's remedy     */
        SPH_C_NONFINITE,          /* particles whose a, du/dt or dS/dt was not finite in the last CLOSE      */
+       SPH_C_TILES_DIRTY,        /* sph_params.skin > 0: tiles whose lists are rebuilt in every step since the
+                                    last full build (0 right after one)                                      */
        SPH_C_COUNT };
 
 typedef struct sph_ctx sph_ctx;   /* opaque, library-owned (host memory) */
@@ -136,6 +138,17 @@ typedef struct sph_params {
                                   particle may have (8 bytes of workspace per particle and unit);
                                   <= 0 selects 64 (256 neighbours).  Tiles that need more are served by
                                   the tree-walk kernels and counted in SPH_C_LIST_OVERFLOW.           */
+    float skin;                /* list reuse inside sph_step: > 0: a full neighbour build
+                                  (re-sort + lists) keeps every pair within (1 + skin) of its cut-off, and the
+                                  following steps reuse those lists -- the exact fp32 predicate (reading Q4) is
+                                  evaluated on the current positions inside the pair passes, so the neighbour
+                                  SETS are the same as with skin = 0 -- until the next full build; tiles whose
+                                  surroundings moved by more than skin * H against them are rebuilt in every
+                                  step (SPH_C_TILES_DIRTY).  <= 0: every step is a full build.             */
+    int rebuild_every;         /* skin > 0: steps from one full build to the next (<= 0 selects 8)          */
+    int adapt_h_every;         /* > 0: sph_step runs one iteration of sph_adapt_h (Eq. 2)
+                                  every adapt_h_every steps, before the neighbour build of that step, with  */
+    float adapt_h_target;      /* ... this n_target (the method's remedy for Omega -> 0, SPH_C_OMEGA_SMALL)  */
 } sph_params;
 
 /* NEXT-3: a tabulated EOS for one material (P and T are computed from rho and u by the EOS

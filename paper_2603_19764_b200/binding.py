@@ -25,7 +25,7 @@ F = dict(RHO=0, OMEGA=1, P=2, CS=3, T=4, GAMMA=5, Y=6, MUMAX=7, DUDT=8, DT=9, EA
          CFLAG=13, NGATHER=14, NSYMMETRIC=15, H=16, A=32, V=36, X=40, SPRED=48, S=56, DSDT=64, F=80, CINV=96, G=112)
 T_SLOTS = ("build", "density", "predict", "gradient", "force", "close", "kickdrift", "step")
 C_SLOTS = ("pairs_gather", "pairs_symmetric", "tests_density", "tests_force", "cfallback", "tests_cull",
-           "candidates", "list_overflow", "bad_material", "omega_small", "nonfinite")
+           "candidates", "list_overflow", "bad_material", "omega_small", "nonfinite", "tiles_dirty")
 
 FLOAT_FIELDS = ("x", "y", "z", "m", "h", "vx", "vy", "vz", "u", "Sxx", "Syy", "Sxy", "Sxz", "Syz")
 OPT_FIELDS = ("gx", "gy", "gz")
@@ -51,7 +51,8 @@ class sph_material(C.Structure):
 class sph_params(C.Structure):
     _fields_ = [("kappa", C.c_float), ("alpha", C.c_float), ("beta", C.c_float), ("eps_av", C.c_float),
                 ("eta_C", C.c_float), ("eta_a", C.c_float), ("n_materials", C.c_int), ("flags", C.c_uint),
-                ("mat", sph_material * MAX_MATERIALS), ("list_budget", C.c_int)]
+                ("mat", sph_material * MAX_MATERIALS), ("list_budget", C.c_int),
+                ("skin", C.c_float), ("rebuild_every", C.c_int), ("adapt_h_every", C.c_int), ("adapt_h_target", C.c_float)]
 
 
 class sph_state(C.Structure):
@@ -146,6 +147,10 @@ def make_params(p) -> sph_params:
     out.eta_C, out.eta_a = p.eta_C, p.eta_a
     out.flags = int(p.flags)
     out.list_budget = int(getattr(p, "list_budget", 0))
+    out.skin = float(getattr(p, "skin", 0.0))
+    out.rebuild_every = int(getattr(p, "rebuild_every", 0))
+    out.adapt_h_every = int(getattr(p, "adapt_h_every", 0))
+    out.adapt_h_target = float(getattr(p, "adapt_h_target", 0.0))
     out.n_materials = len(p.materials)
     for k, m in enumerate(p.materials):
         for name, _ in sph_material._fields_:

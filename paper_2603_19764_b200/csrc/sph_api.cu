@@ -53,7 +53,13 @@ static int device_sm_count()
     return sm_count_cached;
 }
 
-static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap, bool lists)
+static float skin_of(const sph_params *p)
+{
+    if (!(p->skin > 0.f) || (p->flags & SPH_NO_LISTS)) return 0.f;
+    return p->skin > 0.5f ? 0.5f : p->skin;
+}
+
+static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap, bool lists, float skin)
 {
     const int sm_count = device_sm_count();
     Bump b{base, 0};
@@ -73,7 +79,11 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
         size_t c = L < nlev ? (size_t)count[L] : 1;
         o.tree.lo[L] = b.take<float4>(c);
         o.tree.hi[L] = b.take<float4>(c);
+        o.tree.dlo[L] = b.take<float4>(skin > 0.f ? c : 1);
+        o.tree.dhi[L] = b.take<float4>(skin > 0.f ? c : 1);
     }
+    o.skin = skin;
+    o.xref = b.take<float4>(skin > 0.f ? N : 1);
     for (int k = 0; k < 3; ++k) o.vfull[k] = b.take<float>(N);
     o.ufull = b.take<float>(N);
     for (int k = 0; k < 5; ++k) o.Sfull[k] = b.take<float>(N);
@@ -100,9 +110,11 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
     o.heavy_list = b.take<unsigned>(o.heavy_cap);
     o.nheavy = b.take<unsigned>(1);
     o.heavy_mark = b.take<unsigned char>(ntile);
-    o.cand_cursor = b.take<unsigned long long>(1);
+    o.tile_dirty = b.take<unsigned char>(ntile);
+    o.cand_cursor = b.take<unsigned long long>(2);
     o.cand_cap = lists ? (unsigned long long)ntile * (2 * SPH_SE) : 1;   // pool: twice the one-round average
-    o.cand = b.take<unsigned>((size_t)o.cand_cap);
+    o.cand_cap_dirty = (lists && skin > 0.f) ? (unsigned long long)ntile * SPH_SE : 0;
+    o.cand = b.take<unsigned>((size_t)(o.cand_cap + o.cand_cap_dirty));
     o.rows_cap = kcap;
     o.rowptr = b.take<unsigned short>(lists ? nchunk * (SPH_MAXROUND + 1) : 1);
     o.nlist = b.take<uint2>(lists ? nchunk * (size_t)kcap * 32 : 1);
@@ -136,7 +148,7 @@ static bool params_ok(const sph_params *p)
 extern "C" size_t sph_workspace_bytes(const sph_params *params, long long n_max)
 {
     if (!params_ok(params) || n_max < 0 || n_max > 2000000000ll) return 0;
-    return carve(nullptr, nullptr, nullptr, n_max, kcap_of(params), !(params->flags & SPH_NO_LISTS));
+    return carve(nullptr, nullptr, nullptr, n_max, kcap_of(params), !(params->flags & SPH_NO_LISTS), skin_of(params));
 }
 
 extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max, void *workspace,
@@ -146,7 +158,7 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
     *out = nullptr;
     if (!params_ok(params) || n_max < 0 || n_max > 2000000000ll || !workspace) return SPH_EINVAL;
     if (((uintptr_t)workspace & 255u) != 0) return SPH_EINVAL;
-    size_t need = carve(nullptr, nullptr, nullptr, n_max, kcap_of(params), !(params->flags & SPH_NO_LISTS));
+    size_t need = carve(nullptr, nullptr, nullptr, n_max, kcap_of(params), !(params->flags & SPH_NO_LISTS), skin_of(params));
     if (workspace_bytes < need) return SPH_ENOMEM;
     sph_ctx *c = new (std::nothrow) sph_ctx();
     if (!c) return SPH_ENOMEM;
@@ -160,7 +172,9 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
     // a capture cannot be taken on the legacy default stream
     c->use_graph = !(params->flags & SPH_NO_GRAPH) && cuda_stream != nullptr && (cudaStream_t)cuda_stream != cudaStreamLegacy
                    && (cudaStream_t)cuda_stream != cudaStreamPerThread;
-    c->ws_bytes = carve(&c->d, &c->stage, (char *)workspace, n_max, kcap_of(params), c->use_lists);
+    c->ws_bytes = carve(&c->d, &c->stage, (char *)workspace, n_max, kcap_of(params), c->use_lists, skin_of(params));
+    c->rebuild_every = params->rebuild_every > 0 ? params->rebuild_every : 8;
+    c->force_full = true;
     c->d.n = 0; c->d.nchunk = 0;
     for (int k = 0; k < 2 * SPH_T_COUNT; ++k) {
         cudaError_t e = cudaEventCreate(&c->ev[k]);
@@ -178,6 +192,7 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
         if (e == cudaSuccess) e = cudaMemsetAsync(c->d.cull_cycles, 0, sizeof(unsigned long long), c->stream);
         if (e == cudaSuccess) e = cudaMemsetAsync(c->d.nheavy, 0, sizeof(unsigned), c->stream);
         if (e == cudaSuccess) e = cudaMemsetAsync(c->d.heavy_mark, 0, ntile, c->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d.tile_dirty, 0, ntile, c->stream);
     }
     if (e == cudaSuccess) e = cudaMemsetAsync(c->d.dt_next, 0, sizeof(float), c->stream);
     if (e != cudaSuccess) { sph_destroy(c); return SPH_ECUDA; }
@@ -188,7 +203,8 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
 static void drop_graphs(sph_ctx *c)
 {
     for (int k = 0; k < 2; ++k)
-        if (c->gexec[k]) { cudaGraphExecDestroy(c->gexec[k]); c->gexec[k] = nullptr; }
+        for (int s = 0; s < 2; ++s)
+            if (c->gexec[k][s]) { cudaGraphExecDestroy(c->gexec[k][s]); c->gexec[k][s] = nullptr; }
 }
 
 extern "C" void sph_destroy(sph_ctx *c)
@@ -248,9 +264,30 @@ extern "C" int sph_build_neighbors(sph_ctx *c, const sph_state *state, long long
     }
     c->have_density = c->have_predict = c->have_grad = c->have_force = false;
     if (c->use_lists) {
-        rc = sph_launch_cull(c);
+        rc = sph_launch_set_ref(c);          // list reuse: the positions this full build refers to
+        if (rc) return rc;
+        rc = sph_launch_cull(c, false);
         if (rc) return rc;
     }
+    c->steps_since_full = 0;
+    c->force_full = false;
+    return SPH_OK;
+}
+
+// The neighbour structure of a step that REUSES the lists of the last full build (sph_params.skin > 0): chunk
+// boxes and tree at the current positions (with the displacement boxes), the check of every tile, and the
+// rebuild of the dirty ones.  The particle order stays.
+static int reuse_neighbors(sph_ctx *c)
+{
+    PassTimer t(c, SPH_T_BUILD);
+    int rc = sph_launch_tree(c);
+    if (rc) return rc;
+    rc = sph_launch_check(c);
+    if (rc) return rc;
+    rc = sph_launch_cull(c, true);
+    if (rc) return rc;
+    c->have_density = c->have_predict = c->have_grad = c->have_force = false;
+    c->steps_since_full++;
     return SPH_OK;
 }
 
@@ -282,8 +319,11 @@ extern "C" int sph_adapt_h(sph_ctx *c, float n_target, int iterations, float *ma
         rc = sph_launch_tree(c);
         if (rc) return rc;
         if (c->use_lists) {
-            rc = sph_launch_cull(c);
+            rc = sph_launch_set_ref(c);
             if (rc) return rc;
+            rc = sph_launch_cull(c, false);
+            if (rc) return rc;
+            c->steps_since_full = 0;
         }
         c->have_density = c->have_predict = c->have_grad = c->have_force = false;
     }
@@ -367,6 +407,12 @@ static int derivative_passes(sph_ctx *c)
     return sph_gradients_forces(c);
 }
 
+// does the next step rebuild everything (re-sort, full list build) or reuse the lists?
+static bool step_is_full(const sph_ctx *c)
+{
+    return !(c->d.skin > 0.f) || !c->use_lists || c->force_full || c->steps_since_full + 1 >= c->rebuild_every;
+}
+
 static int step_body(sph_ctx *c, sph_state *state, long long n, float dt, float *dt_used)
 {
     int rc;
@@ -389,7 +435,7 @@ static int step_body(sph_ctx *c, sph_state *state, long long n, float dt, float 
         rc = sph_launch_kick_drift(c, dt);
         if (rc) return rc;
     }
-    rc = sph_build_neighbors(c, nullptr, 0);
+    rc = step_is_full(c) ? sph_build_neighbors(c, nullptr, 0) : reuse_neighbors(c);
     if (rc) return rc;
     rc = derivative_passes(c);
     if (rc) return rc;
@@ -412,12 +458,18 @@ extern "C" int sph_step(sph_ctx *c, sph_state *state, long long n, float dt, flo
     if (!c) return SPH_EINVAL;
     const bool graphable = c->use_graph && c->resident && c->have_derivs && !state && !(dt > 0.f) && c->d.n > 0;
     if (!graphable) return step_body(c, state, n, dt, dt_used);
+    const int kind = step_is_full(c) ? 0 : 1;       // a step with a full build (re-sort) or one that reuses the lists
     const int s = c->parity;
-    if (c->gexec[s] && (c->gkey_n[s] != c->d.n || c->gkey_dtused[s] != (const void *)dt_used)) {
-        cudaGraphExecDestroy(c->gexec[s]);
-        c->gexec[s] = nullptr;
+    if (c->gexec[kind][s] && (c->gkey_n[kind][s] != c->d.n || c->gkey_dtused[kind][s] != (const void *)dt_used)) {
+        cudaGraphExecDestroy(c->gexec[kind][s]);
+        c->gexec[kind][s] = nullptr;
     }
-    if (!c->gexec[s]) {
+    if (!c->gexec[kind][s]) {
+        // everything step_body changes on the host, in case the capture fails half way (no kernel has run then)
+        const Resident r0 = c->d.r, alt0 = c->d.alt;
+        const int parity0 = c->parity, since0 = c->steps_since_full;
+        const bool force0 = c->force_full, hd = c->have_density, hp = c->have_predict, hg = c->have_grad,
+                   hf = c->have_force, hv = c->have_derivs;
         cudaGraph_t g = nullptr;
         const long long l0 = c->launches;
         SPH_CUDA(c, cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal));
@@ -425,26 +477,39 @@ extern "C" int sph_step(sph_ctx *c, sph_state *state, long long n, float dt, flo
         const int rc = step_body(c, nullptr, 0, dt, dt_used);         // records; runs nothing
         c->capturing = false;
         cudaError_t e = cudaStreamEndCapture(c->stream, &g);
-        if (rc || e != cudaSuccess || !g) {
-            if (g) cudaGraphDestroy(g);
-            c->last_cuda = (int)e;
-            return rc ? rc : SPH_ECUDA;
+        if (!rc && e == cudaSuccess && g) {
+            e = cudaGraphInstantiate(&c->gexec[kind][s], g, 0);
+            if (e != cudaSuccess) c->gexec[kind][s] = nullptr;
         }
-        e = cudaGraphInstantiate(&c->gexec[s], g, 0);
-        cudaGraphDestroy(g);
-        if (e != cudaSuccess) { c->gexec[s] = nullptr; c->last_cuda = (int)e; return SPH_ECUDA; }
-        c->glaunches[s] = c->launches - l0;
-        c->gkey_n[s] = c->d.n;
-        c->gkey_dtused[s] = (const void *)dt_used;
-        SPH_CUDA(c, cudaGraphLaunch(c->gexec[s], c->stream));         // the host effects were applied by step_body
+        if (g) cudaGraphDestroy(g);
+        if (rc || e != cudaSuccess || !c->gexec[kind][s]) {
+            c->d.r = r0; c->d.alt = alt0; c->parity = parity0; c->steps_since_full = since0; c->force_full = force0;
+            c->have_density = hd; c->have_predict = hp; c->have_grad = hg; c->have_force = hf; c->have_derivs = hv;
+            c->launches = l0;
+            (void)cudaGetLastError();
+            if (rc) return rc;
+            c->last_cuda = (int)e;
+            c->use_graph = false;                                     // from now on kernel by kernel
+            return step_body(c, state, n, dt, dt_used);
+        }
+        c->glaunches[kind][s] = c->launches - l0;
+        c->gkey_n[kind][s] = c->d.n;
+        c->gkey_dtused[kind][s] = (const void *)dt_used;
+        SPH_CUDA(c, cudaGraphLaunch(c->gexec[kind][s], c->stream));   // the host effects were applied by step_body
         return SPH_OK;
     }
-    SPH_CUDA(c, cudaGraphLaunch(c->gexec[s], c->stream));
+    SPH_CUDA(c, cudaGraphLaunch(c->gexec[kind][s], c->stream));
     {                                                                 // what step_body does on the host
         Dev &d = c->d;
-        Resident t = d.r; d.r = d.alt; d.alt = t;
-        c->parity ^= 1;
-        c->launches += c->glaunches[s];
+        if (kind == 0) {
+            Resident t = d.r; d.r = d.alt; d.alt = t;
+            c->parity ^= 1;
+            c->steps_since_full = 0;
+            c->force_full = false;
+        } else {
+            c->steps_since_full++;
+        }
+        c->launches += c->glaunches[kind][s];
         c->have_density = c->have_predict = c->have_force = c->have_derivs = true;
         c->have_grad = (c->p.flags & SPH_STRENGTH) != 0;
         for (int k = 0; k < SPH_T_COUNT; ++k) c->ev_used[k] = c->ev_used[k] || k != SPH_T_GRADIENT;
@@ -504,6 +569,7 @@ extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, f
     if (c->resident && n > 0) {
         k_refresh<<<sph_div_up(n, 256), 256, 0, c->stream>>>(c->d, ds);
         c->launches++;
+        c->force_full = true;                 // the caller's positions: nothing the lists were built on holds
         SPH_CUDA(c, cudaGetLastError());
     }
     rc = sph_step(c, &ds, n, dt, nullptr);

@@ -183,8 +183,10 @@ __global__ void __launch_bounds__(256) k_permute(Dev d, const unsigned *__restri
 }
 
 // ------------------------------------------------------------------------------------------
-// chunk boxes (level 0) and inner levels of the implicit tree
+// chunk boxes (level 0) and inner levels of the implicit tree.  DISP (list reuse, Dev::skin > 0): also the
+// box of the displacements x - xref since the last full list build and the smallest H of the node.
 // ------------------------------------------------------------------------------------------
+template <bool DISP>
 __global__ void __launch_bounds__(256) k_chunk_boxes(Dev d, float kappa)
 {
     int chunk = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -192,10 +194,16 @@ __global__ void __launch_bounds__(256) k_chunk_boxes(Dev d, float kappa)
     int lane = threadIdx.x & 31;
     long long i = (long long)chunk * SPH_CHUNK + lane;
     float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, H = 0.f;
+    float dl[3] = {3.0e38f, 3.0e38f, 3.0e38f}, dh[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, Hmin = 3.0e38f;
     if (i < d.n) {
         float4 q = d.r.pm[i];
         lo[0] = hi[0] = q.x; lo[1] = hi[1] = q.y; lo[2] = hi[2] = q.z;
         H = sph_H(kappa, d.r.vh[i].w);
+        if (DISP) {
+            const float4 r = d.xref[i];
+            dl[0] = dh[0] = q.x - r.x; dl[1] = dh[1] = q.y - r.y; dl[2] = dh[2] = q.z - r.z;
+            Hmin = H;
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -203,15 +211,25 @@ __global__ void __launch_bounds__(256) k_chunk_boxes(Dev d, float kappa)
         for (int a = 0; a < 3; ++a) {
             lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
             hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+            if (DISP) {
+                dl[a] = fminf(dl[a], __shfl_xor_sync(0xffffffffu, dl[a], o));
+                dh[a] = fmaxf(dh[a], __shfl_xor_sync(0xffffffffu, dh[a], o));
+            }
         }
         H = fmaxf(H, __shfl_xor_sync(0xffffffffu, H, o));
+        if (DISP) Hmin = fminf(Hmin, __shfl_xor_sync(0xffffffffu, Hmin, o));
     }
     if (lane == 0) {
         d.tree.lo[0][chunk] = make_float4(lo[0], lo[1], lo[2], H);
         d.tree.hi[0][chunk] = make_float4(hi[0], hi[1], hi[2], 0.f);
+        if (DISP) {
+            d.tree.dlo[0][chunk] = make_float4(dl[0], dl[1], dl[2], Hmin);
+            d.tree.dhi[0][chunk] = make_float4(dh[0], dh[1], dh[2], 0.f);
+        }
     }
 }
 
+template <bool DISP>
 __global__ void __launch_bounds__(256) k_tree_level(Tree t, int L)
 {
     int node = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
@@ -219,10 +237,16 @@ __global__ void __launch_bounds__(256) k_tree_level(Tree t, int L)
     int lane = threadIdx.x & 31;
     int child = node * SPH_ARITY + lane;
     float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, H = 0.f;
+    float dl[3] = {3.0e38f, 3.0e38f, 3.0e38f}, dh[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, Hmin = 3.0e38f;
     if (child < t.count[L - 1]) {
         float4 a = t.lo[L - 1][child], b = t.hi[L - 1][child];
         lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; H = a.w;
         hi[0] = b.x; hi[1] = b.y; hi[2] = b.z;
+        if (DISP) {
+            a = t.dlo[L - 1][child]; b = t.dhi[L - 1][child];
+            dl[0] = a.x; dl[1] = a.y; dl[2] = a.z; Hmin = a.w;
+            dh[0] = b.x; dh[1] = b.y; dh[2] = b.z;
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -230,13 +254,29 @@ __global__ void __launch_bounds__(256) k_tree_level(Tree t, int L)
         for (int a = 0; a < 3; ++a) {
             lo[a] = fminf(lo[a], __shfl_xor_sync(0xffffffffu, lo[a], o));
             hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xffffffffu, hi[a], o));
+            if (DISP) {
+                dl[a] = fminf(dl[a], __shfl_xor_sync(0xffffffffu, dl[a], o));
+                dh[a] = fmaxf(dh[a], __shfl_xor_sync(0xffffffffu, dh[a], o));
+            }
         }
         H = fmaxf(H, __shfl_xor_sync(0xffffffffu, H, o));
+        if (DISP) Hmin = fminf(Hmin, __shfl_xor_sync(0xffffffffu, Hmin, o));
     }
     if (lane == 0) {
         t.lo[L][node] = make_float4(lo[0], lo[1], lo[2], H);
         t.hi[L][node] = make_float4(hi[0], hi[1], hi[2], 0.f);
+        if (DISP) {
+            t.dlo[L][node] = make_float4(dl[0], dl[1], dl[2], Hmin);
+            t.dhi[L][node] = make_float4(dh[0], dh[1], dh[2], 0.f);
+        }
     }
+}
+
+// the reference positions of the list reuse: xref = x (at a full list build)
+__global__ void __launch_bounds__(256) k_set_ref(Dev d)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i < d.n) d.xref[i] = d.r.pm[i];
 }
 
 // ------------------------------------------------------------------------------------------
@@ -280,12 +320,25 @@ int sph_launch_tree(sph_ctx *c)
 {
     Dev &d = c->d;
     if (d.n == 0) return SPH_OK;
-    k_chunk_boxes<<<sph_div_up(d.nchunk, 8), 256, 0, c->stream>>>(d, c->p.kappa);
+    const bool disp = d.skin > 0.f;
+    if (disp) k_chunk_boxes<true><<<sph_div_up(d.nchunk, 8), 256, 0, c->stream>>>(d, c->p.kappa);
+    else k_chunk_boxes<false><<<sph_div_up(d.nchunk, 8), 256, 0, c->stream>>>(d, c->p.kappa);
     c->launches++;
     for (int L = 1; L < d.tree.nlev; ++L) {
-        k_tree_level<<<sph_div_up(d.tree.count[L], 8), 256, 0, c->stream>>>(d.tree, L);
+        if (disp) k_tree_level<true><<<sph_div_up(d.tree.count[L], 8), 256, 0, c->stream>>>(d.tree, L);
+        else k_tree_level<false><<<sph_div_up(d.tree.count[L], 8), 256, 0, c->stream>>>(d.tree, L);
         c->launches++;
     }
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_set_ref(sph_ctx *c)
+{
+    Dev &d = c->d;
+    if (d.n == 0 || !(d.skin > 0.f)) return SPH_OK;
+    k_set_ref<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d);
+    c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
 }

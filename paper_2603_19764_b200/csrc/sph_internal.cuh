@@ -62,11 +62,15 @@ struct Resident {
 
 // Implicit 32-ary tree over the Morton-sorted chunk array: node k of level L covers chunks
 // [k 32^L, (k+1) 32^L).  lo.w = max H of the node, hi.w unused.
+// dlo / dhi (list reuse, see Dev::skin): per node the box of the DISPLACEMENTS x - xref of its particles since
+// the last full list build; dlo.w = smallest support radius H in the node.
 struct Tree {
     int nlev;                        // levels stored; level nlev-1 has <= 32 nodes
     int count[SPH_MAX_LEVELS];
     float4 *lo[SPH_MAX_LEVELS];
     float4 *hi[SPH_MAX_LEVELS];
+    float4 *dlo[SPH_MAX_LEVELS];
+    float4 *dhi[SPH_MAX_LEVELS];
 };
 
 // Everything the kernels need, passed by value.
@@ -90,8 +94,16 @@ struct Dev {
     int *tile_ncand;                        // candidates per tile
     unsigned *cand;                         // candidate pool: global indices, tile after tile, ascending per tile
     unsigned long long *tile_off;           // where each tile's candidates start in the pool
-    unsigned long long *cand_cursor;        // bump allocator of the pool
-    unsigned long long cand_cap;            // pool capacity (entries)
+    unsigned long long *cand_cursor;        // bump allocators of the pool: [0] full builds, [1] per-step rebuilds of dirty tiles
+    unsigned long long cand_cap;            // pool capacity (entries) of a full build; the entries behind it
+    unsigned long long cand_cap_dirty;      //   serve the dirty tiles of the steps in between
+    // list reuse (sph_params.skin > 0): the lists of a full build hold every pair within (1 + skin) of its
+    // cut-off and stay in use, with the exact predicate evaluated in the pair passes, until the next full
+    // build; a tile whose surroundings moved too much against it (k_check) is DIRTY: its lists are rebuilt
+    // at the current positions in every step until then
+    float skin;                             // 0: off (every step is a full build)
+    float4 *xref;                           // positions at the last full build (current sorted order)
+    unsigned char *tile_dirty;              // sticky until the next full build
     uint2 *nlist;                           // [chunk][row-group][lane]: 4 x u16 per lane = byte offsets (slot * 16)
                                             // into the round's staged arrays; 0xFFFF = no entry
     int rows_cap;                           // row-groups reserved per chunk
@@ -133,10 +145,15 @@ struct sph_ctx {
     // ping-pong (the kernels take the array pointers by value); see sph_step
     bool use_graph, capturing;
     int parity;                      // which half of the ping-pong is current
-    cudaGraphExec_t gexec[2];
-    long long glaunches[2];          // launches one replay stands for
-    long long gkey_n[2];
-    const void *gkey_dtused[2];
+    // graphs of the resident step: [kind][parity], kind 0 = step with a full list build (re-sort), 1 = step that
+    // reuses the lists
+    cudaGraphExec_t gexec[2][2];
+    long long glaunches[2][2];       // launches one replay stands for
+    long long gkey_n[2][2];
+    const void *gkey_dtused[2][2];
+    int rebuild_every;               // steps between two full list builds when skin > 0
+    int steps_since_full;            // steps taken since the last full build
+    bool force_full;                 // the next step must do a full build (state refreshed, h changed, ...)
     bool resident, have_density, have_predict, have_grad, have_force, have_derivs;
     cudaEvent_t ev[2 * SPH_T_COUNT];
     bool ev_used[SPH_T_COUNT];
@@ -161,6 +178,8 @@ size_t sph_cub_temp_bytes(long long n_max);
 int sph_launch_ingest(sph_ctx *c, const sph_state *st, long long n);
 int sph_launch_resort(sph_ctx *c);
 int sph_launch_tree(sph_ctx *c);
+int sph_launch_set_ref(sph_ctx *c);
+int sph_launch_check(sph_ctx *c);
 int sph_launch_density(sph_ctx *c, bool flagged_only);
 int sph_launch_pair(sph_ctx *c, bool grad, bool force, bool flagged_only);
 int sph_launch_predict(sph_ctx *c);
@@ -173,7 +192,8 @@ int sph_launch_diagnostics(sph_ctx *c, double *out);
 int sph_launch_h_update(sph_ctx *c, float n_target);
 int sph_launch_neighbors(sph_ctx *c, int which, int *counts, const long long *offsets, int *list, bool flagged_only);
 int sph_launch_download(sph_ctx *c, sph_state *st);
-int sph_launch_cull(sph_ctx *c);
+int sph_launch_cull(sph_ctx *c, bool dirty_only);
+int sph_launch_list_sort(sph_ctx *c);
 int sph_launch_density_l(sph_ctx *c);
 int sph_launch_pair_l(sph_ctx *c, bool grad, bool force);
 int sph_launch_neighbors_l(sph_ctx *c, int which, int *counts, const long long *offsets, int *list);

@@ -130,7 +130,11 @@ __device__ __forceinline__ int scan_popc(const unsigned *mask, unsigned short *o
     return __shfl_sync(FULL, incl, 31);
 }
 
-__global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile)
+// infl2 = (1 + skin)^2 (1 with no list reuse): every support radius of this kernel -- box reaches and the exact
+// test alike -- is inflated by 1 + skin, so that the lists hold every pair with r < (1 + skin) max(H_i, H_j) and
+// the pair passes, which evaluate the exact predicate themselves, can go on using them while the particles move.
+// dirty: only the tiles k_check marked (their candidates go to the second region of the pool).
+__global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float infl, float infl2, int ntile, int dirty)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     CullSmem &sm = *reinterpret_cast<CullSmem *>(smem_raw);
@@ -139,7 +143,14 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     {
     const int tile = sph_tile_of_block(d, blockIdx.x);
     if (tile < 0 || tile >= ntile) return;
+    if (dirty) {
+        if (!d.tile_dirty[tile]) return;
+    } else if (d.skin > 0.f && threadIdx.x == 0) {
+        d.tile_dirty[tile] = 0;
+    }
     const long long t_begin = clock64();
+    // SPH_C_LIST_OVERFLOW counts the tiles that are flagged NOW: a rebuilt dirty tile may change sides
+    const int was_flagged = (dirty && d.tile_flag[tile]) ? 1 : 0;
     const int chunk0 = tile * SPH_TILE_CHUNKS;
     const int nch = min(SPH_TILE_CHUNKS, d.nchunk - chunk0);
 
@@ -149,10 +160,10 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     // lanes without a particle sit where every r2 overflows to +inf (and differs from the table sentinel)
     const float4 pi = valid ? d.r.pm[i] : make_float4(-1.0e30f, -1.0e30f, -1.0e30f, 0.f);
     const float Hi = sph_H(kappa, valid ? d.r.vh[i].w : 1.f);
-    const float H2i = valid ? __fmul_rn(Hi, Hi) : -1.f;
+    const float H2i = valid ? __fmul_rn(__fmul_rn(Hi, Hi), infl2) : -1.f;
     {
         float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, Hm = 0.f;
-        if (valid) { lo[0] = hi[0] = pi.x; lo[1] = hi[1] = pi.y; lo[2] = hi[2] = pi.z; Hm = Hi; }
+        if (valid) { lo[0] = hi[0] = pi.x; lo[1] = hi[1] = pi.y; lo[2] = hi[2] = pi.z; Hm = Hi * infl; }
 #pragma unroll
         for (int o = 4; o > 0; o >>= 1) {
 #pragma unroll
@@ -167,7 +178,9 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
                             sm.gc[4 * warp + (lane >> 3)], sm.ge[4 * warp + (lane >> 3)]);
     }
     if (threadIdx.x < nch) {
-        const float4 lo = d.tree.lo[0][chunk0 + threadIdx.x], hi = d.tree.hi[0][chunk0 + threadIdx.x];
+        float4 lo = d.tree.lo[0][chunk0 + threadIdx.x];
+        const float4 hi = d.tree.hi[0][chunk0 + threadIdx.x];
+        lo.w *= infl;
         sm.blo[threadIdx.x] = lo;
         sm.bhi[threadIdx.x] = hi;
         box_centre_form(lo, hi, sm.bc[threadIdx.x], sm.be[threadIdx.x]);
@@ -222,7 +235,9 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
                 int cnt = min(SPH_ARITY, d.tree.count[L] - first);
                 unsigned cm = 0;
                 if (lane < cnt) {
-                    float4 clo = d.tree.lo[L][first + lane], chi = d.tree.hi[L][first + lane];
+                    float4 clo = d.tree.lo[L][first + lane];
+                    const float4 chi = d.tree.hi[L][first + lane];
+                    clo.w *= infl;
                     if (box_reach_sym(clo, chi, tlo, thi)) {
                         for (int w = 0; w < nch; ++w)
                             if (box_reach_sym(clo, chi, sm.blo[w], sm.bhi[w])) cm |= 1u << w;
@@ -292,11 +307,11 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
         unsigned f = 0, f2 = 0;
         if (j < d.n) {
             const float Hj = sph_H(kappa, h);
-            f = reach_chunks(sm, sm.cmask[k], q.x, q.y, q.z, Hj * Hj * SPH_REACH_SLACK);
+            f = reach_chunks(sm, sm.cmask[k], q.x, q.y, q.z, Hj * Hj * infl2 * SPH_REACH_SLACK);
         }
         if (j2 < d.n) {
             const float Hj = sph_H(kappa, h2);
-            f2 = reach_chunks(sm, sm.cmask[k2], q2.x, q2.y, q2.z, Hj * Hj * SPH_REACH_SLACK);
+            f2 = reach_chunks(sm, sm.cmask[k2], q2.x, q2.y, q2.z, Hj * Hj * infl2 * SPH_REACH_SLACK);
         }
         if (k < SPH_CULL_CFCACHE) sm.cf[k][lane] = (unsigned char)f;
         const unsigned m = __ballot_sync(FULL, f != 0);
@@ -311,8 +326,10 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
     if (warp == 0) {
         int total = scan_popc(sm.mask, sm.off, nsrc, lane);
         if (lane == 0) {
-            unsigned long long co = atomicAdd(d.cand_cursor, (unsigned long long)total);
-            if (co + (unsigned long long)total > d.cand_cap) sm.overflow |= 2;
+            // the pool: [0, cand_cap) for full builds, [cand_cap, cand_cap + cand_cap_dirty) for dirty tiles
+            unsigned long long co = atomicAdd(d.cand_cursor + (dirty ? 1 : 0), (unsigned long long)total);
+            if (co + (unsigned long long)total > (dirty ? d.cand_cap_dirty : d.cand_cap)) sm.overflow |= 2;
+            if (dirty) co += d.cand_cap;
             if (total > SPH_MAXROUND * SPH_SE) sm.overflow |= 4;
             sm.ntotal = total;
             sm.cand_off = co;
@@ -324,10 +341,10 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
             d.tile_flag[tile] = (unsigned char)sm.overflow;     // which capacity: 1 walk, 2 pool, 4 rounds
             d.tile_ncand[tile] = 0;
             d.tile_off[tile] = 0;
-            atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], 1ull);
+            if (!was_flagged) atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], 1ull);
         }
         if (valid) d.nsym[i] = 0;
-        if (threadIdx.x == 0) {
+        if (threadIdx.x == 0 && !dirty) {
             const unsigned cyc = (unsigned)(clock64() - t_begin);
             d.tile_cycles[tile] = cyc;
             atomicAdd(d.cull_cycles, (unsigned long long)cyc);
@@ -404,8 +421,8 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
                 if (slot[t] < 0) continue;
                 const int kk = k + t * SPH_TILE_CHUNKS;
                 const float Hj = sph_H(kappa, hh[t]);
-                sm.pos[slot[t]] = make_float4(q[t].x, q[t].y, q[t].z, __fmul_rn(Hj, Hj));
-                const float H2s = Hj * Hj * SPH_REACH_SLACK;
+                sm.pos[slot[t]] = make_float4(q[t].x, q[t].y, q[t].z, __fmul_rn(__fmul_rn(Hj, Hj), infl2));
+                const float H2s = Hj * Hj * infl2 * SPH_REACH_SLACK;
                 const unsigned fc = kk < SPH_CULL_CFCACHE ? (unsigned)sm.cf[kk][lane]
                                                           : reach_chunks(sm, sm.cmask[kk], q[t].x, q[t].y, q[t].z, H2s);
                 sm.flag[slot[t]] = (unsigned char)fc;
@@ -542,18 +559,30 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, int ntile
 #undef LIST_FLUSH
     if (threadIdx.x == 0) {
         d.tile_flag[tile] = (unsigned char)sm.overflow;         // 8: list rows
-        const unsigned cyc = (unsigned)(clock64() - t_begin);
-        d.tile_cycles[tile] = cyc;
-        atomicAdd(d.cull_cycles, (unsigned long long)cyc);
-        if (sm.overflow) atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], 1ull);
+        if (!dirty) {                                           // the cost statistics are those of full builds
+            const unsigned cyc = (unsigned)(clock64() - t_begin);
+            d.tile_cycles[tile] = cyc;
+            atomicAdd(d.cull_cycles, (unsigned long long)cyc);
+        }
+        const int now_flagged = sm.overflow ? 1 : 0;
+        if (now_flagged > was_flagged) atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], 1ull);
+        if (now_flagged < was_flagged) atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], ~0ull);      // minus one
     }
     }
 }
 
 // Head of a list build, ONE block: which tiles go first (those that cost more than 1.5x the average in the previous
 // build), and the resets the build needs (list-build counters, candidate pool cursor, cycle sum).
-__global__ void __launch_bounds__(1024) k_tile_plan(Dev d, int ntile)
+__global__ void __launch_bounds__(1024) k_tile_plan(Dev d, int ntile, int dirty)
 {
+    if (dirty) {                  // a step that reuses the lists: only the second region of the pool starts over
+        if (threadIdx.x == 0) {
+            d.cand_cursor[1] = 0ull;
+            d.counters[SPH_C_TESTS_CULL] = 0ull;
+            d.counters[SPH_C_CANDIDATES] = 0ull;
+        }
+        return;
+    }
     __shared__ unsigned s_n;
     if (threadIdx.x == 0) s_n = 0u;
     __syncthreads();
@@ -571,11 +600,102 @@ __global__ void __launch_bounds__(1024) k_tile_plan(Dev d, int ntile)
     if (threadIdx.x == 0) {
         *d.nheavy = min(s_n, (unsigned)d.heavy_cap);
         *d.cull_cycles = 0ull;
-        *d.cand_cursor = 0ull;
+        d.cand_cursor[0] = 0ull;
+        d.cand_cursor[1] = 0ull;
         d.counters[SPH_C_TESTS_CULL] = 0ull;
         d.counters[SPH_C_CANDIDATES] = 0ull;
         d.counters[SPH_C_LIST_OVERFLOW] = 0ull;
+        d.counters[SPH_C_TILES_DIRTY] = 0ull;
     }
+}
+
+// ------------------------------------------------------------------------------------------
+// k_list_sort (after a full build when the lists are reused, sph_params.skin > 0: its cost is spread over the steps
+// that reuse them -- as a pass of every step it did not pay, profiles/r01_v5): reorder every lane's list entries of a
+// round so that lane l reads bank class
+// (l + n) mod 8 at step n (class = slot mod 8 = which 16-byte bank group the slot's float4 sits in).  The eight
+// lanes of a quarter-warp phase then hit eight different bank groups in the pair kernel's gathers instead of
+// random ones (2.47 wavefronts per phase).  Per lane: count the classes, bucket the entries by class in shared
+// memory (counting sort, cursors packed 8 x 8 bit), emit them round-robin over the classes starting at the
+// lane's own; when the wanted class has run out, the next one in cyclic order that has entries.  One warp per
+// chunk, all lanes in lockstep over the positions of the round; rounds with a lane over SORT_CAP entries stay as
+// they are.  The order of a lane's entries has no meaning (a set), so results change only by summation order.
+// ------------------------------------------------------------------------------------------
+#define SORT_CAP 160
+#define SORT_STRIDE (SORT_CAP * 2 + 4)       // bytes per lane: 81 words
+#define SORT_WARPS 4
+__global__ void __launch_bounds__(SORT_WARPS * 32) k_list_sort(Dev d)
+{
+    __shared__ __align__(4) unsigned char s_buf[SORT_WARPS * 32 * SORT_STRIDE];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int chunk = blockIdx.x * SORT_WARPS + warp;
+    if (chunk >= d.nchunk) return;
+    const int tile = chunk / SPH_TILE_CHUNKS;
+    if (d.tile_flag[tile]) return;
+    const int nround = (d.tile_ncand[tile] + SPH_SE - 1) / SPH_SE;
+    uint2 *lp = d.nlist + ((size_t)chunk * d.rows_cap) * 32 + lane;
+    const unsigned short *rp = d.rowptr + (size_t)chunk * ROWPTR_STRIDE;
+    unsigned short *buf = reinterpret_cast<unsigned short *>(s_buf + (size_t)threadIdx.x * SORT_STRIDE);
+    for (int r = 0; r < nround; ++r) {
+        const int g0 = rp[r], g1 = rp[r + 1];
+        if (g1 <= g0) continue;
+        // pass 1: class counts
+        unsigned long long cnt = 0ull;
+        int N = 0;
+        for (int gq = g0; gq < g1; ++gq) {
+            const uint2 w = lp[(size_t)gq * 32];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const unsigned x = (e & 2) ? w.y : w.x;
+                const unsigned off = (e & 1) ? (x >> 16) : (x & 0xffffu);
+                if (off != 0xffffu) { cnt += 1ull << (((off >> 4) & 7u) << 3); ++N; }
+            }
+        }
+        if (__any_sync(FULL, N > SORT_CAP)) continue;
+        const unsigned long long base = cnt * 0x0101010101010100ull;     // field c = entries of the classes below c
+        // pass 2: bucket by class
+        unsigned long long cur = base;
+        for (int gq = g0; gq < g1; ++gq) {
+            const uint2 w = lp[(size_t)gq * 32];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+                const unsigned x = (e & 2) ? w.y : w.x;
+                const unsigned off = (e & 1) ? (x >> 16) : (x & 0xffffu);
+                if (off != 0xffffu) {
+                    const unsigned c8 = ((off >> 4) & 7u) << 3;
+                    buf[(unsigned)(cur >> c8) & 0xffu] = (unsigned short)off;
+                    cur += 1ull << c8;
+                }
+            }
+        }
+        const unsigned long long end = cur;
+        unsigned long long tk = base;
+        // pass 3: emit round-robin over the classes, all lanes in lockstep over the positions
+        const int nmax = (g1 - g0) * 4;
+        unsigned w0 = 0u, w1 = 0u;
+        for (int n = 0; n < nmax; ++n) {
+            unsigned entry = 0xffffu;
+            if (n < N) {
+                unsigned c8 = ((unsigned)(lane + n) & 7u) << 3;
+                while (((unsigned)(tk >> c8) & 0xffu) >= ((unsigned)(end >> c8) & 0xffu)) c8 = (c8 + 8u) & 63u;
+                entry = buf[(unsigned)(tk >> c8) & 0xffu];
+                tk += 1ull << c8;
+            }
+            w0 = __byte_perm(w0, w1, 0x5432);
+            w1 = __byte_perm(w1, entry, 0x5432);
+            if ((n & 3) == 3) lp[(size_t)(g0 + (n >> 2)) * 32] = make_uint2(w0, w1);
+        }
+    }
+}
+
+int sph_launch_list_sort(sph_ctx *c)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    k_list_sort<<<sph_div_up(d.nchunk, SORT_WARPS), SORT_WARPS * 32, 0, c->stream>>>(d);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
 }
 
 // entry e (0..3) of a row-group word pair
@@ -690,6 +810,7 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p)
     const long long i = (long long)tile * SPH_TILE + threadIdx.x;
     const bool valid = i < d.n;
     const PairTarget t = pair_target_load(d, valid ? i : 0, p.kappa);
+    const float H2i = __fmul_rn(t.H, t.H);
     PairConst kc;
     kc.beta = p.beta; kc.alpha2 = 0.5f * p.alpha; kc.eps = p.eps_av; kc.hk = 0.5f / p.kappa;
     const uint2 *lp = d.nlist + ((size_t)(haschunk ? chunk : 0) * d.rows_cap) * 32 + lane;
@@ -723,11 +844,15 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p)
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
                     unsigned off = list_entry(w, e);
-                    const bool v = off != 0xffffu;
+                    bool v = off != 0xffffu;
                     off = v ? off : 0u;
-                    cnt += v ? 1 : 0;
                     const float4 q1 = *reinterpret_cast<const float4 *>(s1 + off);
                     const float4 q2 = *reinterpret_cast<const float4 *>(s2 + off);
+                    // the lists may hold pairs of the skin (list reuse): membership is the exact predicate on the
+                    // current positions (reading Q4), evaluated here
+                    const float r2x = sph_r2(__fsub_rn(t.x, q1.x), __fsub_rn(t.y, q1.y), __fsub_rn(t.z, q1.z));
+                    v = v && r2x < fmaxf(H2i, __fmul_rn(q2.w, q2.w));
+                    cnt += v ? 1 : 0;
                     const float4 q3 = *reinterpret_cast<const float4 *>(s3 + off);
                     float4 q4 = make_float4(0.f, 0.f, 0.f, 0.f);
                     float q5 = 0.f;
@@ -742,7 +867,10 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p)
         __syncthreads();
     }
 
-    if (valid) pair_store<GRAD, FORCE>(d, i, A);
+    if (valid) {
+        pair_store<GRAD, FORCE>(d, i, A);
+        d.nsym[i] = cnt;
+    }
     if (FORCE) {
         unsigned long long hits = valid ? (unsigned long long)cnt : 0ull;
 #pragma unroll
@@ -777,6 +905,7 @@ __global__ void __launch_bounds__(256) k_neighbors_l(Dev d, float kappa, int *co
     float Hi = sph_H(kappa, d.r.vh[i].w);
     float H2i = __fmul_rn(Hi, Hi);
     int out = 0;
+    // the lists may hold pairs of the skin: the sets are defined by the exact predicate (reading Q4)
     if (!SYM) {
         if (list) list[base] = (int)oi;
         out = 1;
@@ -789,10 +918,12 @@ __global__ void __launch_bounds__(256) k_neighbors_l(Dev d, float kappa, int *co
                 const unsigned off = list_entry(w, e);
                 if (off == 0xffffu) continue;
                 unsigned j = cand[r0 + (int)(off >> 4)];
-                bool hit = true;
-                if (!SYM) {
-                    float4 q = d.r.pm[j];
-                    hit = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z)) < H2i;
+                const float4 q = d.r.pm[j];
+                const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
+                bool hit = r2 < H2i;
+                if (SYM) {
+                    const float Hj = sph_H(kappa, d.r.vh[j].w);
+                    hit = r2 < fmaxf(H2i, __fmul_rn(Hj, Hj));
                 }
                 if (hit) {
                     if (list) list[base + out] = (int)orig[j];
@@ -813,7 +944,7 @@ static int set_smem(sph_ctx *c, const void *fn, size_t bytes)
     return SPH_OK;
 }
 
-int sph_launch_cull(sph_ctx *c)
+int sph_launch_cull(sph_ctx *c, bool dirty_only)
 {
     Dev &d = c->d;
     if (d.n == 0) {
@@ -823,9 +954,116 @@ int sph_launch_cull(sph_ctx *c)
     int rc = set_smem(c, (const void *)k_cull, sizeof(CullSmem));
     if (rc) return rc;
     int ntile = sph_div_up(d.nchunk, SPH_TILE_CHUNKS);
-    k_tile_plan<<<1, 1024, 0, c->stream>>>(d, ntile);
-    k_cull<<<d.heavy_cap + ntile, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, ntile);
+    const float infl = 1.f + (d.skin > 0.f ? d.skin : 0.f);
+    k_tile_plan<<<1, 1024, 0, c->stream>>>(d, ntile, dirty_only ? 1 : 0);
+    k_cull<<<d.heavy_cap + ntile, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, infl, infl * infl, ntile,
+                                                                            dirty_only ? 1 : 0);
     c->launches += 2;
+    SPH_CUDA(c, cudaGetLastError());
+    if (!dirty_only && d.skin > 0.f) return sph_launch_list_sort(c);      // lists that will be reused: order them
+    return SPH_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// k_check (list reuse): may tile T go on using the lists of the last full build?  Those lists hold every pair
+// that was within (1 + skin) max(H_i, H_j) then.  A pair (t, j) that is within max(H_t, H_j) NOW and is not in
+// t's list must have closed in by more than skin max(H_t, H_j) >= skin H_t:  |d_t - d_j| > skin H_t, d = x - xref.
+// With D_T the centre of the box of the tile's displacements and E_T its half diagonal, that cannot happen if
+//     max_{j in N} |d_j - D_T| + E_T <= 0.95 skin min_T H
+// for every tree node N whose box is within reach of the tile's box now (0.95 covers the rounding of the two
+// predicates).  One warp per tile walks the chunk tree: a node out of reach is skipped, a node that satisfies
+// the bound is done with all its descendants, others are opened; a CHUNK that fails makes the tile DIRTY -- its
+// lists are then rebuilt at the current positions in every step until the next full build (sticky).
+// Rigid motion of a body costs nothing here (its displacement boxes are points); a tile at a contact surface
+// gets dirty at once, and only it and its like are rebuilt.
+// ------------------------------------------------------------------------------------------
+#define CHECK_STACK (SPH_ARITY * (SPH_MAX_LEVELS - 1))
+__global__ void __launch_bounds__(SPH_TILE) k_check(Dev d, float thr, int ntile)
+{
+    __shared__ unsigned s_stack[SPH_TILE_CHUNKS][CHECK_STACK];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int tile = blockIdx.x * SPH_TILE_CHUNKS + warp;
+    if (tile >= ntile || d.tile_dirty[tile]) return;
+    const int chunk0 = tile * SPH_TILE_CHUNKS;
+    const int nch = min(SPH_TILE_CHUNKS, d.nchunk - chunk0);
+    float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, H = 0.f;
+    float dl[3] = {3.0e38f, 3.0e38f, 3.0e38f}, dh[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, Hmin = 3.0e38f;
+    if (lane < nch) {
+        float4 a = d.tree.lo[0][chunk0 + lane], b = d.tree.hi[0][chunk0 + lane];
+        lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; H = a.w;
+        hi[0] = b.x; hi[1] = b.y; hi[2] = b.z;
+        a = d.tree.dlo[0][chunk0 + lane]; b = d.tree.dhi[0][chunk0 + lane];
+        dl[0] = a.x; dl[1] = a.y; dl[2] = a.z; Hmin = a.w;
+        dh[0] = b.x; dh[1] = b.y; dh[2] = b.z;
+    }
+#pragma unroll
+    for (int o = 4; o > 0; o >>= 1) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            lo[a] = fminf(lo[a], __shfl_xor_sync(FULL, lo[a], o));
+            hi[a] = fmaxf(hi[a], __shfl_xor_sync(FULL, hi[a], o));
+            dl[a] = fminf(dl[a], __shfl_xor_sync(FULL, dl[a], o));
+            dh[a] = fmaxf(dh[a], __shfl_xor_sync(FULL, dh[a], o));
+        }
+        H = fmaxf(H, __shfl_xor_sync(FULL, H, o));
+        Hmin = fminf(Hmin, __shfl_xor_sync(FULL, Hmin, o));
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        lo[a] = __shfl_sync(FULL, lo[a], 0); hi[a] = __shfl_sync(FULL, hi[a], 0);
+        dl[a] = __shfl_sync(FULL, dl[a], 0); dh[a] = __shfl_sync(FULL, dh[a], 0);
+    }
+    H = __shfl_sync(FULL, H, 0);
+    Hmin = __shfl_sync(FULL, Hmin, 0);
+    const float4 tlo = make_float4(lo[0], lo[1], lo[2], H), thi = make_float4(hi[0], hi[1], hi[2], 0.f);
+    const float Dx = 0.5f * (dl[0] + dh[0]), Dy = 0.5f * (dl[1] + dh[1]), Dz = 0.5f * (dl[2] + dh[2]);
+    const float ex = 0.5f * (dh[0] - dl[0]), ey = 0.5f * (dh[1] - dl[1]), ez = 0.5f * (dh[2] - dl[2]);
+    const float E = sqrtf(ex * ex + ey * ey + ez * ez) * 1.000001f;
+    const float budget = thr * Hmin - E;          // what a node's displacements may differ from D_T by
+    bool dirty = !(budget > 0.f);
+    const float budget2 = budget * budget;
+    unsigned *stack = s_stack[warp];
+    int sp = 0;
+    int L = d.tree.nlev - 1, first = 0, cnt = d.tree.count[L];
+    while (!dirty) {
+        bool open = false;
+        if (lane < cnt) {
+            const float4 clo = d.tree.lo[L][first + lane], chi = d.tree.hi[L][first + lane];
+            if (box_reach_sym(clo, chi, tlo, thi)) {
+                const float4 a = d.tree.dlo[L][first + lane], b = d.tree.dhi[L][first + lane];
+                const float fx = fmaxf(fabsf(a.x - Dx), fabsf(b.x - Dx)), fy = fmaxf(fabsf(a.y - Dy), fabsf(b.y - Dy)),
+                            fz = fmaxf(fabsf(a.z - Dz), fabsf(b.z - Dz));
+                open = !(fx * fx + fy * fy + fz * fz <= budget2);
+            }
+        }
+        const unsigned mask = __ballot_sync(FULL, open);
+        if (L == 0) {
+            if (mask) { dirty = true; break; }
+        } else {
+            if (open) stack[sp + __popc(mask & ((1u << lane) - 1u))] = ((unsigned)L << 27) | (unsigned)(first + lane);
+            sp += __popc(mask);
+            __syncwarp();
+        }
+        if (sp == 0) break;
+        const unsigned e = stack[--sp];
+        __syncwarp();
+        L = (int)(e >> 27) - 1;
+        first = (int)(e & 0x7ffffffu) * SPH_ARITY;
+        cnt = min(SPH_ARITY, d.tree.count[L] - first);
+    }
+    if (dirty && lane == 0) {
+        d.tile_dirty[tile] = 1;
+        atomicAdd(&d.counters[SPH_C_TILES_DIRTY], 1ull);
+    }
+}
+
+int sph_launch_check(sph_ctx *c)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    const int ntile = sph_div_up(d.nchunk, SPH_TILE_CHUNKS);
+    k_check<<<sph_div_up(ntile, SPH_TILE_CHUNKS), SPH_TILE, 0, c->stream>>>(d, 0.95f * d.skin, ntile);
+    c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
 }

@@ -84,7 +84,11 @@ class Params:
     eta_C: float = 0.3
     eta_a: float = 0.0
     flags: int = FLAG_STRENGTH | FLAG_CORRECTION_TENSOR
-    list_budget: int = 0       # neighbour-mask words per particle of the CUDA path (0 = library default)
+    list_budget: int = 0       # neighbour-list rows per particle of the CUDA path (0 = library default)
+    skin: float = 0.0          # CUDA path: list reuse between full neighbour builds (sph_params.skin); no effect on results
+    rebuild_every: int = 0     # CUDA path: steps between full builds when skin > 0 (0 = library default)
+    adapt_h_every: int = 0     # sph_step: one smoothing-length iteration every so many steps (0 = never)
+    adapt_h_target: float = 0.0
     materials: List[Material] = field(default_factory=lambda: [Material()])
 
 
@@ -372,20 +376,27 @@ def oblique_impact(n_total: int = 30_000, v_impact: float = 100.0, seed: int = S
     return wl
 
 
+# list reuse of the CUDA path per config (skin as a fraction of H, steps between full builds): measured choices,
+# DESIGN.md section 7; they change how often the neighbour lists are rebuilt, never a result
+LIST_REUSE = {1: (0.05, 16), 2: (0.05, 16), 3: (0.03, 16), 4: (0.03, 16)}
+
+
 def config(k: int, scale: float = 1.0) -> Workload:
     """BASELINE.json configs[k]; ``scale`` < 1 shrinks particle counts (parity-sized cases)."""
     if k == 0:
         return elastic_block(16 if scale >= 1.0 else max(4, int(round(16 * scale))))
     if k == 1:
-        return granular_column(scale)
-    if k == 2:
-        return gravitating_sphere(int(1_000_000 * scale ** 3) if scale < 1.0 else 1_000_000)
-    if k == 3:
-        return impact_pair(int(4_400_000 * (scale ** 3 if scale < 1.0 else 1.0)), SEED_BASE + 3, 100.0, 1.214,
-                           name="impact_pair_c3")
-    if k == 4:
+        wl = granular_column(scale)
+    elif k == 2:
+        wl = gravitating_sphere(int(1_000_000 * scale ** 3) if scale < 1.0 else 1_000_000)
+    elif k == 3:
+        wl = impact_pair(int(4_400_000 * (scale ** 3 if scale < 1.0 else 1.0)), SEED_BASE + 3, 100.0, 1.214,
+                         name="impact_pair_c3")
+    elif k == 4:
         wl = impact_pair(int(32_000_000 * (scale ** 3 if scale < 1.0 else 1.0)), SEED_BASE + 4, 1000.0, 1.530,
                          name="impact_pair_c4")
         wl.params.list_budget = 96        # ~120 neighbours: room for 384 list entries per particle (default 256)
-        return wl
-    raise ValueError(f"no config {k}")
+    else:
+        raise ValueError(f"no config {k}")
+    wl.params.skin, wl.params.rebuild_every = LIST_REUSE[k]
+    return wl

@@ -35,7 +35,7 @@ def test_library_exports_every_declared_symbol(lib):
 def test_struct_layout_matches_header():
     from paper_2603_19764_b200 import binding as B
     assert C.sizeof(B.sph_material) == 11 * 4
-    assert C.sizeof(B.sph_params) == 6 * 4 + 4 + 4 + 8 * 11 * 4 + 4
+    assert C.sizeof(B.sph_params) == 6 * 4 + 4 + 4 + 8 * 11 * 4 + 4 + 4 * 4
     assert C.sizeof(B.sph_state) == 19 * C.sizeof(C.c_void_p)
 
 

@@ -328,3 +328,70 @@ def test_graph_replay_equals_kernel_by_kernel_step():
         assert np.array_equal(out[0][0][k], out[1][0][k]), k
     assert out[0][1] == out[1][1] and out[0][2] == out[1][2]
     assert np.array_equal(out[0][3], out[1][3])
+
+
+# ---- list reuse (sph_params.skin > 0): same neighbour sets, same numbers --------------------------------------
+def test_skin_lists_give_the_same_single_pass():
+    """With skin > 0 the lists hold the pairs within (1 + skin) of the cut-off and the pair passes evaluate the
+    exact predicate themselves: a pair of the skin contributes exactly zero, so the neighbour sets and counts are
+    those of the exact lists, and the fields differ only by the order of summation (reused lists are ordered by
+    shared-memory bank class)."""
+    out = []
+    for skin in (0.0, 0.12):
+        wl = W.elastic_block(12, h_spread=0.3, two_materials=True)
+        wl.params.skin = skin
+        g = U.gpu_single_pass(wl, split=False)
+        out.append(g)
+        U.compare_single_pass(g, O.single_pass(wl), wl)
+        U.neighbor_sets_equal(g["_sph"], wl, mode="brute")
+    assert out[1]["counters"]["candidates"] > out[0]["counters"]["candidates"]
+    for k in ("ngather", "nsymmetric", "cflag"):
+        assert np.array_equal(out[0][k], out[1][k]), k
+    for k in ("rho", "a", "dudt", "dsdt", "s", "f", "cinv"):
+        assert U.maxnorm_err(out[1][k], out[0][k]) <= 2e-6, k
+
+
+@pytest.mark.parametrize("case", ["block", "impact"])
+def test_reused_lists_keep_the_exact_neighbour_sets_over_steps(case):
+    """sph_step with list reuse (full build every 5 steps, skin 5 %): after every step the neighbour sets the
+    passes used are the exact sets of the CURRENT positions (oracle on the downloaded positions), dirty tiles
+    included (the impact pair has a contact surface moving at 3 km/s), and the state follows the oracle's
+    stepper like the step without reuse does."""
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    if case == "block":
+        wl = W.elastic_block(14, h_spread=0.2)
+        for q in ("vx", "vy", "vz"):                          # a violent velocity field: lists go stale quickly
+            wl.arrays[q] *= 30.0
+    else:
+        wl = W.impact_pair(20000, W.SEED_BASE + 3, 100.0, 1.214)
+    wl.params.skin = 0.05
+    wl.params.rebuild_every = 5
+    st = O.Stepper(wl, mode="grid")
+    dirty_seen = 0
+    with torch.cuda.stream(torch.cuda.Stream()):
+        s = B.Sph(wl.params, wl.n)
+        t = s.upload(wl)
+        dtu = torch.zeros(1, dtype=torch.float32, device="cuda")
+        s.build_neighbors(t, wl.n)
+        for step in range(12):
+            s.step(None, 0, 0.0, dtu)
+            dt_o = st.step(0.0)
+            assert float(dtu.item()) == pytest.approx(dt_o, rel=1e-4)
+            c = s.get_counters()
+            dirty_seen = max(dirty_seen, c["tiles_dirty"])
+            assert c["list_overflow"] == 0 and c["nonfinite"] == 0
+            if step in (2, 3, 4, 8, 11):
+                s.download_state(t)
+                cur = W.Workload(wl.name, wl.params, {k: t[k].cpu().numpy() for k in W.FIELDS}, wl.mat, wl.fixed, 0.0)
+                U.neighbor_sets_equal(s, cur, mode="grid")
+        s.download_state(t)
+        torch.cuda.synchronize()
+    x = np.stack([t[k].cpu().numpy() for k in ("x", "y", "z")])
+    v = np.stack([t[k].cpu().numpy() for k in ("vx", "vy", "vz")])
+    S = np.stack([t[k].cpu().numpy() for k in ("Sxx", "Syy", "Sxy", "Sxz", "Syz")])
+    errs = {"x": U.maxnorm_err(x, st.x), "v": U.maxnorm_err(v, st.v), "S": U.maxnorm_err(S, st.S)}
+    print(case, "dirty tiles seen", dirty_seen, {k: float(f"{e:.3g}") for k, e in errs.items()})
+    assert errs["x"] <= 1e-5 and errs["v"] <= 1e-3 and errs["S"] <= 1e-2       # 12 steps: chaotic growth of rounding
+    if case == "impact":
+        assert dirty_seen > 0
