@@ -112,6 +112,8 @@ enum { SPH_C_PAIRS_GATHER = 0,   /* sum_i |gather set(i)|   (true pairs of the d
        SPH_C_NONFINITE,          /* particles whose a, du/dt or dS/dt was not finite in the last CLOSE      */
        SPH_C_TILES_DIRTY,        /* sph_params.skin > 0: tiles whose lists are rebuilt in every step since the
                                     last full build (0 right after one)                                      */
+       SPH_C_LIST_SLOTS,         /* list slots the pair passes step through per launch: entries plus the padding
+                                    that makes the 32 lists of a chunk equally long in every round (last build) */
        SPH_C_COUNT };
 
 typedef struct sph_ctx sph_ctx;   /* opaque, library-owned (host memory) */

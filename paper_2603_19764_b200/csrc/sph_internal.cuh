@@ -216,6 +216,13 @@ __device__ __forceinline__ int sph_tile_of_block(const Dev &d, int b)
     return d.heavy_mark[t] ? -1 : t;
 }
 
+// Rounds of a tile with ncand candidates: SPH_SE slots each, the last one shorter.  (Measured on configs[4], 1967
+// candidates per tile on average, i.e. 1632 + 335: the 32 lists of a chunk are padded to equal length in every
+// round, 30 % of the slots the pair passes step through are padding; rounds of EQUAL size, 2 x 984, were tried
+// and are worse, 56 % -- the candidates are in curve order, an even split cuts through every chunk's neighbourhood.)
+__host__ __device__ __forceinline__ int sph_round_count(int ncand) { return (ncand + SPH_SE - 1) / SPH_SE; }
+__host__ __device__ __forceinline__ int sph_round_size(int) { return SPH_SE; }
+
 // order-preserving float <-> int map for atomicMin/atomicMax on floats
 __device__ __forceinline__ int sph_f2ord(float f)
 {

@@ -372,7 +372,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float inf
     unsigned wp = lb;                     // where the next entry goes
     int G = 0;                            // row-groups of this lane in the global list so far (padding included)
     int nhit = 0;                         // true neighbours
-    unsigned tests = 0;
+    unsigned tests = 0, slots = 0;
     int Gstart = 0;                       // first row-group of the current round
     // write the complete row-groups of the buffer out, keep the 0..3 entries left over
 #define LIST_FLUSH()                                                                        \
@@ -390,8 +390,9 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float inf
     if (warp < nch && lane == 0) rp[0] = 0;
 
     int round = 0;
-    for (int r0 = 0; r0 < ntotal; r0 += SPH_SE, ++round) {
-        const int nr = min(SPH_SE, ntotal - r0);
+    const int se = sph_round_size(ntotal);
+    for (int r0 = 0; r0 < ntotal; r0 += se, ++round) {
+        const int nr = min(se, ntotal - r0);
         // ---- A3: compact this round's survivors into shared memory and the global candidate list
         // (two source chunks per trip, as in A2: the loads of both are issued before either is used)
         for (int k = warp; k < nsrc; k += 2 * SPH_TILE_CHUNKS) {
@@ -546,7 +547,10 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float inf
                 if (gg < d.rows_cap) lp[(size_t)gg * 32] = make_uint2(0xffffffffu, 0xffffffffu);
             G = Gmax;
             if (G > d.rows_cap) sm.overflow = 8;      // list rows exhausted: the tile falls back
-            if (lane == 0) rp[round + 1] = (unsigned short)min(Gmax, d.rows_cap);
+            if (lane == 0) {
+                rp[round + 1] = (unsigned short)min(Gmax, d.rows_cap);
+                slots += (unsigned)(Gmax - Gstart) * 128u;
+            }
         }
         __syncthreads();
     }
@@ -554,7 +558,10 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float inf
     if (warp < nch) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) tests += __shfl_xor_sync(FULL, tests, o);
-        if (lane == 0) atomicAdd(&d.counters[SPH_C_TESTS_CULL], (unsigned long long)tests);
+        if (lane == 0) {
+            atomicAdd(&d.counters[SPH_C_TESTS_CULL], (unsigned long long)tests);
+            atomicAdd(&d.counters[SPH_C_LIST_SLOTS], (unsigned long long)slots);
+        }
     }
 #undef LIST_FLUSH
     if (threadIdx.x == 0) {
@@ -580,6 +587,7 @@ __global__ void __launch_bounds__(1024) k_tile_plan(Dev d, int ntile, int dirty)
             d.cand_cursor[1] = 0ull;
             d.counters[SPH_C_TESTS_CULL] = 0ull;
             d.counters[SPH_C_CANDIDATES] = 0ull;
+            d.counters[SPH_C_LIST_SLOTS] = 0ull;
         }
         return;
     }
@@ -606,6 +614,7 @@ __global__ void __launch_bounds__(1024) k_tile_plan(Dev d, int ntile, int dirty)
         d.counters[SPH_C_CANDIDATES] = 0ull;
         d.counters[SPH_C_LIST_OVERFLOW] = 0ull;
         d.counters[SPH_C_TILES_DIRTY] = 0ull;
+        d.counters[SPH_C_LIST_SLOTS] = 0ull;
     }
 }
 
@@ -632,7 +641,7 @@ __global__ void __launch_bounds__(SORT_WARPS * 32) k_list_sort(Dev d)
     if (chunk >= d.nchunk) return;
     const int tile = chunk / SPH_TILE_CHUNKS;
     if (d.tile_flag[tile]) return;
-    const int nround = (d.tile_ncand[tile] + SPH_SE - 1) / SPH_SE;
+    const int nround = sph_round_count(d.tile_ncand[tile]);
     uint2 *lp = d.nlist + ((size_t)chunk * d.rows_cap) * 32 + lane;
     const unsigned short *rp = d.rowptr + (size_t)chunk * ROWPTR_STRIDE;
     unsigned short *buf = reinterpret_cast<unsigned short *>(s_buf + (size_t)threadIdx.x * SORT_STRIDE);
@@ -739,8 +748,9 @@ __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
     A.sum = (double)pi.w; A.sh = 3.f * pi.w; A.n = 1;          // self term: q = 0, t = 1
     int ntest = 1;
     int round = 0;
-    for (int r0 = 0; r0 < ncand; r0 += SPH_SE, ++round) {
-        const int nr = min(SPH_SE, ncand - r0);
+    const int se = sph_round_size(ncand);
+    for (int r0 = 0; r0 < ncand; r0 += se, ++round) {
+        const int nr = min(se, ncand - r0);
         for (int s = threadIdx.x; s < nr; s += SPH_TILE) s_pm[s] = d.r.pm[cand[r0 + s]];
         __syncthreads();
         if (haschunk) {
@@ -817,11 +827,12 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p)
     const unsigned short *rp = d.rowptr + (size_t)(haschunk ? chunk : 0) * ROWPTR_STRIDE;
     PairAcc A;
     pair_acc_zero(A);
-    int cnt = 0;
+    int cnt = 0, nent = 0;
 
     int round = 0;
-    for (int r0 = 0; r0 < ncand; r0 += SPH_SE, ++round) {
-        const int nr = min(SPH_SE, ncand - r0);
+    const int se = sph_round_size(ncand);
+    for (int r0 = 0; r0 < ncand; r0 += se, ++round) {
+        const int nr = min(se, ncand - r0);
         for (int s = threadIdx.x; s < nr; s += SPH_TILE) {
             const unsigned j = cand[r0 + s];
             float4 vh = d.r.vh[j];
@@ -845,6 +856,7 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p)
                 for (int e = 0; e < 4; ++e) {
                     unsigned off = list_entry(w, e);
                     bool v = off != 0xffffu;
+                    nent += v ? 1 : 0;
                     off = v ? off : 0u;
                     const float4 q1 = *reinterpret_cast<const float4 *>(s1 + off);
                     const float4 q2 = *reinterpret_cast<const float4 *>(s2 + off);
@@ -872,12 +884,15 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p)
         d.nsym[i] = cnt;
     }
     if (FORCE) {
-        unsigned long long hits = valid ? (unsigned long long)cnt : 0ull;
+        unsigned long long hits = valid ? (unsigned long long)cnt : 0ull, ents = valid ? (unsigned long long)nent : 0ull;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) hits += __shfl_xor_sync(FULL, hits, o);
+        for (int o = 16; o > 0; o >>= 1) {
+            hits += __shfl_xor_sync(FULL, hits, o);
+            ents += __shfl_xor_sync(FULL, ents, o);
+        }
         if (lane == 0) {
             atomicAdd(&d.counters[SPH_C_PAIRS_SYMMETRIC], hits);
-            atomicAdd(&d.counters[SPH_C_TESTS_FORCE], hits);
+            atomicAdd(&d.counters[SPH_C_TESTS_FORCE], ents);          // list entries examined (skin pairs included)
         }
     }
 }
@@ -911,7 +926,8 @@ __global__ void __launch_bounds__(256) k_neighbors_l(Dev d, float kappa, int *co
         out = 1;
     }
     int round = 0;
-    for (int r0 = 0; r0 < ncand; r0 += SPH_SE, ++round) {
+    const int se = sph_round_size(ncand);
+    for (int r0 = 0; r0 < ncand; r0 += se, ++round) {
         for (int gq = rp[round]; gq < rp[round + 1]; ++gq) {
             const uint2 w = lp[(size_t)gq * 32];
             for (int e = 0; e < 4; ++e) {
