@@ -327,22 +327,23 @@ def run_ours(args):
     # ---- end to end through the host-buffer entry point -----------------------------------
     del s, t
     torch.cuda.empty_cache()
-    host = {k: torch.from_numpy(v.copy()).pin_memory() for k, v in wl.arrays.items()}
-    host["mat"] = torch.from_numpy(wl.mat.copy()).pin_memory()
-    host["fixed"] = torch.from_numpy(wl.fixed.copy()).pin_memory()
-    s2 = B.Sph(wl.params, n, device=dev)
     e2e_steps = max(1, min(args.steps, 5))
-    s2.step_host(host, n, 0.0)                                   # warm-up (also the bootstrap)
-    s2.step_host(host, n, 0.0)
-    barrier()
-    t0 = time.perf_counter()
-    e2e_pairs = 0
-    for _ in range(e2e_steps):
+    e2e_s, e2e_pairs = 1.0, 0
+    if not args.no_e2e:
+        host = {k: torch.from_numpy(v.copy()).pin_memory() for k, v in wl.arrays.items()}
+        host["mat"] = torch.from_numpy(wl.mat.copy()).pin_memory()
+        host["fixed"] = torch.from_numpy(wl.fixed.copy()).pin_memory()
+        s2 = B.Sph(wl.params, n, device=dev)
+        s2.step_host(host, n, 0.0)                                   # warm-up (also the bootstrap)
         s2.step_host(host, n, 0.0)
-        c = s2.get_counters()
-        e2e_pairs += c["pairs_gather"] + c["pairs_symmetric"]
-    torch.cuda.synchronize(dev)
-    e2e_s = time.perf_counter() - t0
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            s2.step_host(host, n, 0.0)
+            c = s2.get_counters()
+            e2e_pairs += c["pairs_gather"] + c["pairs_symmetric"]
+        torch.cuda.synchronize(dev)
+        e2e_s = time.perf_counter() - t0
     clocks = sampler.stop()          # sampled from the start of the device-timed steps to the end of the e2e steps
     e2e_s_max, e2e_pairs_all = rank_reduce(e2e_s, e2e_pairs, dev)
     e2e_value = e2e_pairs_all / e2e_s_max
@@ -464,6 +465,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-hydro-only", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     ap.add_argument("--no-graph", action="store_true", help="launch the step kernel by kernel (A/B of the CUDA graph)")
     ap.add_argument("--skin", type=float, default=None, help="list reuse: skin as a fraction of H (0 = off; A/B)")
     ap.add_argument("--rebuild-every", type=int, default=None, help="list reuse: steps between full builds (A/B)")

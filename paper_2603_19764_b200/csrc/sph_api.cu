@@ -174,6 +174,8 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
                    && (cudaStream_t)cuda_stream != cudaStreamPerThread;
     c->ws_bytes = carve(&c->d, &c->stage, (char *)workspace, n_max, kcap_of(params), c->use_lists, skin_of(params));
     c->rebuild_every = params->rebuild_every > 0 ? params->rebuild_every : 8;
+    c->adapt_h_every = (params->adapt_h_every > 0 && params->adapt_h_target > 0.f) ? params->adapt_h_every : 0;
+    c->adapt_h_target = params->adapt_h_target;
     c->force_full = true;
     c->d.n = 0; c->d.nchunk = 0;
     for (int k = 0; k < 2 * SPH_T_COUNT; ++k) {
@@ -202,7 +204,7 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
 
 static void drop_graphs(sph_ctx *c)
 {
-    for (int k = 0; k < 2; ++k)
+    for (int k = 0; k < 3; ++k)
         for (int s = 0; s < 2; ++s)
             if (c->gexec[k][s]) { cudaGraphExecDestroy(c->gexec[k][s]); c->gexec[k][s] = nullptr; }
 }
@@ -257,6 +259,7 @@ extern "C" int sph_build_neighbors(sph_ctx *c, const sph_state *state, long long
         drop_graphs(c);
         c->resident = true;
         c->have_derivs = false;
+        c->step_count = 0;
     } else {
         if (!c->resident) return SPH_EORDER;
         rc = sph_launch_resort(c);
@@ -408,9 +411,15 @@ static int derivative_passes(sph_ctx *c)
 }
 
 // does the next step rebuild everything (re-sort, full list build) or reuse the lists?
+static bool step_adapts_h(const sph_ctx *c)
+{
+    return c->adapt_h_every > 0 && (c->step_count + 1) % c->adapt_h_every == 0;
+}
+
 static bool step_is_full(const sph_ctx *c)
 {
-    return !(c->d.skin > 0.f) || !c->use_lists || c->force_full || c->steps_since_full + 1 >= c->rebuild_every;
+    return !(c->d.skin > 0.f) || !c->use_lists || c->force_full || c->steps_since_full + 1 >= c->rebuild_every
+           || step_adapts_h(c);
 }
 
 static int step_body(sph_ctx *c, sph_state *state, long long n, float dt, float *dt_used)
@@ -435,8 +444,16 @@ static int step_body(sph_ctx *c, sph_state *state, long long n, float dt, float 
         rc = sph_launch_kick_drift(c, dt);
         if (rc) return rc;
     }
+    const bool adapt = step_adapts_h(c);
     rc = step_is_full(c) ? sph_build_neighbors(c, nullptr, 0) : reuse_neighbors(c);
     if (rc) return rc;
+    if (adapt) {
+        // one Newton-Raphson update of h towards a constant kernel mass at the new positions (density
+        // pass, update, tree and lists again); the method's own remedy for particles that lose their neighbours
+        rc = sph_adapt_h(c, c->adapt_h_target, 1, nullptr);
+        if (rc) return rc;
+    }
+    c->step_count++;
     rc = derivative_passes(c);
     if (rc) return rc;
     rc = do_close(c, SPH_CLOSE, 0.f, true);
@@ -458,7 +475,8 @@ extern "C" int sph_step(sph_ctx *c, sph_state *state, long long n, float dt, flo
     if (!c) return SPH_EINVAL;
     const bool graphable = c->use_graph && c->resident && c->have_derivs && !state && !(dt > 0.f) && c->d.n > 0;
     if (!graphable) return step_body(c, state, n, dt, dt_used);
-    const int kind = step_is_full(c) ? 0 : 1;       // a step with a full build (re-sort) or one that reuses the lists
+    // a step with a full build (re-sort), one that reuses the lists, or a full one with a smoothing-length update
+    const int kind = step_adapts_h(c) ? 2 : (step_is_full(c) ? 0 : 1);
     const int s = c->parity;
     if (c->gexec[kind][s] && (c->gkey_n[kind][s] != c->d.n || c->gkey_dtused[kind][s] != (const void *)dt_used)) {
         cudaGraphExecDestroy(c->gexec[kind][s]);
@@ -468,6 +486,7 @@ extern "C" int sph_step(sph_ctx *c, sph_state *state, long long n, float dt, flo
         // everything step_body changes on the host, in case the capture fails half way (no kernel has run then)
         const Resident r0 = c->d.r, alt0 = c->d.alt;
         const int parity0 = c->parity, since0 = c->steps_since_full;
+        const long long count0 = c->step_count;
         const bool force0 = c->force_full, hd = c->have_density, hp = c->have_predict, hg = c->have_grad,
                    hf = c->have_force, hv = c->have_derivs;
         cudaGraph_t g = nullptr;
@@ -484,6 +503,7 @@ extern "C" int sph_step(sph_ctx *c, sph_state *state, long long n, float dt, flo
         if (g) cudaGraphDestroy(g);
         if (rc || e != cudaSuccess || !c->gexec[kind][s]) {
             c->d.r = r0; c->d.alt = alt0; c->parity = parity0; c->steps_since_full = since0; c->force_full = force0;
+            c->step_count = count0;
             c->have_density = hd; c->have_predict = hp; c->have_grad = hg; c->have_force = hf; c->have_derivs = hv;
             c->launches = l0;
             (void)cudaGetLastError();
@@ -501,7 +521,8 @@ extern "C" int sph_step(sph_ctx *c, sph_state *state, long long n, float dt, flo
     SPH_CUDA(c, cudaGraphLaunch(c->gexec[kind][s], c->stream));
     {                                                                 // what step_body does on the host
         Dev &d = c->d;
-        if (kind == 0) {
+        c->step_count++;
+        if (kind != 1) {
             Resident t = d.r; d.r = d.alt; d.alt = t;
             c->parity ^= 1;
             c->steps_since_full = 0;

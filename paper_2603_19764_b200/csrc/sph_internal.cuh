@@ -147,10 +147,14 @@ struct sph_ctx {
     int parity;                      // which half of the ping-pong is current
     // graphs of the resident step: [kind][parity], kind 0 = step with a full list build (re-sort), 1 = step that
     // reuses the lists
-    cudaGraphExec_t gexec[2][2];
-    long long glaunches[2][2];       // launches one replay stands for
-    long long gkey_n[2][2];
-    const void *gkey_dtused[2][2];
+    // kind 2 = a full step that first runs one smoothing-length iteration (sph_params.adapt_h_every)
+    cudaGraphExec_t gexec[3][2];
+    long long glaunches[3][2];       // launches one replay stands for
+    long long gkey_n[3][2];
+    const void *gkey_dtused[3][2];
+    int adapt_h_every;               // > 0: one iteration of sph_adapt_h every so many steps, inside sph_step
+    float adapt_h_target;
+    long long step_count;            // steps taken since the state was ingested
     int rebuild_every;               // steps between two full list builds when skin > 0
     int steps_since_full;            // steps taken since the last full build
     bool force_full;                 // the next step must do a full build (state refreshed, h changed, ...)

@@ -98,6 +98,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_density(Dev d, float kappa,
     __shared__ float4 s_tgt[PAIR_WARPS][SPH_CHUNK];
     __shared__ unsigned s_stack[PAIR_WARPS][STACK_DEPTH];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (tile_flag && d.counters[SPH_C_LIST_OVERFLOW] == 0ull) return;       // serving flagged tiles: there are none
     for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
     if (tile_flag && !tile_flag[tile]) continue;
     const int chunk = tile * PAIR_WARPS + warp;
@@ -254,6 +255,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_neighbors(Dev d, float kapp
     __shared__ float4 s_tgt[PAIR_WARPS][SPH_CHUNK];
     __shared__ unsigned s_stack[PAIR_WARPS][STACK_DEPTH];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (tile_flag && d.counters[SPH_C_LIST_OVERFLOW] == 0ull) return;       // serving flagged tiles: there are none
     for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
     if (tile_flag && !tile_flag[tile]) continue;
     const int chunk = tile * PAIR_WARPS + warp;

@@ -37,7 +37,39 @@ def test_correction_tensor_keeps_angular_momentum():
     fluid, p3 = _drift(W.FLAG_PCLIP_GLOBAL, 800)
     print(f"|dL|/L0 after 2000 steps: with C {with_c:.3e}, C = 1 {without_c:.3e}; fluid (800 steps) {fluid:.3e}; "
           f"|dP|/(M v) {p1:.1e} {p2:.1e} {p3:.1e}")
-    assert with_c < 2e-3                     # paper: < 1e-3 with the correction tensor
-    assert without_c > 5e-3 and without_c > 5.0 * with_c      # paper: > 1 % without it
+    assert with_c < 1e-3                     # paper: < 1e-3 with the correction tensor
+    assert without_c > 1e-2 and without_c > 5.0 * with_c      # paper: > 1 % without it
     assert fluid < 1e-5                      # paper: ~1e-5 for a fluid
     assert max(p1, p2, p3) < 1e-6            # linear momentum: antisymmetric pair forces
+
+
+def test_fluid_run_with_smoothing_length_iteration_survives_ejecta():
+    """DESIGN.md section 9 (round 1): with h fixed, the strength-off oblique impact goes non-finite after ~1300
+    steps, when ejecta lose their neighbours (Omega -> 0, Eq. 3).  The method's remedy is its smoothing-length
+    iteration (Eq. 2): sph_params.adapt_h_every runs one Newton-Raphson update every so many
+    steps inside sph_step.  With it the run stays finite past 2000 steps and the counter of particles with
+    |Omega| < 0.1 stays at zero; without it the same counter flags the trouble before the state breaks."""
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    out = {}
+    for every in (5, 0):
+        base = W.oblique_impact()
+        p = dataclasses.replace(base.params, flags=W.FLAG_PCLIP_GLOBAL, adapt_h_every=every, adapt_h_target=73.6)
+        wl = dataclasses.replace(base, params=p)
+        with torch.cuda.stream(torch.cuda.Stream()):
+            s = B.Sph(wl.params, wl.n)
+            t = s.upload(wl)
+            s.build_neighbors(t, wl.n)
+            small_max = bad = 0
+            for k in range(2000):
+                s.step(None, 0, 0.0)
+                if k % 50 == 49:
+                    c = s.get_counters()
+                    small_max = max(small_max, c["omega_small"]); bad = max(bad, c["nonfinite"])
+            d1 = s.get_diagnostics().cpu().numpy()
+            h = s.get_field("H").cpu().numpy()
+        out[every] = (small_max, bad, bool(np.all(np.isfinite(d1))), float(h.max() / h.min()))
+    print("adapt_h_every -> (max omega_small, max nonfinite, finite diagnostics, h max/min):", out)
+    assert out[5][0] == 0 and out[5][1] == 0 and out[5][2]
+    assert out[5][3] > 1.05                                # h did adapt
+    assert out[0][0] > 0 or out[0][1] > 0 or not out[0][2]  # and the fixed-h run is the one that gets into trouble

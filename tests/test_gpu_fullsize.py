@@ -55,22 +55,21 @@ def test_full_config_sampled(k, where):
     print(f"config{k} {where}: n={wl.n}, oracle sample {ns}, fallback tiles {nfb} of {(wl.n + 255) // 256}", {q: float(f"{v:.3g}") for q, v in errs.items()})
 
 
-@pytest.mark.parametrize("k,steps", [(1, 4), (2, 2)])
+@pytest.mark.parametrize("k,steps", [(1, 4), (2, 3)])
 def test_full_config_steps_in_bench_configuration(k, steps):
-    """sph_step as bench.py runs it -- resident state, fused gradient + force pass, CFL time step, a capturable
-    stream so that the step is captured into a CUDA graph and (configs[1]) replayed -- against the oracle's
-    stepper, every particle.
+    """sph_step as bench.py runs it -- resident state, fused gradient + force pass, CFL time step, list reuse
+    (a full build every 3 steps here, so that both kinds of step occur), a capturable stream so that the steps
+    are captured into CUDA graphs and replayed -- against the oracle's stepper, every particle.
 
-    Tolerances after SEVERAL steps (BASELINE.json states its 1e-4 for one step): x, v, u keep the one-step
-    tolerances.  S does not, in the max norm: the CUDA path stores positions in fp32 (BASELINE.json: "particle
-    SoA storage in fp32"), the oracle carries fp64 state, and half an ulp of a position (4e-6 of a particle
-    spacing at |x| / dx = 60) moves rho by ~1e-7..1e-6 relative, P = c0^2 (rho - rho0) by 1e3..1e4 Pa and the
-    yield-limited S (|S| = Y ~ mu P) with it, for the particles whose drift crosses a rounding boundary.  So:
-    rms and 99.9th percentile of |dS| stay within 1e-4 / 1e-3 of max |S|, the maximum within 1e-2."""
+    BASELINE.json fixes the STORAGE of the particle state as fp32, so the oracle runs in its fp32-storage mode
+    (Stepper(store_fp32=True): every stored quantity rounded to fp32 once, all arithmetic fp64) and is given the
+    GPU's time steps (checked against its own CFL steps first).  Round 1 compared with the fp64-state stepper
+    and had to widen S to 1e-2 in the max norm; what is left with like storage is reported below."""
     import torch
     from paper_2603_19764_b200 import binding as B
     wl = W.config(k)
-    st = O.Stepper(wl, mode="grid")
+    wl.params.rebuild_every = 3
+    st = O.Stepper(wl, mode="grid", store_fp32=True)
     with torch.cuda.stream(torch.cuda.Stream()):
         s = B.Sph(wl.params, wl.n)
         t = s.upload(wl)
@@ -78,23 +77,122 @@ def test_full_config_steps_in_bench_configuration(k, steps):
         s.step(t, wl.n, 0.0, dtu)                       # ingest + bootstrap + step (kernel by kernel)
         dts = [float(dtu.item())]
         for _ in range(steps - 1):
-            s.step(None, 0, 0.0, dtu)                   # captured (twice), then replayed
+            s.step(None, 0, 0.0, dtu)                   # captured, then replayed
             dts.append(float(dtu.item()))
         s.download_state(t)
         eacc = s.get_field("EACC")
         torch.cuda.synchronize()
         got = {q: t[q].cpu().numpy() for q in ("x", "y", "z", "vx", "vy", "vz", "u", "Sxx", "Syy", "Sxy", "Sxz", "Syz")}
         eacc = eacc.cpu().numpy()
-        assert s.get_counters()["list_overflow"] == 0
+        c = s.get_counters()
+        assert c["list_overflow"] == 0 and c["nonfinite"] == 0
     for n in range(steps):
-        assert dts[n] == pytest.approx(st.step(0.0), rel=2e-5)
+        if st.d is None:
+            st.bootstrap()
+        assert dts[n] == pytest.approx(st.dt_next, rel=2e-5)       # the oracle's own CFL step
+        st.step(dts[n])                                            # ... then the GPU's fp32 value of it
     x = np.stack([got["x"], got["y"], got["z"]]); v = np.stack([got["vx"], got["vy"], got["vz"]])
     S = np.stack([got[q] for q in ("Sxx", "Syy", "Sxy", "Sxz", "Syz")])
     smax = np.abs(st.S).max()
     errs = {"x": U.maxnorm_err(x, st.x), "v": U.maxnorm_err(v, st.v), "u": U.maxnorm_err(got["u"], st.u),
             "S_max": U.maxnorm_err(S, st.S), "S_rms": float(np.sqrt(((S - st.S) ** 2).mean()) / smax),
-            "S_p999": float(np.percentile(np.abs(S - st.S), 99.9) / smax), "eacc": U.maxnorm_err(eacc, st.e_acc)}
+            "S_p999": float(np.percentile(np.abs(S - st.S), 99.9) / smax), "eacc": U.maxnorm_err(eacc, st.e_acc),
+            "x_bitwise_equal_fraction": float((x == st.x).mean())}
     print(f"config{k} n={wl.n} {steps} steps", {q: float(f"{e:.3g}") for q, e in errs.items()})
     assert errs["x"] <= 1e-6 and errs["v"] <= U.TOL_STATE and errs["u"] <= U.TOL_STATE
-    assert errs["S_rms"] <= U.TOL_STATE and errs["S_p999"] <= 1e-3 and errs["S_max"] <= 1e-2
+    assert errs["S_rms"] <= 1e-5 and errs["S_p999"] <= U.TOL_STATE and errs["S_max"] <= S_MAX_TOL[k]
     assert errs["eacc"] <= 1e-3
+
+
+# S after several steps, max norm, against the fp32-storage stepper: what the particles whose fp32 drift lands on
+# the other side of a rounding boundary (x differs by one ulp between fp32 and fp64 arithmetic) leave
+S_MAX_TOL = {1: 2e-4, 2: 2e-4}        # measured: 6.1e-5 (configs[1], x bitwise equal), 1.01e-4 (configs[2], 0.2 % of x off by an ulp)
+
+
+def _invariants(s, wl, tag):
+    """sqrt(J2) <= Y (1 + 1e-6) for every particle (after the closing rescale), finite state,
+    counters clean; on the device (torch), nothing is downloaded."""
+    import torch
+    S = s.get_fields("S", 5)
+    Y = s.get_field("Y")
+    szz = -S[0] - S[1]
+    sj = torch.sqrt(0.5 * (S[0] ** 2 + S[1] ** 2 + szz ** 2) + S[2] ** 2 + S[3] ** 2 + S[4] ** 2)
+    worst = float((sj - Y * (1.0 + 1e-6)).max().item())
+    assert worst <= 1e-3 * float(Y.max().item()) * 1e-6 + 1e-6, (tag, worst)
+    for name, nc in (("V", 3), ("X", 3)):
+        assert bool(torch.isfinite(s.get_fields(name, nc)).all().item()), (tag, name)
+    assert bool(torch.isfinite(s.get_field("U")).all().item()), tag
+    c = s.get_counters()
+    assert c["nonfinite"] == 0 and c["list_overflow"] == 0, (tag, c)
+    return c
+
+
+def _internal_momentum_drift(s, wl, d0, t_elapsed):
+    """|sum m v - (sum m v)_0 - t sum m g| / sum m |v|: what the INTERNAL pair forces did to the linear momentum
+    (antisymmetric pair terms conserve it; a_ext, constant per particle, is taken out)."""
+    import torch
+    d1 = s.get_diagnostics().cpu().numpy()
+    m = wl.arrays["m"].astype(np.float64)
+    g = np.stack([wl.arrays[q].astype(np.float64) for q in ("gx", "gy", "gz")])
+    free = (wl.fixed == 0)
+    ext = (m * g * free).sum(axis=1) * t_elapsed
+    v = s.get_fields("V", 3).double()
+    scale = float((torch.as_tensor(m, device=v.device) * v.abs()).sum().item()) + 1e-300
+    return float(np.abs(d1[1:4] - d0[1:4] - ext).max() / scale), scale
+
+
+def test_config1_200_steps_floor_fixed_yield_bounded_pass_split():
+    """BASELINE.json configs[1]: "200 time steps with Courant factor 0.3.  Report per-step time split by pass."
+    Floor particles bit-identical in x with v = 0; sqrt(J2) <= Y every 20 steps; no NaN; the split is printed."""
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    wl = W.config(1)
+    fx = torch.as_tensor(wl.fixed.astype(bool))
+    with torch.cuda.stream(torch.cuda.Stream()):
+        s = B.Sph(wl.params, wl.n)
+        t = s.upload(wl)
+        s.build_neighbors(t, wl.n)
+        tm_sum = {q: 0.0 for q in B.T_SLOTS}
+        for step in range(200):
+            s.step(None, 0, 0.0)
+            if (step + 1) % 20 == 0:
+                _invariants(s, wl, f"config1 step {step + 1}")
+                tm = s.get_timings()
+                for q in B.T_SLOTS:
+                    tm_sum[q] += tm[q] / 10.0
+        X = s.get_fields("X", 3).cpu(); V = s.get_fields("V", 3).cpu()
+        torch.cuda.synchronize()
+    x0 = torch.stack([torch.as_tensor(wl.arrays[q]) for q in ("x", "y", "z")])
+    assert torch.equal(X[:, fx], x0[:, fx]) and bool((V[:, fx] == 0).all())
+    assert float((X[:, ~fx] - x0[:, ~fx]).abs().max()) > 0.0
+    print("config1 200 steps, mean ms per pass over the sampled steps:", {q: round(v, 4) for q, v in tm_sum.items()})
+
+
+@pytest.mark.parametrize("k,steps", [(2, 20), (3, 10), (4, 5)])
+def test_config_multi_step_invariants(k, steps):
+    """BASELINE.json configs[2] "Run 20 steps and check that S stays bounded and momentum is conserved",
+    configs[3] 10 steps, configs[4] 5 steps: sqrt(J2) <= Y after every step, internal forces leave sum m v alone
+    to 1e-5 of sum m |v|, no list overflow, nothing non-finite."""
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    need = {2: 3e9, 3: 10e9, 4: 60e9}[k]
+    if _free_gpu_bytes() < need:
+        pytest.skip("not enough free device memory for configs[%d]" % k)
+    wl = W.config(k)
+    wl.params.rebuild_every = 4                       # both kinds of step within the run
+    with torch.cuda.stream(torch.cuda.Stream()):
+        s = B.Sph(wl.params, wl.n)
+        t = s.upload(wl)
+        s.build_neighbors(t, wl.n)
+        d0 = s.get_diagnostics().cpu().numpy()
+        dtu = torch.zeros(1, dtype=torch.float32, device="cuda")
+        elapsed = 0.0
+        for step in range(steps):
+            s.step(None, 0, 0.0, dtu)
+            elapsed += float(dtu.item())
+            c = _invariants(s, wl, f"config{k} step {step + 1}")
+        drift, scale = _internal_momentum_drift(s, wl, d0, elapsed)
+        torch.cuda.synchronize()
+    print(f"config{k} n={wl.n} {steps} steps: internal momentum drift {drift:.3g} of sum m|v| = {scale:.3g};"
+          f" dirty tiles {c['tiles_dirty']}, omega_small {c['omega_small']}")
+    assert drift <= 1e-5
