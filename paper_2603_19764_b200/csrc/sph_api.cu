@@ -186,6 +186,12 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
             return SPH_ECUDA;
         }
     }
+    if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess
+        || cudaEventCreateWithFlags(&c->ev_pos, cudaEventDisableTiming) != cudaSuccess
+        || cudaEventCreateWithFlags(&c->ev_copied, cudaEventDisableTiming) != cudaSuccess) {
+        sph_destroy(c);
+        return SPH_ECUDA;
+    }
     cudaError_t e = cudaMemsetAsync(c->d.counters, 0, SPH_C_COUNT * sizeof(unsigned long long), c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->d.dt_cur, 0, sizeof(float), c->stream);
     {
@@ -213,7 +219,11 @@ extern "C" void sph_destroy(sph_ctx *c)
 {
     if (!c) return;
     drop_graphs(c);
-    for (int k = 0; k < 2 * SPH_T_COUNT; ++k) cudaEventDestroy(c->ev[k]);
+    for (int k = 0; k < 2 * SPH_T_COUNT; ++k)
+        if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+    if (c->ev_pos) cudaEventDestroy(c->ev_pos);
+    if (c->ev_copied) cudaEventDestroy(c->ev_copied);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
 }
 
@@ -447,6 +457,19 @@ static int step_body(sph_ctx *c, sph_state *state, long long n, float dt, float 
     const bool adapt = step_adapts_h(c);
     rc = step_is_full(c) ? sph_build_neighbors(c, nullptr, 0) : reuse_neighbors(c);
     if (rc) return rc;
+    if (c->host_out && c->d.n > 0) {
+        // sph_step_host: the positions are final (drift and re-sort done): scatter them to the staging arrays and let
+        // the second stream carry them to the host while the pair passes run on this one
+        rc = sph_launch_download(c, c->host_out, 1);
+        if (rc) return rc;
+        SPH_CUDA(c, cudaEventRecord(c->ev_pos, c->stream));
+        SPH_CUDA(c, cudaStreamWaitEvent(c->copy_stream, c->ev_pos, 0));
+        float *src[3] = {c->host_out->x, c->host_out->y, c->host_out->z};
+        for (int k = 0; k < 3; ++k)
+            SPH_CUDA(c, cudaMemcpyAsync(c->host_dst[k], src[k], (size_t)c->d.n * sizeof(float), cudaMemcpyDeviceToHost,
+                                        c->copy_stream));
+        SPH_CUDA(c, cudaEventRecord(c->ev_copied, c->copy_stream));
+    }
     if (adapt) {
         // one Newton-Raphson update of h towards a constant kernel mass at the new positions (density
         // pass, update, tree and lists again); the method's own remedy for particles that lose their neighbours
@@ -460,7 +483,7 @@ static int step_body(sph_ctx *c, sph_state *state, long long n, float dt, float 
     if (rc) return rc;
     if (dt_used) SPH_CUDA(c, cudaMemcpyAsync(dt_used, c->d.dt_cur, sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
     if (state) {
-        rc = sph_launch_download(c, state);
+        rc = sph_launch_download(c, state, c->host_out ? 2 : 0);
         if (rc) return rc;
     }
     return SPH_OK;
@@ -593,16 +616,27 @@ extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, f
         c->force_full = true;                 // the caller's positions: nothing the lists were built on holds
         SPH_CUDA(c, cudaGetLastError());
     }
+    // every host-buffer step ingests the caller's positions, so its lists serve one step: built without skin and
+    // without the ordering pass; x, y, z go back on the second stream as soon as the drift is done (step_body)
+    c->no_reuse_now = true;
+    const bool overlap = c->resident && n > 0;          // (the very first call ingests and bootstraps first)
+    if (overlap) {
+        c->host_out = &ds;
+        c->host_dst[0] = hs->x; c->host_dst[1] = hs->y; c->host_dst[2] = hs->z;
+    }
     rc = sph_step(c, &ds, n, dt, nullptr);
+    c->host_out = nullptr;
+    c->no_reuse_now = false;
     if (rc) return rc;
     float *dst[14] = {hs->x, hs->y, hs->z, nullptr, nullptr, hs->vx, hs->vy, hs->vz, hs->u,
                       hs->Sxx, hs->Syy, hs->Sxy, hs->Sxz, hs->Syz};
-    for (int k = 0; k < 14; ++k) {
+    for (int k = overlap ? 3 : 0; k < 14; ++k) {
         if (n > 0 && dst[k])
             SPH_CUDA(c, cudaMemcpyAsync(dst[k], dev[k], (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     }
     if (dt_used) SPH_CUDA(c, cudaMemcpyAsync(dt_used, c->d.dt_cur, sizeof(float), cudaMemcpyDeviceToHost, c->stream));
     SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (overlap) SPH_CUDA(c, cudaEventSynchronize(c->ev_copied));
     return SPH_OK;
 }
 
@@ -610,7 +644,7 @@ extern "C" int sph_download_state(sph_ctx *c, sph_state *state)
 {
     if (!c || !state_ok(state)) return SPH_EINVAL;
     if (!c->resident) return SPH_EORDER;
-    return sph_launch_download(c, state);
+    return sph_launch_download(c, state, 0);
 }
 
 // ------------------------------------------------------------------------------------------

@@ -161,8 +161,14 @@ struct sph_ctx {
     bool resident, have_density, have_predict, have_grad, have_force, have_derivs;
     cudaEvent_t ev[2 * SPH_T_COUNT];
     bool ev_used[SPH_T_COUNT];
-    // host staging for sph_step_host
-    float *stage;            // device: 17 floats + 2 words per particle
+    // sph_step_host: device staging (17 floats + 2 words per particle), a second stream that carries the positions back
+    // to the host while the pair passes still run, and the state they go to
+    float *stage;
+    cudaStream_t copy_stream;
+    cudaEvent_t ev_pos, ev_copied;
+    sph_state *host_out;     // != NULL inside sph_step_host: {device staging arrays}; host_dst: where x, y, z go on the host
+    float *host_dst[3];
+    bool no_reuse_now;       // the lists of this build will not be reused (host-buffer steps): no skin, no ordering pass
     size_t ws_bytes;
 };
 
@@ -195,7 +201,7 @@ int sph_launch_get_h(sph_ctx *c, float *dst);
 int sph_launch_diagnostics(sph_ctx *c, double *out);
 int sph_launch_h_update(sph_ctx *c, float n_target);
 int sph_launch_neighbors(sph_ctx *c, int which, int *counts, const long long *offsets, int *list, bool flagged_only);
-int sph_launch_download(sph_ctx *c, sph_state *st);
+int sph_launch_download(sph_ctx *c, sph_state *st, int part);      // part: 0 everything, 1 positions, 2 the rest
 int sph_launch_cull(sph_ctx *c, bool dirty_only);
 int sph_launch_list_sort(sph_ctx *c);
 int sph_launch_density_l(sph_ctx *c);

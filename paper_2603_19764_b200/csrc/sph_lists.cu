@@ -970,13 +970,14 @@ int sph_launch_cull(sph_ctx *c, bool dirty_only)
     int rc = set_smem(c, (const void *)k_cull, sizeof(CullSmem));
     if (rc) return rc;
     int ntile = sph_div_up(d.nchunk, SPH_TILE_CHUNKS);
-    const float infl = 1.f + (d.skin > 0.f ? d.skin : 0.f);
+    const bool reuse = d.skin > 0.f && !c->no_reuse_now;
+    const float infl = 1.f + (reuse ? d.skin : 0.f);
     k_tile_plan<<<1, 1024, 0, c->stream>>>(d, ntile, dirty_only ? 1 : 0);
     k_cull<<<d.heavy_cap + ntile, SPH_TILE, sizeof(CullSmem), c->stream>>>(d, c->p.kappa, infl, infl * infl, ntile,
                                                                             dirty_only ? 1 : 0);
     c->launches += 2;
     SPH_CUDA(c, cudaGetLastError());
-    if (!dirty_only && d.skin > 0.f) return sph_launch_list_sort(c);      // lists that will be reused: order them
+    if (!dirty_only && reuse) return sph_launch_list_sort(c);      // lists that will be reused: order them
     return SPH_OK;
 }
 

@@ -178,6 +178,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(Dev d, DevParams p, co
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     PairConst kc;
     kc.beta = p.beta; kc.alpha2 = 0.5f * p.alpha; kc.eps = p.eps_av; kc.hk = 0.5f / p.kappa;
+    if (tile_flag && d.counters[SPH_C_LIST_OVERFLOW] == 0ull) return;       // serving flagged tiles: there are none
     for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
     if (tile_flag && !tile_flag[tile]) continue;
     const int chunk = tile * PAIR_WARPS + warp;

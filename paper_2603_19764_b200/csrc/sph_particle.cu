@@ -303,13 +303,17 @@ __global__ void __launch_bounds__(256) k_scatter_pos(const float4 *__restrict__ 
     dst[orig[i]] = comp == 0 ? q.x : (comp == 1 ? q.y : q.z);
 }
 
-__global__ void __launch_bounds__(256) k_download(Dev d, sph_state st)
+// part: 0 everything, 1 the positions only (final once the drift is done), 2 everything but the positions
+__global__ void __launch_bounds__(256) k_download(Dev d, sph_state st, int part)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= d.n) return;
     unsigned o = ((const unsigned *)d.r.s[PP_ORIG])[i];
-    float4 pm = d.r.pm[i];
-    st.x[o] = pm.x; st.y[o] = pm.y; st.z[o] = pm.z;
+    if (part != 2) {
+        float4 pm = d.r.pm[i];
+        st.x[o] = pm.x; st.y[o] = pm.y; st.z[o] = pm.z;
+    }
+    if (part == 1) return;
     st.vx[o] = d.vfull[0][i]; st.vy[o] = d.vfull[1][i]; st.vz[o] = d.vfull[2][i];
     st.u[o] = d.ufull[i];
     st.Sxx[o] = d.Sfull[0][i]; st.Syy[o] = d.Sfull[1][i]; st.Sxy[o] = d.Sfull[2][i];
@@ -491,11 +495,11 @@ int sph_launch_get_position(sph_ctx *c, int comp, float *dst)
     return SPH_OK;
 }
 
-int sph_launch_download(sph_ctx *c, sph_state *st)
+int sph_launch_download(sph_ctx *c, sph_state *st, int part)
 {
     Dev &d = c->d;
     if (d.n == 0) return SPH_OK;
-    k_download<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, *st);
+    k_download<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, *st, part);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
