@@ -509,3 +509,109 @@ class Stepper:
         self.d = d
         self.dt_next = float(d["dt_i"].min())
         return dt
+
+
+# ---------------------------------------------------------------------------
+# NEXT-4: individual (hierarchical) time steps on power-of-two rungs ("the hierarchical individual
+# timestep scheme described in Paper I"; "8 substeps").  Paper I is not available: reading Q23.
+# ---------------------------------------------------------------------------
+def rung_for(dt_i, dT, max_rung):
+    """Smallest rung r in [0, max_rung] with dT / 2^r <= dt_i (rung 0 takes the whole big step dT; a particle
+    whose limit is below dT / 2^max_rung sits on max_rung: the caller chose dT too large for it)."""
+    with np.errstate(divide="ignore"):
+        r = np.ceil(np.log2(dT / dt_i))
+    r = np.where(np.isnan(r), 0.0, r)                     # dt_i = 0 -> +inf -> max_rung; dt_i = inf -> -inf -> 0
+    return np.clip(r, 0, max_rung).astype(np.int64)
+
+
+def next_rung(wanted, current, n_done, max_rung):
+    """Rung of a particle that has just finished a step at the end of substep n_done - 1 (n_done substeps of the
+    big step are done).  It may always move to a FINER rung; to a coarser one only as far as that rung's step
+    boundaries line up with the present time: rung r has steps of 2^(max_rung - r) substeps, so it may start at
+    n_done only if n_done is a multiple of that."""
+    out = np.maximum(wanted, 0).copy()
+    for r in range(max_rung + 1):                         # coarsest admissible rung at this time
+        ok = (n_done % (1 << (max_rung - r))) == 0
+        if ok:
+            coarsest = r
+            break
+    out = np.maximum(out, coarsest)
+    return np.minimum(out, max_rung)
+
+
+class RungStepper(Stepper):
+    """Kick-drift-kick on block time steps (reading Q23).  One BIG step dT = 2^R substeps of delta = dT / 2^R.
+    A particle on rung r takes steps of dt_r = dT / 2^r.  In every substep
+      * particles that START a step get the opening kick with their own dt_r (Eq. 42),
+      * EVERY particle drifts by delta with its half-step velocity,
+      * the values of every particle are PREDICTED to the new time from its last derivatives
+        (Eq. 40 generalised: q_pred = q_half + (t - t_mid) dq/dt, t_mid the middle of the particle's step),
+      * the derivatives are evaluated from the predicted values; particles that END a step here (the ACTIVE ones)
+        take them, get the closing kick with their own dt_r (Eq. 41) and the rescale, and choose their next rung
+        from their new limit (Eq. 38-39); the others keep their old derivatives and only lend their predicted
+        values to their active neighbours.
+    rho, P, Y, ... of every particle are evaluated at the current positions in every substep (they depend on
+    positions and predicted u only; nothing is extrapolated).  With every particle on rung 0 and R = 0 this is
+    Stepper.step(dT), operation for operation."""
+
+    def __init__(self, wl, mode="grid", store_fp32=False):
+        super().__init__(wl, mode, store_fp32)
+        self.rung = None
+        self.kicks = None           # closing kicks each particle received in the last big step
+        self.trace = []             # per substep: predicted S handed to the derivative evaluation (pins)
+
+    def big_step(self, dT, max_rung, rungs=None):
+        if self.d is None:
+            self.bootstrap()
+        R = int(max_rung)
+        nsubs = 1 << R
+        delta = dT / nsubs
+        n = self.u.shape[0]
+        fr = self.free[None, :]
+        st = self._st
+        self.rung = rung_for(self.d["dt_i"], dT, R) if rungs is None else np.asarray(rungs, dtype=np.int64).copy()
+        self.kicks = np.zeros(n, dtype=np.int64)
+        self.trace = []
+        a, dudt, dS = self.d["a"].copy(), self.d["dudt"].copy(), self.d["dS"].copy()
+        dt_i = self.d["dt_i"].copy()
+        v_half = self.v.copy(); u_half = self.u.copy(); S_half = self.S.copy()
+        last = None
+        for k in range(nsubs):
+            per = 1 << (R - self.rung)                      # substeps per step of each particle's rung
+            dtr = dT / (1 << self.rung)                     # its step
+            start = (k % per) == 0
+            # opening kick (PAPER.md:246, Eq. 42) of the particles that start a step now
+            v_half = np.where(start[None, :], st(self.v + 0.5 * dtr * a * fr), v_half)
+            u_half = np.where(start, st(self.u + 0.5 * dtr * dudt), u_half)
+            S_half = np.where(start[None, :], st(self.S + 0.5 * dtr * dS), S_half)
+            # drift of every particle
+            self.x = st(self.x + delta * v_half * fr)
+            # prediction to the new time from each particle's own last derivatives (Eq. 40 generalised)
+            tau = ((k % per) + 1) * delta - 0.5 * dtr         # t_new - t_mid
+            v_pred = st(v_half + tau * a * fr)
+            u_pred = st(u_half + tau * dudt)
+            S_pred = st(S_half + tau * dS)
+            d = self._derivs(v_pred, u_pred, S_pred)
+            act = ((k + 1) % per) == 0
+            self.trace.append({"S_pred_in": S_pred.copy(), "active": act.copy(), "rung": self.rung.copy()})
+            # closing kick (Eq. 41) and rescale (PAPER.md:244) of the active particles, with their own step
+            self.v = np.where(act[None, :], st(v_half + 0.5 * dtr * d["a"] * fr), self.v)
+            self.u = np.where(act, st(u_half + 0.5 * dtr * d["dudt"]), self.u)
+            if self.strength:
+                Sc = st(project(S_half + 0.5 * dtr * d["dS"], d["Y"])[0])
+                self.S = np.where(act[None, :], Sc, self.S)
+            self.e_acc = np.where(act, st(self.e_acc + dtr * d["eps2"]), self.e_acc)
+            a = np.where(act[None, :], d["a"], a)
+            dudt = np.where(act, d["dudt"], dudt)
+            dS = np.where(act[None, :], d["dS"], dS)
+            dt_i = np.where(act, d["dt_i"], dt_i)
+            self.kicks += act
+            if rungs is None:
+                nr = next_rung(rung_for(dt_i, dT, R), self.rung, k + 1, R)
+                self.rung = np.where(act, nr, self.rung)
+            last = d
+        # every particle has finished a step at the end of the big step: the state is synchronised
+        self.d = dict(last)
+        self.d.update(a=a, dudt=dudt, dS=dS, dt_i=dt_i)
+        self.dt_next = float(dt_i.min())
+        return dT
