@@ -79,6 +79,7 @@ enum {
     SPH_F_NGATHER,      /* |gather set| as float                          */
     SPH_F_NSYMMETRIC,   /* |symmetric set| as float                       */
     SPH_F_H,            /* smoothing length (after sph_adapt_h)           */
+    SPH_F_RUNG,         /* rung of the last sph_step_rungs, as float      */
     SPH_F_A = 32,       /* +0..2   acceleration, Eq. 18 (+ a_ext)         */
     SPH_F_V = 36,       /* +0..2   velocity after the closing kick        */
     SPH_F_X = 40,       /* +0..2   position                               */
@@ -112,6 +113,9 @@ enum { SPH_C_PAIRS_GATHER = 0,   /* sum_i |gather set(i)|   (true pairs of the d
        SPH_C_NONFINITE,          /* particles whose a, du/dt or dS/dt was not finite in the last CLOSE      */
        SPH_C_TILES_DIRTY,        /* sph_params.skin > 0: tiles whose lists are rebuilt in every step since the
                                     last full build (0 right after one)                                      */
+       SPH_C_ACTIVE_UPDATES,     /* sph_step_rungs: closing kicks done in the last big step (n 2^max_rung if every
+                                    particle sat on the finest rung)                                           */
+       SPH_C_ACTIVE_TILES,       /* sph_step_rungs: tiles the pair pass worked on, summed over the substeps    */
        SPH_C_LIST_SLOTS,         /* list slots the pair passes step through per launch: entries plus the padding
                                     that makes the 32 lists of a chunk equally long in every round (last build) */
        SPH_C_COUNT };
@@ -232,6 +236,20 @@ int sph_gradients_forces(sph_ctx *ctx);
  * end; state == NULL: everything stays resident.  dt > 0: use it; dt <= 0: use the CFL step of
  * the previous derivatives (Eq. 39).  dt_used: DEVICE pointer to one float, or NULL. */
 int sph_step(sph_ctx *ctx, sph_state *state, long long n, float dt, float *dt_used);
+
+/* NEXT-4 ("hierarchical individual timestep scheme"; reading Q23 in DESIGN.md): ONE BIG
+ * STEP dT of the resident particles on power-of-two rungs.  dT is split into 2^max_rung substeps; a particle on rung r
+ * takes steps dT / 2^r, r the smallest rung whose step is within the particle's limit (Eq. 38-39) from its last
+ * CLOSE.  Per substep: opening kick of the particles that start a step, drift of all, prediction of all to the new
+ * time from their own last derivatives, neighbour lists (reused, checked, rebuilt where dirty), then density and
+ * PREDICT for the tiles that hold an active particle or a neighbour of one, the fused pair pass for the tiles that
+ * hold an active particle, CLOSE (own step, rescale, next rung) for the active particles only: tiles (256 particles)
+ * without active particles cost nothing in the pair passes.  The particle order is kept for the whole big step.
+ * rungs: DEVICE unsigned char[n] in caller order = fixed rungs for this big step (test hook), or NULL = from the
+ * limits.  max_rung in [0, 16]; dT > 0.  Needs a resident state; derivatives are bootstrapped if none are carried.
+ * Afterwards every particle is at t + dT; SPH_F_RUNG has the rungs, SPH_C_ACTIVE_UPDATES the closing kicks done.
+ * Errors: EINVAL, EORDER. */
+int sph_step_rungs(sph_ctx *ctx, float dT, int max_rung, const unsigned char *rungs);
 
 /* The same step through HOST buffers: copies the state host->device into library-owned staging,
  * steps, copies x, v, u, S back device->host, and synchronises the stream.  dt_used: HOST. */

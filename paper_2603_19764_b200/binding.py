@@ -22,17 +22,17 @@ PREDICT, CLOSE, DERIVATIVES = 0, 1, 2
 GATHER, SYMMETRIC = 0, 1
 
 F = dict(RHO=0, OMEGA=1, P=2, CS=3, T=4, GAMMA=5, Y=6, MUMAX=7, DUDT=8, DT=9, EACC=10, EPS2=11, U=12,
-         CFLAG=13, NGATHER=14, NSYMMETRIC=15, H=16, A=32, V=36, X=40, SPRED=48, S=56, DSDT=64, F=80, CINV=96, G=112)
+         CFLAG=13, NGATHER=14, NSYMMETRIC=15, H=16, RUNG=17, A=32, V=36, X=40, SPRED=48, S=56, DSDT=64, F=80, CINV=96, G=112)
 T_SLOTS = ("build", "density", "predict", "gradient", "force", "close", "kickdrift", "step")
 C_SLOTS = ("pairs_gather", "pairs_symmetric", "tests_density", "tests_force", "cfallback", "tests_cull",
-           "candidates", "list_overflow", "bad_material", "omega_small", "nonfinite", "tiles_dirty", "list_slots")
+           "candidates", "list_overflow", "bad_material", "omega_small", "nonfinite", "tiles_dirty", "active_updates", "active_tiles", "list_slots")
 
 FLOAT_FIELDS = ("x", "y", "z", "m", "h", "vx", "vy", "vz", "u", "Sxx", "Syy", "Sxy", "Sxz", "Syz")
 OPT_FIELDS = ("gx", "gy", "gz")
 
 # every symbol include/sph.h declares (tests check the library exports all of them)
 SYMBOLS = ("sph_workspace_bytes", "sph_init", "sph_build_neighbors", "sph_density", "sph_strength_update",
-           "sph_gradients", "sph_forces", "sph_gradients_forces", "sph_fp32_peak", "sph_adapt_h", "sph_set_eos_table", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
+           "sph_gradients", "sph_forces", "sph_gradients_forces", "sph_fp32_peak", "sph_step_rungs", "sph_adapt_h", "sph_set_eos_table", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
            "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_get_diagnostics", "sph_launch_count",
            "sph_last_cuda_error", "sph_strerror", "sph_destroy")
 
@@ -110,6 +110,8 @@ def load():
     lib.sph_gradients_forces.restype = i
     lib.sph_fp32_peak.argtypes = [vp, i, C.POINTER(C.c_double)]
     lib.sph_fp32_peak.restype = i
+    lib.sph_step_rungs.argtypes = [vp, fl, i, vp]
+    lib.sph_step_rungs.restype = i
     lib.sph_step.argtypes = [vp, C.POINTER(sph_state), ll, fl, vp]
     lib.sph_step_host.argtypes = [vp, C.POINTER(sph_state), ll, fl, vp]
     lib.sph_download_state.argtypes = [vp, C.POINTER(sph_state)]
@@ -259,6 +261,10 @@ class Sph:
         if tensors is not None:
             self.n = n
         self._check(self.lib.sph_step(self.ctx, st, n, dt, _ptr(dt_used)), "sph_step")
+
+    def step_rungs(self, dT: float, max_rung: int, rungs=None):
+        """sph_step_rungs; rungs: optional uint8 device tensor [n] in caller order (fixed rungs)."""
+        self._check(self.lib.sph_step_rungs(self.ctx, float(dT), int(max_rung), _ptr(rungs)), "sph_step_rungs")
 
     def step_host(self, host: Dict[str, object], n: int, dt: float = 0.0) -> float:
         """host: dict of (pinned) CPU torch tensors / numpy arrays keyed like sph_state."""

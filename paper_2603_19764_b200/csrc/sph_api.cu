@@ -111,6 +111,9 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
     o.nheavy = b.take<unsigned>(1);
     o.heavy_mark = b.take<unsigned char>(ntile);
     o.tile_dirty = b.take<unsigned char>(ntile);
+    o.tile_act = b.take<unsigned char>(ntile);
+    o.tile_need = b.take<unsigned char>(ntile);
+    o.rung = b.take<unsigned char>(N);
     o.cand_cursor = b.take<unsigned long long>(2);
     o.cand_cap = lists ? (unsigned long long)ntile * (2 * SPH_SE) : 1;   // pool: twice the one-round average
     o.cand_cap_dirty = (lists && skin > 0.f) ? (unsigned long long)ntile * SPH_SE : 0;
@@ -561,6 +564,67 @@ extern "C" int sph_step(sph_ctx *c, sph_state *state, long long n, float dt, flo
     return SPH_OK;
 }
 
+// NEXT-4: one big step on power-of-two rungs (reading Q23; include/sph.h).  Kernel by kernel: every substep has its
+// own arguments, and most of them touch a fraction of the tiles only.
+extern "C" int sph_step_rungs(sph_ctx *c, float dT, int max_rung, const unsigned char *rungs)
+{
+    if (!c || !(dT > 0.f) || max_rung < 0 || max_rung > 16) return SPH_EINVAL;
+    if (!c->resident) return SPH_EORDER;
+    int rc;
+    PassTimer ts(c, SPH_T_STEP);
+    if (!c->have_derivs) {          // a_0, du_0/dt, dS_0/dt and the limits from the current state
+        rc = derivative_passes(c);
+        if (rc) return rc;
+        rc = do_close(c, SPH_DERIVATIVES, 0.f, false);
+        if (rc) return rc;
+    }
+    Dev &d = c->d;
+    // the lists of the big step: built here at the current positions, particle order kept throughout
+    if (c->use_lists) {
+        PassTimer t(c, SPH_T_BUILD);
+        rc = sph_launch_tree(c);
+        if (rc) return rc;
+        rc = sph_launch_set_ref(c);
+        if (rc) return rc;
+        rc = sph_launch_cull(c, false);
+        if (rc) return rc;
+        c->steps_since_full = 0;
+        c->force_full = false;
+    }
+    rc = sph_launch_rung_assign(c, dT, max_rung, rungs);
+    if (rc) return rc;
+    SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_ACTIVE_UPDATES], 0, 2 * sizeof(unsigned long long), c->stream));
+    const bool strength = (c->p.flags & SPH_STRENGTH) != 0;
+    for (int n = 0; n < (1 << max_rung); ++n) {
+        {
+            PassTimer t(c, SPH_T_KICKDRIFT);
+            rc = sph_launch_kick_drift_rung(c, n, max_rung, dT);
+            if (rc) return rc;
+        }
+        if (c->use_lists && d.skin > 0.f) {
+            rc = reuse_neighbors(c);
+        } else {
+            PassTimer t(c, SPH_T_BUILD);
+            rc = sph_launch_tree(c);
+            if (!rc && c->use_lists) rc = sph_launch_cull(c, false);
+            c->have_density = c->have_predict = c->have_grad = c->have_force = false;
+        }
+        if (rc) return rc;
+        rc = sph_launch_mark_need(c);
+        if (rc) return rc;
+        c->rc.on = 1; c->rc.n1 = n + 1; c->rc.R = max_rung; c->rc.dT = dT; c->rc.fixed_rungs = rungs ? 1 : 0;
+        c->rc.rung = d.rung; c->rc.tile_act = d.tile_act; c->rc.tile_need = d.tile_need;
+        rc = derivative_passes(c);
+        if (!rc) rc = do_close(c, SPH_CLOSE, 0.f, false);
+        c->rc.on = 0;
+        if (rc) return rc;
+        (void)strength;
+    }
+    c->step_count++;
+    c->force_full = true;            // a global step after this starts from a full build (re-sort)
+    return SPH_OK;
+}
+
 // refresh the resident state from caller-order device arrays, keeping order and derivatives
 __global__ void __launch_bounds__(256) k_refresh(Dev d, sph_state st)
 {
@@ -675,6 +739,7 @@ extern "C" int sph_get_field(sph_ctx *c, int id, float *dst)
     case SPH_F_NGATHER: src = (const float *)d.ngather; as_int = 1; break;
     case SPH_F_NSYMMETRIC: src = (const float *)d.nsym; as_int = 1; break;
     case SPH_F_H: return sph_launch_get_h(c, dst);
+    case SPH_F_RUNG: src = (const float *)d.rung; as_int = 2; break;
     default: break;
     }
     if (!src) {

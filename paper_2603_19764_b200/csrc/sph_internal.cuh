@@ -73,6 +73,19 @@ struct Tree {
     float4 *dhi[SPH_MAX_LEVELS];
 };
 
+// NEXT-4 (sph_step_rungs): which particles / tiles a pass of a substep works on.  on == 0: everything (global step).
+// A particle on rung r is ACTIVE at the end of substep n (n1 = n + 1 substeps done) iff n1 is a multiple of
+// 2^(R - r).  need: tiles that hold an active particle or a candidate neighbour of one (density, PREDICT);
+// act: tiles that hold an active particle (pair pass).
+struct RungCtl {
+    int on;
+    int n1, R;
+    float dT;
+    int fixed_rungs;                 // keep the rungs (test hook)
+    const unsigned char *rung;       // per particle, current sorted order
+    const unsigned char *tile_act, *tile_need;
+};
+
 // Everything the kernels need, passed by value.
 struct Dev {
     long long n;       // particles resident
@@ -103,6 +116,8 @@ struct Dev {
     // at the current positions in every step until then
     float skin;                             // 0: off (every step is a full build)
     float4 *xref;                           // positions at the last full build (current sorted order)
+    unsigned char *rung;                    // NEXT-4: rung per particle (current sorted order)
+    unsigned char *tile_act, *tile_need;    // NEXT-4: per tile, see RungCtl
     unsigned char *tile_dirty;              // sticky until the next full build
     uint2 *nlist;                           // [chunk][row-group][lane]: 4 x u16 per lane = byte offsets (slot * 16)
                                             // into the round's staged arrays; 0xFFFF = no entry
@@ -155,6 +170,7 @@ struct sph_ctx {
     int adapt_h_every;               // > 0: one iteration of sph_adapt_h every so many steps, inside sph_step
     float adapt_h_target;
     long long step_count;            // steps taken since the state was ingested
+    RungCtl rc;                      // on only inside sph_step_rungs
     int rebuild_every;               // steps between two full list builds when skin > 0
     int steps_since_full;            // steps taken since the last full build
     bool force_full;                 // the next step must do a full build (state refreshed, h changed, ...)
@@ -195,6 +211,9 @@ int sph_launch_pair(sph_ctx *c, bool grad, bool force, bool flagged_only);
 int sph_launch_predict(sph_ctx *c);
 int sph_launch_close(sph_ctx *c, int phase, float dt, bool dt_from_device);
 int sph_launch_kick_drift(sph_ctx *c, float dt);
+int sph_launch_rung_assign(sph_ctx *c, float dT, int R, const unsigned char *rungs);
+int sph_launch_kick_drift_rung(sph_ctx *c, int n, int R, float dT);
+int sph_launch_mark_need(sph_ctx *c);
 int sph_launch_get_field(sph_ctx *c, const float *src, float *dst, int as_int);
 int sph_launch_get_position(sph_ctx *c, int comp, float *dst);
 int sph_launch_get_h(sph_ctx *c, float *dst);
@@ -210,6 +229,12 @@ int sph_launch_neighbors_l(sph_ctx *c, int which, int *counts, const long long *
 
 // ---- small device helpers ----------------------------------------------------------------
 #ifdef __CUDACC__
+// is particle i active at the end of this substep? (everything is, outside sph_step_rungs)
+__device__ __forceinline__ bool sph_active(const RungCtl &rc, long long i)
+{
+    return !rc.on || ((rc.n1 & ((1 << (rc.R - (int)rc.rung[i])) - 1)) == 0);
+}
+
 __device__ __forceinline__ float sph_r2(float dx, float dy, float dz)
 {
     // reading Q4: every multiply and add rounded separately (no FMA contraction)

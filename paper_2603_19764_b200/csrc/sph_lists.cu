@@ -722,12 +722,13 @@ __device__ __forceinline__ unsigned list_entry(uint2 w, int e)
 // staged a second time widened to fp64 (48 B per slot, no conversions in the loop): 0.39 ms with one or two
 // warps per chunk -- three random LDS.128 per pair instead of one: the shared-memory pipe binds: rejected.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
+__global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa, RungCtl rc)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4 *s_pm = reinterpret_cast<float4 *>(smem_raw);
     const int tile = sph_tile_of_block(d, blockIdx.x);
     if (tile < 0 || d.tile_flag[tile]) return;
+    if (rc.on && !rc.tile_need[tile]) return;              // NEXT-4: no active particle reads this tile's density now
     const int ncand = d.tile_ncand[tile];
     const unsigned *cand = d.cand + d.tile_off[tile];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -805,13 +806,14 @@ __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa)
 // hydro-only variant stages the first three arrays only).
 // ------------------------------------------------------------------------------------------
 template <bool GRAD, bool FORCE, bool TENSOR>
-__global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p)
+__global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p, RungCtl rc)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     unsigned char *s1 = smem_raw, *s2 = s1 + SPH_SE * 16, *s3 = s2 + SPH_SE * 16, *s4 = s3 + SPH_SE * 16,
                   *s5 = s4 + SPH_SE * 16;
     const int tile = sph_tile_of_block(d, blockIdx.x);
     if (tile < 0 || d.tile_flag[tile]) return;
+    if (rc.on && !rc.tile_act[tile]) return;               // NEXT-4: no particle of this tile ends a step now
     const int ncand = d.tile_ncand[tile];
     const unsigned *cand = d.cand + d.tile_off[tile];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -879,12 +881,13 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p)
         __syncthreads();
     }
 
-    if (valid) {
+    const bool keep = valid && sph_active(rc, i);          // NEXT-4: an inactive particle keeps its old derivatives
+    if (keep) {
         pair_store<GRAD, FORCE>(d, i, A);
         d.nsym[i] = cnt;
     }
     if (FORCE) {
-        unsigned long long hits = valid ? (unsigned long long)cnt : 0ull, ents = valid ? (unsigned long long)nent : 0ull;
+        unsigned long long hits = keep ? (unsigned long long)cnt : 0ull, ents = valid ? (unsigned long long)nent : 0ull;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             hits += __shfl_xor_sync(FULL, hits, o);
@@ -1095,7 +1098,7 @@ int sph_launch_density_l(sph_ctx *c)
     size_t bytes = (size_t)SPH_SE * sizeof(float4);
     int rc = set_smem(c, (const void *)k_density_l, bytes);
     if (rc) return rc;
-    k_density_l<<<d.heavy_cap + sph_div_up(d.nchunk, SPH_TILE_CHUNKS), SPH_TILE, bytes, c->stream>>>(d, c->p.kappa);
+    k_density_l<<<d.heavy_cap + sph_div_up(d.nchunk, SPH_TILE_CHUNKS), SPH_TILE, bytes, c->stream>>>(d, c->p.kappa, c->rc);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return sph_launch_density(c, true);               // the flagged tiles, if any
@@ -1108,7 +1111,7 @@ static int launch_pair_l(sph_ctx *c)
     size_t bytes = (size_t)SPH_SE * (TENSOR ? 68 : 48);
     int rc = set_smem(c, (const void *)k_pair_l<GRAD, FORCE, TENSOR>, bytes);
     if (rc) return rc;
-    k_pair_l<GRAD, FORCE, TENSOR><<<d.heavy_cap + sph_div_up(d.nchunk, SPH_TILE_CHUNKS), SPH_TILE, bytes, c->stream>>>(d, c->p);
+    k_pair_l<GRAD, FORCE, TENSOR><<<d.heavy_cap + sph_div_up(d.nchunk, SPH_TILE_CHUNKS), SPH_TILE, bytes, c->stream>>>(d, c->p, c->rc);
     return SPH_OK;
 }
 

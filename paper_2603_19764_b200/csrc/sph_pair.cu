@@ -169,7 +169,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_density(Dev d, float kappa,
 // Equations and operand packing: sph_pairterm.cuh.
 // ------------------------------------------------------------------------------------------
 template <bool GRAD, bool FORCE, bool EXACT>
-__global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(Dev d, DevParams p, const unsigned char *__restrict__ tile_flag, int ntile)
+__global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(Dev d, DevParams p, const unsigned char *__restrict__ tile_flag, int ntile, RungCtl rc)
 {
     __shared__ float4 s_src[PAIR_WARPS][4][SPH_CHUNK];
     __shared__ float s_src5[PAIR_WARPS][SPH_CHUNK];
@@ -227,12 +227,13 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(Dev d, DevParams p, co
         __syncwarp();
     });
 
-    if (valid) {
+    const bool keep = valid && sph_active(rc, i);          // NEXT-4: an inactive particle keeps its old derivatives
+    if (keep) {
         pair_store<GRAD, FORCE>(d, i, A);
         d.nsym[i] = cnt_i;
     }
     if (FORCE) {
-        unsigned long long hits = valid ? (unsigned long long)cnt_i : 0ull;
+        unsigned long long hits = keep ? (unsigned long long)cnt_i : 0ull;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) hits += __shfl_xor_sync(0xffffffffu, hits, o);
         if (lane == 0) {
@@ -342,13 +343,13 @@ int sph_launch_pair(sph_ctx *c, bool grad, bool force, bool flagged_only)
     dim3 grid(walk_grid_of(d, flagged_only, ntile)), block(PAIR_WARPS * 32);
     const unsigned char *tf = flagged_only ? d.tile_flag : nullptr;
     if (flagged_only) {
-        if (grad && force) k_pair<true, true, true><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
-        else if (grad) k_pair<true, false, true><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
-        else k_pair<false, true, true><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
+        if (grad && force) k_pair<true, true, true><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile, c->rc);
+        else if (grad) k_pair<true, false, true><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile, c->rc);
+        else k_pair<false, true, true><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile, c->rc);
     } else {
-        if (grad && force) k_pair<true, true, false><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
-        else if (grad) k_pair<true, false, false><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
-        else k_pair<false, true, false><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile);
+        if (grad && force) k_pair<true, true, false><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile, c->rc);
+        else if (grad) k_pair<true, false, false><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile, c->rc);
+        else k_pair<false, true, false><<<grid, block, 0, c->stream>>>(d, c->p, tf, ntile, c->rc);
     }
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());

@@ -54,10 +54,11 @@ __device__ __forceinline__ float plastic_factor(const float S[5], float Y)
 //   B3 = {rho, c, w, st_xx}, B4 = {st_yy, st_zz, st_xy, st_xz}, B5 = st_yz
 //   w = 1/(Omega rho), st = (-P delta + S_pred)/(Omega rho^2)
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_predict(Dev d, DevParams p, DevTabs tabs)
+__global__ void __launch_bounds__(256) k_predict(Dev d, DevParams p, DevTabs tabs, RungCtl rc)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= d.n) return;
+    if (rc.on && !rc.tile_need[i / SPH_TILE]) return;        // NEXT-4: nobody reads this particle in this substep
     unsigned mf = ((const unsigned *)d.r.s[PP_MATFIX])[i];
     const sph_material &m = p.mat[mf & 0xffu];
     float rho = d.rho[i], om = d.omega[i], u = d.r.s[PP_UPRED][i];
@@ -109,13 +110,16 @@ __global__ void __launch_bounds__(256) k_predict(Dev d, DevParams p, DevTabs tab
 // ------------------------------------------------------------------------------------------
 // Also S8: the block's minimum of dt_i goes into dt_next with one atomicMin (positive floats order like
 // unsigned ints; k_dt_select / k_dt_reset set dt_next to +inf before), and the robustness counters.
-__global__ void __launch_bounds__(256) k_close(Dev d, DevParams p, int phase, float dt_arg, int dt_from_device)
+// NEXT-4 (rc.on): only the active particles; the step of the closing kick is the particle's own, dT / 2^rung, and
+// the particle chooses its next rung from its new limit (reading Q23).
+__global__ void __launch_bounds__(256) k_close(Dev d, DevParams p, int phase, float dt_arg, int dt_from_device, RungCtl rc)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     float dti = __int_as_float(0x7f800000);
-    unsigned nfall = 0u, nbad = 0u;
-    if (i < d.n) {
-    const float dt = dt_from_device ? *d.dt_cur : dt_arg;
+    unsigned nfall = 0u, nbad = 0u, nact = 0u;
+    if (i < d.n && sph_active(rc, i)) {
+    float dt = dt_from_device ? *d.dt_cur : dt_arg;
+    if (rc.on) { dt = rc.dT / (float)(1 << (int)d.rung[i]); nact = 1u; }
     const bool strength = (p.flags & SPH_STRENGTH) != 0;
     unsigned mf = ((const unsigned *)d.r.s[PP_MATFIX])[i];
     const bool fixed = (mf >> 8) & 1u;
@@ -208,11 +212,23 @@ __global__ void __launch_bounds__(256) k_close(Dev d, DevParams p, int phase, fl
         for (int c = 0; c < 5; ++c) d.Sfull[c][i] = S[c];
         d.r.s[PP_EACC][i] = fmaf(dt, eps2, d.r.s[PP_EACC][i]);
     }
-    }   // i < d.n
+    if (rc.on && !rc.fixed_rungs) {
+        // next rung: the smallest one whose step is within the new limit, but no coarser than the rungs whose
+        // steps line up with the present time (n1 substeps of 2^R done)
+        int want = 0;
+        while (want < rc.R && rc.dT / (float)(1 << want) > dti) ++want;
+        const int tz = rc.n1 >= (1 << rc.R) ? rc.R : (__ffs(rc.n1) - 1);
+        d.rung[i] = (unsigned char)min(rc.R, max(want, rc.R - tz));
+    }
+    }   // i < d.n and active
     // S8 and the counters: one atomic per block
     __shared__ float s_dt[8];
     __shared__ unsigned s_cnt[8];
     unsigned packed = nfall | (nbad << 16);
+    if (rc.on) {
+        const unsigned na = __popc(__ballot_sync(0xffffffffu, nact != 0u));
+        if ((threadIdx.x & 31) == 0 && na) atomicAdd(&d.counters[SPH_C_ACTIVE_UPDATES], (unsigned long long)na);
+    }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         dti = fminf(dti, __shfl_xor_sync(0xffffffffu, dti, o));
@@ -284,6 +300,121 @@ __global__ void __launch_bounds__(256) k_kick_drift(Dev d, DevParams p)
 }
 
 // ------------------------------------------------------------------------------------------
+// NEXT-4: rungs (reading Q23).  k_rung_assign: at the start of a big step, from the limits of the last CLOSE (or the
+// caller's fixed rungs).  k_kick_drift_rung: substep n of 2^R: opening kick (Eq. 42, own step) of the particles that
+// start a step, drift of all by delta, prediction of all to the new time (Eq. 40 generalised), and the tiles that
+// hold a particle which ends a step now.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_rung_assign(Dev d, float dT, int R, const unsigned char *__restrict__ fixed_rungs)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    int r = 0;
+    if (fixed_rungs) r = min((int)fixed_rungs[((const unsigned *)d.r.s[PP_ORIG])[i]], R);
+    else {
+        const float dti = d.dti[i];
+        while (r < R && dT / (float)(1 << r) > dti) ++r;
+    }
+    d.rung[i] = (unsigned char)r;
+}
+
+__global__ void __launch_bounds__(256) k_kick_drift_rung(Dev d, DevParams p, int n, int R, float dT)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i >= d.n) return;
+    const int r = (int)d.rung[i], per = 1 << (R - r), kk = n & (per - 1);
+    const float dtr = dT / (float)(1 << r), delta = dT / (float)(1 << R), hdt = 0.5f * dtr;
+    const float tau = (float)(kk + 1) * delta - hdt;                 // new time minus the middle of the particle's step
+    unsigned mf = ((const unsigned *)d.r.s[PP_MATFIX])[i];
+    const bool fixed = (mf >> 8) & 1u;
+    const bool start = kk == 0;
+    float4 pm = d.r.pm[i];
+    const float h = d.r.vh[i].w;
+    const float a[3] = {d.a[0][i], d.a[1][i], d.a[2][i]};
+    float vh[3], vp[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        if (start) {
+            const float v = d.vfull[k][i];
+            vh[k] = fixed ? v : fmaf(hdt, a[k], v);
+            d.r.s[PP_VHALF + k][i] = vh[k];
+        } else {
+            vh[k] = d.r.s[PP_VHALF + k][i];
+        }
+        vp[k] = fixed ? vh[k] : fmaf(tau, a[k], vh[k]);
+    }
+    if (!fixed) { pm.x = fmaf(delta, vh[0], pm.x); pm.y = fmaf(delta, vh[1], pm.y); pm.z = fmaf(delta, vh[2], pm.z); }
+    d.r.pm[i] = pm;
+    d.r.vh[i] = make_float4(vp[0], vp[1], vp[2], h);
+    const float du = d.dudt[i];
+    float uh;
+    if (start) { uh = fmaf(hdt, du, d.ufull[i]); d.r.s[PP_UHALF][i] = uh; }
+    else uh = d.r.s[PP_UHALF][i];
+    d.r.s[PP_UPRED][i] = fmaf(tau, du, uh);
+#pragma unroll
+    for (int c = 0; c < 5; ++c) {
+        const float ds = d.dS[c][i];
+        float sh;
+        if (start) { sh = fmaf(hdt, ds, d.Sfull[c][i]); d.r.s[PP_SHALF + c][i] = sh; }
+        else sh = d.r.s[PP_SHALF + c][i];
+        d.r.s[PP_SPRED + c][i] = fmaf(tau, ds, sh);
+    }
+    if (((n + 1) & (per - 1)) == 0) d.tile_act[i / SPH_TILE] = 1;    // ends a step now: active (same value from all)
+}
+
+// tiles that hold a candidate neighbour of an active tile need their density and PREDICT in this substep
+__global__ void __launch_bounds__(256) k_mark_need(Dev d, int ntile)
+{
+    const int tile = blockIdx.x;
+    if (tile >= ntile || !d.tile_act[tile]) return;
+    if (threadIdx.x == 0) {
+        d.tile_need[tile] = 1;
+        atomicAdd(&d.counters[SPH_C_ACTIVE_TILES], 1ull);
+    }
+    if (d.tile_flag[tile]) {                              // no candidate list (served by the tree walk): everything
+        for (int t = threadIdx.x; t < ntile; t += blockDim.x) d.tile_need[t] = 1;
+        return;
+    }
+    const int nc = d.tile_ncand[tile];
+    const unsigned *cand = d.cand + d.tile_off[tile];
+    for (int s = threadIdx.x; s < nc; s += blockDim.x) d.tile_need[cand[s] / SPH_TILE] = 1;
+}
+
+int sph_launch_rung_assign(sph_ctx *c, float dT, int R, const unsigned char *rungs)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    k_rung_assign<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, dT, R, rungs);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_kick_drift_rung(sph_ctx *c, int n, int R, float dT)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    const size_t ntile = (size_t)sph_div_up(d.nchunk, SPH_TILE_CHUNKS);
+    SPH_CUDA(c, cudaMemsetAsync(d.tile_act, 0, ntile, c->stream));
+    SPH_CUDA(c, cudaMemsetAsync(d.tile_need, 0, ntile, c->stream));
+    k_kick_drift_rung<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, c->p, n, R, dT);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+int sph_launch_mark_need(sph_ctx *c)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    const int ntile = sph_div_up(d.nchunk, SPH_TILE_CHUNKS);
+    k_mark_need<<<ntile, 256, 0, c->stream>>>(d, ntile);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
+// ------------------------------------------------------------------------------------------
 // caller-order scatter helpers
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_scatter(const float *__restrict__ src, const unsigned *__restrict__ orig,
@@ -291,7 +422,7 @@ __global__ void __launch_bounds__(256) k_scatter(const float *__restrict__ src, 
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= n) return;
-    dst[orig[i]] = as_int ? (float)((const int *)src)[i] : src[i];
+    dst[orig[i]] = as_int == 2 ? (float)((const unsigned char *)src)[i] : (as_int ? (float)((const int *)src)[i] : src[i]);
 }
 
 __global__ void __launch_bounds__(256) k_scatter_pos(const float4 *__restrict__ pm, const unsigned *__restrict__ orig,
@@ -327,7 +458,7 @@ int sph_launch_predict(sph_ctx *c)
 {
     Dev &d = c->d;
     if (d.n == 0) return SPH_OK;
-    k_predict<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, c->p, c->tabs);
+    k_predict<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, c->p, c->tabs, c->rc);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;
@@ -343,7 +474,7 @@ int sph_launch_close(sph_ctx *c, int phase, float dt, bool dt_from_device)
         c->launches++;
     }
     if (d.n > 0) {
-        k_close<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, c->p, phase, dt, dt_from_device ? 1 : 0);
+        k_close<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, c->p, phase, dt, dt_from_device ? 1 : 0, c->rc);
         c->launches++;
     }
     SPH_CUDA(c, cudaGetLastError());

@@ -1,0 +1,107 @@
+"""NEXT-4 on the GPU: sph_step_rungs (individual time steps on power-of-two rungs, reading Q23) against the oracle's
+RungStepper, element by element, on the configs[3] construction at parity size (h varying ~5x: three to four rungs)."""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2603_19764_b200 import workloads as W
+from tests import parity_util as U
+
+pytestmark = pytest.mark.gpu
+
+
+def _state(s, t):
+    import torch
+    s.download_state(t)
+    torch.cuda.synchronize()
+    x = np.stack([t[k].cpu().numpy() for k in ("x", "y", "z")])
+    v = np.stack([t[k].cpu().numpy() for k in ("vx", "vy", "vz")])
+    S = np.stack([t[k].cpu().numpy() for k in ("Sxx", "Syy", "Sxy", "Sxz", "Syz")])
+    return x, v, t["u"].cpu().numpy(), S
+
+
+def _compare(s, t, st, tol_v=U.TOL_STATE, tol_S=U.TOL_STATE):
+    x, v, u, S = _state(s, t)
+    errs = {"x": U.maxnorm_err(x, st.x), "v": U.maxnorm_err(v, st.v), "u": U.maxnorm_err(u, st.u),
+            "S": U.maxnorm_err(S, st.S), "eacc": U.maxnorm_err(s.get_field("EACC").cpu().numpy(), st.e_acc)}
+    assert errs["x"] <= 1e-6 and errs["v"] <= tol_v and errs["u"] <= U.TOL_STATE and errs["S"] <= tol_S, errs
+    return errs
+
+
+@pytest.mark.parametrize("skin", [0.0, 0.06])
+def test_big_step_with_fixed_rungs_matches_the_oracle(skin):
+    """The rungs of the big step are handed to both sides (the oracle's own assignment), so every decision is the
+    same and the states must agree like those of a global step do; the counter of closing kicks is sum 2^rung."""
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    wl = W.impact_pair(20000, W.SEED_BASE + 3, 100.0, 1.214)
+    wl.params.skin = skin
+    wl.params.rebuild_every = 4
+    st = O.RungStepper(wl, mode="grid")
+    st.bootstrap()
+    R = 3
+    dT = float(np.percentile(st.d["dt_i"], 99.5))
+    rungs = O.rung_for(st.d["dt_i"], dT, R)
+    assert len(np.unique(rungs)) >= 3
+    st.big_step(dT, R, rungs=rungs)
+    with torch.cuda.stream(torch.cuda.Stream()):
+        s = B.Sph(wl.params, wl.n)
+        t = s.upload(wl)
+        s.build_neighbors(t, wl.n)
+        rd = torch.as_tensor(rungs.astype(np.uint8), device="cuda")
+        s.step_rungs(dT, R, rd)
+        c = s.get_counters()
+        errs = _compare(s, t, st)
+        assert np.array_equal(s.get_field("RUNG").cpu().numpy().astype(np.int64), rungs)
+    assert c["active_updates"] == int((1 << rungs).sum()) == int(st.kicks.sum())
+    assert c["list_overflow"] == 0 and c["nonfinite"] == 0
+    assert c["active_tiles"] < (1 << R) * ((wl.n + 255) // 256)          # tiles without active particles were skipped
+    print(f"fixed rungs, skin {skin}: rung histogram {np.bincount(rungs).tolist()}, closing kicks {c['active_updates']} of "
+          f"{wl.n << R}, active tiles {c['active_tiles']} of {(1 << R) * ((wl.n + 255) // 256)}", {k: float(f'{e:.3g}') for k, e in errs.items()})
+
+
+def test_big_steps_with_rungs_from_the_limits_match_the_oracle():
+    """Rungs chosen on each side from its own limits (fp32 on the GPU, fp64 in the oracle): the same for all but
+    particles whose limit sits on a power-of-two boundary; two big steps, so the rungs carried over and the rung
+    changes inside a big step are exercised."""
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    wl = W.impact_pair(20000, W.SEED_BASE + 3, 100.0, 1.214)
+    wl.params.skin = 0.05
+    st = O.RungStepper(wl, mode="grid")
+    st.bootstrap()
+    R = 3
+    dT = float(np.percentile(st.d["dt_i"], 99.5)) * 0.97
+    with torch.cuda.stream(torch.cuda.Stream()):
+        s = B.Sph(wl.params, wl.n)
+        t = s.upload(wl)
+        s.build_neighbors(t, wl.n)
+        for big in range(2):
+            st.big_step(dT, R)
+            s.step_rungs(dT, R)
+            rg = s.get_field("RUNG").cpu().numpy().astype(np.int64)
+            differ = int((rg != st.rung).sum())
+            kicks = s.get_counters()["active_updates"]
+            print(f"big step {big}: rung histogram {np.bincount(rg).tolist()}, {differ} rungs differ, closing kicks gpu {kicks} oracle {int(st.kicks.sum())}")
+            assert differ <= max(2, wl.n // 2000)
+            assert abs(kicks - int(st.kicks.sum())) <= 8 * max(2, wl.n // 2000)
+        errs = _compare(s, t, st, tol_v=1e-3, tol_S=1e-2)
+    print({k: float(f"{e:.3g}") for k, e in errs.items()})
+
+
+def test_single_rung_big_step_is_a_global_step():
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    wl = W.elastic_block(12, h_spread=0.2)
+    out = []
+    for mode in ("global", "rungs"):
+        s = B.Sph(wl.params, wl.n)
+        t = s.upload(wl)
+        s.build_neighbors(t, wl.n)
+        if mode == "global":
+            s.step(None, 0, 3e-7); s.step(None, 0, 3e-7)
+        else:
+            s.step_rungs(3e-7, 0); s.step_rungs(3e-7, 0)
+        out.append(_state(s, t))
+    for a, b in zip(out[0], out[1]):
+        assert U.maxnorm_err(b, a) <= 2e-6
