@@ -297,6 +297,34 @@ def run_ours(args):
     total_ms_max, pairs_all = rank_reduce(total_ms, pairs, dev)
     value = pairs_all / (total_ms_max * 1e-3)
 
+    # ---- NEXT-4 (optional): big steps on 2^R rungs, the finest rung at the CFL step of the global stepper -------------
+    rungs = None
+    if args.rungs > 0:
+        R = args.rungs
+        dtu = torch.zeros(1, dtype=torch.float32, device=dev)
+        s.step(None, 0, 0.0, dtu)
+        dT = float(dtu.item()) * (1 << R)
+        s.step_rungs(dT, R)                                   # warm-up
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nbig = 3
+        upd = tiles = 0
+        barrier()
+        e0.record(s.stream)
+        for _ in range(nbig):
+            s.step_rungs(dT, R)
+            c = s.get_counters()
+            upd += c["active_updates"]; tiles += c["active_tiles"]
+        e1.record(s.stream)
+        barrier()
+        big_ms = e0.elapsed_time(e1) / nbig
+        rg = s.get_field("RUNG")
+        rungs = {"max_rung": R, "dT": dT, "ms_per_big_step": big_ms,
+                 "ms_of_the_same_span_on_one_rung": (total_ms / args.steps) * (1 << R),
+                 "closing_kicks_per_big_step": upd / nbig, "of_global": upd / nbig / (n * (1 << R)),
+                 "active_tiles_per_big_step": tiles / nbig, "of_all_tiles": tiles / nbig / (((n + 255) // 256) * (1 << R)),
+                 "rung_histogram": torch.bincount(rg.to(torch.int64), minlength=R + 1).tolist(),
+                 "particle_updates_per_s": upd / nbig / (big_ms * 1e-3)}
+
     # ---- the same step with strength off (S == 0, hydro only): BASELINE.json's "<= 30 % over hydro-only"
     hydro = None
     if strength and not args.no_hydro_only:
@@ -449,6 +477,7 @@ def run_ours(args):
         "roofline": roofline,
         "cpu_baseline": cpu,
         "hydro_only": hydro,
+        "rungs": rungs,
     }
     print(json.dumps(line), flush=True)
     if world > 1:
@@ -475,6 +504,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-hydro-only", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
+    ap.add_argument("--rungs", type=int, default=0, help="NEXT-4: also time big steps on 2^R rungs (sph_step_rungs)")
     ap.add_argument("--no-graph", action="store_true", help="launch the step kernel by kernel (A/B of the CUDA graph)")
     ap.add_argument("--skin", type=float, default=None, help="list reuse: skin as a fraction of H (0 = off; A/B)")
     ap.add_argument("--rebuild-every", type=int, default=None, help="list reuse: steps between full builds (A/B)")
