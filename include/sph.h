@@ -116,6 +116,8 @@ enum { SPH_C_PAIRS_GATHER = 0,   /* sum_i |gather set(i)|   (true pairs of the d
        SPH_C_ACTIVE_UPDATES,     /* sph_step_rungs: closing kicks done in the last big step (n 2^max_rung if every
                                     particle sat on the finest rung)                                           */
        SPH_C_ACTIVE_TILES,       /* sph_step_rungs: tiles the pair pass worked on, summed over the substeps    */
+       SPH_C_PAIRS_INTILE,       /* symmetric pairs whose two particles sit in the same tile (counted by
+                                    sph_get_neighbors(SPH_SYMMETRIC): the share a tile could evaluate once)     */
        SPH_C_LIST_SLOTS,         /* list slots the pair passes step through per launch: entries plus the padding
                                     that makes the 32 lists of a chunk equally long in every round (last build) */
        SPH_C_COUNT };
@@ -299,6 +301,13 @@ int sph_get_tile_stats(sph_ctx *ctx, int *ncand, unsigned *cycles, unsigned char
  * `repeats` launches timed with CUDA events on `cuda_stream`.  tflops: HOST.  Synchronises the stream.
  * It is the denominator of the ALU-bound roofline entries of bench.py. */
 int sph_fp32_peak(void *cuda_stream, int repeats, double *tflops);
+
+/* Measurement aid for the design question "symmetric-pair accumulation" (BASELINE.json north_star; DESIGN.md
+ * section 6): the rate at which one tile's CTA (256 threads, two CTAs per SM as in the pair pass) can add the j side
+ * of a pair into `accumulators` shared-memory floats per target (20 for the fused pass: F 9, C^-1 6, a 3, du/dt,
+ * mu_max; 5 hydro only) at random targets of the tile, with atomicAdd -- on sm_100a a compare-and-swap loop
+ * (ATOMS.CAST.SPIN).  pairs_per_s: HOST, scatters of one pair per second over the whole device.  Synchronises. */
+int sph_shared_scatter_rate(void *cuda_stream, int accumulators, double *pairs_per_s);
 
 /* Number of this library's kernel launches since sph_init (HOST; no synchronisation). */
 long long sph_launch_count(const sph_ctx *ctx);

@@ -25,14 +25,14 @@ F = dict(RHO=0, OMEGA=1, P=2, CS=3, T=4, GAMMA=5, Y=6, MUMAX=7, DUDT=8, DT=9, EA
          CFLAG=13, NGATHER=14, NSYMMETRIC=15, H=16, RUNG=17, A=32, V=36, X=40, SPRED=48, S=56, DSDT=64, F=80, CINV=96, G=112)
 T_SLOTS = ("build", "density", "predict", "gradient", "force", "close", "kickdrift", "step")
 C_SLOTS = ("pairs_gather", "pairs_symmetric", "tests_density", "tests_force", "cfallback", "tests_cull",
-           "candidates", "list_overflow", "bad_material", "omega_small", "nonfinite", "tiles_dirty", "active_updates", "active_tiles", "list_slots")
+           "candidates", "list_overflow", "bad_material", "omega_small", "nonfinite", "tiles_dirty", "active_updates", "active_tiles", "pairs_intile", "list_slots")
 
 FLOAT_FIELDS = ("x", "y", "z", "m", "h", "vx", "vy", "vz", "u", "Sxx", "Syy", "Sxy", "Sxz", "Syz")
 OPT_FIELDS = ("gx", "gy", "gz")
 
 # every symbol include/sph.h declares (tests check the library exports all of them)
 SYMBOLS = ("sph_workspace_bytes", "sph_init", "sph_build_neighbors", "sph_density", "sph_strength_update",
-           "sph_gradients", "sph_forces", "sph_gradients_forces", "sph_fp32_peak", "sph_step_rungs", "sph_adapt_h", "sph_set_eos_table", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
+           "sph_gradients", "sph_forces", "sph_gradients_forces", "sph_fp32_peak", "sph_shared_scatter_rate", "sph_step_rungs", "sph_adapt_h", "sph_set_eos_table", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
            "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_get_diagnostics", "sph_launch_count",
            "sph_last_cuda_error", "sph_strerror", "sph_destroy")
 
@@ -110,6 +110,8 @@ def load():
     lib.sph_gradients_forces.restype = i
     lib.sph_fp32_peak.argtypes = [vp, i, C.POINTER(C.c_double)]
     lib.sph_fp32_peak.restype = i
+    lib.sph_shared_scatter_rate.argtypes = [vp, i, C.POINTER(C.c_double)]
+    lib.sph_shared_scatter_rate.restype = i
     lib.sph_step_rungs.argtypes = [vp, fl, i, vp]
     lib.sph_step_rungs.restype = i
     lib.sph_step.argtypes = [vp, C.POINTER(sph_state), ll, fl, vp]
@@ -254,6 +256,13 @@ class Sph:
         """sph_fp32_peak: TFLOP/s of independent FFMA chains on this device (measurement aid)."""
         out = C.c_double(0.0)
         self._check(self.lib.sph_fp32_peak(self.stream.cuda_stream, int(repeats), C.byref(out)), "sph_fp32_peak")
+        return float(out.value)
+
+    def shared_scatter_rate(self, accumulators: int) -> float:
+        """sph_shared_scatter_rate: pair scatters per second into shared-memory accumulators (measurement aid)."""
+        out = C.c_double(0.0)
+        self._check(self.lib.sph_shared_scatter_rate(self.stream.cuda_stream, int(accumulators), C.byref(out)),
+                    "sph_shared_scatter_rate")
         return float(out.value)
 
     def step(self, tensors: Optional[Dict[str, object]] = None, n: int = 0, dt: float = 0.0, dt_used=None):

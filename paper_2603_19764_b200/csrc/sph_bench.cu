@@ -57,3 +57,62 @@ extern "C" int sph_fp32_peak(void *cuda_stream, int repeats, double *tflops)
     *tflops = best;
     return rc;
 }
+
+// ------------------------------------------------------------------------------------------
+// Shared-memory scatter rate (see include/sph.h): every thread adds NACC values to the accumulators of a
+// pseudo-random target of its tile, SCATTER_ITERS times; shared-memory float atomicAdd is a CAS loop on sm_100a.
+// ------------------------------------------------------------------------------------------
+#define SCATTER_ITERS 2048
+template <int NACC>
+__global__ void __launch_bounds__(256, 2) k_shared_scatter(float *out)
+{
+    __shared__ float acc[NACC][256];
+    for (int k = threadIdx.x; k < NACC * 256; k += 256) (&acc[0][0])[k] = 0.f;
+    __syncthreads();
+    unsigned x = (blockIdx.x * 256u + threadIdx.x) * 2654435761u + 12345u;
+    float v = 1.0f + (float)threadIdx.x * 1.0e-3f;
+    for (int it = 0; it < SCATTER_ITERS; ++it) {
+        x = x * 1664525u + 1013904223u;
+        const int j = (int)(x >> 24);
+#pragma unroll
+        for (int c = 0; c < NACC; ++c) atomicAdd(&acc[c][j], v);
+        v += 1.0e-6f;
+    }
+    __syncthreads();
+    float s = 0.f;
+    for (int c = 0; c < NACC; ++c) s += acc[c][threadIdx.x];
+    if (s == -1.f) out[0] = s;
+}
+
+extern "C" int sph_shared_scatter_rate(void *cuda_stream, int accumulators, double *pairs_per_s)
+{
+    if (!pairs_per_s || (accumulators != 5 && accumulators != 20)) return SPH_EINVAL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return SPH_ECUDA;
+    float *out = nullptr;
+    if (cudaMalloc(&out, sizeof(float)) != cudaSuccess) return SPH_ECUDA;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int blocks = nsm * 2 * 4;
+    double best = 0.0;
+    int rc = SPH_OK;
+    for (int r = 0; r < 4; ++r) {
+        cudaEventRecord(e0, st);
+        if (accumulators == 20) k_shared_scatter<20><<<blocks, 256, 0, st>>>(out);
+        else k_shared_scatter<5><<<blocks, 256, 0, st>>>(out);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { rc = SPH_ECUDA; break; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (r > 0 && ms > 0.f) best = fmax(best, (double)blocks * 256.0 * SCATTER_ITERS / (ms * 1.0e-3));
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(out);
+    if (rc == SPH_OK && cudaGetLastError() != cudaSuccess) rc = SPH_ECUDA;
+    *pairs_per_s = best;
+    return rc;
+}

@@ -936,7 +936,7 @@ __global__ void __launch_bounds__(256) k_neighbors_l(Dev d, float kappa, int *co
     float4 pi = d.r.pm[i];
     float Hi = sph_H(kappa, d.r.vh[i].w);
     float H2i = __fmul_rn(Hi, Hi);
-    int out = 0;
+    int out = 0, intile = 0;
     // the lists may hold pairs of the skin: the sets are defined by the exact predicate (reading Q4)
     if (!SYM) {
         if (list) list[base] = (int)oi;
@@ -961,11 +961,13 @@ __global__ void __launch_bounds__(256) k_neighbors_l(Dev d, float kappa, int *co
                 if (hit) {
                     if (list) list[base + out] = (int)orig[j];
                     ++out;
+                    if (SYM && (long long)j / SPH_TILE == i / SPH_TILE) ++intile;
                 }
             }
         }
     }
     counts[oi] = out;
+    if (SYM && intile) atomicAdd(&d.counters[SPH_C_PAIRS_INTILE], (unsigned long long)intile);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1155,6 +1157,7 @@ int sph_launch_neighbors_l(sph_ctx *c, int which, int *counts, const long long *
     Dev &d = c->d;
     if (d.n == 0) return SPH_OK;
     int nb = sph_div_up(d.n, 256);
+    if (which == SPH_SYMMETRIC) SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_PAIRS_INTILE], 0, sizeof(unsigned long long), c->stream));
     if (which == SPH_SYMMETRIC) k_neighbors_l<true><<<nb, 256, 0, c->stream>>>(d, c->p.kappa, counts, offsets, list);
     else k_neighbors_l<false><<<nb, 256, 0, c->stream>>>(d, c->p.kappa, counts, offsets, list);
     c->launches++;
