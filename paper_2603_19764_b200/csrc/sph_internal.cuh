@@ -20,7 +20,9 @@
 #define SPH_CULL_MAXSRC 768   // source chunks a tile may accept in the tree walk
 #define SPH_CULL_MAXPAR 128   // level-1 nodes a tile may expand in the last level of the walk
 #define SPH_GCAP 128          // entries of a quarter-warp's candidate table in k_cull (multiple of 32)
-#define SPH_CULL_CFCACHE 256  // source chunks whose per-particle chunk flags are kept between the two passes
+#define SPH_CULL_CFCACHE 128  // source chunks whose per-particle chunk flags are kept between the two passes
+#define SPH_CULL_LATE 1       // a candidate within reach of at most this many chunk boxes of a tile that needs several
+                              // rounds goes to the END of the tile's candidate list (k_cull, A2; measured 1..4 on configs[4])
 #define SPH_ROWS_DEFAULT 64   // default row-groups (4 neighbours per lane each) reserved per chunk
 
 // indices into Resident::s (scalar ping-pong arrays)

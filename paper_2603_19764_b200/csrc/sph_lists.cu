@@ -78,7 +78,10 @@ struct CullSmem {
     unsigned char flag[SPH_SE];          // bit w: within reach of the box of chunk (warp) w of the tile
     unsigned chunks[SPH_CULL_MAXSRC];    // frontier / accepted source chunks, ascending
     unsigned mask[SPH_CULL_MAXSRC];      // surviving lanes (children / particles) of each entry
-    unsigned short off[SPH_CULL_MAXSRC]; // exclusive prefix of popc(mask) (< SPH_MAXROUND * SPH_SE + 32 < 65536)
+    unsigned short off[SPH_CULL_MAXSRC]; // exclusive prefix of popc(mask) (< SPH_MAXROUND * SPH_SE + 32 < 65536); in A2/A3: of
+                                         // the survivors that are not "late"
+    unsigned maskB[SPH_CULL_MAXSRC];     // A2/A3: the "late" survivors (within reach of <= SPH_CULL_LATE chunk boxes)
+    unsigned short offB[SPH_CULL_MAXSRC];// A2/A3: exclusive prefix of popc(maskB)
     unsigned char cmask[SPH_CULL_MAXSRC];                // chunk boxes of the tile a source chunk box reaches
     union alignas(16) {
         struct {                                         // the tree walk (A1) only
@@ -98,7 +101,7 @@ struct CullSmem {
     alignas(16) unsigned short sentinels[32];            // a block of padding offsets (pos[SPH_SE])
     alignas(16) unsigned short gl[SPH_TILE_CHUNKS][4][SPH_GCAP];     // per quarter-warp: candidates still to test, ascending,
                                                          // as byte offsets (slot * 16) into pos[]
-    int nsrc, ntotal, nfront, overflow;
+    int nsrc, ntotal, ntotalA, nfront, overflow;
     unsigned long long cand_off;
 };
 
@@ -315,17 +318,30 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float inf
         }
         if (k < SPH_CULL_CFCACHE) sm.cf[k][lane] = (unsigned char)f;
         const unsigned m = __ballot_sync(FULL, f != 0);
-        if (lane == 0) sm.mask[k] = m;
+        const unsigned mB = __ballot_sync(FULL, f != 0 && __popc(f) <= SPH_CULL_LATE);
+        if (lane == 0) { sm.mask[k] = m & ~mB; sm.maskB[k] = mB; }
         if (has2) {
             if (k2 < SPH_CULL_CFCACHE) sm.cf[k2][lane] = (unsigned char)f2;
             const unsigned m2 = __ballot_sync(FULL, f2 != 0);
-            if (lane == 0) sm.mask[k2] = m2;
+            const unsigned m2B = __ballot_sync(FULL, f2 != 0 && __popc(f2) <= SPH_CULL_LATE);
+            if (lane == 0) { sm.mask[k2] = m2 & ~m2B; sm.maskB[k2] = m2B; }
         }
     }
     __syncthreads();
+    // The candidate list of a tile that fits one round is in ascending index order.  One that needs several rounds is
+    // split: first the candidates within reach of more than SPH_CULL_LATE chunk boxes, then the "late" ones, which
+    // only one of the eight chunks can have as neighbours.  The last round then holds fewer entries for most warps: the
+    // 32 lists of a chunk are padded to equal length in every round it has entries in, and on configs[4] (1 967
+    // candidates per tile, 1 632 slots per round) that padding was 30 % of the slots the pair passes step through;
+    // with the late candidates last it is 14 % (SPH_CULL_LATE = 1; 2: 19 %, 3: 23 %, 4: 26 %), 49.5 -> 45.3 ms per step.
     if (warp == 0) {
-        int total = scan_popc(sm.mask, sm.off, nsrc, lane);
+        const int totalA = scan_popc(sm.mask, sm.off, nsrc, lane);
+        const int totalB = scan_popc(sm.maskB, sm.offB, nsrc, lane);
+        const int total = totalA + totalB;
         if (lane == 0) {
+            // -1: ascending order (one round; or more than three: a tile that straddles a gap of the curve -- there the
+            // split would spread a chunk's entries over more rounds and use up its list rows)
+            sm.ntotalA = (total > SPH_SE && total <= 3 * SPH_SE) ? totalA : -1;
             // the pool: [0, cand_cap) for full builds, [cand_cap, cand_cap + cand_cap_dirty) for dirty tiles
             unsigned long long co = atomicAdd(d.cand_cursor + (dirty ? 1 : 0), (unsigned long long)total);
             if (co + (unsigned long long)total > (dirty ? d.cand_cap_dirty : d.cand_cap)) sm.overflow |= 2;
@@ -351,7 +367,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float inf
         }
         return;
     }
-    const int ntotal = sm.ntotal;
+    const int ntotal = sm.ntotal, ntotalA = sm.ntotalA;
     unsigned *cand = d.cand + sm.cand_off;
     if (threadIdx.x == 0) {
         d.tile_ncand[tile] = ntotal;
@@ -406,10 +422,13 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float inf
                 slot[t] = -1;
                 jj[t] = 0;
                 if (kk < nsrc) {
-                    const unsigned m = sm.mask[kk];
-                    const int o = (int)sm.off[kk];
-                    if (o < r0 + nr && o + 32 > r0 && ((m >> lane) & 1u)) {
-                        const int sl = o + __popc(m & lt) - r0;
+                    const unsigned mA = sm.mask[kk], mB = sm.maskB[kk];
+                    if (((mA | mB) >> lane) & 1u) {
+                        int sl;
+                        if (ntotalA < 0) sl = (int)sm.off[kk] + (int)sm.offB[kk] + __popc((mA | mB) & lt);
+                        else if ((mB >> lane) & 1u) sl = ntotalA + (int)sm.offB[kk] + __popc(mB & lt);
+                        else sl = (int)sm.off[kk] + __popc(mA & lt);
+                        sl -= r0;
                         if (sl >= 0 && sl < nr) { slot[t] = sl; jj[t] = (long long)sm.chunks[kk] * SPH_CHUNK + lane; }
                     }
                 }

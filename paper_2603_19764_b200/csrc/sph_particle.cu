@@ -112,7 +112,7 @@ __global__ void __launch_bounds__(256) k_predict(Dev d, DevParams p, DevTabs tab
 // unsigned ints; k_dt_select / k_dt_reset set dt_next to +inf before), and the robustness counters.
 // NEXT-4 (rc.on): only the active particles; the step of the closing kick is the particle's own, dT / 2^rung, and
 // the particle chooses its next rung from its new limit (reading Q23).
-__global__ void __launch_bounds__(256) k_close(Dev d, DevParams p, int phase, float dt_arg, int dt_from_device, RungCtl rc)
+__global__ void __launch_bounds__(256, 6) k_close(Dev d, DevParams p, int phase, float dt_arg, int dt_from_device, RungCtl rc)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     float dti = __int_as_float(0x7f800000);
