@@ -496,7 +496,8 @@ def measured_hbm_gbs():
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=16)
+    ap.add_argument("--steps", type=int, default=32,
+                    help="timed steps; the default covers one whole cycle of the list reuse of configs[4] (a full build every 32 steps)")
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="c4", choices=["c0", "c1", "c2", "c3", "c4"],
                     help="BASELINE.json configs[k]; default: the largest single-GPU configuration")

@@ -799,7 +799,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa, Rung
                     const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
                     if (r2 < H2i)
                         density_term(A, r2, q.w, invH, pxd - (double)q.x, pyd - (double)q.y, pzd - (double)q.z,
-                                     (double)q.w, invHd);
+                                     sph_widen_pos(q.w), invHd);
                 }
             }
         }

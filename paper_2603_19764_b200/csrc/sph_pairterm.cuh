@@ -50,6 +50,14 @@ struct DensAcc {
 __device__ __forceinline__ void density_term(DensAcc &A, float r2, float mj, float invH, double ex, double ey,
                                              double ez, double md, double invHd);
 
+// fp32 -> fp64 of a POSITIVE NORMAL float by integer operations (exact): the conversion instruction runs on the XU
+// pipe (16 per clock and SM), which bounds the density kernel; three ALU instructions do not.  Zero becomes 2^-127.
+__device__ __forceinline__ double sph_widen_pos(float f)
+{
+    const unsigned b = __float_as_uint(f);
+    return __hiloint2double((int)((b >> 3) + 0x38000000u), (int)(b << 29));
+}
+
 struct PairConst {
     float beta;       // Eq. 5
     float alpha2;     // alpha / 2: alpha cbar = alpha2 (c_i + c_j)
@@ -152,7 +160,7 @@ __device__ __forceinline__ void density_term(DensAcc &A, float r2, float mj, flo
     const float t = fmaxf(0.f, 1.f - q);
     A.sh = fmaf(mj * (t * t * t), fmaf(q, fmaf(-32.f, q, 9.f), 3.f), A.sh);
     const double r2d = fma(ex, ex, fma(ey, ey, ez * ez));
-    const double yd = (double)rinv, td0 = r2d * yd;
+    const double yd = sph_widen_pos(rinv), td0 = r2d * yd;
     const double rd = fma(0.5 * td0, fma(-td0, yd, 1.0), td0);
     const double qd = rd * invHd;
     // no clamp at 0: membership (r2 < H_i^2 in fp32) already says q < 1 up to rounding, and (1 - q)^4 of a q that
