@@ -76,12 +76,13 @@ def _ensure_built():
     from . import build as _build
     if os.environ.get("LOCAL_RANK", "0") == "0":
         try:
-            _build.build()
-        except Exception as e:                      # reported by the missing-file check in load()
-            sys.stderr.write(f"building {LIB_PATH} failed: {e}\n")
+            _build.build()                          # compiles to a temporary file and renames it into place
+        except Exception as e:
+            # a failed rebuild must not run a stale binary silently
+            raise RuntimeError(f"building {LIB_PATH} failed: {e} (there is no CPU fallback)") from e
         return
     t0 = time.time()
-    while not os.path.exists(LIB_PATH) and time.time() - t0 < 600.0:
+    while _build.stale() and time.time() - t0 < 600.0:        # until rank 0 has renamed a current library into place
         time.sleep(1.0)
 
 

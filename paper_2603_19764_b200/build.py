@@ -21,6 +21,10 @@ def sources():
     return sorted(glob.glob(os.path.join(CSRC, "*.cu")))
 
 
+def stale() -> bool:
+    return _stale()
+
+
 def _stale() -> bool:
     if not os.path.exists(OUT):
         return True
@@ -33,11 +37,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return OUT
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    tmp = OUT + ".tmp.%d" % os.getpid()              # never leave a half-written library where load() looks
     cmd = [nvcc, "-O3", "-std=c++17", *ARCH, "-lineinfo", "-diag-suppress", "128", "-Xcompiler", "-fPIC", "-shared",
-           "-o", OUT, *sources()]
+           "-o", tmp, *sources()]
     if verbose:
         cmd += ["-Xptxas", "-v"]
-    subprocess.check_call(cmd)
+    try:
+        subprocess.check_call(cmd)
+        os.replace(tmp, OUT)
+    finally:
+        if os.path.exists(tmp):
+            os.remove(tmp)
     return OUT
 
 

@@ -26,7 +26,7 @@ import numpy as np
 
 SEED_BASE = 260319764
 
-# flag bits of sph_params.flags (mirrored in include/sph.h and oracle/sph_oracle.h;
+# flag bits of sph_params.flags (mirrored in include/sph.h and oracle/oracle.py;
 # plain constants, no arithmetic)
 FLAG_STRENGTH = 1
 FLAG_CORRECTION_TENSOR = 2
