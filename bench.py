@@ -400,6 +400,8 @@ def run_ours(args):
         out = {"kernel": kernel, "bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
                "frac_of_nominal": ach / peak_nominal, "kernel_ms": ms, "share_of_step": ms / step_avg,
                "work": what, "traffic": prof.get("traffic_bytes"), "traffic_unit": "bytes per launch"}
+        if prof.get("traffic_bytes") and ms > 0:
+            out["dram_gbs"] = prof["traffic_bytes"] / (ms * 1e-3) / 1e9       # measured DRAM bytes of a launch over this run's time
         if ex and ms > 0:
             # executed FP32 flop of one launch (2 ffma + fmul + fadd, ncu capture in profiles/) over THIS run's kernel time
             out["executed_achieved"] = ex / (ms * 1e-3) / 1e12
@@ -458,6 +460,8 @@ def run_ours(args):
         "data": "synthetic",
         "config": {"workload": wl.name, "n_particles": n, "strength": strength,
                    "mean_neighbours": pairs_s / args.steps / max(n, 1),
+                   "pair_count": "value = gather pairs (Eq. 1, 3; the particle itself included: the self term is evaluated) "
+                                 "+ symmetric pairs (Eq. 18-21; self excluded) per second",
                    "l2": "flushed between steps (256 MiB fill outside the timed events)",
                    "working_set_bytes": working_set, "parallelism": "replicas x%d" % world,
                    "cuda_graph": not args.no_graph,

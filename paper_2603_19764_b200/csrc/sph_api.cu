@@ -691,6 +691,7 @@ extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, f
     rc = sph_step(c, &ds, n, dt, nullptr);
     c->host_out = nullptr;
     c->no_reuse_now = false;
+    c->force_full = true;          // these lists have no skin: whatever step comes next must not reuse them
     if (rc) return rc;
     float *dst[14] = {hs->x, hs->y, hs->z, nullptr, nullptr, hs->vx, hs->vy, hs->vz, hs->u,
                       hs->Sxx, hs->Syy, hs->Sxy, hs->Sxz, hs->Syz};

@@ -395,3 +395,28 @@ def test_reused_lists_keep_the_exact_neighbour_sets_over_steps(case):
     assert errs["x"] <= 1e-5 and errs["v"] <= 1e-3 and errs["S"] <= 1e-2       # 12 steps: chaotic growth of rounding
     if case == "impact":
         assert dirty_seen > 0
+
+
+def test_device_step_after_a_host_buffer_step_does_not_reuse_its_lists():
+    """sph_step_host builds exact lists (no skin: its positions come from the caller every step).  A resident step
+    right after it must start from a full build instead of reusing them."""
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    wl = W.elastic_block(12, h_spread=0.2)
+    for q in ("vx", "vy", "vz"):
+        wl.arrays[q] *= 30.0
+    wl.params.skin = 0.05
+    wl.params.rebuild_every = 8
+    host = {k: torch.from_numpy(v.copy()).pin_memory() for k, v in wl.arrays.items()}
+    host["mat"] = torch.from_numpy(wl.mat.copy()).pin_memory()
+    host["fixed"] = torch.from_numpy(wl.fixed.copy()).pin_memory()
+    with torch.cuda.stream(torch.cuda.Stream()):
+        s = B.Sph(wl.params, wl.n)
+        s.step_host(host, wl.n, 0.0)
+        s.step_host(host, wl.n, 0.0)
+        t = {k: v.cuda() for k, v in host.items()}
+        for _ in range(3):
+            s.step(None, 0, 0.0)
+        s.download_state(t)
+        cur = W.Workload(wl.name, wl.params, {k: t[k].cpu().numpy() for k in W.FIELDS}, wl.mat, wl.fixed, 0.0)
+        U.neighbor_sets_equal(s, cur, mode="grid")

@@ -67,3 +67,13 @@ def test_reference_arm_runs_on_rank0_only(monkeypatch):
     class A:
         workload = "c0"; steps = 1; warmup = 0; gpus = 2
     bench.run_reference(A())
+
+
+def test_bench_refuses_to_time_fewer_gpus_than_asked(capsys):
+    """`python bench.py --gpus N` outside torchrun starts the N replica ranks itself; with fewer than N devices
+    visible (none here) it must refuse with a clear message instead of timing one GPU and calling it N."""
+    import argparse
+    import bench
+    rc = bench._respawn_under_torchrun(argparse.Namespace(gpus=8))
+    assert rc == 2
+    assert "refusing" in capsys.readouterr().err
