@@ -237,6 +237,10 @@ def run_ours(args):
         wl.params.skin = args.skin
     if args.rebuild_every is not None:
         wl.params.rebuild_every = args.rebuild_every
+    elif wl.params.skin > 0.0 and 0 < args.steps < wl.params.rebuild_every:
+        # fewer timed steps than the list-reuse cycle: shorten the cycle so that the timed steps still hold one full
+        # neighbour build (never time a window without the build it lives on)
+        wl.params.rebuild_every = args.steps
     n = wl.n
     strength = bool(wl.params.flags & B.STRENGTH)
     reuse = wl.params.skin > 0.0
