@@ -750,8 +750,13 @@ __device__ __forceinline__ unsigned list_entry(uint2 w, int e)
 // 0.151 ms but rho only to 1.4e-7 and S_pred of configs[0] at 1.02e-4 (tolerance 1e-4): rejected; candidates
 // staged a second time widened to fp64 (48 B per slot, no conversions in the loop): 0.39 ms with one or two
 // warps per chunk -- three random LDS.128 per pair instead of one: the shared-memory pipe binds: rejected.
+// What did help: (1) the register budget.  With the default budget (48 registers) ptxas re-converted the TARGET's
+// x, y, z to fp64 for every pair instead of keeping three doubles alive: six conversions per pair in the SASS where
+// the source has three.  __launch_bounds__(256, 4) allows 55 registers: 0.228 -> 0.207 ms (configs[2]), 11.7 ->
+// 10.8 ms (configs[4]).  (2) mass and rsqrt widened by integer operations (sph_widen_pos) instead of on the XU pipe.
+// XU operations per gather pair: 7 (round 1) -> 4.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(SPH_TILE) k_density_l(Dev d, float kappa, RungCtl rc)
+__global__ void __launch_bounds__(SPH_TILE, 4) k_density_l(Dev d, float kappa, RungCtl rc)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float4 *s_pm = reinterpret_cast<float4 *>(smem_raw);
