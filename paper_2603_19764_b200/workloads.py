@@ -378,7 +378,7 @@ def oblique_impact(n_total: int = 30_000, v_impact: float = 100.0, seed: int = S
 
 # list reuse of the CUDA path per config (skin as a fraction of H, steps between full builds): measured choices,
 # DESIGN.md section 7; they change how often the neighbour lists are rebuilt, never a result
-LIST_REUSE = {1: (0.05, 16), 2: (0.05, 16), 3: (0.04, 16), 4: (0.03, 32)}
+LIST_REUSE = {1: (0.05, 16), 2: (0.05, 16), 3: (0.04, 16), 4: (0.025, 32)}
 
 
 def config(k: int, scale: float = 1.0) -> Workload:
