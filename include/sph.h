@@ -254,7 +254,9 @@ int sph_step(sph_ctx *ctx, sph_state *state, long long n, float dt, float *dt_us
 int sph_step_rungs(sph_ctx *ctx, float dT, int max_rung, const unsigned char *rungs);
 
 /* The same step through HOST buffers: copies the state host->device into library-owned staging,
- * steps, copies x, v, u, S back device->host, and synchronises the stream.  dt_used: HOST. */
+ * steps, copies x, v, u, S back device->host, and synchronises the stream.  dt_used: HOST.
+ * If the caller's x, y, z, h equal the resident ones bit for bit (a loop that hands back what it was given) the
+ * neighbour lists stay in use as in sph_step; if anything moved, the step starts from a full neighbour build. */
 int sph_step_host(sph_ctx *ctx, sph_state *host_state, long long n, float dt, float *dt_used);
 
 /* Write x, v, u, S of the resident particles to the caller's DEVICE arrays in caller order. */

@@ -127,6 +127,7 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
     o.dt_cur = b.take<float>(1);
     o.dt_next = b.take<float>(1);
     o.hchange = b.take<float>(1);
+    o.refresh_changed = b.take<int>(1);
     o.diag_part = b.take<double>(592 * 8);
     o.counters = b.take<unsigned long long>(SPH_C_COUNT);
     o.keys = b.take<unsigned long long>(N); o.keys_alt = b.take<unsigned long long>(N);
@@ -625,14 +626,20 @@ extern "C" int sph_step_rungs(sph_ctx *c, float dT, int max_rung, const unsigned
     return SPH_OK;
 }
 
-// refresh the resident state from caller-order device arrays, keeping order and derivatives
+// refresh the resident state from caller-order device arrays, keeping order and derivatives.  What the neighbour lists
+// depend on -- x, y, z, h -- is compared with the resident values first: a caller that hands back the state it was
+// given (the usual host-buffer loop) leaves them bit for bit, and the lists (with their skin and their validity
+// check) stay in use; any difference sets the flag and the step starts from a full build.
 __global__ void __launch_bounds__(256) k_refresh(Dev d, sph_state st)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= d.n) return;
     unsigned o = ((const unsigned *)d.r.s[PP_ORIG])[i];
-    d.r.pm[i] = make_float4(st.x[o], st.y[o], st.z[o], st.m[o]);
-    d.r.vh[i].w = st.h[o];
+    const float4 np = make_float4(st.x[o], st.y[o], st.z[o], st.m[o]), op = d.r.pm[i];
+    const float nh = st.h[o];
+    if (!(np.x == op.x && np.y == op.y && np.z == op.z && nh == d.r.vh[i].w)) *d.refresh_changed = 1;
+    d.r.pm[i] = np;
+    d.r.vh[i].w = nh;
     d.vfull[0][i] = st.vx[o]; d.vfull[1][i] = st.vy[o]; d.vfull[2][i] = st.vz[o];
     d.ufull[i] = st.u[o];
     d.Sfull[0][i] = st.Sxx[o]; d.Sfull[1][i] = st.Syy[o]; d.Sfull[2][i] = st.Sxy[o];
@@ -674,15 +681,21 @@ extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, f
         ds.fixed = dfix;
     }
     int rc;
+    bool changed = false;
     if (c->resident && n > 0) {
+        SPH_CUDA(c, cudaMemsetAsync(c->d.refresh_changed, 0, sizeof(int), c->stream));
         k_refresh<<<sph_div_up(n, 256), 256, 0, c->stream>>>(c->d, ds);
         c->launches++;
-        c->force_full = true;                 // the caller's positions: nothing the lists were built on holds
         SPH_CUDA(c, cudaGetLastError());
+        int h_changed = 1;
+        SPH_CUDA(c, cudaMemcpyAsync(&h_changed, c->d.refresh_changed, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        SPH_CUDA(c, cudaStreamSynchronize(c->stream));     // the step cannot start before the copies have landed anyway
+        changed = h_changed != 0;
+        if (changed) c->force_full = true;    // the caller moved particles: nothing the lists were built on holds
     }
-    // every host-buffer step ingests the caller's positions, so its lists serve one step: built without skin and
-    // without the ordering pass; x, y, z go back on the second stream as soon as the drift is done (step_body)
-    c->no_reuse_now = true;
+    // a step on positions the caller changed builds lists that serve this step only: no skin, no ordering pass.
+    // x, y, z go back on the second stream as soon as the drift is done (step_body)
+    c->no_reuse_now = changed;
     const bool overlap = c->resident && n > 0;          // (the very first call ingests and bootstraps first)
     if (overlap) {
         c->host_out = &ds;
@@ -691,7 +704,7 @@ extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, f
     rc = sph_step(c, &ds, n, dt, nullptr);
     c->host_out = nullptr;
     c->no_reuse_now = false;
-    c->force_full = true;          // these lists have no skin: whatever step comes next must not reuse them
+    if (changed) c->force_full = true;     // those lists have no skin: whatever step comes next must not reuse them
     if (rc) return rc;
     float *dst[14] = {hs->x, hs->y, hs->z, nullptr, nullptr, hs->vx, hs->vy, hs->vz, hs->u,
                       hs->Sxx, hs->Syy, hs->Sxy, hs->Sxz, hs->Syz};

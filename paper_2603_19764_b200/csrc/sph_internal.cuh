@@ -142,6 +142,7 @@ struct Dev {
     float *dt_cur, *dt_next;                // step in use / CFL step from the last CLOSE
     double *diag_part;                      // [592][8] per-block partial sums of sph_get_diagnostics
     float *hchange;                         // max |factor - 1| of the last smoothing-length update
+    int *refresh_changed;                   // sph_step_host: != 0 if the caller's x, y, z or h differ from the resident ones
     unsigned long long *counters;           // SPH_C_COUNT
     // sort scratch
     unsigned long long *keys, *keys_alt;
