@@ -98,7 +98,7 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
     for (int k = 0; k < 9; ++k) o.F[k] = b.take<float>(N);
     for (int k = 0; k < 9; ++k) o.Cinv[k] = b.take<float>(N);
     for (int k = 0; k < 9; ++k) o.G[k] = b.take<float>(N);
-    o.B3 = b.take<float4>(N); o.B4 = b.take<float4>(N); o.B5 = b.take<float>(N);
+    o.B3 = b.take<float4>(N); o.B4 = b.take<float4>(N); o.B5 = b.take<float2>(N);
     size_t ntile = (N + SPH_TILE - 1) / SPH_TILE;
     size_t nchunk = (N + SPH_CHUNK - 1) / SPH_CHUNK;
     o.tile_ncand = b.take<int>(ntile);
@@ -121,6 +121,8 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
     o.rows_cap = kcap;
     o.rowptr = b.take<unsigned short>(lists ? nchunk * (SPH_MAXROUND + 1) : 1);
     o.nlist = b.take<uint2>(lists ? nchunk * (size_t)kcap * 32 : 1);
+    o.far_point = b.take<float4>(1);
+    o.nlen = b.take<int>(N);
     o.cull_grid = (int)ntile;
     o.walk_grid = 2 * sm_count;
     o.bbox = b.take<float>(8);

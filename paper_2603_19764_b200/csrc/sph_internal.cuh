@@ -15,7 +15,8 @@
 // neighbour-list machinery (sph_lists.cu)
 #define SPH_TILE_CHUNKS 8     // chunks per tile = warps per CTA of the list kernels
 #define SPH_TILE (SPH_TILE_CHUNKS * SPH_CHUNK)
-#define SPH_SE 1632           // candidates staged per round; the cull, density and pair kernels agree on it
+#define SPH_SE 1600           // candidates staged per round; the cull, density and pair kernels agree on it
+                              // (18 floats per slot plus the dummy slot, twice per SM: 1601 x 72 B <= 115 712 B)
 #define SPH_MAXROUND 15       // rounds a tile may need (more: the tile falls back to the tree-walk kernels)
 #define SPH_CULL_MAXSRC 768   // source chunks a tile may accept in the tree walk
 #define SPH_CULL_MAXPAR 128   // level-1 nodes a tile may expand in the last level of the walk
@@ -104,7 +105,8 @@ struct Dev {
     int *ngather, *nsym;
     float *F[9], *Cinv[9], *G[9];
     float4 *B3, *B4;                        // packed pair-pass operands (see k_predict):
-    float *B5;                              //   B3 = {rho, c, w, st_xx}, B4 = {st_yy, st_zz, st_xy, st_xz}, B5 = st_yz
+    float2 *B5;                             //   B3 = {rho, c, w, st_xx}, B4 = {st_yy, st_zz, st_xy, st_xz}, B5 = {st_yz, m K},
+                                            //   K = 20 SIGMA / H^5 (Wendland C2: -(dW/dr)/r = K (1 - r/H)^3)
     // neighbour lists (sph_lists.cu)
     int *tile_ncand;                        // candidates per tile
     unsigned *cand;                         // candidate pool: global indices, tile after tile, ascending per tile
@@ -135,6 +137,8 @@ struct Dev {
     unsigned char *heavy_mark;              // [tile] != 0: in heavy_list
     int heavy_cap;                          // blocks reserved in front of the grid for heavy_list
     unsigned char *tile_flag;               // != 0: the tile exceeded a capacity; the tree-walk kernels serve it
+    float4 *far_point;                      // x, y, z out of everybody's reach and the largest support radius (sph_far_point)
+    int *nlen;                              // per particle: entries of its neighbour list (pairs of the skin included)
     int cull_grid;                          // persistent CTAs of k_cull
     int walk_grid;                          // persistent CTAs of the tree-walk kernels when they serve flagged tiles
     // scalars on the device

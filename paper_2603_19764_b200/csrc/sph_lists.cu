@@ -359,7 +359,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float inf
             d.tile_off[tile] = 0;
             if (!was_flagged) atomicAdd(&d.counters[SPH_C_LIST_OVERFLOW], 1ull);
         }
-        if (valid) d.nsym[i] = 0;
+        if (valid) { d.nsym[i] = 0; d.nlen[i] = 0; }
         if (threadIdx.x == 0 && !dirty) {
             const unsigned cyc = (unsigned)(clock64() - t_begin);
             d.tile_cycles[tile] = cyc;
@@ -573,7 +573,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float inf
         }
         __syncthreads();
     }
-    if (valid) d.nsym[i] = nhit;
+    if (valid) { d.nsym[i] = nhit; d.nlen[i] = nhit; }      // nlen: entries of the particle's list (pairs of the skin included)
     if (warp < nch) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) tests += __shfl_xor_sync(FULL, tests, o);
@@ -597,10 +597,39 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float inf
     }
 }
 
+// A point no particle can reach and that reaches no particle, from the top level of the chunk tree at the current
+// positions (warp-wide): beyond the box of everything by twice its extent plus eight times the largest support radius,
+// carrying that radius.  The padding entries of the neighbour lists stand for a source of mass 0 there.
+__device__ __forceinline__ void sph_far_point(const Dev &d, int lane)
+{
+    const int L = d.tree.nlev - 1, cnt = d.tree.count[L];
+    float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, H = 0.f;
+    if (lane < cnt) {
+        const float4 a = d.tree.lo[L][lane], b = d.tree.hi[L][lane];
+        lo[0] = a.x; lo[1] = a.y; lo[2] = a.z; H = a.w;
+        hi[0] = b.x; hi[1] = b.y; hi[2] = b.z;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            lo[a] = fminf(lo[a], __shfl_xor_sync(FULL, lo[a], o));
+            hi[a] = fmaxf(hi[a], __shfl_xor_sync(FULL, hi[a], o));
+        }
+        H = fmaxf(H, __shfl_xor_sync(FULL, H, o));
+    }
+    if (lane == 0) {
+        const float ext = fmaxf(hi[0] - lo[0], fmaxf(hi[1] - lo[1], hi[2] - lo[2]));
+        const float off = 2.f * ext + 8.f * H;
+        *d.far_point = make_float4(hi[0] + off, hi[1] + off, hi[2] + off, H);
+    }
+}
+
 // Head of a list build, ONE block: which tiles go first (those that cost more than 1.5x the average in the previous
 // build), and the resets the build needs (list-build counters, candidate pool cursor, cycle sum).
 __global__ void __launch_bounds__(1024) k_tile_plan(Dev d, int ntile, int dirty)
 {
+    if (threadIdx.x < 32) sph_far_point(d, threadIdx.x);
     if (dirty) {                  // a step that reuses the lists: only the second region of the pool starts over
         if (threadIdx.x == 0) {
             d.cand_cursor[1] = 0ull;
@@ -731,6 +760,10 @@ __device__ __forceinline__ void cp_async16(void *smem, const void *gmem)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
 }
+__device__ __forceinline__ void cp_async8(void *smem, const void *gmem)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
+}
 __device__ __forceinline__ void cp_async4(void *smem, const void *gmem)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((unsigned)__cvta_generic_to_shared(smem)), "l"(gmem));
@@ -781,7 +814,11 @@ __global__ void __launch_bounds__(SPH_TILE, 4) k_density_l(Dev d, float kappa, R
     const unsigned short *rp = d.rowptr + (size_t)(haschunk ? chunk : 0) * ROWPTR_STRIDE;
     DensAcc A;
     A.sum = (double)pi.w; A.sh = 3.f * pi.w; A.n = 1;          // self term: q = 0, t = 1
-    int ntest = 1;
+    // slot SPH_SE: the far dummy source the padding entries of the lists point at (out of everybody's reach)
+    if (threadIdx.x == 0) {
+        const float4 fp = *d.far_point;
+        s_pm[SPH_SE] = make_float4(fp.x, fp.y, fp.z, 0.f);
+    }
     int round = 0;
     const int se = sph_round_size(ncand);
     for (int r0 = 0; r0 < ncand; r0 += se, ++round) {
@@ -797,9 +834,7 @@ __global__ void __launch_bounds__(SPH_TILE, 4) k_density_l(Dev d, float kappa, R
                 if (gq + 1 < g1) nxt = lp[(size_t)(gq + 1) * 32];
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    const unsigned off = list_entry(w, e);
-                    if (off == 0xffffu) continue;
-                    ++ntest;
+                    const unsigned off = min(list_entry(w, e), (unsigned)(SPH_SE << 4));      // padding (0xFFFF): the dummy
                     const float4 q = *reinterpret_cast<const float4 *>(smem_raw + off);
                     const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
                     if (r2 < H2i)
@@ -821,7 +856,7 @@ __global__ void __launch_bounds__(SPH_TILE, 4) k_density_l(Dev d, float kappa, R
         d.ngather[i] = A.n;
         small = fabsf(om) < 0.1f ? 1u : 0u;
     }
-    unsigned long long hits = valid ? (unsigned long long)A.n : 0ull, tests = valid ? (unsigned long long)ntest : 0ull;
+    unsigned long long hits = valid ? (unsigned long long)A.n : 0ull, tests = valid ? (unsigned long long)(d.nlen[i] + 1) : 0ull;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         hits += __shfl_xor_sync(FULL, hits, o);
@@ -843,12 +878,32 @@ __global__ void __launch_bounds__(SPH_TILE, 4) k_density_l(Dev d, float kappa, R
 // The candidates are staged with cp.async (measured against loads and stores through registers, round 2: force pass
 // 0.452 -> 0.437 ms on configs[2], 27.9 -> 26.8 ms on configs[4]; 126 -> 102 registers); the staged h is the raw
 // smoothing length, H_j = kappa h_j is formed per list entry.
+// One list entry (staged at byte offset off) that may lie inside the band |u| <= SPH_UBAND: if it does, the exact
+// predicate (reading Q4) decides whether it is a neighbour: the count and mu_max of Eq. 39.
+template <bool FORCE>
+__device__ __forceinline__ void pair_decide(const PairTarget &t, const PairConst &kc, PairAcc &A, int &cnt, float H2i,
+                                            float kappa, const unsigned char *s1, const unsigned char *s2, unsigned off)
+{
+    const float4 q1 = *reinterpret_cast<const float4 *>(s1 + off);
+    float4 q2 = *reinterpret_cast<const float4 *>(s2 + off);
+    q2.w = sph_H(kappa, q2.w);
+    const PairGeom g = pair_geom(t, q1, q2.w);
+    const float um = fmaxf(g.ui, g.uj);
+    if (um >= -SPH_UBAND && !(um > SPH_UBAND)) {
+        const float r2x = sph_r2(g.dx, g.dy, g.dz);
+        if (r2x < fmaxf(H2i, __fmul_rn(q2.w, q2.w))) {
+            ++cnt;
+            if (FORCE) A.mumax = fmaxf(A.mumax, pair_neg_mu(t, kc, g, q2));
+        }
+    }
+}
+
 template <bool GRAD, bool FORCE, bool TENSOR>
 __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p, RungCtl rc)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    unsigned char *s1 = smem_raw, *s2 = s1 + SPH_SE * 16, *s3 = s2 + SPH_SE * 16, *s4 = s3 + SPH_SE * 16,
-                  *s5 = s4 + SPH_SE * 16;
+    unsigned char *s1 = smem_raw, *s2 = s1 + (SPH_SE + 1) * 16, *s3 = s2 + (SPH_SE + 1) * 16, *s4 = s3 + (SPH_SE + 1) * 16,
+                  *s5 = s4 + (SPH_SE + 1) * 16;
     const int tile = sph_tile_of_block(d, blockIdx.x);
     if (tile < 0 || d.tile_flag[tile]) return;
     if (rc.on && !rc.tile_act[tile]) return;               // NEXT-4: no particle of this tile ends a step now
@@ -861,13 +916,24 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p, Rung
     const bool valid = i < d.n;
     const PairTarget t = pair_target_load(d, valid ? i : 0, p.kappa);
     const float H2i = __fmul_rn(t.H, t.H);
-    PairConst kc;
-    kc.beta = p.beta; kc.alpha2 = 0.5f * p.alpha; kc.eps = p.eps_av; kc.hk = 0.5f / p.kappa;
+    const PairConst kc = pair_const(p.alpha, p.beta, p.eps_av, p.kappa);
     const uint2 *lp = d.nlist + ((size_t)(haschunk ? chunk : 0) * d.rows_cap) * 32 + lane;
     const unsigned short *rp = d.rowptr + (size_t)(haschunk ? chunk : 0) * ROWPTR_STRIDE;
     PairAcc A;
     pair_acc_zero(A);
-    int cnt = 0, nent = 0;
+    int cnt = 0;
+    // slot SPH_SE of the staged arrays: the far dummy source the padding entries of the lists point at (mass 0, out of
+    // everybody's reach: sph_far_point), so that the inner loop needs no test for padding
+    if (threadIdx.x == 0) {
+        const float4 fp = *d.far_point;
+        *reinterpret_cast<float4 *>(s1 + 16 * SPH_SE) = make_float4(fp.x, fp.y, fp.z, 0.f);
+        *reinterpret_cast<float4 *>(s2 + 16 * SPH_SE) = make_float4(0.f, 0.f, 0.f, fp.w);
+        *reinterpret_cast<float4 *>(s3 + 16 * SPH_SE) = make_float4(1.f, 0.f, 0.f, 0.f);
+        if (TENSOR) {
+            *reinterpret_cast<float4 *>(s4 + 16 * SPH_SE) = make_float4(0.f, 0.f, 0.f, 0.f);
+            *reinterpret_cast<float2 *>(s5 + 8 * SPH_SE) = make_float2(0.f, 0.f);
+        }
+    }
 
     int round = 0;
     const int se = sph_round_size(ncand);
@@ -880,7 +946,7 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p, Rung
             cp_async16(s3 + 16 * s, &d.B3[j]);
             if (TENSOR) {
                 cp_async16(s4 + 16 * s, &d.B4[j]);
-                cp_async4(s5 + 4 * s, &d.B5[j]);
+                cp_async8(s5 + 8 * s, &d.B5[j]);
             }
         }
         asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory");
@@ -888,31 +954,46 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p, Rung
         if (haschunk) {
             const int g0 = rp[round], g1 = rp[round + 1];
             uint2 nxt = g0 < g1 ? lp[(size_t)g0 * 32] : make_uint2(0xffffffffu, 0xffffffffu);
+            int namb = 0;
+            unsigned amboff = 0u;
             for (int gq = g0; gq < g1; ++gq) {
                 const uint2 w = nxt;
                 if (gq + 1 < g1) nxt = lp[(size_t)(gq + 1) * 32];
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    unsigned off = list_entry(w, e);
-                    bool v = off != 0xffffu;
-                    nent += v ? 1 : 0;
-                    off = v ? off : 0u;
+                    const unsigned off = min(list_entry(w, e), (unsigned)(SPH_SE << 4));      // padding (0xFFFF): the dummy
                     const float4 q1 = *reinterpret_cast<const float4 *>(s1 + off);
                     float4 q2 = *reinterpret_cast<const float4 *>(s2 + off);
                     q2.w = sph_H(p.kappa, q2.w);
-                    // the lists may hold pairs of the skin (list reuse): membership is the exact predicate on the
-                    // current positions (reading Q4), evaluated here
-                    const float r2x = sph_r2(__fsub_rn(t.x, q1.x), __fsub_rn(t.y, q1.y), __fsub_rn(t.z, q1.z));
-                    v = v && r2x < fmaxf(H2i, __fmul_rn(q2.w, q2.w));
-                    cnt += v ? 1 : 0;
                     const float4 q3 = *reinterpret_cast<const float4 *>(s3 + off);
                     float4 q4 = make_float4(0.f, 0.f, 0.f, 0.f);
-                    float q5 = 0.f;
+                    float2 q5 = make_float2(0.f, 0.f);
                     if (TENSOR) {
                         q4 = *reinterpret_cast<const float4 *>(s4 + off);
-                        q5 = *reinterpret_cast<const float *>(s5 + (off >> 2));
+                        q5 = *reinterpret_cast<const float2 *>(s5 + (off >> 1));
                     }
-                    pair_term<GRAD, FORCE, TENSOR>(t, kc, A, q1, q2, q3, q4, q5, v);
+                    // The lists may hold pairs of the skin (list reuse) and padding.  Membership is the exact predicate
+                    // on the current positions (reading Q4); pair_term decides it from u = max(1 - r/H_i, 1 - r/H_j)
+                    // wherever |u| > SPH_UBAND and reports the entries inside the band, which are decided below.
+                    bool v, amb;
+                    pair_term<GRAD, FORCE, TENSOR, true>(t, kc, A, q1, q2, q3, q4, q5, v, amb);
+                    cnt += v ? 1 : 0;
+                    namb += amb ? 1 : 0;
+                    amboff = amb ? off : amboff;
+                }
+            }
+            // Entries inside the band (one list entry in 10^5) are decided with the exact predicate: the count, and
+            // mu_max of Eq. 39 (the sums got their < 1e-17 either way).  A lane with one such entry has its offset;
+            // a lane with several walks the round's rows again.
+            if (__any_sync(FULL, namb > 0)) {
+                if (namb == 1) pair_decide<FORCE>(t, kc, A, cnt, H2i, p.kappa, s1, s2, amboff);
+                if (__any_sync(FULL, namb > 1)) {
+                    for (int gq = g0; gq < g1; ++gq) {
+                        const uint2 w = lp[(size_t)gq * 32];
+                        for (int e = 0; e < 4; ++e)
+                            if (namb > 1)
+                                pair_decide<FORCE>(t, kc, A, cnt, H2i, p.kappa, s1, s2, min(list_entry(w, e), (unsigned)(SPH_SE << 4)));
+                    }
                 }
             }
         }
@@ -921,11 +1002,11 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p, Rung
 
     const bool keep = valid && sph_active(rc, i);          // NEXT-4: an inactive particle keeps its old derivatives
     if (keep) {
-        pair_store<GRAD, FORCE>(d, i, A);
+        pair_store<GRAD, FORCE>(d, i, A, kc);
         d.nsym[i] = cnt;
     }
     if (FORCE) {
-        unsigned long long hits = keep ? (unsigned long long)cnt : 0ull, ents = valid ? (unsigned long long)nent : 0ull;
+        unsigned long long hits = keep ? (unsigned long long)cnt : 0ull, ents = valid ? (unsigned long long)d.nlen[i] : 0ull;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             hits += __shfl_xor_sync(FULL, hits, o);
@@ -1135,7 +1216,7 @@ int sph_launch_density_l(sph_ctx *c)
     SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_TESTS_DENSITY], 0, sizeof(unsigned long long), c->stream));
     SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_OMEGA_SMALL], 0, sizeof(unsigned long long), c->stream));
     if (d.n == 0) return SPH_OK;
-    size_t bytes = (size_t)SPH_SE * sizeof(float4);
+    size_t bytes = (size_t)(SPH_SE + 1) * sizeof(float4);
     int rc = set_smem(c, (const void *)k_density_l, bytes);
     if (rc) return rc;
     k_density_l<<<d.heavy_cap + sph_div_up(d.nchunk, SPH_TILE_CHUNKS), SPH_TILE, bytes, c->stream>>>(d, c->p.kappa, c->rc);
@@ -1148,7 +1229,7 @@ template <bool GRAD, bool FORCE, bool TENSOR>
 static int launch_pair_l(sph_ctx *c)
 {
     Dev &d = c->d;
-    size_t bytes = (size_t)SPH_SE * (TENSOR ? 68 : 48);
+    size_t bytes = (size_t)(SPH_SE + 1) * (TENSOR ? 72 : 48);
     const int grid = d.heavy_cap + sph_div_up(d.nchunk, SPH_TILE_CHUNKS);
     int rc = set_smem(c, (const void *)k_pair_l<GRAD, FORCE, TENSOR>, bytes);
     if (rc) return rc;

@@ -172,12 +172,11 @@ template <bool GRAD, bool FORCE, bool EXACT>
 __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(Dev d, DevParams p, const unsigned char *__restrict__ tile_flag, int ntile, RungCtl rc)
 {
     __shared__ float4 s_src[PAIR_WARPS][4][SPH_CHUNK];
-    __shared__ float s_src5[PAIR_WARPS][SPH_CHUNK];
+    __shared__ float2 s_src5[PAIR_WARPS][SPH_CHUNK];
     __shared__ float4 s_tgt[PAIR_WARPS][SPH_CHUNK];
     __shared__ unsigned s_stack[PAIR_WARPS][STACK_DEPTH];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    PairConst kc;
-    kc.beta = p.beta; kc.alpha2 = 0.5f * p.alpha; kc.eps = p.eps_av; kc.hk = 0.5f / p.kappa;
+    const PairConst kc = pair_const(p.alpha, p.beta, p.eps_av, p.kappa);
     if (tile_flag && d.counters[SPH_C_LIST_OVERFLOW] == 0ull) return;       // serving flagged tiles: there are none
     for (int tile = blockIdx.x; tile < ntile; tile += gridDim.x) {
     if (tile_flag && !tile_flag[tile]) continue;
@@ -229,7 +228,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(Dev d, DevParams p, co
 
     const bool keep = valid && sph_active(rc, i);          // NEXT-4: an inactive particle keeps its old derivatives
     if (keep) {
-        pair_store<GRAD, FORCE>(d, i, A);
+        pair_store<GRAD, FORCE>(d, i, A, kc);
         d.nsym[i] = cnt_i;
     }
     if (FORCE) {

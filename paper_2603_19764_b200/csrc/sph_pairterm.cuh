@@ -33,6 +33,14 @@ __device__ __forceinline__ float sph_rsqrt(float y)
     return r;
 }
 
+// sqrt(y) by one MUFU.SQRT (max relative error 2^-23; sqrt(0) = 0, so no clamp and no multiply as with rsqrt)
+__device__ __forceinline__ float sph_sqrt(float y)
+{
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(y));
+    return r;
+}
+
 // ---- S2: one term of Eq. 1 and Eq. 3 (Wendland C2, reading Q3) ---------------------------------------------
 //   W = SIGMA/H^3 t^4 (1 + 4q),  dW/dh = -SIGMA/(H^3 h) t^3 (3 + 9q - 32 q^2),  q = r/H, t = 1 - q
 // rho is evaluated and accumulated in fp64: P = c0^2 (rho - rho0) amplifies the relative error of rho by
@@ -58,12 +66,23 @@ __device__ __forceinline__ double sph_widen_pos(float f)
     return __hiloint2double((int)((b >> 3) + 0x38000000u), (int)(b << 29));
 }
 
+// Eq. 5-6 with hbar = hk (H_i + H_j), hk = 1 / (2 kappa), and mu = hk mu', mu' = (H_i + H_j) v.x / (r^2 + eps hbar^2):
+// the factor hk is folded into the constants, and the kernels carry max(-mu') (pair_store scales it back)
 struct PairConst {
-    float beta;       // Eq. 5
-    float alpha2;     // alpha / 2: alpha cbar = alpha2 (c_i + c_j)
-    float eps;        // Eq. 6
-    float hk;         // 1 / (2 kappa): hbar = hk (H_i + H_j)
+    float beta_h2;    // beta hk^2
+    float alpha2_h;   // alpha / 2 * hk: alpha cbar mu = alpha2_h (c_i + c_j) mu'
+    float eps_h2;     // eps hk^2
+    float hk;         // 1 / (2 kappa)
 };
+__device__ __forceinline__ PairConst pair_const(float alpha, float beta, float eps_av, float kappa)
+{
+    PairConst k;
+    k.hk = 0.5f / kappa;
+    k.beta_h2 = beta * k.hk * k.hk;
+    k.alpha2_h = 0.5f * alpha * k.hk;
+    k.eps_h2 = eps_av * k.hk * k.hk;
+    return k;
+}
 
 // per-target operands, constant over the neighbour loop
 struct PairTarget {
@@ -78,7 +97,8 @@ struct PairTarget {
 
 struct PairAcc {
     float F[9], C[6];
-    float ax, ay, az, du, mumax;
+    float ax, ay, az, du, mumax;     // mumax: max(-mu') (see PairConst)
+    float duv;                       // sum_j 1/2 m_j Pi_ij (D_i + D_j) v_ij.x_ij: du/dt gets -1/2 of it (Eq. 8)
 };
 
 __device__ __forceinline__ void pair_acc_zero(PairAcc &A)
@@ -87,28 +107,64 @@ __device__ __forceinline__ void pair_acc_zero(PairAcc &A)
     for (int k = 0; k < 9; ++k) A.F[k] = 0.f;
 #pragma unroll
     for (int k = 0; k < 6; ++k) A.C[k] = 0.f;
-    A.ax = A.ay = A.az = A.du = A.mumax = 0.f;
+    A.ax = A.ay = A.az = A.du = A.mumax = A.duv = 0.f;
+}
+
+// Membership band of the list-driven kernel (SELFMASK): u = max(1 - r/H_i, 1 - r/H_j) computed here differs from the
+// exact value by < 5e-7 (r2 by FMA 2.4e-7 hence r 1.2e-7, sqrt.approx 1.2e-7, the reciprocals 1.2e-7, roundings), and the fp32
+// predicate of reading Q4 from the real-number boundary by 1e-7: outside |u| <= SPH_UBAND the sign of u IS the predicate.
+#ifndef SPH_UBAND
+#define SPH_UBAND 2.0e-6f
+#endif
+
+// the geometry both the pair term and the re-walk of the ambiguous entries evaluate, operation for operation
+struct PairGeom {
+    float dx, dy, dz, r2, r, invHj, ui, uj;
+};
+__device__ __forceinline__ PairGeom pair_geom(const PairTarget &t, float4 q1, float Hj)
+{
+    PairGeom g;
+    g.dx = __fsub_rn(t.x, q1.x); g.dy = __fsub_rn(t.y, q1.y); g.dz = __fsub_rn(t.z, q1.z);
+    g.r2 = __fmaf_rn(g.dz, g.dz, __fmaf_rn(g.dy, g.dy, __fmul_rn(g.dx, g.dx)));
+    g.r = sph_sqrt(g.r2);
+    g.invHj = sph_rcp(Hj);
+    g.ui = __fmaf_rn(-g.r, t.invH, 1.f);
+    g.uj = __fmaf_rn(-g.r, g.invHj, 1.f);
+    return g;
 }
 
 // q1 = {x, y, z, m}_j   q2 = {vx, vy, vz, H}_j   q3 = {rho, c, w, st_xx}_j   q4 = {st_yy, st_zz, st_xy, st_xz}_j
-// q5 = st_yz_j.  valid == false: the entry contributes nothing (list padding).
+// q5 = {st_yz, m K}_j with K_j = 20 SIGMA / H_j^5 (TENSOR only; the hydro-only pass forms m_j K_j itself).
+// SELFMASK == false: valid == false means the entry contributes nothing (list padding).
+// SELFMASK == true (list-driven kernel; lists with a skin, padding entries pointing at a far dummy source of mass 0):
+// nothing is masked by hand -- outside both supports t_i = t_j = 0 and every sum gets an exact zero -- except mu_max
+// and the viscosity, which take v = (u > SPH_UBAND); v is returned in `valid`, amb = (|u| <= SPH_UBAND): the caller
+// decides such an entry with the exact predicate (its weight is < 1e-17 of a neighbour's either way).
 // TENSOR == false (hydro only, S == 0): st is the scalar -P/(Omega rho^2) held in t.kxx / q3.w.
-template <bool GRAD, bool FORCE, bool TENSOR = true>
+template <bool GRAD, bool FORCE, bool TENSOR = true, bool SELFMASK = false>
 __device__ __forceinline__ void pair_term(const PairTarget &t, const PairConst &k, PairAcc &A, float4 q1, float4 q2,
-                                          float4 q3, float4 q4, float q5, bool valid)
+                                          float4 q3, float4 q4, float2 q5, bool &valid, bool &amb)
 {
-    const float dx = t.x - q1.x, dy = t.y - q1.y, dz = t.z - q1.z;
-    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    const float r = r2 * sph_rsqrt(fmaxf(r2, 1.0e-37f));
-    const float invHj = sph_rcp(q2.w);
-    const float ti = fmaxf(0.f, fmaf(-r, t.invH, 1.f));
-    const float tj = fmaxf(0.f, fmaf(-r, invHj, 1.f));
+    const PairGeom g = pair_geom(t, q1, q2.w);
+    const float dx = g.dx, dy = g.dy, dz = g.dz, r2 = g.r2, invHj = g.invHj;
+    if (SELFMASK) {
+        const float um = fmaxf(g.ui, g.uj);
+        valid = um > SPH_UBAND;
+        amb = um >= -SPH_UBAND && !valid;
+    }
+    const float ti = fmaxf(0.f, g.ui);
+    const float tj = fmaxf(0.f, g.uj);
     const float ti3 = ti * ti * ti, tj3 = tj * tj * tj;
-    const float g2 = invHj * invHj;
-    const float Kj = (SPH_WC2_K20 * invHj) * (g2 * g2);
-    const float mj = valid ? q1.w : 0.f;
-    const float di = mj * ti3;                       // m_j t_i^3       (D_i = K_i t_i^3)
-    const float dj = mj * Kj * tj3;                  // m_j D_j
+    float mKj;
+    if (TENSOR) {
+        mKj = q5.y;
+    } else {
+        const float g2 = invHj * invHj;
+        mKj = q1.w * ((SPH_WC2_K20 * invHj) * (g2 * g2));
+    }
+    const bool on = SELFMASK || valid;
+    const float di = (on ? q1.w : 0.f) * ti3;        // m_j t_i^3       (D_i = K_i t_i^3)
+    const float dj = (on ? mKj : 0.f) * tj3;         // m_j D_j
     const float dvx = t.vx - q2.x, dvy = t.vy - q2.y, dvz = t.vz - q2.z;
     if (GRAD) {
         const float s = fmaf(di, t.wK, dj * q3.z);   // m_j (w_i D_i + w_j D_j)
@@ -130,8 +186,8 @@ __device__ __forceinline__ void pair_term(const PairTarget &t, const PairConst &
             A.du = fmaf(di, fmaf(zx, dvx, fmaf(zy, dvy, zz * dvz)), A.du);
             // j side: y = st_j x_ij
             const float yx = fmaf(q3.w, dx, fmaf(q4.z, dy, q4.w * dz));
-            const float yy = fmaf(q4.z, dx, fmaf(q4.x, dy, q5 * dz));
-            const float yz = fmaf(q4.w, dx, fmaf(q5, dy, q4.y * dz));
+            const float yy = fmaf(q4.z, dx, fmaf(q4.x, dy, q5.x * dz));
+            const float yz = fmaf(q4.w, dx, fmaf(q5.x, dy, q4.y * dz));
             A.ax = fmaf(-dj, yx, A.ax); A.ay = fmaf(-dj, yy, A.ay); A.az = fmaf(-dj, yz, A.az);
         } else {
             const float si = di * t.kxx;                                     // m_j D_i st_i
@@ -142,14 +198,31 @@ __device__ __forceinline__ void pair_term(const PairTarget &t, const PairConst &
         // artificial viscosity (only approaching pairs: min(v.x, 0))
         float vr = fminf(vx_, 0.f);
         vr = valid ? vr : 0.f;
-        const float hb = k.hk * (t.H + q2.w);
-        const float mu = (hb * vr) * sph_rcp(fmaf(k.eps * hb, hb, r2));
-        const float P2 = (mu * fmaf(k.beta, mu, -k.alpha2 * (t.c + q3.y))) * sph_rcp(t.rho + q3.x);   // Pi_ij / 2
+        const float hs = t.H + q2.w;
+        const float mu = (hs * vr) * sph_rcp(fmaf(k.eps_h2 * hs, hs, r2));                              // mu'
+        const float P2 = (mu * fmaf(k.beta_h2, mu, -k.alpha2_h * (t.c + q3.y))) * sph_rcp(t.rho + q3.x);   // Pi_ij / 2
         const float kk = P2 * fmaf(t.K, di, dj);     // 1/2 m_j Pi_ij (D_i + D_j)
         A.ax = fmaf(kk, dx, A.ax); A.ay = fmaf(kk, dy, A.ay); A.az = fmaf(kk, dz, A.az);
-        A.du = fmaf(-0.5f * kk, vr, A.du);
+        A.duv = fmaf(kk, vr, A.duv);
         A.mumax = fmaxf(A.mumax, -mu);
     }
+}
+
+template <bool GRAD, bool FORCE, bool TENSOR = true>
+__device__ __forceinline__ void pair_term(const PairTarget &t, const PairConst &k, PairAcc &A, float4 q1, float4 q2,
+                                          float4 q3, float4 q4, float2 q5, bool valid)
+{
+    bool amb = false;
+    pair_term<GRAD, FORCE, TENSOR, false>(t, k, A, q1, q2, q3, q4, q5, valid, amb);
+}
+
+// -mu' (>= 0) of one pair: the entries of the list-driven kernel that the exact predicate decides
+__device__ __forceinline__ float pair_neg_mu(const PairTarget &t, const PairConst &k, const PairGeom &g, float4 q2)
+{
+    const float dvx = t.vx - q2.x, dvy = t.vy - q2.y, dvz = t.vz - q2.z;
+    const float vr = fminf(fmaf(dvx, g.dx, fmaf(dvy, g.dy, dvz * g.dz)), 0.f);
+    const float hs = t.H + q2.w;
+    return -(hs * vr) * sph_rcp(fmaf(k.eps_h2 * hs, hs, g.r2));
 }
 
 __device__ __forceinline__ void density_term(DensAcc &A, float r2, float mj, float invH, double ex, double ey,
@@ -184,7 +257,7 @@ __device__ __forceinline__ void density_finish(const DensAcc &A, float invH, dou
 __device__ __forceinline__ PairTarget pair_target_load(const Dev &d, long long i, float kappa)
 {
     const float4 pi = d.r.pm[i], vi = d.r.vh[i], b3 = d.B3[i], b4 = d.B4[i];
-    const float b5 = d.B5[i];
+    const float b5 = d.B5[i].x;
     PairTarget t;
     t.x = pi.x; t.y = pi.y; t.z = pi.z;
     t.vx = vi.x; t.vy = vi.y; t.vz = vi.z;
@@ -200,7 +273,7 @@ __device__ __forceinline__ PairTarget pair_target_load(const Dev &d, long long i
 }
 
 template <bool GRAD, bool FORCE>
-__device__ __forceinline__ void pair_store(const Dev &d, long long i, const PairAcc &A)
+__device__ __forceinline__ void pair_store(const Dev &d, long long i, const PairAcc &A, const PairConst &k)
 {
     if (GRAD) {
 #pragma unroll
@@ -215,7 +288,7 @@ __device__ __forceinline__ void pair_store(const Dev &d, long long i, const Pair
         d.a[0][i] = A.ax + d.r.s[PP_G + 0][i];
         d.a[1][i] = A.ay + d.r.s[PP_G + 1][i];
         d.a[2][i] = A.az + d.r.s[PP_G + 2][i];
-        d.dudt[i] = A.du;
-        d.mumax[i] = A.mumax;
+        d.dudt[i] = fmaf(-0.5f, A.duv, A.du);
+        d.mumax[i] = k.hk * A.mumax;
     }
 }
