@@ -91,11 +91,14 @@ def load():
     global _lib
     if _lib is not None:
         return _lib
-    _ensure_built()
-    if not os.path.exists(LIB_PATH):
-        raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2603_19764_b200.build` "
+    path = os.environ.get("SPH_LIB")             # another build of the same sources (build.build(out=..., defines=...))
+    if not path:
+        path = LIB_PATH
+        _ensure_built()
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: run `python -m paper_2603_19764_b200.build` "
                            "(there is no CPU fallback)")
-    lib = C.CDLL(LIB_PATH)
+    lib = C.CDLL(path)
     for s in SYMBOLS:
         getattr(lib, s)                      # AttributeError if a declared symbol is not exported
     vp, ll, fl, i = C.c_void_p, C.c_longlong, C.c_float, C.c_int

@@ -33,22 +33,25 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not _stale():
+def build(force: bool = False, verbose: bool = False, out: str | None = None, defines=()) -> str:
+    """out / defines: a second library with other compile-time constants (e.g. defines=("SPH_UBAND=1.0e-3f",), which
+    tests/test_gpu_band.py loads through SPH_LIB to drive the rare paths of k_pair_l); the default builds libsph.so."""
+    target = out or OUT
+    if out is None and not force and not _stale():
         return OUT
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    tmp = OUT + ".tmp.%d" % os.getpid()              # never leave a half-written library where load() looks
+    tmp = target + ".tmp.%d" % os.getpid()           # never leave a half-written library where load() looks
     cmd = [nvcc, "-O3", "-std=c++17", *ARCH, "-lineinfo", "-diag-suppress", "128", "-Xcompiler", "-fPIC", "-shared",
-           "-o", tmp, *sources()]
+           *["-D" + d for d in defines], "-o", tmp, *sources()]
     if verbose:
         cmd += ["-Xptxas", "-v"]
     try:
         subprocess.check_call(cmd)
-        os.replace(tmp, OUT)
+        os.replace(tmp, target)
     finally:
         if os.path.exists(tmp):
             os.remove(tmp)
-    return OUT
+    return target
 
 
 if __name__ == "__main__":

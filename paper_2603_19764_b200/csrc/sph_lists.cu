@@ -18,7 +18,7 @@
 //                     buffer in shared memory; complete row-groups of 4 entries go to the global list,
 //                     which is stored transposed ([chunk][row-group][lane]) so that a warp reads one
 //                     coalesced 256-byte row-group per four pairs.  Rounds start at a common row-group
-//                     (rowptr); 0xFFFF pads.
+//                     (rowptr); LIST_PAD pads.
 //   k_density_l : stages {x,y,z,m} of the round's candidates in shared memory (coalesced gathers of index
 //                 runs) and walks the lists; the gather set is the subset with r2 < H_i^2, plus self.
 //   k_pair_l    : same with the 17 floats per source of the fused gradient + force pass.
@@ -34,6 +34,9 @@
 
 #define FULL 0xffffffffu
 #define ROWPTR_STRIDE (SPH_MAXROUND + 1)
+#define LIST_PAD ((unsigned)(SPH_SE << 4))         // padding entry of a list: the byte offset of slot SPH_SE, where the
+                                                   // density and pair kernels keep a far dummy source of mass 0
+#define LIST_PAD2 (LIST_PAD | (LIST_PAD << 16))
 #define LBUF_ENTRIES 32                    // u16 entries a lane can hold between two flushes
 #define LBUF_STRIDE (LBUF_ENTRIES * 2 + 8) // bytes per lane: 18 words, so lanes at the same fill level spread over banks
 
@@ -557,13 +560,13 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float inf
             // ---- end of the round: pad the last row-group, flush, pad every lane to the warp's longest list
             nhit += 4 * (G - Gstart) + ((int)(wp - lb) >> 1);
             while ((int)(wp - lb) & 7) {
-                *reinterpret_cast<unsigned short *>(smem_raw + wp) = 0xffffu;
+                *reinterpret_cast<unsigned short *>(smem_raw + wp) = (unsigned short)LIST_PAD;
                 wp += 2;
             }
             LIST_FLUSH();
             const int Gmax = __reduce_max_sync(FULL, G);
             for (int gg = G; gg < Gmax; ++gg)
-                if (gg < d.rows_cap) lp[(size_t)gg * 32] = make_uint2(0xffffffffu, 0xffffffffu);
+                if (gg < d.rows_cap) lp[(size_t)gg * 32] = make_uint2(LIST_PAD2, LIST_PAD2);
             G = Gmax;
             if (G > d.rows_cap) sm.overflow = 8;      // list rows exhausted: the tile falls back
             if (lane == 0) {
@@ -705,7 +708,7 @@ __global__ void __launch_bounds__(SORT_WARPS * 32) k_list_sort(Dev d)
             for (int e = 0; e < 4; ++e) {
                 const unsigned x = (e & 2) ? w.y : w.x;
                 const unsigned off = (e & 1) ? (x >> 16) : (x & 0xffffu);
-                if (off != 0xffffu) { cnt += 1ull << (((off >> 4) & 7u) << 3); ++N; }
+                if (off != LIST_PAD) { cnt += 1ull << (((off >> 4) & 7u) << 3); ++N; }
             }
         }
         if (__any_sync(FULL, N > SORT_CAP)) continue;
@@ -718,7 +721,7 @@ __global__ void __launch_bounds__(SORT_WARPS * 32) k_list_sort(Dev d)
             for (int e = 0; e < 4; ++e) {
                 const unsigned x = (e & 2) ? w.y : w.x;
                 const unsigned off = (e & 1) ? (x >> 16) : (x & 0xffffu);
-                if (off != 0xffffu) {
+                if (off != LIST_PAD) {
                     const unsigned c8 = ((off >> 4) & 7u) << 3;
                     buf[(unsigned)(cur >> c8) & 0xffu] = (unsigned short)off;
                     cur += 1ull << c8;
@@ -731,7 +734,7 @@ __global__ void __launch_bounds__(SORT_WARPS * 32) k_list_sort(Dev d)
         const int nmax = (g1 - g0) * 4;
         unsigned w0 = 0u, w1 = 0u;
         for (int n = 0; n < nmax; ++n) {
-            unsigned entry = 0xffffu;
+            unsigned entry = LIST_PAD;
             if (n < N) {
                 unsigned c8 = ((unsigned)(lane + n) & 7u) << 3;
                 while (((unsigned)(tk >> c8) & 0xffu) >= ((unsigned)(end >> c8) & 0xffu)) c8 = (c8 + 8u) & 63u;
@@ -828,13 +831,13 @@ __global__ void __launch_bounds__(SPH_TILE, 4) k_density_l(Dev d, float kappa, R
         __syncthreads();
         if (haschunk) {
             const int g0 = rp[round], g1 = rp[round + 1];
-            uint2 nxt = g0 < g1 ? lp[(size_t)g0 * 32] : make_uint2(0xffffffffu, 0xffffffffu);
+            uint2 nxt = g0 < g1 ? lp[(size_t)g0 * 32] : make_uint2(LIST_PAD2, LIST_PAD2);
             for (int gq = g0; gq < g1; ++gq) {
                 const uint2 w = nxt;
                 if (gq + 1 < g1) nxt = lp[(size_t)(gq + 1) * 32];
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    const unsigned off = min(list_entry(w, e), (unsigned)(SPH_SE << 4));      // padding (0xFFFF): the dummy
+                    const unsigned off = list_entry(w, e);               // padding (LIST_PAD): the dummy
                     const float4 q = *reinterpret_cast<const float4 *>(smem_raw + off);
                     const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
                     if (r2 < H2i)
@@ -953,7 +956,7 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p, Rung
         __syncthreads();
         if (haschunk) {
             const int g0 = rp[round], g1 = rp[round + 1];
-            uint2 nxt = g0 < g1 ? lp[(size_t)g0 * 32] : make_uint2(0xffffffffu, 0xffffffffu);
+            uint2 nxt = g0 < g1 ? lp[(size_t)g0 * 32] : make_uint2(LIST_PAD2, LIST_PAD2);
             int namb = 0;
             unsigned amboff = 0u;
             for (int gq = g0; gq < g1; ++gq) {
@@ -961,7 +964,7 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p, Rung
                 if (gq + 1 < g1) nxt = lp[(size_t)(gq + 1) * 32];
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
-                    const unsigned off = min(list_entry(w, e), (unsigned)(SPH_SE << 4));      // padding (0xFFFF): the dummy
+                    const unsigned off = list_entry(w, e);               // padding (LIST_PAD): the dummy
                     const float4 q1 = *reinterpret_cast<const float4 *>(s1 + off);
                     float4 q2 = *reinterpret_cast<const float4 *>(s2 + off);
                     q2.w = sph_H(p.kappa, q2.w);
@@ -992,7 +995,7 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p, Rung
                         const uint2 w = lp[(size_t)gq * 32];
                         for (int e = 0; e < 4; ++e)
                             if (namb > 1)
-                                pair_decide<FORCE>(t, kc, A, cnt, H2i, p.kappa, s1, s2, min(list_entry(w, e), (unsigned)(SPH_SE << 4)));
+                                pair_decide<FORCE>(t, kc, A, cnt, H2i, p.kappa, s1, s2, list_entry(w, e));
                     }
                 }
             }
@@ -1054,7 +1057,7 @@ __global__ void __launch_bounds__(256) k_neighbors_l(Dev d, float kappa, int *co
             const uint2 w = lp[(size_t)gq * 32];
             for (int e = 0; e < 4; ++e) {
                 const unsigned off = list_entry(w, e);
-                if (off == 0xffffu) continue;
+                if (off == LIST_PAD) continue;
                 unsigned j = cand[r0 + (int)(off >> 4)];
                 const float4 q = d.r.pm[j];
                 const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
