@@ -957,11 +957,11 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p, Rung
         if (haschunk) {
             const int g0 = rp[round], g1 = rp[round + 1];
             uint2 nxt = g0 < g1 ? lp[(size_t)g0 * 32] : make_uint2(LIST_PAD2, LIST_PAD2);
-            int namb = 0;
-            unsigned amboff = 0u;
+            int namb = 0, ambrow = 0;              // row-groups of this lane with an entry inside the band; the last one
             for (int gq = g0; gq < g1; ++gq) {
                 const uint2 w = nxt;
                 if (gq + 1 < g1) nxt = lp[(size_t)(gq + 1) * 32];
+                float umin = 3.0e38f;
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
                     const unsigned off = list_entry(w, e);               // padding (LIST_PAD): the dummy
@@ -977,25 +977,28 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p, Rung
                     }
                     // The lists may hold pairs of the skin (list reuse) and padding.  Membership is the exact predicate
                     // on the current positions (reading Q4); pair_term decides it from u = max(1 - r/H_i, 1 - r/H_j)
-                    // wherever |u| > SPH_UBAND and reports the entries inside the band, which are decided below.
-                    bool v, amb;
-                    pair_term<GRAD, FORCE, TENSOR, true>(t, kc, A, q1, q2, q3, q4, q5, v, amb);
+                    // wherever |u| > SPH_UBAND; the entries inside the band are decided below.
+                    bool v;
+                    float um;
+                    pair_term<GRAD, FORCE, TENSOR, true>(t, kc, A, q1, q2, q3, q4, q5, v, um);
                     cnt += v ? 1 : 0;
-                    namb += amb ? 1 : 0;
-                    amboff = amb ? off : amboff;
+                    umin = fminf(umin, fabsf(um));
                 }
+                if (umin <= SPH_UBAND) { ++namb; ambrow = gq; }
             }
             // Entries inside the band (one list entry in 10^5) are decided with the exact predicate: the count, and
-            // mu_max of Eq. 39 (the sums got their < 1e-17 either way).  A lane with one such entry has its offset;
-            // a lane with several walks the round's rows again.
+            // mu_max of Eq. 39 (the sums got their < 1e-17 either way).  A lane with one such row-group looks at its
+            // four entries; a lane with several walks the round's rows again.
             if (__any_sync(FULL, namb > 0)) {
-                if (namb == 1) pair_decide<FORCE>(t, kc, A, cnt, H2i, p.kappa, s1, s2, amboff);
+                if (namb == 1) {
+                    const uint2 w = lp[(size_t)ambrow * 32];
+                    for (int e = 0; e < 4; ++e) pair_decide<FORCE>(t, kc, A, cnt, H2i, p.kappa, s1, s2, list_entry(w, e));
+                }
                 if (__any_sync(FULL, namb > 1)) {
                     for (int gq = g0; gq < g1; ++gq) {
                         const uint2 w = lp[(size_t)gq * 32];
                         for (int e = 0; e < 4; ++e)
-                            if (namb > 1)
-                                pair_decide<FORCE>(t, kc, A, cnt, H2i, p.kappa, s1, s2, list_entry(w, e));
+                            if (namb > 1) pair_decide<FORCE>(t, kc, A, cnt, H2i, p.kappa, s1, s2, list_entry(w, e));
                     }
                 }
             }

@@ -138,19 +138,18 @@ __device__ __forceinline__ PairGeom pair_geom(const PairTarget &t, float4 q1, fl
 // SELFMASK == false: valid == false means the entry contributes nothing (list padding).
 // SELFMASK == true (list-driven kernel; lists with a skin, padding entries pointing at a far dummy source of mass 0):
 // nothing is masked by hand -- outside both supports t_i = t_j = 0 and every sum gets an exact zero -- except mu_max
-// and the viscosity, which take v = (u > SPH_UBAND); v is returned in `valid`, amb = (|u| <= SPH_UBAND): the caller
-// decides such an entry with the exact predicate (its weight is < 1e-17 of a neighbour's either way).
+// and the viscosity, which take v = (u > SPH_UBAND); v is returned in `valid` and u in `um`: an entry with
+// |u| <= SPH_UBAND is decided by the caller with the exact predicate (its weight is < 1e-17 of a neighbour's either way).
 // TENSOR == false (hydro only, S == 0): st is the scalar -P/(Omega rho^2) held in t.kxx / q3.w.
 template <bool GRAD, bool FORCE, bool TENSOR = true, bool SELFMASK = false>
 __device__ __forceinline__ void pair_term(const PairTarget &t, const PairConst &k, PairAcc &A, float4 q1, float4 q2,
-                                          float4 q3, float4 q4, float2 q5, bool &valid, bool &amb)
+                                          float4 q3, float4 q4, float2 q5, bool &valid, float &um)
 {
     const PairGeom g = pair_geom(t, q1, q2.w);
     const float dx = g.dx, dy = g.dy, dz = g.dz, r2 = g.r2, invHj = g.invHj;
     if (SELFMASK) {
-        const float um = fmaxf(g.ui, g.uj);
+        um = fmaxf(g.ui, g.uj);
         valid = um > SPH_UBAND;
-        amb = um >= -SPH_UBAND && !valid;
     }
     const float ti = fmaxf(0.f, g.ui);
     const float tj = fmaxf(0.f, g.uj);
@@ -212,8 +211,8 @@ template <bool GRAD, bool FORCE, bool TENSOR = true>
 __device__ __forceinline__ void pair_term(const PairTarget &t, const PairConst &k, PairAcc &A, float4 q1, float4 q2,
                                           float4 q3, float4 q4, float2 q5, bool valid)
 {
-    bool amb = false;
-    pair_term<GRAD, FORCE, TENSOR, false>(t, k, A, q1, q2, q3, q4, q5, valid, amb);
+    float um = 0.f;
+    pair_term<GRAD, FORCE, TENSOR, false>(t, k, A, q1, q2, q3, q4, q5, valid, um);
 }
 
 // -mu' (>= 0) of one pair: the entries of the list-driven kernel that the exact predicate decides
@@ -230,7 +229,7 @@ __device__ __forceinline__ void density_term(DensAcc &A, float r2, float mj, flo
 {
     const float rinv = sph_rsqrt(fmaxf(r2, 1.0e-37f));
     const float q = (r2 * rinv) * invH;
-    const float t = fmaxf(0.f, 1.f - q);
+    const float t = 1.f - q;        // no clamp: membership says q < 1 up to rounding, and t^3 of a t of -1e-7 is -1e-21
     A.sh = fmaf(mj * (t * t * t), fmaf(q, fmaf(-32.f, q, 9.f), 3.f), A.sh);
     const double r2d = fma(ex, ex, fma(ey, ey, ez * ez));
     const double yd = sph_widen_pos(rinv), td0 = r2d * yd;
