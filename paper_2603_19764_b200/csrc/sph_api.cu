@@ -94,6 +94,7 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
     o.T = b.take<float>(N); o.Gamma = b.take<float>(N); o.Y = b.take<float>(N); o.mumax = b.take<float>(N);
     o.dti = b.take<float>(N); o.eps2 = b.take<float>(N); o.cflag = b.take<float>(N);
     o.rho64 = b.take<double>(N);
+    o.mK = b.take<float>(N);
     o.ngather = b.take<int>(N); o.nsym = b.take<int>(N);
     for (int k = 0; k < 9; ++k) o.F[k] = b.take<float>(N);
     for (int k = 0; k < 9; ++k) o.Cinv[k] = b.take<float>(N);

@@ -102,6 +102,7 @@ struct Dev {
     float *a[3], *dudt, *dS[5];             // derivatives at the full step
     float *rho, *omega, *P, *cs, *T, *Gamma, *Y, *mumax, *dti, *eps2, *cflag;
     double *rho64;                          // fp64 density for the EOS (see k_density)
+    float *mK;                              // m K, K = 20 SIGMA / H^5 (written by the density kernels, packed into B5 by k_predict)
     int *ngather, *nsym;
     float *F[9], *Cinv[9], *G[9];
     float4 *B3, *B4;                        // packed pair-pass operands (see k_predict):

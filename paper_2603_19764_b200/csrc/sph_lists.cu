@@ -857,6 +857,7 @@ __global__ void __launch_bounds__(SPH_TILE, 4) k_density_l(Dev d, float kappa, R
         d.rho[i] = rho;
         d.omega[i] = om;
         d.ngather[i] = A.n;
+        d.mK[i] = sph_mK(pi.w, invH);
         small = fabsf(om) < 0.1f ? 1u : 0u;
     }
     unsigned long long hits = valid ? (unsigned long long)A.n : 0ull, tests = valid ? (unsigned long long)(d.nlen[i] + 1) : 0ull;

@@ -149,6 +149,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_density(Dev d, float kappa,
         d.rho[i] = rho;
         d.omega[i] = om;
         d.ngather[i] = A.n;
+        d.mK[i] = sph_mK(pi.w, invH);
         small = fabsf(om) < 0.1f ? 1u : 0u;
     }
     small = __popc(__ballot_sync(0xffffffffu, small != 0u));

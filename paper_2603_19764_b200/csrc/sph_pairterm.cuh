@@ -33,6 +33,13 @@ __device__ __forceinline__ float sph_rsqrt(float y)
     return r;
 }
 
+// m K with K = 20 SIGMA / H^5: -(dW/dr)/r = K (1 - r/H)^3 for Wendland C2 (reading Q3); invH = 1 / H
+__device__ __forceinline__ float sph_mK(float m, float invH)
+{
+    const float g2 = invH * invH;
+    return m * ((SPH_WC2_K20 * invH) * (g2 * g2));
+}
+
 // sqrt(y) by one MUFU.SQRT (max relative error 2^-23; sqrt(0) = 0, so no clamp and no multiply as with rsqrt)
 __device__ __forceinline__ float sph_sqrt(float y)
 {
@@ -158,8 +165,7 @@ __device__ __forceinline__ void pair_term(const PairTarget &t, const PairConst &
     if (TENSOR) {
         mKj = q5.y;
     } else {
-        const float g2 = invHj * invHj;
-        mKj = q1.w * ((SPH_WC2_K20 * invHj) * (g2 * g2));
+        mKj = sph_mK(q1.w, invHj);
     }
     const bool on = SELFMASK || valid;
     const float di = (on ? q1.w : 0.f) * ti3;        // m_j t_i^3       (D_i = K_i t_i^3)

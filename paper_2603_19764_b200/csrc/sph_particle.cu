@@ -99,9 +99,7 @@ __global__ void __launch_bounds__(256) k_predict(Dev d, DevParams p, DevTabs tab
     float g = w / rho;                                // 1 / (Omega rho^2)
     d.B3[i] = make_float4(rho, cs, w, g * (S[0] - P));
     d.B4[i] = make_float4(g * (S[1] - P), g * (-S[0] - S[1] - P), g * S[2], g * S[3]);
-    const float4 pm = d.r.pm[i];
-    const float invH = 1.f / sph_H(p.kappa, d.r.vh[i].w), g2 = invH * invH;
-    d.B5[i] = make_float2(g * S[4], pm.w * ((66.845076098596046f * invH) * (g2 * g2)));      // m K, K = 20 * 21 / (2 pi) / H^5
+    d.B5[i] = make_float2(g * S[4], d.mK[i]);
 }
 
 // ------------------------------------------------------------------------------------------
