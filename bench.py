@@ -26,8 +26,8 @@ if ROOT not in sys.path:
 
 # Algorithmic flops per TRUE pair evaluation, hand-counted from the equations as the kernels
 # evaluate them (FMA = 2, rsqrt / div / min / max / compare = 1); DESIGN.md section 6.
-FLOPS_PAIR_FUSED = 148      # Eq. 18-21 + 5-8, gradient and force in one pass, with S
-FLOPS_PAIR_HYDRO = 82       # force pass with S == 0 (no gradient sums)
+FLOPS_PAIR_FUSED = 147      # Eq. 18-21 + 5-8, gradient and force in one pass, with S (DESIGN.md section 5 has the breakdown)
+FLOPS_PAIR_HYDRO = 78       # force pass with S == 0 (no gradient sums; forms m_j K_j itself)
 FLOPS_PAIR_DENSITY = 44     # Eq. 1 + 3: 20 fp32 + 12 fp64 (counted as 2 each)
 FP32_LANES_PER_SM = 128
 
@@ -180,7 +180,7 @@ def run_reference(args):
 
 
 # Algorithmic HBM bytes per particle of the HBM-bound passes
-BYTES_PER_PARTICLE = {"predict": 120, "close": 230, "kickdrift": 160,
+BYTES_PER_PARTICLE = {"predict": 128, "close": 230, "kickdrift": 160,
                       # S1 with a full build: keys 12 r + 12 w, radix sort 4-5 digit passes x 24, reorder 116 r + 116 w
                       "build_full": 24 + 5 * 24 + 232}
 
