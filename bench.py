@@ -379,7 +379,7 @@ def run_ours(args):
     clocks = sampler.stop()          # sampled from the start of the device-timed steps to the end of the e2e steps
     e2e_s_max, e2e_pairs_all = rank_reduce(e2e_s, e2e_pairs, dev)
     e2e_value = e2e_pairs_all / e2e_s_max
-    h2d = n * (17 * 4 + 4 + 1)
+    h2d = n * 17 * 4               # 17 float arrays per step (material and fixed flags travel with the first call only)
     d2h = n * 12 * 4 + 4
 
     if rank != 0:
@@ -482,7 +482,8 @@ def run_ours(args):
         "e2e": {"value": e2e_value, "unit": "pairs/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s_max / e2e_steps,
                 "note": "host buffers in and out every step; the loop hands back the state it received, so the library "
-                        "finds x, y, z, h unchanged and keeps reusing its neighbour lists"},
+                        "finds x, y, z, h unchanged and keeps reusing its neighbour lists; on such steps u, S and a_ext "
+                        "arrive while the list check and the density pass run, and x, y, z leave during the pair pass"},
         "roofline": roofline,
         "cpu_baseline": cpu,
         "hydro_only": hydro,

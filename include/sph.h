@@ -256,7 +256,11 @@ int sph_step_rungs(sph_ctx *ctx, float dT, int max_rung, const unsigned char *ru
 /* The same step through HOST buffers: copies the state host->device into library-owned staging,
  * steps, copies x, v, u, S back device->host, and synchronises the stream.  dt_used: HOST.
  * If the caller's x, y, z, h equal the resident ones bit for bit (a loop that hands back what it was given) the
- * neighbour lists stay in use as in sph_step; if anything moved, the step starts from a full neighbour build. */
+ * neighbour lists stay in use as in sph_step; if anything moved, the step starts from a full neighbour build.
+ * mat and fixed are read at the FIRST call only (they stay with the resident particles).  Copies overlap the step
+ * where the data flow allows: on a step that reuses the lists u, S and a_ext arrive on a second stream while the
+ * first half of the kick, the list check and the density pass run; x, y, z leave during the pair pass.  All host
+ * arrays should be pinned (pageable memory works, without the overlap) and must not be touched during the call. */
 int sph_step_host(sph_ctx *ctx, sph_state *host_state, long long n, float dt, float *dt_used);
 
 /* Write x, v, u, S of the resident particles to the caller's DEVICE arrays in caller order. */

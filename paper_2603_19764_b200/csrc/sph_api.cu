@@ -195,7 +195,10 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
     }
     if (cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking) != cudaSuccess
         || cudaEventCreateWithFlags(&c->ev_pos, cudaEventDisableTiming) != cudaSuccess
-        || cudaEventCreateWithFlags(&c->ev_copied, cudaEventDisableTiming) != cudaSuccess) {
+        || cudaEventCreateWithFlags(&c->ev_copied, cudaEventDisableTiming) != cudaSuccess
+        || cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking) != cudaSuccess
+        || cudaEventCreateWithFlags(&c->ev_first, cudaEventDisableTiming) != cudaSuccess
+        || cudaEventCreateWithFlags(&c->ev_second, cudaEventDisableTiming) != cudaSuccess) {
         sph_destroy(c);
         return SPH_ECUDA;
     }
@@ -230,6 +233,9 @@ extern "C" void sph_destroy(sph_ctx *c)
         if (c->ev[k]) cudaEventDestroy(c->ev[k]);
     if (c->ev_pos) cudaEventDestroy(c->ev_pos);
     if (c->ev_copied) cudaEventDestroy(c->ev_copied);
+    if (c->ev_first) cudaEventDestroy(c->ev_first);
+    if (c->ev_second) cudaEventDestroy(c->ev_second);
+    if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
 }
@@ -418,10 +424,16 @@ extern "C" int sph_strength_update(sph_ctx *c, int phase, float dt)
 }
 
 // density -> predict -> fused gradient + force
+static int take_second_group(sph_ctx *c);
+
 static int derivative_passes(sph_ctx *c)
 {
     int rc = c->have_density ? SPH_OK : sph_density(c);
     if (rc) return rc;
+    if (c->host_in) {                 // sph_step_host: u, S, a_ext have landed by now; second half of the kick
+        rc = take_second_group(c);
+        if (rc) return rc;
+    }
     rc = sph_strength_update(c, SPH_PREDICT, 0.f);
     if (rc) return rc;
     return sph_gradients_forces(c);
@@ -458,7 +470,7 @@ static int step_body(sph_ctx *c, sph_state *state, long long n, float dt, float 
     }
     {
         PassTimer t(c, SPH_T_KICKDRIFT);
-        rc = sph_launch_kick_drift(c, dt);
+        rc = sph_launch_kick_drift(c, dt, c->host_in ? 1 : 3);
         if (rc) return rc;
     }
     const bool adapt = step_adapts_h(c);
@@ -633,23 +645,42 @@ extern "C" int sph_step_rungs(sph_ctx *c, float dT, int max_rung, const unsigned
 // depend on -- x, y, z, h -- is compared with the resident values first: a caller that hands back the state it was
 // given (the usual host-buffer loop) leaves them bit for bit, and the lists (with their skin and their validity
 // check) stay in use; any difference sets the flag and the step starts from a full build.
+// PARTS: 1 = x, y, z, m, h, v (and the test whether the caller moved anything), 2 = u, S, a_ext, 3 = both
+template <int PARTS>
 __global__ void __launch_bounds__(256) k_refresh(Dev d, sph_state st)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= d.n) return;
     unsigned o = ((const unsigned *)d.r.s[PP_ORIG])[i];
-    const float4 np = make_float4(st.x[o], st.y[o], st.z[o], st.m[o]), op = d.r.pm[i];
-    const float nh = st.h[o];
-    if (!(np.x == op.x && np.y == op.y && np.z == op.z && nh == d.r.vh[i].w)) *d.refresh_changed = 1;
-    d.r.pm[i] = np;
-    d.r.vh[i].w = nh;
-    d.vfull[0][i] = st.vx[o]; d.vfull[1][i] = st.vy[o]; d.vfull[2][i] = st.vz[o];
-    d.ufull[i] = st.u[o];
-    d.Sfull[0][i] = st.Sxx[o]; d.Sfull[1][i] = st.Syy[o]; d.Sfull[2][i] = st.Sxy[o];
-    d.Sfull[3][i] = st.Sxz[o]; d.Sfull[4][i] = st.Syz[o];
-    d.r.s[PP_G + 0][i] = st.gx ? st.gx[o] : 0.f;
-    d.r.s[PP_G + 1][i] = st.gy ? st.gy[o] : 0.f;
-    d.r.s[PP_G + 2][i] = st.gz ? st.gz[o] : 0.f;
+    if (PARTS & 1) {
+        const float4 np = make_float4(st.x[o], st.y[o], st.z[o], st.m[o]), op = d.r.pm[i];
+        const float nh = st.h[o];
+        if (!(np.x == op.x && np.y == op.y && np.z == op.z && nh == d.r.vh[i].w)) *d.refresh_changed = 1;
+        d.r.pm[i] = np;
+        d.r.vh[i].w = nh;
+        d.vfull[0][i] = st.vx[o]; d.vfull[1][i] = st.vy[o]; d.vfull[2][i] = st.vz[o];
+    }
+    if (PARTS & 2) {
+        d.ufull[i] = st.u[o];
+        d.Sfull[0][i] = st.Sxx[o]; d.Sfull[1][i] = st.Syy[o]; d.Sfull[2][i] = st.Sxy[o];
+        d.Sfull[3][i] = st.Sxz[o]; d.Sfull[4][i] = st.Syz[o];
+        d.r.s[PP_G + 0][i] = st.gx ? st.gx[o] : 0.f;
+        d.r.s[PP_G + 1][i] = st.gy ? st.gy[o] : 0.f;
+        d.r.s[PP_G + 2][i] = st.gz ? st.gz[o] : 0.f;
+    }
+}
+
+// sph_step_host, a step that reuses the lists: the second group of host arrays (u, S, a_ext) has been travelling on
+// h2d_stream while the first half of the kick, the list check and the density pass ran; take it in and kick u and S
+static int take_second_group(sph_ctx *c)
+{
+    sph_state *ds = c->host_in;
+    c->host_in = nullptr;
+    SPH_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_second, 0));
+    k_refresh<2><<<sph_div_up(c->d.n, 256), 256, 0, c->stream>>>(c->d, *ds);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return sph_launch_kick_drift(c, 0.f, 2);
 }
 
 extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, float *dt_used)
@@ -667,34 +698,55 @@ extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, f
                             hs->Sxx, hs->Syy, hs->Sxy, hs->Sxz, hs->Syz, hs->gx, hs->gy, hs->gz};
     sph_state ds;
     memset(&ds, 0, sizeof(ds));
-    for (int k = 0; k < 17; ++k) {
-        if (n > 0 && src[k])
-            SPH_CUDA(c, cudaMemcpyAsync(dev[k], src[k], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    // first group: what the first half of the kick, the list check and the density pass need (x, y, z, m, h, v);
+    // second group (u, S, a_ext) on its own stream behind it when the particles are resident already
+    const bool split = c->resident && n > 0;
+    for (int k = 0; k < 8; ++k)
+        if (n > 0) SPH_CUDA(c, cudaMemcpyAsync(dev[k], src[k], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    cudaStream_t s2 = c->stream;
+    if (split) {
+        SPH_CUDA(c, cudaEventRecord(c->ev_first, c->stream));
+        SPH_CUDA(c, cudaStreamWaitEvent(c->h2d_stream, c->ev_first, 0));
+        s2 = c->h2d_stream;
     }
+    for (int k = 8; k < 17; ++k)
+        if (n > 0 && src[k]) SPH_CUDA(c, cudaMemcpyAsync(dev[k], src[k], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, s2));
+    if (split) SPH_CUDA(c, cudaEventRecord(c->ev_second, c->h2d_stream));
     ds.x = dev[0]; ds.y = dev[1]; ds.z = dev[2]; ds.m = dev[3]; ds.h = dev[4];
     ds.vx = dev[5]; ds.vy = dev[6]; ds.vz = dev[7]; ds.u = dev[8];
     ds.Sxx = dev[9]; ds.Syy = dev[10]; ds.Sxy = dev[11]; ds.Sxz = dev[12]; ds.Syz = dev[13];
     ds.gx = hs->gx ? dev[14] : nullptr; ds.gy = hs->gy ? dev[15] : nullptr; ds.gz = hs->gz ? dev[16] : nullptr;
-    if (n > 0 && hs->mat) {
+    // material and fixed flags are read at the first call only (they stay with the resident particles)
+    if (n > 0 && hs->mat && !c->resident) {
         SPH_CUDA(c, cudaMemcpyAsync(dmat, hs->mat, (size_t)n * sizeof(int), cudaMemcpyHostToDevice, c->stream));
         ds.mat = dmat;
     }
-    if (n > 0 && hs->fixed) {
+    if (n > 0 && hs->fixed && !c->resident) {
         SPH_CUDA(c, cudaMemcpyAsync(dfix, hs->fixed, (size_t)n, cudaMemcpyHostToDevice, c->stream));
         ds.fixed = dfix;
     }
     int rc;
     bool changed = false;
-    if (c->resident && n > 0) {
+    if (split) {
         SPH_CUDA(c, cudaMemsetAsync(c->d.refresh_changed, 0, sizeof(int), c->stream));
-        k_refresh<<<sph_div_up(n, 256), 256, 0, c->stream>>>(c->d, ds);
+        k_refresh<1><<<sph_div_up(n, 256), 256, 0, c->stream>>>(c->d, ds);
         c->launches++;
         SPH_CUDA(c, cudaGetLastError());
         int h_changed = 1;
         SPH_CUDA(c, cudaMemcpyAsync(&h_changed, c->d.refresh_changed, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-        SPH_CUDA(c, cudaStreamSynchronize(c->stream));     // the step cannot start before the copies have landed anyway
+        SPH_CUDA(c, cudaStreamSynchronize(c->stream));     // the step cannot start before these copies have landed anyway
         changed = h_changed != 0;
         if (changed) c->force_full = true;    // the caller moved particles: nothing the lists were built on holds
+        // A step that reuses the lists keeps the particle order, so u and S can be taken in and kicked after the
+        // density pass (take_second_group); a step with a re-sort permutes them, so it waits for them here.
+        if (c->have_derivs && !step_is_full(c)) {
+            c->host_in = &ds;
+        } else {
+            SPH_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_second, 0));
+            k_refresh<2><<<sph_div_up(n, 256), 256, 0, c->stream>>>(c->d, ds);
+            c->launches++;
+            SPH_CUDA(c, cudaGetLastError());
+        }
     }
     // a step on positions the caller changed builds lists that serve this step only: no skin, no ordering pass.
     // x, y, z go back on the second stream as soon as the drift is done (step_body)
@@ -706,6 +758,7 @@ extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, f
     }
     rc = sph_step(c, &ds, n, dt, nullptr);
     c->host_out = nullptr;
+    c->host_in = nullptr;
     c->no_reuse_now = false;
     if (changed) c->force_full = true;     // those lists have no skin: whatever step comes next must not reuse them
     if (rc) return rc;

@@ -190,6 +190,11 @@ struct sph_ctx {
     float *stage;
     cudaStream_t copy_stream;
     cudaEvent_t ev_pos, ev_copied;
+    // sph_step_host on a step that reuses the lists: u, S and a_ext travel on h2d_stream behind x, m, h, v and are taken
+    // into the resident arrays (k_refresh<2>, second half of the kick) after the density pass
+    cudaStream_t h2d_stream;
+    cudaEvent_t ev_first, ev_second;     // the first group of copies is issued / the second group has landed
+    sph_state *host_in;                  // != NULL: the staging arrays whose second group is still to be taken in
     sph_state *host_out;     // != NULL inside sph_step_host: {device staging arrays}; host_dst: where x, y, z go on the host
     float *host_dst[3];
     bool no_reuse_now;       // the lists of this build will not be reused (host-buffer steps): no skin, no ordering pass
@@ -218,7 +223,7 @@ int sph_launch_density(sph_ctx *c, bool flagged_only);
 int sph_launch_pair(sph_ctx *c, bool grad, bool force, bool flagged_only);
 int sph_launch_predict(sph_ctx *c);
 int sph_launch_close(sph_ctx *c, int phase, float dt, bool dt_from_device);
-int sph_launch_kick_drift(sph_ctx *c, float dt);
+int sph_launch_kick_drift(sph_ctx *c, float dt, int parts = 3);
 int sph_launch_rung_assign(sph_ctx *c, float dT, int R, const unsigned char *rungs);
 int sph_launch_kick_drift_rung(sph_ctx *c, int n, int R, float dT);
 int sph_launch_mark_need(sph_ctx *c);

@@ -265,37 +265,44 @@ __global__ void k_dt_select(float dt_arg, float *dt_cur, float *dt_next, float *
 // ------------------------------------------------------------------------------------------
 // S7 opening kick (Eq. 42), drift, prediction (Eq. 40); fixed particles keep x and v
 // ------------------------------------------------------------------------------------------
+// PARTS: 1 = x and v, 2 = u and S, 3 = both.  The two halves are independent; sph_step_host runs the second one after
+// the list check and the density pass, while u, S and a_ext are still on their way from the host.
+template <int PARTS>
 __global__ void __launch_bounds__(256) k_kick_drift(Dev d, DevParams p)
 {
     long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (i >= d.n) return;
     const float dt = *d.dt_cur, hdt = 0.5f * dt;
-    unsigned mf = ((const unsigned *)d.r.s[PP_MATFIX])[i];
-    const bool fixed = (mf >> 8) & 1u;
-    float4 pm = d.r.pm[i];
-    float h = d.r.vh[i].w;
-    float v[3] = {d.vfull[0][i], d.vfull[1][i], d.vfull[2][i]};
-    float a[3] = {d.a[0][i], d.a[1][i], d.a[2][i]};
-    float vh[3], vp[3];
+    if (PARTS & 1) {
+        unsigned mf = ((const unsigned *)d.r.s[PP_MATFIX])[i];
+        const bool fixed = (mf >> 8) & 1u;
+        float4 pm = d.r.pm[i];
+        float h = d.r.vh[i].w;
+        float v[3] = {d.vfull[0][i], d.vfull[1][i], d.vfull[2][i]};
+        float a[3] = {d.a[0][i], d.a[1][i], d.a[2][i]};
+        float vh[3], vp[3];
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-        vh[k] = fixed ? v[k] : fmaf(hdt, a[k], v[k]);
-        vp[k] = fixed ? v[k] : fmaf(hdt, a[k], vh[k]);
-        d.r.s[PP_VHALF + k][i] = vh[k];
+        for (int k = 0; k < 3; ++k) {
+            vh[k] = fixed ? v[k] : fmaf(hdt, a[k], v[k]);
+            vp[k] = fixed ? v[k] : fmaf(hdt, a[k], vh[k]);
+            d.r.s[PP_VHALF + k][i] = vh[k];
+        }
+        if (!fixed) { pm.x = fmaf(dt, vh[0], pm.x); pm.y = fmaf(dt, vh[1], pm.y); pm.z = fmaf(dt, vh[2], pm.z); }
+        d.r.pm[i] = pm;
+        d.r.vh[i] = make_float4(vp[0], vp[1], vp[2], h);
     }
-    if (!fixed) { pm.x = fmaf(dt, vh[0], pm.x); pm.y = fmaf(dt, vh[1], pm.y); pm.z = fmaf(dt, vh[2], pm.z); }
-    d.r.pm[i] = pm;
-    d.r.vh[i] = make_float4(vp[0], vp[1], vp[2], h);
-    float du = d.dudt[i];
-    float uh = fmaf(hdt, du, d.ufull[i]);
-    d.r.s[PP_UHALF][i] = uh;
-    d.r.s[PP_UPRED][i] = fmaf(hdt, du, uh);
+    if (PARTS & 2) {
+        float du = d.dudt[i];
+        float uh = fmaf(hdt, du, d.ufull[i]);
+        d.r.s[PP_UHALF][i] = uh;
+        d.r.s[PP_UPRED][i] = fmaf(hdt, du, uh);
 #pragma unroll
-    for (int c = 0; c < 5; ++c) {
-        float ds = d.dS[c][i];
-        float sh = fmaf(hdt, ds, d.Sfull[c][i]);
-        d.r.s[PP_SHALF + c][i] = sh;
-        d.r.s[PP_SPRED + c][i] = fmaf(hdt, ds, sh);
+        for (int c = 0; c < 5; ++c) {
+            float ds = d.dS[c][i];
+            float sh = fmaf(hdt, ds, d.Sfull[c][i]);
+            d.r.s[PP_SHALF + c][i] = sh;
+            d.r.s[PP_SPRED + c][i] = fmaf(hdt, ds, sh);
+        }
     }
 }
 
@@ -481,13 +488,19 @@ int sph_launch_close(sph_ctx *c, int phase, float dt, bool dt_from_device)
     return SPH_OK;
 }
 
-int sph_launch_kick_drift(sph_ctx *c, float dt)
+// parts: 1 = x and v (selects the time step first), 2 = u and S (with the step already selected), 3 = everything
+int sph_launch_kick_drift(sph_ctx *c, float dt, int parts)
 {
     Dev &d = c->d;
-    k_dt_select<<<1, 1, 0, c->stream>>>(dt, d.dt_cur, d.dt_next, nullptr);
-    c->launches++;
+    if (parts & 1) {
+        k_dt_select<<<1, 1, 0, c->stream>>>(dt, d.dt_cur, d.dt_next, nullptr);
+        c->launches++;
+    }
     if (d.n > 0) {
-        k_kick_drift<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>(d, c->p);
+        const int nb = sph_div_up(d.n, 256);
+        if (parts == 3) k_kick_drift<3><<<nb, 256, 0, c->stream>>>(d, c->p);
+        else if (parts == 1) k_kick_drift<1><<<nb, 256, 0, c->stream>>>(d, c->p);
+        else k_kick_drift<2><<<nb, 256, 0, c->stream>>>(d, c->p);
         c->launches++;
     }
     SPH_CUDA(c, cudaGetLastError());
