@@ -816,7 +816,7 @@ __global__ void __launch_bounds__(SPH_TILE, 4) k_density_l(Dev d, float kappa, R
     const uint2 *lp = d.nlist + ((size_t)(haschunk ? chunk : 0) * d.rows_cap) * 32 + lane;
     const unsigned short *rp = d.rowptr + (size_t)(haschunk ? chunk : 0) * ROWPTR_STRIDE;
     DensAcc A;
-    A.sum = (double)pi.w; A.sh = 3.f * pi.w; A.n = 1;          // self term: q = 0, t = 1
+    A.sum = (double)pi.w; A.sh = 3.0 * (double)pi.w; A.n = 1;          // self term: q = 0, t = 1
     // slot SPH_SE: the far dummy source the padding entries of the lists point at (out of everybody's reach)
     if (threadIdx.x == 0) {
         const float4 fp = *d.far_point;
@@ -841,7 +841,7 @@ __global__ void __launch_bounds__(SPH_TILE, 4) k_density_l(Dev d, float kappa, R
                     const float4 q = *reinterpret_cast<const float4 *>(smem_raw + off);
                     const float r2 = sph_r2(__fsub_rn(pi.x, q.x), __fsub_rn(pi.y, q.y), __fsub_rn(pi.z, q.z));
                     if (r2 < H2i)
-                        density_term(A, r2, q.w, invH, pxd - (double)q.x, pyd - (double)q.y, pzd - (double)q.z,
+                        density_term(A, r2, pxd - (double)q.x, pyd - (double)q.y, pzd - (double)q.z,
                                      sph_widen_pos(q.w), invHd);
                 }
             }

@@ -114,7 +114,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_density(Dev d, float kappa,
     const double pxd = (double)pi.x, pyd = (double)pi.y, pzd = (double)pi.z;
     float4 blo = d.tree.lo[0][chunk], bhi = d.tree.hi[0][chunk];
     DensAcc A;
-    A.sum = 0.0; A.sh = 0.f; A.n = 0;                  // the walk meets the particle itself (r2 = 0)
+    A.sum = 0.0; A.sh = 0.0; A.n = 0;                  // the walk meets the particle itself (r2 = 0)
     unsigned long long tests = 0;
     const unsigned vmask = __ballot_sync(0xffffffffu, valid);
     if (EXACT) {
@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_density(Dev d, float kappa,
             float dx = __fsub_rn(pi.x, q.x), dy = __fsub_rn(pi.y, q.y), dz = __fsub_rn(pi.z, q.z);
             float r2 = sph_r2(dx, dy, dz);
             if (r2 < H2i)
-                density_term(A, r2, q.w, invH, pxd - (double)q.x, pyd - (double)q.y, pzd - (double)q.z, (double)q.w, invHd);
+                density_term(A, r2, pxd - (double)q.x, pyd - (double)q.y, pzd - (double)q.z, (double)q.w, invHd);
         }
         __syncwarp();
     });

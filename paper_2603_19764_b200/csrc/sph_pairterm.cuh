@@ -54,16 +54,16 @@ __device__ __forceinline__ float sph_sqrt(float y)
 // rho/(rho - rho0) ~ 100 on a lattice, and a yielding particle (Y small against rho0 c0^2) passes the error of P
 // on to the rescaled S: BASELINE.json configs[0] needs rho to ~2e-8 for its 1e-4 on the yielded state, which is
 // below what fp32 geometry can give (measured in round 2: fp32 terms with an fp64 accumulator leave 1.4e-7 in rho
-// and 1.02e-4 in S_pred).  The Omega sum (Eq. 3) stays fp32.  r = sqrt(r2) by one Newton step, in fp64, on the
+// and 1.02e-4 in S_pred).  The Omega sum (Eq. 3) uses the same fp64 q and t.  r = sqrt(r2) by one Newton step, in fp64, on the
 // fp32 rsqrt.  ex, ey, ez: x_i - x_j in fp64 (exact: both are fp32 values); md = m_j.
 struct DensAcc {
     double sum;     // sum_j m_j t^4 (1 + 4q)
-    float sh;       // sum_j m_j t^3 (3 + 9q - 32 q^2)
+    double sh;      // sum_j m_j t^3 (3 + 9q - 32 q^2)
     int n;          // |gather set|
 };
 
-__device__ __forceinline__ void density_term(DensAcc &A, float r2, float mj, float invH, double ex, double ey,
-                                             double ez, double md, double invHd);
+__device__ __forceinline__ void density_term(DensAcc &A, float r2, double ex, double ey, double ez, double md,
+                                             double invHd);
 
 // fp32 -> fp64 of a POSITIVE NORMAL float by integer operations (exact): the conversion instruction runs on the XU
 // pipe (16 per clock and SM), which bounds the density kernel; three ALU instructions do not.  Zero becomes 2^-127.
@@ -230,21 +230,21 @@ __device__ __forceinline__ float pair_neg_mu(const PairTarget &t, const PairCons
     return -(hs * vr) * sph_rcp(fmaf(k.eps_h2 * hs, hs, g.r2));
 }
 
-__device__ __forceinline__ void density_term(DensAcc &A, float r2, float mj, float invH, double ex, double ey,
-                                             double ez, double md, double invHd)
+__device__ __forceinline__ void density_term(DensAcc &A, float r2, double ex, double ey, double ez, double md,
+                                             double invHd)
 {
     const float rinv = sph_rsqrt(fmaxf(r2, 1.0e-37f));
-    const float q = (r2 * rinv) * invH;
-    const float t = 1.f - q;        // no clamp: membership says q < 1 up to rounding, and t^3 of a t of -1e-7 is -1e-21
-    A.sh = fmaf(mj * (t * t * t), fmaf(q, fmaf(-32.f, q, 9.f), 3.f), A.sh);
     const double r2d = fma(ex, ex, fma(ey, ey, ez * ez));
     const double yd = sph_widen_pos(rinv), td0 = r2d * yd;
     const double rd = fma(0.5 * td0, fma(-td0, yd, 1.0), td0);
     const double qd = rd * invHd;
     // no clamp at 0: membership (r2 < H_i^2 in fp32) already says q < 1 up to rounding, and (1 - q)^4 of a q that
     // exceeds 1 by 1e-7 is 1e-28
-    const double td = 1.0 - qd, t2 = td * td;
-    A.sum = fma(md * t2 * t2, fma(4.0, qd, 1.0), A.sum);
+    const double td = 1.0 - qd, a = md * (td * td);
+    // both sums from the fp64 q and t: four more fp64 operations instead of nine fp32 ones (the kernel is bound by
+    // instruction issue: configs[4] 10.08 -> 9.91 ms)
+    A.sh = fma(a * td, fma(qd, fma(-32.0, qd, 9.0), 3.0), A.sh);
+    A.sum = fma(a * (td * td), fma(4.0, qd, 1.0), A.sum);
     A.n++;
 }
 
@@ -255,7 +255,7 @@ __device__ __forceinline__ void density_finish(const DensAcc &A, float invH, dou
     rhod = 3.3422538049298023 * invHd * invHd * invHd * A.sum;
     rho = (float)rhod;
     const float kw = SPH_WC2_SIGMA * invH * invH * invH;
-    omega = 1.f - kw * A.sh / (3.f * rho);
+    omega = 1.f - kw * (float)A.sh / (3.f * rho);
 }
 
 // loads the per-target operands (resident arrays of sph_internal.cuh's Dev)
