@@ -125,7 +125,7 @@ struct Dev {
     unsigned char *tile_act, *tile_need;    // NEXT-4: per tile, see RungCtl
     unsigned char *tile_dirty;              // sticky until the next full build
     uint2 *nlist;                           // [chunk][row-group][lane]: 4 x u16 per lane = byte offsets (slot * 16)
-                                            // into the round's staged arrays; 0xFFFF = no entry
+                                            // into the round's staged arrays; SPH_SE << 4 (the dummy slot) = no entry
     int rows_cap;                           // row-groups reserved per chunk
     unsigned short *rowptr;                 // [chunk][SPH_MAXROUND + 1]: first row-group of each round
     unsigned *tile_cycles;                  // SM clock cycles k_cull spent on each tile in the last build
@@ -265,7 +265,7 @@ __device__ __forceinline__ int sph_tile_of_block(const Dev &d, int b)
 }
 
 // Rounds of a tile with ncand candidates: SPH_SE slots each, the last one shorter.  (Measured on configs[4], 1967
-// candidates per tile on average, i.e. 1632 + 335: the 32 lists of a chunk are padded to equal length in every
+// candidates per tile on average, i.e. 1632 + 335 with the 1632 slots of that measurement: the 32 lists of a chunk are padded to equal length in every
 // round, 30 % of the slots the pair passes step through are padding; rounds of EQUAL size, 2 x 984, were tried
 // and are worse, 56 % -- the candidates are in curve order, an even split cuts through every chunk's neighbourhood.)
 __host__ __device__ __forceinline__ int sph_round_count(int ncand) { return (ncand + SPH_SE - 1) / SPH_SE; }

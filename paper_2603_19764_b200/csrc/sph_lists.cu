@@ -21,7 +21,7 @@
 //                     (rowptr); LIST_PAD pads.
 //   k_density_l : stages {x,y,z,m} of the round's candidates in shared memory (coalesced gathers of index
 //                 runs) and walks the lists; the gather set is the subset with r2 < H_i^2, plus self.
-//   k_pair_l    : same with the 17 floats per source of the fused gradient + force pass.
+//   k_pair_l    : same with the 18 floats per source of the fused gradient + force pass.
 //   A tile that exceeds any capacity (tree-walk frontier, candidate pool, rounds, list rows) is FLAGGED
 //   and served by the tree-walk kernels of sph_pair.cu instead: slower, never wrong.
 //
@@ -335,7 +335,7 @@ __global__ void __launch_bounds__(SPH_TILE) k_cull(Dev d, float kappa, float inf
     // split: first the candidates within reach of more than SPH_CULL_LATE chunk boxes, then the "late" ones, which
     // only one of the eight chunks can have as neighbours.  The last round then holds fewer entries for most warps: the
     // 32 lists of a chunk are padded to equal length in every round it has entries in, and on configs[4] (1 967
-    // candidates per tile, 1 632 slots per round) that padding was 30 % of the slots the pair passes step through;
+    // candidates per tile, 1 632 slots per round at the time) that padding was 30 % of the slots the pair passes step through;
     // with the late candidates last it is 14 % (SPH_CULL_LATE = 1; 2: 19 %, 3: 23 %, 4: 26 %), 49.5 -> 45.3 ms per step.
     if (warp == 0) {
         const int totalA = scan_popc(sm.mask, sm.off, nsrc, lane);
@@ -876,12 +876,15 @@ __global__ void __launch_bounds__(SPH_TILE, 4) k_density_l(Dev d, float kappa, R
 
 // ------------------------------------------------------------------------------------------
 // S4 + S5 from the lists.  Equations and operand packing: sph_pairterm.cuh.
-// Shared memory: four float4 arrays and one float array of SPH_SE slots (68 B per candidate; the
-// hydro-only variant stages the first three arrays only).
+// Shared memory: four float4 arrays and one float2 array of SPH_SE + 1 slots (72 B per candidate; the
+// hydro-only variant stages the first three arrays only); slot SPH_SE is the far dummy source of mass 0 that the
+// padding entries of the lists point at.
 // ------------------------------------------------------------------------------------------
 // The candidates are staged with cp.async (measured against loads and stores through registers, round 2: force pass
-// 0.452 -> 0.437 ms on configs[2], 27.9 -> 26.8 ms on configs[4]; 126 -> 102 registers); the staged h is the raw
-// smoothing length, H_j = kappa h_j is formed per list entry.
+// 0.452 -> 0.437 ms on configs[2], 27.9 -> 26.8 ms on configs[4]); the staged h is the raw smoothing length,
+// H_j = kappa h_j is formed per list entry.  The list loop is bound by instruction issue (profiles/r02_v8_pair_diet.md):
+// 112.5 instructions per entry, no test for padding, membership from u = max(1 - r/H_i, 1 - r/H_j) (pair_term).
+
 // One list entry (staged at byte offset off) that may lie inside the band |u| <= SPH_UBAND: if it does, the exact
 // predicate (reading Q4) decides whether it is a neighbour: the count and mu_max of Eq. 39.
 template <bool FORCE>
