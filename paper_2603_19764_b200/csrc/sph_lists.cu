@@ -714,6 +714,21 @@ __device__ __forceinline__ void sort_emit(uint2 *lp, const unsigned short *buf, 
     }
 }
 
+// walk the row-groups [ga, gb) of a lane's column with four loads in flight (these kernels are bound by the latency
+// of the list reads): f(gq, w)
+template <typename F>
+__device__ __forceinline__ void for_rows(const uint2 *lp, int ga, int gb, F f)
+{
+    for (int gq = ga; gq < gb; gq += 4) {
+        uint2 w[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) w[j] = gq + j < gb ? lp[(size_t)(gq + j) * 32] : make_uint2(LIST_PAD2, LIST_PAD2);
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (gq + j < gb) f(gq + j, w[j]);
+    }
+}
+
 // the entries of one round of a lane's list, row-groups [g0, ge), ordered by bank class (all lanes of a warp together);
 // a round with a lane over SORT_CAP entries stays as it is
 __device__ __forceinline__ void sort_round(uint2 *lp, unsigned short *buf, int g0, int ge, int lane)
@@ -722,20 +737,18 @@ __device__ __forceinline__ void sort_round(uint2 *lp, unsigned short *buf, int g
     // pass 1: class counts
     unsigned long long cnt = 0ull;
     int N = 0;
-    for (int gq = g0; gq < ge; ++gq) {
-        const uint2 w = lp[(size_t)gq * 32];
+    for_rows(lp, g0, ge, [&](int, uint2 w) {
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             const unsigned off = list_entry(w, e);
             if (off != LIST_PAD) { cnt += 1ull << (((off >> 4) & 7u) << 3); ++N; }
         }
-    }
+    });
     if (__any_sync(FULL, N > SORT_CAP)) return;
     const unsigned long long base = cnt * 0x0101010101010100ull;     // field c = entries of the classes below c
     // pass 2: bucket by class
     unsigned long long cur = base;
-    for (int gq = g0; gq < ge; ++gq) {
-        const uint2 w = lp[(size_t)gq * 32];
+    for_rows(lp, g0, ge, [&](int, uint2 w) {
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
             const unsigned off = list_entry(w, e);
@@ -745,7 +758,7 @@ __device__ __forceinline__ void sort_round(uint2 *lp, unsigned short *buf, int g
                 cur += 1ull << c8;
             }
         }
-    }
+    });
     sort_emit(lp, buf, base, cur, N, g0, ge - g0, lane);
 }
 
@@ -784,8 +797,7 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_list_compact_sort(Dev d)
         if (haschunk) {
             g1 = rp[1];
             g2 = nround > 1 ? (int)rp[2] : g1;
-            for (int gq = 0; gq < g2; ++gq) {
-                const uint2 w = lp[(size_t)gq * 32];
+            for_rows(lp, 0, g2, [&](int gq, uint2 w) {
                 const unsigned kb = gq < g1 ? 0u : (unsigned)SPH_SE;
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
@@ -795,7 +807,7 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_list_compact_sort(Dev d)
                         atomicOr(&bits[k >> 5], 1u << (k & 31u));
                     }
                 }
-            }
+            });
             const long long i = (long long)tile * SPH_TILE + threadIdx.x;
             const int tot = __reduce_max_sync(FULL, i < d.n ? d.nlen[i] : 0);
             ok = (2 * g2 - g1 <= d.rows_cap && tot <= SORT_CAP) ? 1 : 0;
@@ -843,8 +855,7 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_list_compact_sort(Dev d)
         // entries of both old rounds together: the new first round in [0, N0) of the buffer, the second in [N0, N0 + N1)
         unsigned long long cnt0 = 0ull, cnt1 = 0ull;
         int N0 = 0, N1 = 0;
-        for (int gq = 0; gq < g2; ++gq) {
-            const uint2 w = lp[(size_t)gq * 32];
+        for_rows(lp, 0, g2, [&](int gq, uint2 w) {
             const unsigned kb = gq < g1 ? 0u : (unsigned)SPH_SE;
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
@@ -855,12 +866,11 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_list_compact_sort(Dev d)
                     else { cnt1 += 1ull << (((ns - SPH_SE) & 7u) << 3); ++N1; }
                 }
             }
-        }
+        });
         const unsigned long long base0 = cnt0 * 0x0101010101010100ull;
         const unsigned long long base1 = cnt1 * 0x0101010101010100ull + (unsigned long long)N0 * 0x0101010101010101ull;
         unsigned long long cur0 = base0, cur1 = base1;
-        for (int gq = 0; gq < g2; ++gq) {
-            const uint2 w = lp[(size_t)gq * 32];
+        for_rows(lp, 0, g2, [&](int gq, uint2 w) {
             const unsigned kb = gq < g1 ? 0u : (unsigned)SPH_SE;
 #pragma unroll
             for (int e = 0; e < 4; ++e) {
@@ -878,7 +888,7 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_list_compact_sort(Dev d)
                     }
                 }
             }
-        }
+        });
         const int R0 = __reduce_max_sync(FULL, (N0 + 3) >> 2), R1 = __reduce_max_sync(FULL, (N1 + 3) >> 2);
         sort_emit(lp, buf, base0, cur0, N0, 0, R0, lane);
         sort_emit(lp, buf, base1, cur1, N1, R0, R1, lane);
