@@ -714,17 +714,21 @@ __device__ __forceinline__ void sort_emit(uint2 *lp, const unsigned short *buf, 
     }
 }
 
-// walk the row-groups [ga, gb) of a lane's column with four loads in flight (these kernels are bound by the latency
-// of the list reads): f(gq, w)
+// walk the row-groups [ga, gb) of a lane's column with SORT_INFLIGHT loads in flight (these kernels are bound by the
+// latency of the list reads): f(gq, w)
+#ifndef SORT_INFLIGHT
+#define SORT_INFLIGHT 8
+#endif
 template <typename F>
 __device__ __forceinline__ void for_rows(const uint2 *lp, int ga, int gb, F f)
 {
-    for (int gq = ga; gq < gb; gq += 4) {
-        uint2 w[4];
+    for (int gq = ga; gq < gb; gq += SORT_INFLIGHT) {
+        uint2 w[SORT_INFLIGHT];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) w[j] = gq + j < gb ? lp[(size_t)(gq + j) * 32] : make_uint2(LIST_PAD2, LIST_PAD2);
+        for (int j = 0; j < SORT_INFLIGHT; ++j)
+            w[j] = gq + j < gb ? lp[(size_t)(gq + j) * 32] : make_uint2(LIST_PAD2, LIST_PAD2);
 #pragma unroll
-        for (int j = 0; j < 4; ++j)
+        for (int j = 0; j < SORT_INFLIGHT; ++j)
             if (gq + j < gb) f(gq + j, w[j]);
     }
 }
