@@ -482,8 +482,8 @@ def run_ours(args):
         "e2e": {"value": e2e_value, "unit": "pairs/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "ms_per_step": 1e3 * e2e_s_max / e2e_steps,
                 "note": "host buffers in and out every step; the loop hands back the state it received, so the library "
-                        "finds x, y, z, h unchanged and keeps reusing its neighbour lists; on such steps u, S and a_ext "
-                        "arrive while the list check and the density pass run, and x, y, z leave during the pair pass"},
+                        "finds x, y, z, h unchanged and keeps reusing its neighbour lists; on such steps u and S arrive while "
+                        "the list check and the density pass run, a_ext and the outgoing x, y, z travel during the pair pass"},
         "roofline": roofline,
         "cpu_baseline": cpu,
         "hydro_only": hydro,

@@ -258,8 +258,9 @@ int sph_step_rungs(sph_ctx *ctx, float dT, int max_rung, const unsigned char *ru
  * If the caller's x, y, z, h equal the resident ones bit for bit (a loop that hands back what it was given) the
  * neighbour lists stay in use as in sph_step; if anything moved, the step starts from a full neighbour build.
  * mat and fixed are read at the FIRST call only (they stay with the resident particles).  Copies overlap the step
- * where the data flow allows: on a step that reuses the lists u, S and a_ext arrive on a second stream while the
- * first half of the kick, the list check and the density pass run; x, y, z leave during the pair pass.  All host
+ * where the data flow allows: on a step that reuses the lists u and S arrive on a second stream while the first half
+ * of the kick, the list check and the density pass run, a_ext while the pair pass runs (CLOSE adds it then, with
+ * the same single rounding); x, y, z leave during the pair pass.  All host
  * arrays should be pinned (pageable memory works, without the overlap) and must not be touched during the call. */
 int sph_step_host(sph_ctx *ctx, sph_state *host_state, long long n, float dt, float *dt_used);
 

@@ -172,7 +172,7 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
     memset(c, 0, sizeof(*c));
     c->p.kappa = params->kappa; c->p.alpha = params->alpha; c->p.beta = params->beta;
     c->p.eps_av = params->eps_av; c->p.eta_C = params->eta_C; c->p.eta_a = params->eta_a;
-    c->p.flags = params->flags; c->p.n_materials = params->n_materials;
+    c->p.flags = params->flags & ~SPH_INT_DEFER_AEXT; c->p.n_materials = params->n_materials;
     memcpy(c->p.mat, params->mat, sizeof(params->mat));
     c->stream = (cudaStream_t)cuda_stream;
     c->use_lists = !(params->flags & SPH_NO_LISTS);
@@ -198,7 +198,8 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
         || cudaEventCreateWithFlags(&c->ev_copied, cudaEventDisableTiming) != cudaSuccess
         || cudaStreamCreateWithFlags(&c->h2d_stream, cudaStreamNonBlocking) != cudaSuccess
         || cudaEventCreateWithFlags(&c->ev_first, cudaEventDisableTiming) != cudaSuccess
-        || cudaEventCreateWithFlags(&c->ev_second, cudaEventDisableTiming) != cudaSuccess) {
+        || cudaEventCreateWithFlags(&c->ev_second, cudaEventDisableTiming) != cudaSuccess
+        || cudaEventCreateWithFlags(&c->ev_third, cudaEventDisableTiming) != cudaSuccess) {
         sph_destroy(c);
         return SPH_ECUDA;
     }
@@ -235,6 +236,7 @@ extern "C" void sph_destroy(sph_ctx *c)
     if (c->ev_copied) cudaEventDestroy(c->ev_copied);
     if (c->ev_first) cudaEventDestroy(c->ev_first);
     if (c->ev_second) cudaEventDestroy(c->ev_second);
+    if (c->ev_third) cudaEventDestroy(c->ev_third);
     if (c->h2d_stream) cudaStreamDestroy(c->h2d_stream);
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     delete c;
@@ -393,10 +395,16 @@ extern "C" int sph_gradients_forces(sph_ctx *c)
     return SPH_OK;
 }
 
+static int take_third_group(sph_ctx *c);
+
 static int do_close(sph_ctx *c, int phase, float dt, bool dt_from_device)
 {
     const bool strength = (c->p.flags & SPH_STRENGTH) != 0;
     if (!c->have_force || (strength && !c->have_grad)) return SPH_EORDER;
+    if (c->host_in_g) {               // sph_step_host: a_ext has landed by now; this CLOSE adds it (SPH_INT_DEFER_AEXT)
+        int rc = take_third_group(c);
+        if (rc) return rc;
+    }
     PassTimer t(c, SPH_T_CLOSE);
     int rc = sph_launch_close(c, phase, dt, dt_from_device);
     if (rc) return rc;
@@ -645,7 +653,7 @@ extern "C" int sph_step_rungs(sph_ctx *c, float dT, int max_rung, const unsigned
 // depend on -- x, y, z, h -- is compared with the resident values first: a caller that hands back the state it was
 // given (the usual host-buffer loop) leaves them bit for bit, and the lists (with their skin and their validity
 // check) stay in use; any difference sets the flag and the step starts from a full build.
-// PARTS: 1 = x, y, z, m, h, v (and the test whether the caller moved anything), 2 = u, S, a_ext, 3 = both
+// PARTS: 1 = x, y, z, m, h, v (and the test whether the caller moved anything), 2 = u, S, 4 = a_ext
 template <int PARTS>
 __global__ void __launch_bounds__(256) k_refresh(Dev d, sph_state st)
 {
@@ -664,14 +672,17 @@ __global__ void __launch_bounds__(256) k_refresh(Dev d, sph_state st)
         d.ufull[i] = st.u[o];
         d.Sfull[0][i] = st.Sxx[o]; d.Sfull[1][i] = st.Syy[o]; d.Sfull[2][i] = st.Sxy[o];
         d.Sfull[3][i] = st.Sxz[o]; d.Sfull[4][i] = st.Syz[o];
+    }
+    if (PARTS & 4) {
         d.r.s[PP_G + 0][i] = st.gx ? st.gx[o] : 0.f;
         d.r.s[PP_G + 1][i] = st.gy ? st.gy[o] : 0.f;
         d.r.s[PP_G + 2][i] = st.gz ? st.gz[o] : 0.f;
     }
 }
 
-// sph_step_host, a step that reuses the lists: the second group of host arrays (u, S, a_ext) has been travelling on
-// h2d_stream while the first half of the kick, the list check and the density pass ran; take it in and kick u and S
+// sph_step_host, a step that reuses the lists: the second group of host arrays (u, S) has been travelling on
+// h2d_stream while the first half of the kick, the list check and the density pass ran; take it in and kick u and S.
+// The third group (a_ext) is still on its way: the pair pass leaves it out and CLOSE adds it (take_third_group).
 static int take_second_group(sph_ctx *c)
 {
     sph_state *ds = c->host_in;
@@ -680,7 +691,20 @@ static int take_second_group(sph_ctx *c)
     k_refresh<2><<<sph_div_up(c->d.n, 256), 256, 0, c->stream>>>(c->d, *ds);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
+    c->host_in_g = ds;
+    c->p.flags |= SPH_INT_DEFER_AEXT;
     return sph_launch_kick_drift(c, 0.f, 2);
+}
+
+static int take_third_group(sph_ctx *c)
+{
+    sph_state *ds = c->host_in_g;
+    c->host_in_g = nullptr;
+    SPH_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_third, 0));
+    k_refresh<4><<<sph_div_up(c->d.n, 256), 256, 0, c->stream>>>(c->d, *ds);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
 }
 
 extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, float *dt_used)
@@ -709,9 +733,12 @@ extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, f
         SPH_CUDA(c, cudaStreamWaitEvent(c->h2d_stream, c->ev_first, 0));
         s2 = c->h2d_stream;
     }
-    for (int k = 8; k < 17; ++k)
+    for (int k = 8; k < 14; ++k)
         if (n > 0 && src[k]) SPH_CUDA(c, cudaMemcpyAsync(dev[k], src[k], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, s2));
     if (split) SPH_CUDA(c, cudaEventRecord(c->ev_second, c->h2d_stream));
+    for (int k = 14; k < 17; ++k)
+        if (n > 0 && src[k]) SPH_CUDA(c, cudaMemcpyAsync(dev[k], src[k], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, s2));
+    if (split) SPH_CUDA(c, cudaEventRecord(c->ev_third, c->h2d_stream));
     ds.x = dev[0]; ds.y = dev[1]; ds.z = dev[2]; ds.m = dev[3]; ds.h = dev[4];
     ds.vx = dev[5]; ds.vy = dev[6]; ds.vz = dev[7]; ds.u = dev[8];
     ds.Sxx = dev[9]; ds.Syy = dev[10]; ds.Sxy = dev[11]; ds.Sxz = dev[12]; ds.Syz = dev[13];
@@ -742,8 +769,8 @@ extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, f
         if (c->have_derivs && !step_is_full(c)) {
             c->host_in = &ds;
         } else {
-            SPH_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_second, 0));
-            k_refresh<2><<<sph_div_up(n, 256), 256, 0, c->stream>>>(c->d, ds);
+            SPH_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_third, 0));
+            k_refresh<6><<<sph_div_up(n, 256), 256, 0, c->stream>>>(c->d, ds);
             c->launches++;
             SPH_CUDA(c, cudaGetLastError());
         }
@@ -759,6 +786,8 @@ extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, f
     rc = sph_step(c, &ds, n, dt, nullptr);
     c->host_out = nullptr;
     c->host_in = nullptr;
+    c->host_in_g = nullptr;
+    c->p.flags &= ~SPH_INT_DEFER_AEXT;
     c->no_reuse_now = false;
     if (changed) c->force_full = true;     // those lists have no skin: whatever step comes next must not reuse them
     if (rc) return rc;

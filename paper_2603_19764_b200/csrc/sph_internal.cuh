@@ -12,6 +12,10 @@
 #define SPH_MAX_LEVELS 7      // 32^6 chunks * 32 particles >> any n that fits in HBM
 #define SPH_NPP 21            // scalar (4-byte) resident arrays that are permuted at re-sort
 
+// internal bit of DevParams.flags (never set by callers: sph_init masks it): the pair pass leaves a_ext out and CLOSE adds
+// it -- sph_step_host on a step whose a_ext is still on its way from the host while the pair pass runs
+#define SPH_INT_DEFER_AEXT 0x80000000u
+
 // neighbour-list machinery (sph_lists.cu)
 #define SPH_TILE_CHUNKS 8     // chunks per tile = warps per CTA of the list kernels
 #define SPH_TILE (SPH_TILE_CHUNKS * SPH_CHUNK)
@@ -195,6 +199,8 @@ struct sph_ctx {
     cudaStream_t h2d_stream;
     cudaEvent_t ev_first, ev_second;     // the first group of copies is issued / the second group has landed
     sph_state *host_in;                  // != NULL: the staging arrays whose second group is still to be taken in
+    cudaEvent_t ev_third;                // a_ext has landed (third group: taken in before CLOSE, SPH_INT_DEFER_AEXT)
+    sph_state *host_in_g;                // != NULL: a_ext is still to be taken in
     sph_state *host_out;     // != NULL inside sph_step_host: {device staging arrays}; host_dst: where x, y, z go on the host
     float *host_dst[3];
     bool no_reuse_now;       // the lists of this build will not be reused (host-buffer steps): no skin, no ordering pass

@@ -1193,7 +1193,7 @@ __global__ void __launch_bounds__(SPH_TILE, 2) k_pair_l(Dev d, DevParams p, Rung
 
     const bool keep = valid && sph_active(rc, i);          // NEXT-4: an inactive particle keeps its old derivatives
     if (keep) {
-        pair_store<GRAD, FORCE>(d, i, A, kc);
+        pair_store<GRAD, FORCE>(d, i, A, kc, !(p.flags & SPH_INT_DEFER_AEXT));
         d.nsym[i] = cnt;
     }
     if (FORCE) {

@@ -229,7 +229,7 @@ __global__ void __launch_bounds__(PAIR_WARPS * 32) k_pair(Dev d, DevParams p, co
 
     const bool keep = valid && sph_active(rc, i);          // NEXT-4: an inactive particle keeps its old derivatives
     if (keep) {
-        pair_store<GRAD, FORCE>(d, i, A, kc);
+        pair_store<GRAD, FORCE>(d, i, A, kc, !(p.flags & SPH_INT_DEFER_AEXT));
         d.nsym[i] = cnt_i;
     }
     if (FORCE) {

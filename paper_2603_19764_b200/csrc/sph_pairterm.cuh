@@ -277,8 +277,9 @@ __device__ __forceinline__ PairTarget pair_target_load(const Dev &d, long long i
     return t;
 }
 
+// add_aext == false: a_ext is added by CLOSE instead (SPH_INT_DEFER_AEXT)
 template <bool GRAD, bool FORCE>
-__device__ __forceinline__ void pair_store(const Dev &d, long long i, const PairAcc &A, const PairConst &k)
+__device__ __forceinline__ void pair_store(const Dev &d, long long i, const PairAcc &A, const PairConst &k, bool add_aext)
 {
     if (GRAD) {
 #pragma unroll
@@ -290,9 +291,11 @@ __device__ __forceinline__ void pair_store(const Dev &d, long long i, const Pair
         d.Cinv[6][i] = c2; d.Cinv[7][i] = c4; d.Cinv[8][i] = c5;
     }
     if (FORCE) {
-        d.a[0][i] = A.ax + d.r.s[PP_G + 0][i];
-        d.a[1][i] = A.ay + d.r.s[PP_G + 1][i];
-        d.a[2][i] = A.az + d.r.s[PP_G + 2][i];
+        float gx = 0.f, gy = 0.f, gz = 0.f;
+        if (add_aext) { gx = d.r.s[PP_G + 0][i]; gy = d.r.s[PP_G + 1][i]; gz = d.r.s[PP_G + 2][i]; }
+        d.a[0][i] = A.ax + gx;
+        d.a[1][i] = A.ay + gy;
+        d.a[2][i] = A.az + gz;
         d.dudt[i] = fmaf(-0.5f, A.duv, A.du);
         d.mumax[i] = k.hk * A.mumax;
     }

@@ -184,6 +184,10 @@ __global__ void __launch_bounds__(256, 6) k_close(Dev d, DevParams p, int phase,
     // time-step limit, Eq. 39 (and Eq. 38 with epsilon = h when eta_a > 0)
     float h = d.r.vh[i].w;
     float ax = d.a[0][i], ay = d.a[1][i], az = d.a[2][i];
+    if (p.flags & SPH_INT_DEFER_AEXT) {               // the pair pass left a_ext out (sph_step_host): a = a_int + a_ext
+        ax += d.r.s[PP_G + 0][i]; ay += d.r.s[PP_G + 1][i]; az += d.r.s[PP_G + 2][i];
+        d.a[0][i] = ax; d.a[1][i] = ay; d.a[2][i] = az;
+    }
     dti = p.eta_C * h / ((1.f + 0.6f * p.alpha) * d.cs[i] + 0.6f * p.beta * d.mumax[i]);
     if (p.eta_a > 0.f) {
         float an = sqrtf(ax * ax + ay * ay + az * az);

@@ -432,6 +432,10 @@ def test_host_buffer_loop_reuses_lists_and_notices_moved_particles():
     wl = W.elastic_block(12, h_spread=0.2)
     wl.params.skin = 0.06
     wl.params.rebuild_every = 4
+    # an external acceleration that matters: on the steps that reuse the lists it reaches the device while the pair pass
+    # runs and is added by CLOSE instead (one rounding either way: the states must still agree bit for bit)
+    wl.arrays["gy"] = (-2.0e6 * (1.0 + 5.0 * wl.arrays["x"])).astype(np.float32)
+    wl.arrays["gx"] = (1.0e6 * np.sin(40.0 * wl.arrays["z"])).astype(np.float32)
 
     def pinned():
         h = {k: torch.from_numpy(v.copy()).pin_memory() for k, v in wl.arrays.items()}
