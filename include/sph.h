@@ -292,6 +292,29 @@ int sph_set_eos_table(sph_ctx *ctx, int material, const sph_eos_table *table);
  * in a fixed order (bitwise repeatable).  Asynchronous.  Errors: EINVAL, EORDER. */
 int sph_get_diagnostics(sph_ctx *ctx, double *out);
 
+/* The same eight sums for callers that cannot allocate device memory -- no context, no workspace.
+ * Meant for two kinds of caller: a host code that gave the whole GPU to its own particle pool at start-up, so
+ * that any later cudaMalloc (the workspace sph_init wants) fails; and a time-step loop that cannot afford the
+ * device-wide synchronisation that cudaMalloc / cudaFree bring.  This call allocates nothing: the per-block
+ * partial sums sit in a static __device__ array inside libsph.so (512 KiB; every GPU that loads the library's
+ * kernels holds it until the process exits).  That fixes the limit: n <= SPH_DIAG_NOALLOC_MAX_N.
+ *   state: HOST struct; its x, y, z, m, vx, vy, vz, u are DEVICE float[n] (the other members are not read), in any
+ *          order -- this is the caller's state as it stands, not the resident one.
+ *   out:   DEVICE double[8] = { sum m, sum m v (3), sum m x cross v (3), sum m (v.v/2 + u) },
+ *          fp64, summed in a fixed order that depends on n only: repeatable bit for bit, and equal to
+ *          sph_get_diagnostics of the same state up to the rounding of a different order (1e-12 relative).
+ *   cuda_stream: a cudaStream_t (NULL = default stream); asynchronous on it.  n = 0 writes zeros.
+ *   cuda_error: HOST int receiving the cudaError_t when SPH_ECUDA is returned, or NULL.
+ * The first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device
+ * current); make that first call outside any stream capture.  All calls on a device share the one array, which
+ * keeps the last call's partial sums; a call reads only rows it has just written, so nothing needs clearing.
+ * Calls that can overlap on the GPU (two streams of one device) race on it and give undefined sums: keep them on
+ * one stream or order them with events.  Different devices do not interfere.
+ * Errors: EINVAL (NULL state / out / a needed array, n < 0), ECAPACITY (n > SPH_DIAG_NOALLOC_MAX_N; nothing is
+ * launched), ECUDA. */
+#define SPH_DIAG_NOALLOC_MAX_N 33554432   /* 2^25 particles */
+int sph_diagnostics_noalloc(const sph_state *state, long long n, double *out, void *cuda_stream, int *cuda_error);
+
 /* HOST outputs.  Both synchronise the stream. */
 int sph_get_timings(sph_ctx *ctx, float *ms, int n);            /* SPH_T_* slots              */
 int sph_get_counters(sph_ctx *ctx, long long *counters, int n); /* SPH_C_* slots              */

@@ -33,7 +33,8 @@ OPT_FIELDS = ("gx", "gy", "gz")
 # every symbol include/sph.h declares (tests check the library exports all of them)
 SYMBOLS = ("sph_workspace_bytes", "sph_init", "sph_build_neighbors", "sph_density", "sph_strength_update",
            "sph_gradients", "sph_forces", "sph_gradients_forces", "sph_fp32_peak", "sph_shared_scatter_rate", "sph_step_rungs", "sph_adapt_h", "sph_set_eos_table", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
-           "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_get_diagnostics", "sph_launch_count",
+           "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_get_diagnostics",
+           "sph_diagnostics_noalloc", "sph_launch_count",
            "sph_last_cuda_error", "sph_strerror", "sph_destroy")
 
 
@@ -130,6 +131,8 @@ def load():
     lib.sph_set_eos_table.restype = i
     lib.sph_get_diagnostics.argtypes = [vp, vp]
     lib.sph_get_diagnostics.restype = i
+    lib.sph_diagnostics_noalloc.argtypes = [C.POINTER(sph_state), ll, vp, vp, C.POINTER(i)]
+    lib.sph_diagnostics_noalloc.restype = i
     lib.sph_adapt_h.argtypes = [vp, fl, i, vp]
     lib.sph_adapt_h.restype = i
     lib.sph_launch_count.restype = ll
@@ -168,6 +171,33 @@ def make_params(p) -> sph_params:
 
 def _ptr(t) -> Optional[int]:
     return None if t is None else int(t.data_ptr())
+
+
+DIAG_NOALLOC_MAX_N = 1 << 25       # SPH_DIAG_NOALLOC_MAX_N of include/sph.h
+
+
+def diagnostics_noalloc(tensors: Dict[str, object], n: int, out, stream=None):
+    """sph_diagnostics_noalloc: the eight S8 sums (M, P, L, E) of the caller's own device arrays, written to `out`
+    (float64 device tensor [8], supplied by the caller).  For programs that cannot allocate on the GPU -- all of
+    its memory already belongs to their own pool, or an allocation's device-wide synchronisation would stall their
+    loop: neither the library nor this wrapper allocates anything; the partial sums live in a static array inside
+    libsph.so, which limits n to DIAG_NOALLOC_MAX_N.  tensors: x, y, z, m, vx, vy, vz, u (float32, on out's
+    device, which must be the current one).  Calls on different streams of one device must not overlap."""
+    import torch
+    lib = load()
+    st = sph_state()
+    for k in ("x", "y", "z", "m", "vx", "vy", "vz", "u"):
+        setattr(st, k, _ptr(tensors.get(k)))
+    if stream is None:
+        stream = torch.cuda.current_stream(out.device)
+    err = C.c_int(0)
+    rc = lib.sph_diagnostics_noalloc(C.byref(st), int(n), _ptr(out), stream.cuda_stream, C.byref(err))
+    if rc == ECAPACITY:
+        raise SphError(rc, "sph_diagnostics_noalloc", f"n = {n} is more than the static scratch array holds "
+                                                      f"(SPH_DIAG_NOALLOC_MAX_N = {DIAG_NOALLOC_MAX_N})")
+    if rc != 0:
+        raise SphError(rc, "sph_diagnostics_noalloc", lib.sph_strerror(rc).decode() + (f" cudaError={err.value}" if rc == ECUDA else ""))
+    return out
 
 
 class Sph:
