@@ -276,18 +276,17 @@ def run_ours(args):
     barrier()
     for k in range(args.steps):
         flush.fill_(k & 0xff)
-        # the library's schedule (sph_internal: step_is_full): the step after a full build is number 1 of `every`
-        is_full = (not reuse) or ((args.warmup + k + 1) % every == 0)
         ev[k][0].record(s.stream)
         s.step(None, 0, 0.0)
         ev[k][1].record(s.stream)
         tm = s.get_timings()                 # synchronises; outside the event pair of the next step
+        c = s.get_counters()
+        is_full = c["steps_since_full"] == 0         # what the library did, not a prediction of its schedule
         for q in B.T_SLOTS:
             pass_ms[q] += tm[q]
             (pass_full if is_full else pass_reuse)[q] += tm[q]
         n_full += 1 if is_full else 0
         n_reuse += 0 if is_full else 1
-        c = s.get_counters()
         pairs_g += c["pairs_gather"]; pairs_s += c["pairs_symmetric"]
         entries += c["tests_density"] + c["tests_force"]
         if is_full:
@@ -463,6 +462,8 @@ def run_ours(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
         "config": {"workload": wl.name, "n_particles": n, "strength": strength,
+                   # reading Q1: which rotation sign of Eq. 13 was timed (the cost is the same)
+                   "jaumann": "as_printed" if (wl.params.flags & B.JAUMANN_AS_PRINTED) else "objective",
                    "mean_neighbours": pairs_s / args.steps / max(n, 1),
                    "pair_count": "value = gather pairs (Eq. 1, 3; the particle itself included: the self term is evaluated) "
                                  "+ symmetric pairs (Eq. 18-21; self excluded) per second",

@@ -32,9 +32,11 @@ extern "C" {
 #define SPH_STRENGTH              1u  /* evolve S, add the S terms of Eq. 18-19      */
 #define SPH_CORRECTION_TENSOR     2u  /* G = F.C (Eq. 22); off: C = 1      */
 #define SPH_PCLIP_GLOBAL          4u  /* clip P >= 0 in the EOS too, not only in Eq. 34 (reading Q8)    */
-#define SPH_JAUMANN_AS_PRINTED    8u  /* rotation terms of Eq. 13 with the index order AS PRINTED, S.R - R.S,
+#define SPH_JAUMANN_AS_PRINTED  512u  /* rotation terms of Eq. 13 with the index order AS PRINTED, S.R - R.S,
                                          instead of the objective (co-rotational) Jaumann rate R.S - S.R that
                                          is the default (reading Q1: the print contradicts "objective")     */
+/* Retired bits: 8 (once SPH_JAUMANN_COROTATIONAL, the opposite choice under the opposite default), 128, 256.  sph_init and
+ * sph_workspace_bytes refuse them, and any other bit not listed here, with SPH_EINVAL / 0 instead of ignoring them. */
 #define SPH_NO_LISTS             16u  /* pair passes walk the chunk tree themselves instead of reading
                                          the per-particle neighbour lists (the round-1 "v0" kernels: A/B
                                          measurement; they also serve tiles over a list capacity)           */
@@ -120,6 +122,13 @@ enum { SPH_C_PAIRS_GATHER = 0,   /* sum_i |gather set(i)|   (true pairs of the d
                                     sph_get_neighbors(SPH_SYMMETRIC): the share a tile could evaluate once)     */
        SPH_C_LIST_SLOTS,         /* list slots the pair passes step through per launch: entries plus the padding
                                     that makes the 32 lists of a chunk equally long in every round (last build) */
+       SPH_C_RUNG_CLAMPED,       /* sph_step_rungs with rungs from the limits: rung choices (at the start of the big
+                                    step and at every closing kick) that put a particle on max_rung although its limit
+                                    (Eq. 38-39) is below dT / 2^max_rung, or is not a number: such a particle is stepped
+                                    beyond its limit; raise max_rung or lower dT if this is not 0                     */
+       SPH_C_STEPS_SINCE_FULL,   /* steps taken on the lists of the last full neighbour build: 0 right after a call that
+                                    did a full build (re-sort + lists), k after the k-th step that reused them (kept
+                                    on the host; the way to tell which kind of step the last sph_step was)            */
        SPH_C_COUNT };
 
 typedef struct sph_ctx sph_ctx;   /* opaque, library-owned (host memory) */
@@ -242,7 +251,7 @@ int sph_step(sph_ctx *ctx, sph_state *state, long long n, float dt, float *dt_us
 /* NEXT-4 ("hierarchical individual timestep scheme"; reading Q23 in DESIGN.md): ONE BIG
  * STEP dT of the resident particles on power-of-two rungs.  dT is split into 2^max_rung substeps; a particle on rung r
  * takes steps dT / 2^r, r the smallest rung whose step is within the particle's limit (Eq. 38-39) from its last
- * CLOSE.  Per substep: opening kick of the particles that start a step, drift of all, prediction of all to the new
+ * CLOSE -- or max_rung when even dT / 2^max_rung exceeds the limit (counted in SPH_C_RUNG_CLAMPED; nothing else signals it).  Per substep: opening kick of the particles that start a step, drift of all, prediction of all to the new
  * time from their own last derivatives, neighbour lists (reused, checked, rebuilt where dirty), then density and
  * PREDICT for the tiles that hold an active particle or a neighbour of one, the fused pair pass for the tiles that
  * hold an active particle, CLOSE (own step, rescale, next rung) for the active particles only: tiles (256 particles)
@@ -260,7 +269,11 @@ int sph_step_rungs(sph_ctx *ctx, float dT, int max_rung, const unsigned char *ru
  * mat and fixed are read at the FIRST call only (they stay with the resident particles).  Copies overlap the step
  * where the data flow allows: on a step that reuses the lists u and S arrive on a second stream while the first half
  * of the kick, the list check and the density pass run, a_ext while the pair pass runs (CLOSE adds it then, with
- * the same single rounding); x, y, z leave during the pair pass.  All host
+ * the same single rounding); x, y, z leave during the pair pass.  With
+ * sph_params.adapt_h_every > 0 the smoothing lengths the step adapted are written back to host_state->h as well (the
+ * host state stays the resident one, and the lists stay in use between the adaptation steps); otherwise m and h are
+ * only read.  If the call fails part way it waits for every copy it issued before it returns (the host arrays are the
+ * caller's again), and the next step starts from a full build.  All host
  * arrays should be pinned (pageable memory works, without the overlap) and must not be touched during the call. */
 int sph_step_host(sph_ctx *ctx, sph_state *host_state, long long n, float dt, float *dt_used);
 

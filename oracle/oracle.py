@@ -28,7 +28,7 @@ from . import build as _build
 FLAG_STRENGTH = 1
 FLAG_CORRECTION_TENSOR = 2
 FLAG_PCLIP_GLOBAL = 4
-FLAG_JAUMANN_AS_PRINTED = 8
+FLAG_JAUMANN_AS_PRINTED = 512
 
 GATHER, SYMMETRIC = 0, 1
 CTOL = 1.0e-4          # reading Q9: C = I unless |det C^-1| > CTOL * ||C^-1||_F^3

@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libsph.so")
 
 MAX_MATERIALS = 8
-STRENGTH, CORRECTION_TENSOR, PCLIP_GLOBAL, JAUMANN_AS_PRINTED, NO_LISTS = 1, 2, 4, 8, 16
+STRENGTH, CORRECTION_TENSOR, PCLIP_GLOBAL, JAUMANN_AS_PRINTED, NO_LISTS = 1, 2, 4, 512, 16
 OK, EINVAL, ENOMEM, ECUDA, EORDER, ECAPACITY = 0, -1, -2, -3, -4, -5
 PREDICT, CLOSE, DERIVATIVES = 0, 1, 2
 GATHER, SYMMETRIC = 0, 1
@@ -25,7 +25,8 @@ F = dict(RHO=0, OMEGA=1, P=2, CS=3, T=4, GAMMA=5, Y=6, MUMAX=7, DUDT=8, DT=9, EA
          CFLAG=13, NGATHER=14, NSYMMETRIC=15, H=16, RUNG=17, A=32, V=36, X=40, SPRED=48, S=56, DSDT=64, F=80, CINV=96, G=112)
 T_SLOTS = ("build", "density", "predict", "gradient", "force", "close", "kickdrift", "step")
 C_SLOTS = ("pairs_gather", "pairs_symmetric", "tests_density", "tests_force", "cfallback", "tests_cull",
-           "candidates", "list_overflow", "bad_material", "omega_small", "nonfinite", "tiles_dirty", "active_updates", "active_tiles", "pairs_intile", "list_slots")
+           "candidates", "list_overflow", "bad_material", "omega_small", "nonfinite", "tiles_dirty", "active_updates", "active_tiles", "pairs_intile", "list_slots",
+           "rung_clamped", "steps_since_full")
 
 FLOAT_FIELDS = ("x", "y", "z", "m", "h", "vx", "vy", "vz", "u", "Sxx", "Syy", "Sxy", "Sxz", "Syz")
 OPT_FIELDS = ("gx", "gy", "gz")

@@ -147,6 +147,9 @@ static bool params_ok(const sph_params *p)
     if (!p) return false;
     if (p->n_materials < 1 || p->n_materials > SPH_MAX_MATERIALS) return false;
     if (!(p->kappa > 0.f)) return false;
+    const unsigned known = SPH_STRENGTH | SPH_CORRECTION_TENSOR | SPH_PCLIP_GLOBAL | SPH_JAUMANN_AS_PRINTED | SPH_NO_LISTS
+                           | SPH_NO_GRAPH | SPH_MORTON_ORDER;
+    if (p->flags & ~known) return false;     // retired bits (8, 128, 256) and unknown ones: refused, never ignored
     for (int k = 0; k < p->n_materials; ++k)
         if (!(p->mat[k].rho0 > 0.f) || !(p->mat[k].cv > 0.f) || !(p->mat[k].c0 > 0.f)) return false;
     return true;
@@ -212,6 +215,10 @@ extern "C" int sph_init(sph_ctx **out, const sph_params *params, long long n_max
         if (e == cudaSuccess) e = cudaMemsetAsync(c->d.nheavy, 0, sizeof(unsigned), c->stream);
         if (e == cudaSuccess) e = cudaMemsetAsync(c->d.heavy_mark, 0, ntile, c->stream);
         if (e == cudaSuccess) e = cudaMemsetAsync(c->d.tile_dirty, 0, ntile, c->stream);
+        // never written with SPH_NO_LISTS; the workspace arrives uninitialised
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d.tile_flag, 0, ntile, c->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d.tile_ncand, 0, ntile * sizeof(int), c->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->d.tile_off, 0, ntile * sizeof(unsigned long long), c->stream);
     }
     if (e == cudaSuccess) e = cudaMemsetAsync(c->d.dt_next, 0, sizeof(float), c->stream);
     if (e != cudaSuccess) { sph_destroy(c); return SPH_ECUDA; }
@@ -615,6 +622,7 @@ extern "C" int sph_step_rungs(sph_ctx *c, float dT, int max_rung, const unsigned
         c->steps_since_full = 0;
         c->force_full = false;
     }
+    SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_RUNG_CLAMPED], 0, sizeof(unsigned long long), c->stream));
     rc = sph_launch_rung_assign(c, dT, max_rung, rungs);
     if (rc) return rc;
     SPH_CUDA(c, cudaMemsetAsync(&d.counters[SPH_C_ACTIVE_UPDATES], 0, 2 * sizeof(unsigned long long), c->stream));
@@ -707,11 +715,8 @@ static int take_third_group(sph_ctx *c)
     return SPH_OK;
 }
 
-extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, float *dt_used)
+static int step_host_body(sph_ctx *c, sph_state *hs, long long n, float dt, float *dt_used)
 {
-    if (!c || n < 0 || (n > 0 && !state_ok(hs))) return SPH_EINVAL;
-    if (n > c->d.n_max) return SPH_ECAPACITY;
-    if (c->resident && n != c->d.n) return SPH_EINVAL;
     size_t N = (size_t)(c->d.n_max > 0 ? c->d.n_max : 1);
     float *base = c->stage;
     float *dev[17];
@@ -793,6 +798,14 @@ extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, f
     if (rc) return rc;
     float *dst[14] = {hs->x, hs->y, hs->z, nullptr, nullptr, hs->vx, hs->vy, hs->vz, hs->u,
                       hs->Sxx, hs->Syy, hs->Sxy, hs->Sxz, hs->Syz};
+    if (c->adapt_h_every > 0 && n > 0) {
+        // the step may have updated the smoothing lengths: they go back with the rest of the state, so
+        // that the caller's h stays the resident one (otherwise the next call would see "the caller changed h", put its
+        // stale h back over the adapted one and start from a full build every time)
+        rc = sph_launch_get_h(c, dev[4]);
+        if (rc) return rc;
+        dst[4] = hs->h;
+    }
     for (int k = overlap ? 3 : 0; k < 14; ++k) {
         if (n > 0 && dst[k])
             SPH_CUDA(c, cudaMemcpyAsync(dst[k], dev[k], (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
@@ -801,6 +814,28 @@ extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, f
     SPH_CUDA(c, cudaStreamSynchronize(c->stream));
     if (overlap) SPH_CUDA(c, cudaEventSynchronize(c->ev_copied));
     return SPH_OK;
+}
+
+extern "C" int sph_step_host(sph_ctx *c, sph_state *hs, long long n, float dt, float *dt_used)
+{
+    if (!c || n < 0 || (n > 0 && !state_ok(hs))) return SPH_EINVAL;
+    if (n > c->d.n_max) return SPH_ECAPACITY;
+    if (c->resident && n != c->d.n) return SPH_EINVAL;
+    const int rc = step_host_body(c, hs, n, dt, dt_used);
+    if (rc) {
+        // an error part way: copies into the staging arrays or into the caller's host arrays may still be in flight on
+        // the three streams.  The caller is free to reuse its buffers once this returns, so wait for all of them, and
+        // leave nothing of this call's per-call state behind.
+        cudaStreamSynchronize(c->stream);
+        cudaStreamSynchronize(c->h2d_stream);
+        cudaStreamSynchronize(c->copy_stream);
+        (void)cudaGetLastError();
+        c->host_out = nullptr; c->host_in = nullptr; c->host_in_g = nullptr;
+        c->p.flags &= ~SPH_INT_DEFER_AEXT;
+        c->no_reuse_now = false;
+        c->force_full = true;
+    }
+    return rc;
 }
 
 extern "C" int sph_download_state(sph_ctx *c, sph_state *state)
@@ -881,6 +916,7 @@ extern "C" int sph_get_counters(sph_ctx *c, long long *out, int n)
     unsigned long long h[SPH_C_COUNT];
     SPH_CUDA(c, cudaMemcpyAsync(h, c->d.counters, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    h[SPH_C_STEPS_SINCE_FULL] = (unsigned long long)c->steps_since_full;       // host-side
     for (int k = 0; k < n && k < SPH_C_COUNT; ++k) out[k] = (long long)h[k];
     return SPH_OK;
 }

@@ -219,8 +219,10 @@ __global__ void __launch_bounds__(256, 6) k_close(Dev d, DevParams p, int phase,
     if (rc.on && !rc.fixed_rungs) {
         // next rung: the smallest one whose step is within the new limit, but no coarser than the rungs whose
         // steps line up with the present time (n1 substeps of 2^R done)
+        // (a limit that is not a number sends the particle to the finest rung; a limit below the finest step is counted)
         int want = 0;
-        while (want < rc.R && rc.dT / (float)(1 << want) > dti) ++want;
+        while (want < rc.R && !(rc.dT / (float)(1 << want) <= dti)) ++want;
+        if (!(rc.dT / (float)(1 << rc.R) <= dti)) atomicAdd(&d.counters[SPH_C_RUNG_CLAMPED], 1ull);     // rare
         const int tz = rc.n1 >= (1 << rc.R) ? rc.R : (__ffs(rc.n1) - 1);
         d.rung[i] = (unsigned char)min(rc.R, max(want, rc.R - tz));
     }
@@ -324,7 +326,8 @@ __global__ void __launch_bounds__(256) k_rung_assign(Dev d, float dT, int R, con
     if (fixed_rungs) r = min((int)fixed_rungs[((const unsigned *)d.r.s[PP_ORIG])[i]], R);
     else {
         const float dti = d.dti[i];
-        while (r < R && dT / (float)(1 << r) > dti) ++r;
+        while (r < R && !(dT / (float)(1 << r) <= dti)) ++r;         // NaN limit: the finest rung, not the coarsest
+        if (!(dT / (float)(1 << R) <= dti)) atomicAdd(&d.counters[SPH_C_RUNG_CLAMPED], 1ull);   // beyond its limit even there
     }
     d.rung[i] = (unsigned char)r;
 }
@@ -374,10 +377,20 @@ __global__ void __launch_bounds__(256) k_kick_drift_rung(Dev d, DevParams p, int
 }
 
 // tiles that hold a candidate neighbour of an active tile need their density and PREDICT in this substep
-__global__ void __launch_bounds__(256) k_mark_need(Dev d, int ntile)
+// lists == 0 (SPH_NO_LISTS): there are no candidate lists to follow (tile_flag, tile_ncand, tile_off, cand are never
+// written), and the tree-walk pair pass works on every tile: every tile is needed.
+__global__ void __launch_bounds__(256) k_mark_need(Dev d, int ntile, int lists)
 {
     const int tile = blockIdx.x;
-    if (tile >= ntile || !d.tile_act[tile]) return;
+    if (tile >= ntile) return;
+    if (!lists) {
+        if (threadIdx.x == 0) {
+            d.tile_need[tile] = 1;
+            atomicAdd(&d.counters[SPH_C_ACTIVE_TILES], 1ull);
+        }
+        return;
+    }
+    if (!d.tile_act[tile]) return;
     if (threadIdx.x == 0) {
         d.tile_need[tile] = 1;
         atomicAdd(&d.counters[SPH_C_ACTIVE_TILES], 1ull);
@@ -419,7 +432,7 @@ int sph_launch_mark_need(sph_ctx *c)
     Dev &d = c->d;
     if (d.n == 0) return SPH_OK;
     const int ntile = sph_div_up(d.nchunk, SPH_TILE_CHUNKS);
-    k_mark_need<<<ntile, 256, 0, c->stream>>>(d, ntile);
+    k_mark_need<<<ntile, 256, 0, c->stream>>>(d, ntile, c->use_lists ? 1 : 0);
     c->launches++;
     SPH_CUDA(c, cudaGetLastError());
     return SPH_OK;

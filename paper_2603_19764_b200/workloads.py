@@ -31,7 +31,7 @@ SEED_BASE = 260319764
 FLAG_STRENGTH = 1
 FLAG_CORRECTION_TENSOR = 2
 FLAG_PCLIP_GLOBAL = 4
-FLAG_JAUMANN_AS_PRINTED = 8
+FLAG_JAUMANN_AS_PRINTED = 512
 FLAG_NO_LISTS = 16
 FLAG_NO_GRAPH = 64
 

@@ -163,3 +163,14 @@ def restrict(fields, idx):
     for k, v in fields.items():
         out[k] = v[..., idx] if isinstance(v, np.ndarray) and v.ndim >= 1 else v
     return out
+
+
+def state_errors(x, v, u, S, st):
+    """Errors of a GPU state against an oracle stepper after several steps: max norm per field, and for S also the rms
+    and the 99.9th percentile (both relative to max|S|) -- after many steps a handful of particles whose fp32 drift
+    rounded the other way carry the maximum, the bulk statistic is the sharper check."""
+    smax = np.abs(st.S).max()
+    dS = np.abs(np.asarray(S, dtype=np.float64) - st.S)
+    return {"x": maxnorm_err(x, st.x), "v": maxnorm_err(v, st.v), "u": maxnorm_err(u, st.u),
+            "S_max": float(dS.max() / smax), "S_rms": float(np.sqrt((dS ** 2).mean()) / smax),
+            "S_p999": float(np.percentile(dS, 99.9) / smax)}

@@ -53,6 +53,25 @@ def test_argument_errors_without_gpu(lib):
     lib.sph_destroy(None)
 
 
+def test_retired_and_unknown_flag_bits_are_refused(lib):
+    """Bit 8 once meant the opposite Jaumann choice, 128 and 256 selected kernels that no longer exist: a caller that
+    still passes one of them must hear about it (sph.h), not get something else silently."""
+    from paper_2603_19764_b200 import binding as B, workloads as W
+    p = B.make_params(W.Params())
+    assert lib.sph_workspace_bytes(C.byref(p), 100) > 0
+    for bit in (8, 128, 256, 1024, 1 << 31):
+        q = B.make_params(W.Params())
+        q.flags |= bit
+        assert lib.sph_workspace_bytes(C.byref(q), 100) == 0, bit
+        ctx = C.c_void_p()
+        assert lib.sph_init(C.byref(ctx), C.byref(q), 100, C.c_void_p(256), 1 << 30, None) == B.EINVAL, bit
+    for bit in (1, 2, 4, 16, 32, 64, 512):
+        q = B.make_params(W.Params())
+        q.flags |= bit
+        assert lib.sph_workspace_bytes(C.byref(q), 100) > 0, bit
+    assert B.JAUMANN_AS_PRINTED == W.FLAG_JAUMANN_AS_PRINTED == 512
+
+
 def test_no_cpu_fallback_when_library_missing(monkeypatch, tmp_path):
     from paper_2603_19764_b200 import binding as B
     monkeypatch.setattr(B, "_lib", None)

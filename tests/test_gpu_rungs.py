@@ -28,15 +28,18 @@ def _compare(s, t, st, tol_v=U.TOL_STATE, tol_S=U.TOL_STATE):
     return errs
 
 
-@pytest.mark.parametrize("skin", [0.0, 0.06])
-def test_big_step_with_fixed_rungs_matches_the_oracle(skin):
+@pytest.mark.parametrize("skin,no_lists", [(0.0, False), (0.06, False), (0.0, True)])
+def test_big_step_with_fixed_rungs_matches_the_oracle(skin, no_lists):
     """The rungs of the big step are handed to both sides (the oracle's own assignment), so every decision is the
-    same and the states must agree like those of a global step do; the counter of closing kicks is sum 2^rung."""
+    same and the states must agree like those of a global step do; the counter of closing kicks is sum 2^rung.
+    no_lists: SPH_NO_LISTS, the tree-walk pair passes (no candidate lists to mark needed tiles from: all are)."""
     import torch
     from paper_2603_19764_b200 import binding as B
     wl = W.impact_pair(20000, W.SEED_BASE + 3, 100.0, 1.214)
     wl.params.skin = skin
     wl.params.rebuild_every = 4
+    if no_lists:
+        wl.params.flags |= W.FLAG_NO_LISTS
     st = O.RungStepper(wl, mode="grid")
     st.bootstrap()
     R = 3
@@ -55,7 +58,10 @@ def test_big_step_with_fixed_rungs_matches_the_oracle(skin):
         assert np.array_equal(s.get_field("RUNG").cpu().numpy().astype(np.int64), rungs)
     assert c["active_updates"] == int((1 << rungs).sum()) == int(st.kicks.sum())
     assert c["list_overflow"] == 0 and c["nonfinite"] == 0
-    assert c["active_tiles"] < (1 << R) * ((wl.n + 255) // 256)          # tiles without active particles were skipped
+    if no_lists:
+        assert c["active_tiles"] == (1 << R) * ((wl.n + 255) // 256)     # the tree walk visits every tile
+    else:
+        assert c["active_tiles"] < (1 << R) * ((wl.n + 255) // 256)      # tiles without active particles were skipped
     print(f"fixed rungs, skin {skin}: rung histogram {np.bincount(rungs).tolist()}, closing kicks {c['active_updates']} of "
           f"{wl.n << R}, active tiles {c['active_tiles']} of {(1 << R) * ((wl.n + 255) // 256)}", {k: float(f'{e:.3g}') for k, e in errs.items()})
 
@@ -68,10 +74,10 @@ def test_big_steps_with_rungs_from_the_limits_match_the_oracle():
     from paper_2603_19764_b200 import binding as B
     wl = W.impact_pair(20000, W.SEED_BASE + 3, 100.0, 1.214)
     wl.params.skin = 0.05
-    st = O.RungStepper(wl, mode="grid")
+    st = O.RungStepper(wl, mode="grid", store_fp32=True)          # like storage: fp32 state, fp64 arithmetic
     st.bootstrap()
     R = 3
-    dT = float(np.percentile(st.d["dt_i"], 99.5)) * 0.97
+    dT = float(np.float32(np.percentile(st.d["dt_i"], 99.5) * 0.97))
     with torch.cuda.stream(torch.cuda.Stream()):
         s = B.Sph(wl.params, wl.n)
         t = s.upload(wl)
@@ -85,8 +91,27 @@ def test_big_steps_with_rungs_from_the_limits_match_the_oracle():
             print(f"big step {big}: rung histogram {np.bincount(rg).tolist()}, {differ} rungs differ, closing kicks gpu {kicks} oracle {int(st.kicks.sum())}")
             assert differ <= max(2, wl.n // 2000)
             assert abs(kicks - int(st.kicks.sum())) <= 8 * max(2, wl.n // 2000)
-        errs = _compare(s, t, st, tol_v=1e-3, tol_S=1e-2)
-    print({k: float(f"{e:.3g}") for k, e in errs.items()})
+            assert s.get_counters()["rung_clamped"] == 0               # three rungs hold every limit here
+            agree = (rg == st.rung) if big == 0 else (agree & (rg == st.rung))
+        # A particle whose limit sits on a power-of-two boundary may take another rung on the GPU (fp32 limit) than in
+        # the oracle (fp64): another integration of that particle, not a rounding difference.  Its own state is left
+        # out of the max norms (how many there are is bounded above); its neighbours stay in.
+        x, v, u, S = _state(s, t)
+        sub = type("Sub", (), {})()
+        sub.x, sub.v, sub.u, sub.S = st.x[:, agree], st.v[:, agree], st.u[agree], st.S[:, agree]
+        errs = U.state_errors(x[:, agree], v[:, agree], u[agree], S[:, agree], sub)
+        errs["all_v"], errs["all_S"] = U.maxnorm_err(v, st.v), U.maxnorm_err(S, st.S)
+        assert int((~agree).sum()) <= 2 * max(2, wl.n // 2000)
+        # measured (B200, round 3; no rung differed): v 1.7e-7, u 2.0e-7, S_max 9.4e-7, S_rms 1.8e-8, S_p999 1.6e-7
+        # (the fp64-state stepper needed v 1e-3, S 1e-2 here)
+        assert errs["x"] <= 1e-6 and errs["v"] <= 1e-5 and errs["u"] <= 1e-5, errs
+        assert errs["S_rms"] <= 1e-6 and errs["S_p999"] <= 5e-6 and errs["S_max"] <= 2e-5, errs
+        assert errs["all_v"] <= 1e-3 and errs["all_S"] <= 1e-2, errs
+        # a big step too long for max_rung = 1 (substeps of 3 dT): most particles are stepped beyond their limit, and the counter says so
+        s.step_rungs(6.0 * dT, 1)
+        clamped = s.get_counters()["rung_clamped"]
+        assert clamped >= wl.n // 2, clamped
+    print({k: float(f"{e:.3g}") for k, e in errs.items()}, "clamped on a 6x big step with two rungs:", clamped)
 
 
 def test_single_rung_big_step_is_a_global_step():
