@@ -50,8 +50,7 @@ def test_density_continuum_limit():
         c, o, l = O.neighbors(p[0], p[1], p[2], h, 2.0, O.GATHER, "grid")
         rho, om = O.density(p[0], p[1], p[2], m, h, 2.0, o, l)
         i = np.argmin(((p - p.mean(axis=1, keepdims=True)) ** 2).sum(axis=0))
-        if eta < 3.0 or True:
-            errs.append((abs(rho[i] / rho0 - 1.0), abs(om[i] - 1.0)))
+        errs.append((abs(rho[i] / rho0 - 1.0), abs(om[i] - 1.0)))
     assert errs[0][0] < 2e-2 and errs[1][0] < 2e-3 and errs[2][0] < 2e-4
     assert errs[0][0] > errs[1][0] > errs[2][0]
     assert errs[2][1] < 1e-3

@@ -190,3 +190,75 @@ def test_grid_mode_gives_the_same_step_as_brute():
     a = O.Stepper(wl, mode="brute"); b = O.Stepper(wl, mode="grid")
     a.step(0.0); b.step(0.0)
     assert np.array_equal(a.x, b.x) and np.array_equal(a.S, b.S) and np.array_equal(a.u, b.u)
+
+
+def test_single_pass_closing_half_kick_is_pinned_by_closed_forms():
+    """Pin of oracle.single_pass()'s closing half kick (Eq. 41: v, u, S advance by HALF a step with the
+    new derivatives, then S is rescaled again), by values that do not come from single_pass's own formula:
+
+    (1) pure shear v = (g y, 0, 0) of an unstressed block, constant shear modulus: the corrected gradient is exact for a
+        linear field, so G_xy = g, eps_xy = g/2 and, with S = 0, dS_xy/dt = 2 Gamma eps_xy = Gamma g
+        with every other component 0 (Eq. 13).  Below yield the closed S_xy is therefore Gamma g dt / 2 -- a full-step
+        kick would give twice that;
+    (2) the same with a step so long that Gamma g dt / 2 is beyond the yield strength: the second rescale
+        (PAPER.md:244) puts the state ON the yield surface, sqrt(J2) = |S_xy| = Y, direction kept;
+    (3) a uniform external acceleration on an isolated particle (no neighbour within reach: a = a_ext exactly, du/dt = 0):
+        g_y = -10, dt = 0.2 gives v_y - 1, not - 2; a fixed particle keeps its velocity;
+    (4) the special value dt = 2, where half a step is exactly one unit: u_close - u = du/dt and v_close - v = a,
+        bit for bit (a full-step kick would double them), and dt = 0 returns the input state."""
+    gdot, Gam = 100.0, 22.7e9
+    wl = W.elastic_block(9)
+    A = wl.arrays
+    assert wl.params.materials[0].Gamma == Gam
+    A["vx"] = (gdot * A["y"].astype(np.float64)).astype(np.float32)
+    A["vy"][:] = 0.0; A["vz"][:] = 0.0
+    for k in ("Sxx", "Syy", "Sxy", "Sxz", "Syz"):
+        A[k][:] = 0.0
+    A["u"][:] = 300.0 * wl.params.materials[0].cv          # cold: no thermal softening to speak of (Eq. 37)
+    # the velocity field the oracle sees is the fp32 array: linear up to its rounding (1e-7 relative)
+    dt1 = 1.0e-7                                   # Gamma g dt / 2 = 1.135e5 Pa, far below Y0 = 1e7 Pa
+    d = O.single_pass(wl, dt=dt1)
+    Y = d["Y"]
+    assert Y.min() > 1.0e6
+    want = 0.5 * Gam * gdot * dt1
+    S = d["S_close"]
+    assert np.allclose(S[2], want, rtol=2e-6, atol=0.0)                     # (1): half a step
+    assert np.abs(S[[0, 1, 3, 4]]).max() <= 2e-6 * want
+    assert np.all(d["f_close"] == 1.0)
+    dt2 = 4.0e-5                                   # Gamma g dt / 2 = 4.54e7 Pa: beyond Y for many particles
+    d2 = O.single_pass(wl, dt=dt2)
+    S2, Y2 = d2["S_close"], d2["Y"]
+    over = 0.5 * Gam * gdot * dt2 > Y2
+    assert over.sum() > 50 and (~over).sum() > 0                            # both branches of the rescale are taken
+    assert np.allclose(np.abs(S2[2][over]), Y2[over], rtol=1e-9)            # (2): on the yield surface
+    assert np.allclose(np.sqrt(O.J2(S2))[over], Y2[over], rtol=1e-12)
+    assert np.all(S2[2][over] > 0.0)
+    assert np.allclose(S2[2][~over], 0.5 * Gam * gdot * dt2, rtol=2e-6)     # below yield: untouched by the rescale
+    assert np.all((d2["f_close"] < 1.0) == over)
+
+    # (3) isolated particles under a uniform external acceleration
+    far = W.elastic_block(2)
+    far.arrays["x"] = (np.arange(far.n) * 1.0).astype(np.float32)           # one metre apart, h = 1.3 cm
+    far.arrays["y"][:] = 0.0; far.arrays["z"][:] = 0.0
+    far.arrays["gy"] = np.full(far.n, -10.0, np.float32)
+    far.arrays["vx"][:] = 3.0; far.arrays["vy"][:] = 0.5; far.arrays["vz"][:] = 0.0
+    far.fixed[0] = 1
+    df = O.single_pass(far, dt=0.2)
+    assert np.array_equal(df["a"], np.stack([np.zeros(far.n), np.full(far.n, -10.0), np.zeros(far.n)]))
+    assert np.all(df["dudt"] == 0.0)
+    assert np.array_equal(df["v_close"][:, 1:], np.stack([np.full(far.n - 1, 3.0), np.full(far.n - 1, -0.5),
+                                                          np.zeros(far.n - 1)]))
+    assert np.array_equal(df["v_close"][:, 0], [3.0, 0.5, 0.0])             # fixed: no kick
+    assert np.array_equal(df["u_close"], far.arrays["u"].astype(np.float64))
+
+    # (4) dt = 2 and dt = 0 on the generic block (random S, thermal spread, shear + noise)
+    gen = W.elastic_block(8)
+    g0 = O.single_pass(gen, dt=0.0)
+    gA = {k: v.astype(np.float64) for k, v in gen.arrays.items()}
+    v_in = np.stack([gA["vx"], gA["vy"], gA["vz"]])
+    assert np.array_equal(g0["v_close"], v_in) and np.array_equal(g0["u_close"], gA["u"])
+    g2 = O.single_pass(gen, dt=2.0)
+    assert np.abs(g2["dudt"]).min() > 0.0
+    assert np.allclose(g2["u_close"] - gA["u"], g2["dudt"], rtol=1e-9, atol=0.0)
+    assert np.allclose(g2["v_close"] - v_in, g2["a"], rtol=1e-9, atol=1e-9 * np.abs(g2["a"]).max())
+    assert not np.allclose(g2["u_close"] - gA["u"], 2.0 * g2["dudt"], rtol=0.2)
