@@ -345,12 +345,11 @@ int sph_get_tile_stats(sph_ctx *ctx, int *ncand, unsigned *cycles, unsigned char
  * It is the denominator of the ALU-bound roofline entries of bench.py. */
 int sph_fp32_peak(void *cuda_stream, int repeats, double *tflops);
 
-/* Measurement aid for the design question "symmetric-pair accumulation" (BASELINE.json north_star; DESIGN.md
- * section 6): the rate at which one tile's CTA (256 threads, two CTAs per SM as in the pair pass) can add the j side
- * of a pair into `accumulators` shared-memory floats per target (20 for the fused pass: F 9, C^-1 6, a 3, du/dt,
- * mu_max; 5 hydro only) at random targets of the tile, with atomicAdd -- on sm_100a a compare-and-swap loop
- * (ATOMS.CAST.SPIN).  pairs_per_s: HOST, scatters of one pair per second over the whole device.  Synchronises. */
-int sph_shared_scatter_rate(void *cuda_stream, int accumulators, double *pairs_per_s);
+/* The same measurement for other instruction forms (variant 0 is sph_fp32_peak): 1 = scalar FFMA with three register
+ * operands, 2 = packed FFMA2 (fma.rn.f32x2) with three 64-bit register operands, 3 / 4 = variants 1 / 2 with one independent
+ * integer ALU instruction per FP32 instruction.  TFLOP/s (2 flop per FFMA, 4 per FFMA2).  It answers whether packed FP32
+ * arithmetic frees issue slots on this device; nothing on the step path calls it.  Synchronises. */
+int sph_fp32_rate(void *cuda_stream, int variant, int repeats, double *tflops);
 
 /* Number of this library's kernel launches since sph_init (HOST; no synchronisation). */
 long long sph_launch_count(const sph_ctx *ctx);

@@ -33,7 +33,7 @@ OPT_FIELDS = ("gx", "gy", "gz")
 
 # every symbol include/sph.h declares (tests check the library exports all of them)
 SYMBOLS = ("sph_workspace_bytes", "sph_init", "sph_build_neighbors", "sph_density", "sph_strength_update",
-           "sph_gradients", "sph_forces", "sph_gradients_forces", "sph_fp32_peak", "sph_shared_scatter_rate", "sph_step_rungs", "sph_adapt_h", "sph_set_eos_table", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
+           "sph_gradients", "sph_forces", "sph_gradients_forces", "sph_fp32_peak", "sph_fp32_rate", "sph_step_rungs", "sph_adapt_h", "sph_set_eos_table", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
            "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_get_diagnostics",
            "sph_diagnostics_noalloc", "sph_launch_count",
            "sph_last_cuda_error", "sph_strerror", "sph_destroy")
@@ -116,8 +116,8 @@ def load():
     lib.sph_gradients_forces.restype = i
     lib.sph_fp32_peak.argtypes = [vp, i, C.POINTER(C.c_double)]
     lib.sph_fp32_peak.restype = i
-    lib.sph_shared_scatter_rate.argtypes = [vp, i, C.POINTER(C.c_double)]
-    lib.sph_shared_scatter_rate.restype = i
+    lib.sph_fp32_rate.argtypes = [vp, i, i, C.POINTER(C.c_double)]
+    lib.sph_fp32_rate.restype = i
     lib.sph_step_rungs.argtypes = [vp, fl, i, vp]
     lib.sph_step_rungs.restype = i
     lib.sph_step.argtypes = [vp, C.POINTER(sph_state), ll, fl, vp]
@@ -293,11 +293,10 @@ class Sph:
         self._check(self.lib.sph_fp32_peak(self.stream.cuda_stream, int(repeats), C.byref(out)), "sph_fp32_peak")
         return float(out.value)
 
-    def shared_scatter_rate(self, accumulators: int) -> float:
-        """sph_shared_scatter_rate: pair scatters per second into shared-memory accumulators (measurement aid)."""
+    def fp32_rate(self, variant: int, repeats: int = 5) -> float:
+        """sph_fp32_rate: TFLOP/s of FFMA chains in another instruction form (see include/sph.h)."""
         out = C.c_double(0.0)
-        self._check(self.lib.sph_shared_scatter_rate(self.stream.cuda_stream, int(accumulators), C.byref(out)),
-                    "sph_shared_scatter_rate")
+        self._check(self.lib.sph_fp32_rate(self.stream.cuda_stream, int(variant), int(repeats), C.byref(out)), "sph_fp32_rate")
         return float(out.value)
 
     def step(self, tensors: Optional[Dict[str, object]] = None, n: int = 0, dt: float = 0.0, dt_used=None):

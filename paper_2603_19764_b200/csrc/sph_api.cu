@@ -116,8 +116,8 @@ static size_t carve(Dev *d, float **stage, char *base, long long n_max, int kcap
     o.tile_need = b.take<unsigned char>(ntile);
     o.rung = b.take<unsigned char>(N);
     o.cand_cursor = b.take<unsigned long long>(2);
-    o.cand_cap = lists ? (unsigned long long)ntile * (2 * SPH_SE) : 1;   // pool: twice the one-round average
-    o.cand_cap_dirty = (lists && skin > 0.f) ? (unsigned long long)ntile * SPH_SE : 0;
+    o.cand_cap = lists ? (unsigned long long)ntile * SPH_POOL_PER_TILE : 1;   // pool: twice the one-round average
+    o.cand_cap_dirty = (lists && skin > 0.f) ? (unsigned long long)ntile * (SPH_POOL_PER_TILE / 2) : 0;
     o.cand = b.take<unsigned>((size_t)(o.cand_cap + o.cand_cap_dirty));
     o.rows_cap = kcap;
     o.rowptr = b.take<unsigned short>(lists ? nchunk * (SPH_MAXROUND + 1) : 1);

@@ -19,7 +19,9 @@
 // neighbour-list machinery (sph_lists.cu)
 #define SPH_TILE_CHUNKS 8     // chunks per tile = warps per CTA of the list kernels
 #define SPH_TILE (SPH_TILE_CHUNKS * SPH_CHUNK)
+#ifndef SPH_SE                // (a test build with fewer slots drives the multi-round paths on every tile: tests/test_gpu_rounds.py)
 #define SPH_SE 1600           // candidates staged per round; the cull, density and pair kernels agree on it
+#endif
                               // (18 floats per slot plus the dummy slot, twice per SM: 1601 x 72 B <= 115 712 B)
 #define SPH_MAXROUND 15       // rounds a tile may need (more: the tile falls back to the tree-walk kernels)
 #define SPH_CULL_MAXSRC 768   // source chunks a tile may accept in the tree walk
@@ -28,7 +30,12 @@
 #define SPH_CULL_CFCACHE 128  // source chunks whose per-particle chunk flags are kept between the two passes
 #define SPH_CULL_LATE 1       // a candidate within reach of at most this many chunk boxes of a tile that needs several
                               // rounds goes to the END of the tile's candidate list (k_cull, A2; measured 1..4 on configs[4])
+#ifndef SPH_ROWS_DEFAULT
 #define SPH_ROWS_DEFAULT 64   // default row-groups (4 neighbours per lane each) reserved per chunk
+#endif
+#ifndef SPH_POOL_PER_TILE     // candidate pool: slots per tile on average (twice the one-round capacity); half as much again
+#define SPH_POOL_PER_TILE (2 * SPH_SE)   // for the dirty tiles' region.  (The small-SPH_SE test build keeps the 3 200 of the product.)
+#endif
 
 // indices into Resident::s (scalar ping-pong arrays)
 enum {
