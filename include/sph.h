@@ -82,6 +82,8 @@ enum {
     SPH_F_NSYMMETRIC,   /* |symmetric set| as float                       */
     SPH_F_H,            /* smoothing length (after sph_adapt_h)           */
     SPH_F_RUNG,         /* rung of the last sph_step_rungs, as float      */
+    SPH_F_TILE,         /* tile (256 curve-consecutive resident particles) the particle sits in, as float: the
+                           index into the arrays of sph_get_tile_stats / sph_get_tile_dirty (test hook)       */
     SPH_F_A = 32,       /* +0..2   acceleration, Eq. 18 (+ a_ext)         */
     SPH_F_V = 36,       /* +0..2   velocity after the closing kick        */
     SPH_F_X = 40,       /* +0..2   position                               */
@@ -338,6 +340,12 @@ int sph_get_counters(sph_ctx *ctx, long long *counters, int n); /* SPH_C_* slots
  * Returns the number of tiles (nothing is copied if capacity is smaller), or a negative SPH_E* code.
  * Synchronises the stream. */
 int sph_get_tile_stats(sph_ctx *ctx, int *ncand, unsigned *cycles, unsigned char *flag, int capacity);
+
+/* Diagnostic / test hook: which tiles are "dirty" (sph_params.skin > 0): their surroundings moved by more than the skin
+ * since the last full build, and their lists are rebuilt in every step until the next one (SPH_C_TILES_DIRTY is their
+ * number).  dirty: HOST array of `capacity` bytes (1 = dirty).  Returns the number of tiles (nothing is copied if
+ * capacity is smaller or dirty is NULL), or a negative SPH_E* code.  Synchronises the stream. */
+int sph_get_tile_dirty(sph_ctx *ctx, unsigned char *dirty, int capacity);
 
 /* Measurement aid ("measure an FMA-chain microbenchmark"): the FP32 CUDA-core rate this
  * device sustains on a kernel of independent FFMA chains (2 flop each, no memory traffic), in TFLOP/s, best of

@@ -22,7 +22,7 @@ PREDICT, CLOSE, DERIVATIVES = 0, 1, 2
 GATHER, SYMMETRIC = 0, 1
 
 F = dict(RHO=0, OMEGA=1, P=2, CS=3, T=4, GAMMA=5, Y=6, MUMAX=7, DUDT=8, DT=9, EACC=10, EPS2=11, U=12,
-         CFLAG=13, NGATHER=14, NSYMMETRIC=15, H=16, RUNG=17, A=32, V=36, X=40, SPRED=48, S=56, DSDT=64, F=80, CINV=96, G=112)
+         CFLAG=13, NGATHER=14, NSYMMETRIC=15, H=16, RUNG=17, TILE=18, A=32, V=36, X=40, SPRED=48, S=56, DSDT=64, F=80, CINV=96, G=112)
 T_SLOTS = ("build", "density", "predict", "gradient", "force", "close", "kickdrift", "step")
 C_SLOTS = ("pairs_gather", "pairs_symmetric", "tests_density", "tests_force", "cfallback", "tests_cull",
            "candidates", "list_overflow", "bad_material", "omega_small", "nonfinite", "tiles_dirty", "active_updates", "active_tiles", "pairs_intile", "list_slots",
@@ -34,7 +34,7 @@ OPT_FIELDS = ("gx", "gy", "gz")
 # every symbol include/sph.h declares (tests check the library exports all of them)
 SYMBOLS = ("sph_workspace_bytes", "sph_init", "sph_build_neighbors", "sph_density", "sph_strength_update",
            "sph_gradients", "sph_forces", "sph_gradients_forces", "sph_fp32_peak", "sph_fp32_rate", "sph_step_rungs", "sph_adapt_h", "sph_set_eos_table", "sph_step", "sph_step_host", "sph_download_state", "sph_get_field",
-           "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_get_diagnostics",
+           "sph_get_neighbors", "sph_get_timings", "sph_get_counters", "sph_get_tile_stats", "sph_get_tile_dirty", "sph_get_diagnostics",
            "sph_diagnostics_noalloc", "sph_launch_count",
            "sph_last_cuda_error", "sph_strerror", "sph_destroy")
 
@@ -128,6 +128,8 @@ def load():
     lib.sph_get_timings.argtypes = [vp, C.POINTER(fl), i]
     lib.sph_get_counters.argtypes = [vp, C.POINTER(ll), i]
     lib.sph_get_tile_stats.argtypes = [vp, vp, vp, vp, i]
+    lib.sph_get_tile_dirty.argtypes = [vp, vp, i]
+    lib.sph_get_tile_dirty.restype = i
     lib.sph_set_eos_table.argtypes = [vp, i, vp]
     lib.sph_set_eos_table.restype = i
     lib.sph_get_diagnostics.argtypes = [vp, vp]
@@ -415,6 +417,15 @@ class Sph:
         rc = self.lib.sph_get_tile_stats(self.ctx, nc.ctypes.data, cy.ctypes.data, fl.ctypes.data, nt)
         self._check(min(rc, 0), "sph_get_tile_stats")
         return nc, cy, fl
+
+    def get_tile_dirty(self):
+        """sph_get_tile_dirty: uint8 numpy array, 1 for tiles whose lists are rebuilt in every step (host)."""
+        import numpy as np
+        nt = self.lib.sph_get_tile_dirty(self.ctx, None, 0)
+        self._check(min(nt, 0), "sph_get_tile_dirty")
+        out = np.zeros(nt, np.uint8)
+        self._check(min(self.lib.sph_get_tile_dirty(self.ctx, out.ctypes.data, nt), 0), "sph_get_tile_dirty")
+        return out
 
     def launch_count(self) -> int:
         return int(self.lib.sph_launch_count(self.ctx))

@@ -874,6 +874,7 @@ extern "C" int sph_get_field(sph_ctx *c, int id, float *dst)
     case SPH_F_NSYMMETRIC: src = (const float *)d.nsym; as_int = 1; break;
     case SPH_F_H: return sph_launch_get_h(c, dst);
     case SPH_F_RUNG: src = (const float *)d.rung; as_int = 2; break;
+    case SPH_F_TILE: return sph_launch_get_tile(c, dst);
     default: break;
     }
     if (!src) {
@@ -957,6 +958,17 @@ extern "C" int sph_get_tile_stats(sph_ctx *c, int *ncand, unsigned *cycles, unsi
     if (ncand) SPH_CUDA(c, cudaMemcpyAsync(ncand, c->d.tile_ncand, sizeof(int) * ntile, cudaMemcpyDeviceToHost, c->stream));
     if (cycles) SPH_CUDA(c, cudaMemcpyAsync(cycles, c->d.tile_cycles, sizeof(unsigned) * ntile, cudaMemcpyDeviceToHost, c->stream));
     if (flag) SPH_CUDA(c, cudaMemcpyAsync(flag, c->d.tile_flag, ntile, cudaMemcpyDeviceToHost, c->stream));
+    SPH_CUDA(c, cudaStreamSynchronize(c->stream));
+    return ntile;
+}
+
+extern "C" int sph_get_tile_dirty(sph_ctx *c, unsigned char *dirty, int capacity)
+{
+    if (!c || capacity < 0) return SPH_EINVAL;
+    if (!c->resident) return SPH_EORDER;
+    const int ntile = sph_div_up(c->d.nchunk, SPH_TILE_CHUNKS);
+    if (!c->use_lists || capacity < ntile || !dirty) return ntile;
+    SPH_CUDA(c, cudaMemcpyAsync(dirty, c->d.tile_dirty, ntile, cudaMemcpyDeviceToHost, c->stream));
     SPH_CUDA(c, cudaStreamSynchronize(c->stream));
     return ntile;
 }

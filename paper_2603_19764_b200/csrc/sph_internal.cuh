@@ -243,6 +243,7 @@ int sph_launch_mark_need(sph_ctx *c);
 int sph_launch_get_field(sph_ctx *c, const float *src, float *dst, int as_int);
 int sph_launch_get_position(sph_ctx *c, int comp, float *dst);
 int sph_launch_get_h(sph_ctx *c, float *dst);
+int sph_launch_get_tile(sph_ctx *c, float *dst);
 int sph_launch_diagnostics(sph_ctx *c, double *out);
 int sph_launch_h_update(sph_ctx *c, float n_target);
 int sph_launch_neighbors(sph_ctx *c, int which, int *counts, const long long *offsets, int *list, bool flagged_only);

@@ -626,6 +626,23 @@ __global__ void __launch_bounds__(256) k_scatter_h(const float4 *__restrict__ vh
     if (i < n) dst[orig[i]] = vh[i].w;
 }
 
+// the tile (SPH_TILE curve-consecutive resident particles) each particle sits in, caller order (sph_get_field(SPH_F_TILE))
+__global__ void __launch_bounds__(256) k_scatter_tile(const unsigned *__restrict__ orig, long long n, float *__restrict__ dst)
+{
+    long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (i < n) dst[orig[i]] = (float)(i / SPH_TILE);
+}
+
+int sph_launch_get_tile(sph_ctx *c, float *dst)
+{
+    Dev &d = c->d;
+    if (d.n == 0) return SPH_OK;
+    k_scatter_tile<<<sph_div_up(d.n, 256), 256, 0, c->stream>>>((const unsigned *)d.r.s[PP_ORIG], d.n, dst);
+    c->launches++;
+    SPH_CUDA(c, cudaGetLastError());
+    return SPH_OK;
+}
+
 int sph_launch_get_h(sph_ctx *c, float *dst)
 {
     Dev &d = c->d;

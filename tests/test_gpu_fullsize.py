@@ -196,3 +196,78 @@ def test_config_multi_step_invariants(k, steps):
     print(f"config{k} n={wl.n} {steps} steps: internal momentum drift {drift:.3g} of sum m|v| = {scale:.3g};"
           f" dirty tiles {c['tiles_dirty']}, omega_small {c['omega_small']}")
     assert drift <= 1e-5
+
+
+@pytest.mark.parametrize("k", [3, 4])
+def test_reuse_step_with_dirty_tiles_at_full_size_sampled(k):
+    """The configuration bench.py times, on a step that REUSES the lists of an earlier full build while tiles at the
+    contact are dirty (rebuilt into the second pool region every step): the state before that step is taken from the
+    device, the oracle evaluates the same step's derivatives on two dependency-closed samples (dense core, contact) at
+    the positions after the drift, from the predicted v, u, S of Eq. 40 formed here from the downloaded
+    fp32 state, and rho, a, du/dt, dS/dt and the neighbour ids of the sampled particles must agree.  The samples must
+    hold tiles that need two rounds and, at the contact, dirty tiles -- what the parity-size cases barely contain."""
+    import torch
+    from paper_2603_19764_b200 import binding as B
+    need = {3: 8e9, 4: 60e9}[k]
+    if _free_gpu_bytes() < need:
+        pytest.skip("not enough free device memory for configs[%d]" % k)
+    wl = W.config(k)
+    assert wl.params.skin > 0.0 and not wl.fixed.any()
+    n = wl.n
+    with torch.cuda.stream(torch.cuda.Stream()):
+        s = B.Sph(wl.params, n)
+        t = s.upload(wl)
+        dtu = torch.zeros(1, dtype=torch.float32, device="cuda")
+        s.step(t, n, 0.0, dtu)                                   # ingest, bootstrap, first step
+        for _ in range(12):                                      # until dirty tiles exist and the next step reuses
+            c = s.get_counters()
+            if c["tiles_dirty"] > 0 and 0 < c["steps_since_full"] < wl.params.rebuild_every - 2:
+                break
+            s.step(None, 0, 0.0, dtu)
+        assert c["tiles_dirty"] > 0, c
+        s.download_state(t)                                      # v, u, S at the full step before the checked one
+        prev = {"a": s.get_fields("A", 3), "dudt": s.get_field("DUDT"), "dS": s.get_fields("DSDT", 5)}
+        s.step(None, 0, 0.0, dtu)                                # the checked step
+        dt = float(dtu.item())
+        c = s.get_counters()
+        assert c["steps_since_full"] > 0 and c["tiles_dirty"] > 0 and c["nonfinite"] == 0, c
+        pos_now = s.get_fields("X", 3)
+        cur = W.Workload(wl.name, wl.params, dict(wl.arrays), wl.mat, wl.fixed, 0.0)
+        for q, name in enumerate(("x", "y", "z")):
+            cur.arrays[name] = pos_now[q].cpu().numpy()
+        tile_of = s.get_field("TILE").cpu().numpy().astype(np.int64)
+        ncand, _, flag = s.get_tile_stats()
+        dirty = s.get_tile_dirty()
+        got = {"rho": s.get_field("RHO"), "a": s.get_fields("A", 3), "dudt": s.get_field("DUDT"),
+               "dS": s.get_fields("DSDT", 5)}
+        report = {}
+        for where, centre in (("core", (0.0, 0.0, 0.0)), ("contact", (5.0e4 / np.sqrt(2.0), 5.0e4 / np.sqrt(2.0), 0.0))):
+            idx, pos, V = U.dependency_closed_sample(cur, centre, 30000)
+            di = torch.as_tensor(idx, device="cuda")
+            f64 = lambda a: a.cpu().numpy().astype(np.float64)
+            sub = cur.subset(idx)
+            A = {q: v.astype(np.float64) for q, v in sub.arrays.items()}
+            # Eq. 40: the predicted values this step's derivatives are evaluated from (no fixed particles here)
+            v_pred = np.stack([f64(t[q][di]) for q in ("vx", "vy", "vz")]) + dt * f64(prev["a"][:, di])
+            u_pred = f64(t["u"][di]) + dt * f64(prev["dudt"][di])
+            S_pred = np.stack([f64(t[q][di]) for q in ("Sxx", "Syy", "Sxy", "Sxz", "Syz")]) + dt * f64(prev["dS"][:, di])
+            g = np.stack([A["gx"], A["gy"], A["gz"]])
+            d = O.derivatives(sub.params, A["x"], A["y"], A["z"], A["m"], A["h"], v_pred[0], v_pred[1], v_pred[2],
+                              u_pred, S_pred, sub.mat, g, "grid")
+            dv = torch.as_tensor(V, device="cuda")
+            errs = {"rho": float(np.abs(f64(got["rho"][dv]) / d["rho"][pos] - 1.0).max()),
+                    "a": U.maxnorm_err(f64(got["a"][:, dv]), d["a"][:, pos]),
+                    "dudt": U.maxnorm_err(f64(got["dudt"][dv]), d["dudt"][pos]),
+                    "dS": U.maxnorm_err(f64(got["dS"][:, dv]), d["dS"][:, pos])}
+            U.neighbor_sets_equal(s, cur, mode="grid", select=V, oracle_sample=(idx, pos))
+            tiles = np.unique(tile_of[V])
+            rounds = (ncand[tiles] + 1599) // 1600
+            report[where] = dict(errs, sample=int(idx.size), tiles=int(tiles.size), two_round=int((rounds >= 2).sum()),
+                                 dirty=int(dirty[tiles].sum()), fallback=int((flag[tiles] != 0).sum()))
+            assert errs["rho"] <= U.TOL_RHO and errs["a"] <= U.TOL_RATE and errs["dudt"] <= U.TOL_RATE \
+                and errs["dS"] <= U.TOL_RATE, (where, errs)
+        torch.cuda.synchronize()
+    print(f"config{k} n={n} reuse step {c['steps_since_full']} after a full build, {c['tiles_dirty']} dirty tiles:",
+          {w: {q: (float(f'{v:.3g}') if isinstance(v, float) else v) for q, v in r.items()} for w, r in report.items()})
+    assert report["contact"]["dirty"] > 0                                   # rebuilt tiles are in the sample
+    assert report["core"]["two_round"] + report["contact"]["two_round"] > 0  # and tiles that stage twice
